@@ -1,0 +1,374 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the FDAS hot path on B200 (one step = one DM trial: prepare_spectrum ->
+convolve_plane -> harmonic_sum_peaks on one synthetic SKA-like time series).
+
+    python bench.py --gpus N --steps K --warmup W            # this repo's CUDA path
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle on the host cores
+
+Prints ONE JSON line (rank 0).  `value` = f-fdot plane points per second with the series resident in
+HBM; `e2e` = the same through fdas_search_host with the series in pinned host memory (H2D + D2H
+inside the timed region).  DM trials are independent, so N > 1 is N replicas on sharded trials
+(weak scaling, no data-path collective).  See DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import ctypes as C
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "f-fdot plane points/s (SKA-like DM trial: real FFT + whitening + 193-template convolve+power + 16-harmonic sum/peaks)"
+UNIT = "points/s"
+
+# Algorithmic work of K2 per (segment, template) and per plane point -- DESIGN.md "Kernels / K2".
+L_SEG = 2048
+FLOP_IFFT = 5 * L_SEG * 11          # 5 L log2 L
+FLOP_MUL = 6 * L_SEG
+HBM_BYTES_PER_POINT = {"fp32": 4.05, "bf16": 4.02, "bf16_plane16": 2.02}
+# ALU peak: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (B200_PROFILING.md unit counts/clocks)
+N_SM, LANES, SM_MAX_GHZ = 148, 128, 1.965
+ALU_PEAK_TFLOPS = N_SM * LANES * 2 * SM_MAX_GHZ / 1e3
+# dram__bytes_read.sum + dram__bytes_write.sum of one K2 launch from `ncu --set full`
+# (profiles/); None until captured for that (workload, precision).
+NCU_K2_TRAFFIC_BYTES = {}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured"
+        except Exception:
+            pass
+    return 6650.0, "fallback"
+
+
+def workload_for(name: str, inputs):
+    if name == "ska":
+        return inputs.ska()
+    if name == "ska_half":
+        return inputs.ska(half_res=True)
+    if name == "medium":
+        return inputs.medium()
+    if name == "tiny":
+        return inputs.tiny()
+    raise SystemExit(f"unknown workload {name}")
+
+
+def trial_series(wl_name, trial, inputs):
+    """Distinct seeded series per trial: configs[3] members for the SKA shapes."""
+    if wl_name in ("ska", "ska_half"):
+        w = inputs.batched_member(trial % 64, half_res=(wl_name == "ska_half"))
+        if trial == 0:
+            w = workload_for(wl_name, inputs)      # trial 0 is configs[2] itself (2 injected pulsars)
+        return inputs.series_for(w)
+    w = workload_for(wl_name, inputs)
+    return inputs.make_series(w.n, w.seed + 7919 * trial, w.signals, w.red_knee)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock, power and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.02):
+        super().__init__(daemon=True)
+        self.period, self.samples, self.reasons, self.power = period, [], set(), []
+        self.stop_flag = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:   # no NVML: clocks are reported as unavailable
+            self.err = repr(e)
+            self.sm_max = None
+
+    def energy_mj(self):
+        try:
+            return int(self.nv.nvmlDeviceGetTotalEnergyConsumption(self.h))
+        except Exception:
+            return None
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+            0x80: "hw_power_brake_slowdown",
+        }
+        while not self.stop_flag.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["nvml_unavailable"]}
+        return {"sm_mhz": int(statistics.median(self.samples)), "sm_max_mhz": self.sm_max,
+                "reasons": sorted(self.reasons), "power_w_mean": round(sum(self.power) / len(self.power), 1),
+                "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------- CPU oracle arm
+def oracle_sample(x, wl, budget_s=12.0):
+    """Times the oracle, as it stands, on a bounded sample of one trial: O1+O2 on the whole series
+    (prorated to the sample), O4 plane and O5/O6 harmonic sums + candidates over the first R bins
+    of all nz rows.  Returns (points_per_s, cores, description, seconds)."""
+    from oracle import fdas_oracle as orc
+    t0 = time.perf_counter()
+    X = orc.spectrum(x, wl.nfft)
+    w = orc.whiten(X)
+    t_spec = time.perf_counter() - t0
+    bank = orc.template_bank(wl.zmax, wl.zstep)          # plan-time work, not counted
+    nb = wl.nfft // 2
+    nz = bank.shape[0]
+    R = min(nb, 4096)
+    t0 = time.perf_counter()
+    orc.plane(w, bank, 0, R)
+    t_probe = time.perf_counter() - t0
+    R = int(min(nb, max(R, R * budget_s / max(t_probe, 1e-3))))
+    R = max(4096, (R // 4096) * 4096)
+    t0 = time.perf_counter()
+    P = orc.plane(w, bank, 0, R)
+    t_plane = time.perf_counter() - t0
+    thr = orc.thresholds(wl.nharm, wl.nsigma)
+    t0 = time.perf_counter()
+    orc.candidates(P, wl.nharm, thr, min(wl.r_lo, R - 1))
+    t_harm = time.perf_counter() - t0
+    total = t_spec * (R / nb) + t_plane + t_harm
+    desc = (f"oracle O1+O2 on the full {wl.nfft}-sample series (prorated by R/Nb), O4 plane and O5/O6 "
+            f"harmonic sums over the first R={R} of {nb} bins x {nz} templates")
+    return nz * R / total, orc.num_threads(), desc, total + t_spec * (1 - R / nb)
+
+
+def run_reference(args):
+    from paper_2211_13517_b200 import inputs
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    wl = workload_for(args.workload, inputs)
+    x = trial_series(args.workload, 0, inputs)
+    budget = max(2.0, min(15.0, 120.0 / max(1, args.steps + args.warmup)))
+    vals, secs = [], []
+    cores, desc = 0, ""
+    for i in range(args.warmup + args.steps):
+        v, cores, desc, s = oracle_sample(x, wl, budget)
+        if i >= args.warmup:
+            vals.append(v)
+            secs.append(s)
+    value = len(vals) / sum(1.0 / v for v in vals)
+    nb = wl.nfft // 2
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * wl.nz * nb / value, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{wl.name}: N={wl.n}, nfft={wl.nfft}, nz={wl.nz}, seg_len={wl.seg_len}, H={wl.nharm}",
+                   "note": "ms_per_step is the oracle's time for a whole trial extrapolated from the sample"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ----------------------------------------------------------------------------------- CUDA arm
+def run_cuda(args):
+    import torch
+    from paper_2211_13517_b200 import dist as fd, fdas, inputs
+
+    ctx = fd.init_from_env("nccl")
+    torch.cuda.set_device(ctx.local_rank)
+    dev = torch.device("cuda", ctx.local_rank)
+    wl = workload_for(args.workload, inputs)
+    precision = args.precision
+    plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, precision)
+    info = plan.info
+    points = int(info.nz) * int(info.nbins)
+
+    # seeded pool of distinct series for this rank's trials (trial t -> pool[t % pool])
+    pool_n = max(1, min(args.pool, args.steps))
+    my_trials = [ctx.rank + ctx.world * i for i in range(pool_n)]
+    host_pool = []
+    for t in my_trials:
+        ht = torch.empty(wl.n, dtype=torch.float32).pin_memory()
+        ht.numpy()[:] = trial_series(args.workload, t, inputs)
+        host_pool.append(ht)
+    dev_pool = [h.to(dev, non_blocking=False) for h in host_pool]
+    pool_bytes = pool_n * wl.n * 4
+
+    d_spec, d_plane = plan.alloc_spec(dev), plan.alloc_plane(dev)
+    cap = 1 << 16
+    d_c, d_n = plan.alloc_cands(cap, dev)
+    thr = fdas.thresholds_from_sigma(wl.nharm, wl.nsigma)
+    stream = torch.cuda.current_stream()
+
+    def step(i, evs=None):
+        x = dev_pool[i % pool_n]
+        if evs is not None:
+            evs[0].record(stream)
+        plan.prepare_spectrum(x, d_spec, stream)
+        if evs is not None:
+            evs[1].record(stream)
+        plan.convolve_plane(d_spec, d_plane, stream)
+        if evs is not None:
+            evs[2].record(stream)
+        plan.harmonic_sum_peaks(d_plane, wl.nharm, thr, wl.r_lo, d_c, d_n, stream)
+        if evs is not None:
+            evs[3].record(stream)
+
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+    n_cands = int(d_n.item())
+
+    sampler = ClockSampler(ctx.local_rank)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    launches0 = plan.launch_count()
+    fd.barrier(ctx)
+    torch.cuda.synchronize()
+    sampler.start()
+    e0 = sampler.energy_mj() if sampler.ok else None
+    for i in range(args.steps):
+        step(i, evs[i])
+    torch.cuda.synchronize()
+    e1 = sampler.energy_mj() if sampler.ok else None
+    sampler.stop_flag.set()
+    fd.barrier(ctx)
+    t_total_ms = evs[0][0].elapsed_time(evs[-1][3])
+    launches = plan.launch_count() - launches0
+    sampler.join(timeout=2.0)
+    t_prep = statistics.mean(e[0].elapsed_time(e[1]) for e in evs)
+    t_conv = statistics.mean(e[1].elapsed_time(e[2]) for e in evs)
+    t_harm = statistics.mean(e[2].elapsed_time(e[3]) for e in evs)
+
+    t_max_ms = fd.max_over_ranks(ctx, t_total_ms)
+    total_points = fd.sum_over_ranks(ctx, float(points * args.steps))
+    value = total_points / (t_max_ms * 1e-3)
+
+    # ---- end to end through fdas_search_host: pinned host series in, candidates out, every step
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    out = np.empty(cap, dtype=fdas.CAND_DTYPE)
+    thr_c = thr.ctypes.data_as(C.POINTER(C.c_float))
+    sp = int(stream.cuda_stream)
+    cnt = 0
+    for i in range(min(3, args.warmup)):
+        plan.search_host_raw(host_pool[i % pool_n].data_ptr(), wl.nharm, thr_c, wl.r_lo, out.ctypes.data, cap, sp)
+    fd.barrier(ctx)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    d2h = 0
+    for i in range(e2e_steps):
+        st, cnt = plan.search_host_raw(host_pool[i % pool_n].data_ptr(), wl.nharm, thr_c, wl.r_lo,
+                                       out.ctypes.data, cap, sp)
+        assert st in (fdas.FDAS_OK, fdas.FDAS_EOVERFLOW), st
+        d2h += 8 + 16 * min(cnt, cap)
+    torch.cuda.synchronize()
+    t_e2e = fd.max_over_ranks(ctx, time.perf_counter() - t0)
+    e2e_value = fd.sum_over_ranks(ctx, float(points * e2e_steps)) / t_e2e
+
+    hbm_peak, peak_kind = measured_peaks()
+    seg_flops = FLOP_IFFT + FLOP_MUL + 3 * int(info.valid)
+    k2_flops = int(info.nseg) * (int(info.nz) * seg_flops + FLOP_IFFT)
+    k2_tflops = k2_flops / (t_conv * 1e-3) / 1e12
+    k2_gbs = HBM_BYTES_PER_POINT[precision] * points / (t_conv * 1e-3) / 1e9
+    plane_bytes = points * int(info.plane_elem_bytes)
+    k3_gbs = plane_bytes / (t_harm * 1e-3) / 1e9
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ctx.world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t_max_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {
+            "workload": f"{wl.name}: N={wl.n} samples at {wl.tsamp * 1e6:.0f} us, nfft={info.nfft}, nz={info.nz} "
+                        f"(zmax={wl.zmax:g}), seg_len={info.seg_len}, h={info.halfwidth}, S={info.nseg}, H={wl.nharm}, "
+                        f"{wl.nsigma:g} sigma, storage={precision} (fp32 arithmetic)",
+            "precision": precision, "plane_points_per_step": points,
+            "parallelism": f"dm-trial replicas x{ctx.world} (no data-path collective)",
+            "l2": f"plane of {plane_bytes / 1e9:.2f} GB per step exceeds the 126 MB L2; input pool of "
+                  f"{pool_n} series ({pool_bytes / 1e6:.0f} MB) cycled",
+            "timed": "cuFFT R2C + K1a/K1b whitening + K2 convolve + K3 harmonic sum per step; CUDA events on the launching stream",
+        },
+        "kernel_ms": {"prepare_spectrum": t_prep, "convolve_plane": t_conv, "harmonic_sum_peaks": t_harm},
+        "candidates_last_step": n_cands,
+        "gpu_launches": int(fd.sum_over_ranks(ctx, int(launches))),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": wl.n * 4,
+                "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps,
+                "api": "fdas_search_host (pinned host series -> candidates on host), wall clock"},
+        "roofline": {
+            "kernel": "K2 convolve_kernel", "bound": "alu", "achieved": k2_tflops, "peak": ALU_PEAK_TFLOPS,
+            "unit": "TFLOP/s", "frac": k2_tflops / ALU_PEAK_TFLOPS,
+            "traffic": NCU_K2_TRAFFIC_BYTES.get((args.workload, precision)),
+            "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz",
+            "flops_per_launch": k2_flops,
+        },
+        "roofline_hbm": {
+            "kernel": "K2 convolve_kernel", "bound": "hbm", "achieved": k2_gbs, "peak": hbm_peak, "unit": "GB/s",
+            "frac": k2_gbs / hbm_peak, "peak_kind": f"{peak_kind} copy bandwidth",
+            "bytes_per_point": HBM_BYTES_PER_POINT[precision], "frac_of_8TBs_nominal": k2_gbs / 8000.0,
+        },
+        "roofline_k3": {
+            "kernel": "K3 harmonic_kernel", "bound": "hbm", "achieved": k3_gbs, "peak": hbm_peak, "unit": "GB/s",
+            "frac": k3_gbs / hbm_peak, "note": "algorithmic bytes = one read of the plane; the stride-k gathers "
+                                               "touch ~3.2x that in 32-byte sectors (DESIGN.md)",
+        },
+        "clocks": sampler.summary(),
+    }
+    if e0 is not None and e1 is not None and e1 > e0:
+        line["energy"] = {"joules_per_step": (e1 - e0) / 1e3 / args.steps, "source": "NVML total energy counter"}
+    if ctx.rank == 0 and ctx.world == 1 and not args.no_cpu_baseline:
+        v, cores, desc, _ = oracle_sample(host_pool[0].numpy(), wl, args.cpu_budget)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    if ctx.rank == 0:
+        print(json.dumps(line), flush=True)
+    fd.finalize(ctx)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="ska", choices=["ska", "ska_half", "medium", "tiny"])
+    ap.add_argument("--precision", default="bf16", choices=["fp32", "bf16", "bf16_plane16"])
+    ap.add_argument("--pool", type=int, default=4, help="distinct series cycled per rank")
+    ap.add_argument("--e2e-steps", type=int, default=20)
+    ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle plane work")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,166 @@
+/*
+ * fdas.h -- C ABI of libfdas.so: the data-parallel hot path of the Fourier Domain Acceleration
+ * Search (FDAS), hand-written for NVIDIA B200 (sm_100a).
+ *
+ * Method: arxiv 2211.13517 (White, Adamek, Armour), /root/reference/PAPER.md.  The paper states
+ * the method in words only -- "a matched filtering approach" whose cost "scales linearly with the
+ * number of acceleration values" (section 2.1) that "relies on the Fast Fourier
+ * Transform (FFT) to perform convolutions in the frequency domain", with "the most
+ * computationally demanding section (the convolution stage)" optionally in bfloat16 (PAPER.md:23,
+ * section 2.2), run on an SKA-like workload of "193 acceleration trials" per DM trial
+ * (section 3).  The concrete definitions (FFT length, whitening, template response,
+ * overlap-save bookkeeping, harmonic sums, thresholds) are the readings A1..A19 of DESIGN.md,
+ * which the CPU oracle (oracle/fdas_oracle.c) implements independently.
+ *
+ * Conventions for every call
+ *   - returns an int status (FDAS_OK = 0); nothing throws or aborts across this boundary;
+ *   - pointers named d_* are DEVICE pointers owned by the caller (allocate them with the sizes
+ *     fdas_plan_info reports); pointers named h_* are HOST pointers; the plan owns its templates,
+ *     twiddle tables, cuFFT plan + workspace and whitening scratch;
+ *   - the three per-trial calls only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
+ *     void*, NULL = legacy default stream) and return; they never synchronise, allocate or free;
+ *   - a plan may be used from one stream at a time (its scratch is not duplicated).
+ */
+#ifndef FDAS_H
+#define FDAS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fdas_plan_s* fdas_plan_t; /* opaque, library-owned */
+
+/* Storage precision of the convolution stage (reading A10).  Arithmetic is
+ * always fp32.  FP32: spectrum, templates and plane in fp32.  BF16: whitened spectrum and templates
+ * stored as bfloat16 (round-to-nearest-even), plane fp32.  BF16_PLANE16: plane stored bf16 too. */
+enum { FDAS_FP32 = 0, FDAS_BF16 = 1, FDAS_BF16_PLANE16 = 2 };
+
+enum {
+    FDAS_OK = 0,
+    FDAS_EARG = 1,         /* invalid argument (see each call) */
+    FDAS_EALLOC = 2,       /* host or device allocation failed */
+    FDAS_ECUDA = 3,        /* a CUDA runtime call or kernel launch failed */
+    FDAS_ECUFFT = 4,       /* a cuFFT call failed */
+    FDAS_EOVERFLOW = 5,    /* more candidates than capacity (host-side helper only) */
+    FDAS_EUNSUPPORTED = 6  /* valid request this build does not implement (e.g. seg_len != 2048) */
+};
+
+typedef struct {
+    int64_t n_in;        /* samples in the caller's series (N given to fdas_plan)            */
+    int64_t nfft;        /* FFT length: largest power of two <= n_in (reading A1)            */
+    int64_t nbins;       /* Nb = nfft/2 Fourier bins kept, k = 0..Nb-1 (reading A2)          */
+    int32_t nz;          /* number of templates, z_j = -zmax + j*zstep (reading A6)          */
+    int32_t seg_len;     /* L, overlap-save segment length in complex bins                   */
+    int32_t halfwidth;   /* h: templates have 2h+1 taps (reading A5)                         */
+    int32_t valid;       /* V = L - 2h valid outputs per segment                             */
+    int64_t nseg;        /* S = ceil(Nb / V)                                                 */
+    int64_t plane_pitch; /* elements between consecutive rows of the plane (= Nb)            */
+    int32_t spec_elem_bytes;  /* bytes per COMPLEX spectrum element: 8 (fp32) or 4 (bf16)    */
+    int32_t plane_elem_bytes; /* bytes per plane element: 4 or 2                             */
+    int32_t precision;
+    int32_t reserved;
+    double zmax, zstep, tsamp, tobs; /* tobs = nfft * tsamp; f = r/tobs, fdot = z/tobs^2     */
+} fdas_info_t;
+
+/* One candidate (16 bytes).  zidx is the row j (z = -zmax + zidx*zstep); power is S_h(r, z);
+ * flags bit 0 = local maximum of S_h over the 8 neighbours (r+-1, j+-1) (reading A14). */
+typedef struct {
+    uint32_t r;
+    int16_t zidx;
+    uint16_t h;
+    float power;
+    uint32_t flags;
+} fdas_cand_t;
+
+/*
+ * fdas_plan -- build everything that does not depend on the data (readings A1, A5,
+ * A6): derives nfft, Nb, nz, h, V, S; generates the template bank on the host in double precision
+ * (closed-form Fresnel response of a constant-fdot signal, Ransom et al. 2002 cited at PAPER.md:75,
+ * truncated to 2h+1 taps, unit L2 norm, shifted by h, FFT_L, conjugated, scaled by 1/L), casts it
+ * once to fp32 or bf16 and uploads it in the kernel's register order; creates the cuFFT R2C plan
+ * and the whitening block table.
+ *   N        samples per time series (>= 2*seg_len); tsamp  sampling time in seconds (> 0; units only)
+ *   zmax     largest |z| searched, in Fourier bins of drift over the observation (>= 0)
+ *   zstep    template spacing in z (> 0); 2*zmax/zstep must be an integer (nz = that + 1 <= 32767)
+ *   seg_len  L; this build supports 2048 only (FDAS_EUNSUPPORTED otherwise; FDAS_EARG if not a
+ *            power of two or if V = L - 2h <= 0)
+ *   precision  FDAS_FP32 | FDAS_BF16 | FDAS_BF16_PLANE16
+ * On success *out receives the handle (release with fdas_destroy).
+ */
+int fdas_plan(fdas_plan_t* out, int64_t N, double tsamp, double zmax, double zstep, int seg_len,
+              int precision);
+
+/* Sizes and derived constants of a plan.  FDAS_EARG on NULL. */
+int fdas_plan_info(fdas_plan_t plan, fdas_info_t* out);
+
+/*
+ * fdas_prepare_spectrum -- real FFT + running-median power whitening (BASELINE.json north_star;
+ * readings A1, A2, A3).  X = cuFFT R2C of the first nfft samples (the one library call on the
+ * path); block medians of |X|^2 over the A3 block schedule; w[k] = X[k]*sqrt(ln2/m(k)), w[0] = 0,
+ * stored as complex fp32 (FDAS_FP32) or complex bf16 (RNE).
+ *   d_series  device, n_in float32 samples (only the first nfft are read)
+ *   d_spec    device, nbins complex elements of spec_elem_bytes each (output)
+ */
+int fdas_prepare_spectrum(fdas_plan_t plan, const float* d_series, void* d_spec, void* cuda_stream);
+
+/*
+ * fdas_convolve_plane -- the convolution stage (readings A7, A8, A9): for every
+ * overlap-save segment s and template j, P[j][sV+t] = |IFFT_L(FFT_L(g_s) . K_j)[t]|^2, t < V,
+ * g_s[i] = w[sV-h+i] (zero outside [0,Nb)), which equals |sum_m w[r+m] conj(T_j[m])|^2.
+ *   d_spec   device, as written by fdas_prepare_spectrum
+ *   d_plane  device, nz rows of plane_pitch elements of plane_elem_bytes (output, every element
+ *            with r < nbins is written; 16-byte aligned)
+ */
+int fdas_convolve_plane(fdas_plan_t plan, const void* d_spec, void* d_plane, void* cuda_stream);
+
+/*
+ * fdas_harmonic_sum_peaks -- harmonic summing, thresholding, candidate compaction (BASELINE.json
+ * north_star; readings A12, A13, A14): S_h(r,j) = sum_{k=1..h} P[row(k z_j)][k r] while k r <= Nb-1
+ * and |k z_j| <= zmax; emits (r, j, h, S_h, flags) for every S_h > h_thresholds[h-1] (strict),
+ * r in [r_lo, Nb).
+ *   H             1..32;  h_thresholds  host, H floats (copied at call time)
+ *   d_cands       device, capacity records, filled in unspecified order
+ *   d_count       device; set to 0 by this call, then receives the TRUE number of candidates found
+ *                 (it may exceed capacity; only the first `capacity` claimed slots are stored)
+ * FDAS_EARG: NULL pointers, H out of range, r_lo < 0, capacity < 0.
+ */
+int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const float* h_thresholds,
+                            int64_t r_lo, fdas_cand_t* d_cands, int64_t capacity,
+                            unsigned long long* d_count, void* cuda_stream);
+
+/*
+ * fdas_search_host -- the same three steps for a HOST time series (the end-to-end entry point):
+ * copies h_series (n_in floats) to the device, runs prepare -> convolve -> harmonic_sum_peaks on
+ * `cuda_stream`, copies the count and the first min(count, capacity) candidates back and waits for
+ * them.  Device workspace (series, spectrum, plane, candidates) is allocated on first use and owned
+ * by the plan.  Returns FDAS_EOVERFLOW (after copying `capacity` records) if count > capacity.
+ */
+int fdas_search_host(fdas_plan_t plan, const float* h_series, int H, const float* h_thresholds,
+                     int64_t r_lo, fdas_cand_t* h_cands, int64_t capacity, int64_t* h_count,
+                     void* cuda_stream);
+
+/*
+ * fdas_thresholds_from_sigma -- host helper (reading A13): h_thresholds_out[h-1] = T_h with
+ * Q(h, T_h) = erfc(nsigma/sqrt2)/2, Q the survival function of a sum of h unit exponentials.
+ */
+int fdas_thresholds_from_sigma(int H, double nsigma, float* h_thresholds_out);
+
+/*
+ * fdas_plan_templates_host -- diagnostic: copies the plan's time-domain template bank
+ * (nz x (2h+1) complex doubles, interleaved re/im, unit L2 norm) to h_out.  Host only.
+ */
+int fdas_plan_templates_host(fdas_plan_t plan, double* h_out);
+
+/* Number of kernels the library launched on behalf of this plan since it was created. */
+int64_t fdas_plan_launch_count(fdas_plan_t plan);
+
+int fdas_destroy(fdas_plan_t plan);
+const char* fdas_strerror(int status);
+const char* fdas_last_error_detail(void); /* thread-local text of the last CUDA/cuFFT failure */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FDAS_H */

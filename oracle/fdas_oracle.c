@@ -388,6 +388,31 @@ int orc_harmonic_sums_at(const double* P, int64_t nb, int nz, int H, int64_t r, 
     return hmax;
 }
 
+/* O5 at sampled fundamentals straight from the whitened spectrum (for sizes where the full plane
+ * is too large): S[i*H + (k-1)] = S_k(rr[i], jj[i]) for k <= hmax[i], every needed plane point
+ * computed one by one by the O4 definition. */
+int orc_harmonic_sums_sampled(const double* w_, int64_t nb, const double* bank_, int nz, int h, int H,
+                              const int64_t* rr, const int32_t* jj, int64_t npts, double* S,
+                              int32_t* hmax) {
+    const cplx* w = (const cplx*)w_;
+    const cplx* bank = (const cplx*)bank_;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int64_t i = 0; i < npts; ++i) {
+        double acc = 0.0;
+        int hm = 0;
+        for (int k = 1; k <= H; ++k) {
+            int row;
+            if ((int64_t)k * rr[i] > nb - 1) break;
+            if (!harmonic_row(jj[i], k, nz, &row)) break;
+            acc += plane_point(w, nb, bank + (size_t)row * (2 * h + 1), h, (int64_t)k * rr[i]);
+            S[i * H + (k - 1)] = acc;
+            hm = k;
+        }
+        hmax[i] = hm;
+    }
+    return 0;
+}
+
 static int sum_defined(const double* P, int64_t nb, int nz, int64_t r_lo, int64_t r, int j, int h,
                        double* val) {
     if (j < 0 || j >= nz || r < r_lo || r >= nb) return 0;

@@ -56,6 +56,8 @@ def lib():
         L.orc_plane_points.argtypes = [_d, C.c_int64, _d, C.c_int, C.c_int, _i64, _i32, C.c_int64, _d]
         L.orc_plane_ols_dft.argtypes = [_d, C.c_int64, _d, C.c_int, C.c_int, C.c_int, _d]
         L.orc_harmonic_sums_at.argtypes = [_d, C.c_int64, C.c_int, C.c_int, C.c_int64, C.c_int, _d]
+        L.orc_harmonic_sums_sampled.argtypes = [_d, C.c_int64, _d, C.c_int, C.c_int, C.c_int, _i64, _i32,
+                                                C.c_int64, _d, _i32]
         L.orc_candidates.argtypes = [_d, C.c_int64, C.c_int, C.c_int, _d, C.c_int64,
                                      _i64, _i32, _i32, _d, _i32, C.c_int64]
         L.orc_candidates.restype = C.c_int64
@@ -182,6 +184,21 @@ def harmonic_sums_at(P, H, r, j):
     S = np.zeros(H)
     hmax = lib().orc_harmonic_sums_at(_p(P, _d), nb, nz, H, int(r), int(j), _p(S, _d))
     return S[:hmax]
+
+
+def harmonic_sums_sampled(w, bank, H, rr, jj):
+    """S (npts x H, NaN where undefined) and hmax (npts) at sampled fundamentals, from w directly."""
+    w, wv = _c128(w)
+    bank, bv = _c128(bank)
+    nz, taps = bank.shape
+    h = (taps - 1) // 2
+    rr = np.ascontiguousarray(rr, dtype=np.int64)
+    jj = np.ascontiguousarray(jj, dtype=np.int32)
+    S = np.full((rr.size, H), np.nan)
+    hmax = np.zeros(rr.size, dtype=np.int32)
+    lib().orc_harmonic_sums_sampled(_p(wv, _d), w.size, _p(bv, _d), nz, h, H, _p(rr, _i64),
+                                    _p(jj, _i32), rr.size, _p(S, _d), _p(hmax, _i32))
+    return S, hmax
 
 
 def thresholds(H, nsigma):

@@ -1,0 +1,314 @@
+// fdas_api.cu -- the C ABI of libfdas.so (include/fdas.h): plan construction, the three per-trial
+// calls, the host end-to-end entry point.  No exceptions cross the boundary.
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/fdas.h"
+#include "fdas_fft_core.cuh"
+#include "fdas_host.h"
+#include "fdas_kernels.h"
+
+using namespace fdas;
+
+static thread_local std::string g_detail;
+
+struct fdas_plan_s {
+    fdas_info_t info;
+    std::vector<cd> bank_time;  // nz x (2h+1), kept for diagnostics
+    void* d_bank = nullptr;
+    float2* d_tw1 = nullptr;
+    float2* d_tw2 = nullptr;
+    cufftHandle fft = 0;
+    bool fft_made = false;
+    void* d_fft_work = nullptr;
+    float2* d_X = nullptr;  // nfft/2 + 1
+    int32_t* d_blk_start = nullptr;
+    int32_t* d_blk_len = nullptr;
+    float* d_blk_med = nullptr;
+    int nblk = 0;
+    int nsplit = 1;
+    int64_t launches = 0;
+    // workspace of fdas_search_host (lazy)
+    float* ws_series = nullptr;
+    void* ws_spec = nullptr;
+    void* ws_plane = nullptr;
+    fdas_cand_t* ws_cands = nullptr;
+    int64_t ws_cap = 0;
+    unsigned long long* ws_count = nullptr;
+    unsigned long long* h_count = nullptr;  // pinned
+};
+
+#define CU(call)                                                                        \
+    do {                                                                                \
+        cudaError_t e_ = (call);                                                        \
+        if (e_ != cudaSuccess) {                                                        \
+            g_detail = std::string(#call) + ": " + cudaGetErrorString(e_);              \
+            return (e_ == cudaErrorMemoryAllocation) ? FDAS_EALLOC : FDAS_ECUDA;        \
+        }                                                                               \
+    } while (0)
+
+#define CF(call)                                                                        \
+    do {                                                                                \
+        cufftResult r_ = (call);                                                        \
+        if (r_ != CUFFT_SUCCESS) {                                                      \
+            g_detail = std::string(#call) + ": cufft status " + std::to_string((int)r_); \
+            return (r_ == CUFFT_ALLOC_FAILED) ? FDAS_EALLOC : FDAS_ECUFFT;              \
+        }                                                                               \
+    } while (0)
+
+static void free_plan(fdas_plan_s* p) {
+    if (!p) return;
+    cudaFree(p->d_bank); cudaFree(p->d_tw1); cudaFree(p->d_tw2); cudaFree(p->d_fft_work);
+    cudaFree(p->d_X); cudaFree(p->d_blk_start); cudaFree(p->d_blk_len); cudaFree(p->d_blk_med);
+    cudaFree(p->ws_series); cudaFree(p->ws_spec); cudaFree(p->ws_plane); cudaFree(p->ws_cands);
+    cudaFree(p->ws_count);
+    if (p->h_count) cudaFreeHost(p->h_count);
+    if (p->fft_made) cufftDestroy(p->fft);
+    delete p;
+}
+
+static int derive_info(int64_t N, double tsamp, double zmax, double zstep, int seg_len, int precision,
+                       fdas_info_t* o) {
+    if (N < 2 || !(tsamp > 0.0) || !(zmax >= 0.0) || !(zstep > 0.0) || seg_len < 2) return FDAS_EARG;
+    if (precision != FDAS_FP32 && precision != FDAS_BF16 && precision != FDAS_BF16_PLANE16) return FDAS_EARG;
+    if ((seg_len & (seg_len - 1)) != 0) return FDAS_EARG;
+    if (N < 2 * (int64_t)seg_len) return FDAS_EARG;
+    const double cnt = 2.0 * zmax / zstep;
+    const double rc = std::floor(cnt + 0.5);
+    if (std::fabs(cnt - rc) > 1e-9 * (1.0 + cnt) || rc + 1 > 32767.0) return FDAS_EARG;
+    std::memset(o, 0, sizeof(*o));
+    o->n_in = N;
+    int64_t nfft = 1;
+    while (nfft * 2 <= N) nfft *= 2;
+    if (nfft > ((int64_t)1 << 31)) return FDAS_EARG;  // candidate r is 32-bit
+    o->nfft = nfft;
+    o->nbins = nfft / 2;
+    o->nz = (int)rc + 1;
+    o->seg_len = seg_len;
+    o->halfwidth = template_halfwidth(zmax);
+    o->valid = seg_len - 2 * o->halfwidth;
+    if (o->valid <= 0) return FDAS_EARG;
+    o->nseg = (o->nbins + o->valid - 1) / o->valid;
+    o->plane_pitch = o->nbins;
+    o->spec_elem_bytes = (precision == FDAS_FP32) ? 8 : 4;
+    o->plane_elem_bytes = (precision == FDAS_BF16_PLANE16) ? 2 : 4;
+    o->precision = precision;
+    o->zmax = zmax; o->zstep = zstep; o->tsamp = tsamp; o->tobs = (double)nfft * tsamp;
+    if (seg_len != kL) return FDAS_EUNSUPPORTED;
+    return FDAS_OK;
+}
+
+static int build_plan(fdas_plan_s* p) {
+    const fdas_info_t& in = p->info;
+    Bank bank;
+    build_bank(in.zmax, in.zstep, in.nz, in.halfwidth, in.seg_len, &bank);
+    p->bank_time = bank.time;
+    if (in.precision == FDAS_FP32) {
+        std::vector<float> packed;
+        pack_bank_fp32(bank, &packed);
+        CU(cudaMalloc(&p->d_bank, packed.size() * sizeof(float)));
+        CU(cudaMemcpy(p->d_bank, packed.data(), packed.size() * sizeof(float), cudaMemcpyHostToDevice));
+    } else {
+        std::vector<uint32_t> packed;
+        pack_bank_bf16(bank, &packed);
+        CU(cudaMalloc(&p->d_bank, packed.size() * sizeof(uint32_t)));
+        CU(cudaMemcpy(p->d_bank, packed.data(), packed.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    }
+    std::vector<float> t1, t2;
+    build_twiddles(&t1, &t2);
+    CU(cudaMalloc(&p->d_tw1, t1.size() * sizeof(float)));
+    CU(cudaMalloc(&p->d_tw2, t2.size() * sizeof(float)));
+    CU(cudaMemcpy(p->d_tw1, t1.data(), t1.size() * sizeof(float), cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(p->d_tw2, t2.data(), t2.size() * sizeof(float), cudaMemcpyHostToDevice));
+
+    std::vector<int32_t> bs, bl;
+    whitening_blocks(in.nbins, &bs, &bl);
+    p->nblk = (int)bs.size();
+    CU(cudaMalloc(&p->d_blk_start, bs.size() * sizeof(int32_t)));
+    CU(cudaMalloc(&p->d_blk_len, bl.size() * sizeof(int32_t)));
+    CU(cudaMalloc(&p->d_blk_med, bs.size() * sizeof(float)));
+    CU(cudaMemcpy(p->d_blk_start, bs.data(), bs.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(p->d_blk_len, bl.data(), bl.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+
+    CU(cudaMalloc(&p->d_X, (size_t)(in.nfft / 2 + 1) * sizeof(float2)));
+    size_t ws = 0;
+    CF(cufftCreate(&p->fft));
+    p->fft_made = true;
+    CF(cufftSetAutoAllocation(p->fft, 0));
+    CF(cufftMakePlan1d(p->fft, (int)in.nfft, CUFFT_R2C, 1, &ws));
+    if (ws > 0) CU(cudaMalloc(&p->d_fft_work, ws));
+    CF(cufftSetWorkArea(p->fft, p->d_fft_work));
+
+    int dev = 0, nsm = 148;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    const int64_t slots = 3LL * nsm;  // K2 runs 3 CTAs per SM
+    int nsplit = 1;
+    if (in.nseg < 4 * slots) nsplit = (int)std::min<int64_t>(in.nz, (4 * slots + in.nseg - 1) / in.nseg);
+    if (const char* e = std::getenv("FDAS_NSPLIT")) {
+        const int v = std::atoi(e);
+        if (v >= 1) nsplit = std::min(v, (int)in.nz);
+    }
+    p->nsplit = nsplit;
+    return FDAS_OK;
+}
+
+extern "C" {
+
+int fdas_plan(fdas_plan_t* out, int64_t N, double tsamp, double zmax, double zstep, int seg_len,
+              int precision) {
+    if (!out) return FDAS_EARG;
+    *out = nullptr;
+    fdas_info_t info;
+    const int rc = derive_info(N, tsamp, zmax, zstep, seg_len, precision, &info);
+    if (rc != FDAS_OK) return rc;
+    fdas_plan_s* p = new (std::nothrow) fdas_plan_s();
+    if (!p) return FDAS_EALLOC;
+    p->info = info;
+    int st;
+    try {
+        st = build_plan(p);
+    } catch (const std::bad_alloc&) {
+        st = FDAS_EALLOC;
+    } catch (...) {
+        st = FDAS_ECUDA;
+    }
+    if (st != FDAS_OK) {
+        free_plan(p);
+        return st;
+    }
+    *out = p;
+    return FDAS_OK;
+}
+
+int fdas_plan_info(fdas_plan_t plan, fdas_info_t* out) {
+    if (!plan || !out) return FDAS_EARG;
+    *out = plan->info;
+    return FDAS_OK;
+}
+
+int fdas_prepare_spectrum(fdas_plan_t plan, const float* d_series, void* d_spec, void* cuda_stream) {
+    if (!plan || !d_series || !d_spec) return FDAS_EARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CF(cufftSetStream(plan->fft, st));
+    CF(cufftExecR2C(plan->fft, const_cast<float*>(d_series), reinterpret_cast<cufftComplex*>(plan->d_X)));
+    WhitenParams w;
+    w.X = plan->d_X; w.spec = d_spec;
+    w.blk_start = plan->d_blk_start; w.blk_len = plan->d_blk_len; w.blk_med = plan->d_blk_med;
+    w.nblk = plan->nblk; w.nbins = plan->info.nbins;
+    CU(launch_whiten(plan->info.precision, w, st));
+    plan->launches += 2;
+    return FDAS_OK;
+}
+
+int fdas_convolve_plane(fdas_plan_t plan, const void* d_spec, void* d_plane, void* cuda_stream) {
+    if (!plan || !d_spec || !d_plane) return FDAS_EARG;
+    if ((reinterpret_cast<uintptr_t>(d_plane) & 15u) != 0) return FDAS_EARG;
+    ConvParams c;
+    c.spec = d_spec; c.plane = d_plane; c.bank = plan->d_bank; c.tw1 = plan->d_tw1; c.tw2 = plan->d_tw2;
+    c.nbins = plan->info.nbins; c.pitch = plan->info.plane_pitch;
+    c.nz = plan->info.nz; c.h = plan->info.halfwidth; c.V = plan->info.valid;
+    CU(launch_convolve(plan->info.precision, c, plan->info.nseg, plan->nsplit, (cudaStream_t)cuda_stream));
+    plan->launches += 1;
+    return FDAS_OK;
+}
+
+int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const float* h_thresholds,
+                            int64_t r_lo, fdas_cand_t* d_cands, int64_t capacity,
+                            unsigned long long* d_count, void* cuda_stream) {
+    if (!plan || !d_plane || !h_thresholds || !d_count) return FDAS_EARG;
+    if (H < 1 || H > 32 || r_lo < 0 || capacity < 0 || (capacity > 0 && !d_cands)) return FDAS_EARG;
+    HarmParams hp;
+    hp.plane = d_plane; hp.nbins = plan->info.nbins; hp.pitch = plan->info.plane_pitch;
+    hp.nz = plan->info.nz; hp.H = H; hp.r_lo = r_lo;
+    for (int i = 0; i < 32; ++i) hp.thr[i] = (i < H) ? h_thresholds[i] : INFINITY;
+    hp.cands = d_cands; hp.capacity = capacity; hp.count = d_count;
+    CU(launch_harmonic(plan->info.precision == FDAS_BF16_PLANE16, hp, (cudaStream_t)cuda_stream));
+    plan->launches += 1;
+    return FDAS_OK;
+}
+
+int fdas_search_host(fdas_plan_t plan, const float* h_series, int H, const float* h_thresholds,
+                     int64_t r_lo, fdas_cand_t* h_cands, int64_t capacity, int64_t* h_count,
+                     void* cuda_stream) {
+    if (!plan || !h_series || !h_thresholds || !h_count || capacity < 0 || (capacity > 0 && !h_cands))
+        return FDAS_EARG;
+    const fdas_info_t& in = plan->info;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!plan->ws_series) {
+        CU(cudaMalloc(&plan->ws_series, (size_t)in.n_in * sizeof(float)));
+        CU(cudaMalloc(&plan->ws_spec, (size_t)in.nbins * in.spec_elem_bytes));
+        CU(cudaMalloc(&plan->ws_plane, (size_t)in.nz * in.plane_pitch * in.plane_elem_bytes));
+        CU(cudaMalloc(&plan->ws_count, sizeof(unsigned long long)));
+        CU(cudaMallocHost(&plan->h_count, sizeof(unsigned long long)));
+    }
+    if (plan->ws_cap < capacity) {
+        cudaFree(plan->ws_cands);
+        plan->ws_cands = nullptr;
+        plan->ws_cap = 0;
+        CU(cudaMalloc(&plan->ws_cands, (size_t)capacity * sizeof(fdas_cand_t)));
+        plan->ws_cap = capacity;
+    }
+    CU(cudaMemcpyAsync(plan->ws_series, h_series, (size_t)in.n_in * sizeof(float), cudaMemcpyHostToDevice, st));
+    int rc = fdas_prepare_spectrum(plan, plan->ws_series, plan->ws_spec, cuda_stream);
+    if (rc != FDAS_OK) return rc;
+    rc = fdas_convolve_plane(plan, plan->ws_spec, plan->ws_plane, cuda_stream);
+    if (rc != FDAS_OK) return rc;
+    rc = fdas_harmonic_sum_peaks(plan, plan->ws_plane, H, h_thresholds, r_lo, plan->ws_cands, capacity,
+                                 plan->ws_count, cuda_stream);
+    if (rc != FDAS_OK) return rc;
+    CU(cudaMemcpyAsync(plan->h_count, plan->ws_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    const int64_t found = (int64_t)*plan->h_count;
+    *h_count = found;
+    const int64_t ncopy = found < capacity ? found : capacity;
+    if (ncopy > 0) {
+        CU(cudaMemcpyAsync(h_cands, plan->ws_cands, (size_t)ncopy * sizeof(fdas_cand_t), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
+    return found > capacity ? FDAS_EOVERFLOW : FDAS_OK;
+}
+
+int fdas_thresholds_from_sigma(int H, double nsigma, float* h_thresholds_out) {
+    if (H < 1 || H > 32 || !h_thresholds_out || !(nsigma > 0.0)) return FDAS_EARG;
+    return thresholds_from_sigma(H, nsigma, h_thresholds_out) == 0 ? FDAS_OK : FDAS_EARG;
+}
+
+int fdas_plan_templates_host(fdas_plan_t plan, double* h_out) {
+    if (!plan || !h_out) return FDAS_EARG;
+    std::memcpy(h_out, plan->bank_time.data(), plan->bank_time.size() * sizeof(cd));
+    return FDAS_OK;
+}
+
+int64_t fdas_plan_launch_count(fdas_plan_t plan) { return plan ? plan->launches : -1; }
+
+int fdas_destroy(fdas_plan_t plan) {
+    if (!plan) return FDAS_EARG;
+    free_plan(plan);
+    return FDAS_OK;
+}
+
+const char* fdas_strerror(int status) {
+    switch (status) {
+        case FDAS_OK: return "ok";
+        case FDAS_EARG: return "invalid argument";
+        case FDAS_EALLOC: return "allocation failed";
+        case FDAS_ECUDA: return "CUDA error";
+        case FDAS_ECUFFT: return "cuFFT error";
+        case FDAS_EOVERFLOW: return "more candidates than capacity";
+        case FDAS_EUNSUPPORTED: return "unsupported configuration (this build: seg_len = 2048 only)";
+        default: return "unknown status";
+    }
+}
+
+const char* fdas_last_error_detail(void) { return g_detail.c_str(); }
+
+}  // extern "C"

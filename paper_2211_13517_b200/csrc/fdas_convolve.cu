@@ -1,0 +1,167 @@
+// fdas_convolve.cu -- K2, the fused convolution stage ("the most computationally
+// demanding section (the convolution stage)"; DESIGN.md step a4 + a5).
+//
+// One CTA (128 threads, 16 points per thread) owns one overlap-save segment s and a contiguous
+// chunk of templates:
+//   stage-in   g_s[i] = w[sV - h + i] (zero outside [0,Nb)), read once, coalesced
+//   forward    S = FFT_2048(g_s) in registers/shared memory, kept in 32 registers per thread
+//   loop j     x = S . Khat_j (Khat_j streamed from L2 with 128-bit loads, prefetched one template
+//              ahead), y = IFFT_2048(x) (three register passes, two shared-memory exchanges),
+//              P[j][sV + t] = |y[t]|^2 for the V valid samples only, written once, streaming stores
+// so the spectrum is read once and the plane written once.  fp32 arithmetic throughout; the bf16
+// variants only change the storage format of w, Khat (and optionally P) -- reading A10.
+#include <cuda_bf16.h>
+
+#include "fdas_fft_core.cuh"
+#include "fdas_kernels.h"
+
+namespace fdas {
+
+__device__ __forceinline__ void ifft2048(float2 (&x)[16], float2* X1, float2* X2, const int tid,
+                                         const float2 (&tw1)[15], const float2 (&tw2)[7]) {
+    pass1(x, tw1);
+    x1_store(X1, tid, x);
+    __syncthreads();
+    xrow_load(X1, tid, x);
+    pass2(x);
+    x2_store(X2, tid, x);
+    __syncthreads();
+    xrow_load(X2, tid, x);
+    pass3(x, tw2);
+}
+
+template <int PREC>
+__global__ void __launch_bounds__(kThreads, 3) convolve_kernel(const ConvParams p) {
+    __shared__ __align__(16) float2 X1[kXbufElems];
+    __shared__ __align__(16) float2 X2[kXbufElems];
+    const int tid = threadIdx.x;
+    const int64_t s = blockIdx.x;
+    const int per = (p.nz + (int)gridDim.y - 1) / (int)gridDim.y;
+    const int jbeg = (int)blockIdx.y * per;
+    const int jend = min(p.nz, jbeg + per);
+    if (jbeg >= jend) return;
+
+    float2 tw1[15], tw2[7];
+#pragma unroll
+    for (int i = 0; i < 15; ++i) tw1[i] = __ldg(p.tw1 + tid * 15 + i);
+#pragma unroll
+    for (int i = 0; i < 7; ++i) tw2[i] = __ldg(p.tw2 + (tid >> 3) * 7 + i);
+
+    // ---- stage-in (conjugated: forward FFT = conj(IFFT(conj g)))
+    float2 x[16];
+    const int64_t g0 = s * p.V - p.h + tid;
+#pragma unroll
+    for (int k1 = 0; k1 < 16; ++k1) {
+        const int64_t k = g0 + 128 * k1;
+        float2 v = make_float2(0.f, 0.f);
+        if (k >= 0 && k < p.nbins) {
+            if (PREC == FDAS_FP32) v = __ldg(reinterpret_cast<const float2*>(p.spec) + k);
+            else v = unpack_bf16x2(__ldg(reinterpret_cast<const unsigned int*>(p.spec) + k));
+        }
+        x[k1] = make_float2(v.x, -v.y);
+    }
+    ifft2048(x, X1, X2, tid, tw1, tw2);
+    // x[e*8 + n2b] = conj(S[2 tid + e + 256 n2b]): to natural order through X1, then to (k0, k1) order
+    {
+        float4* lin = reinterpret_cast<float4*>(X1);
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+            lin[tid + 128 * q] = make_float4(x[q].x, -x[q].y, x[8 + q].x, -x[8 + q].y);
+    }
+    __syncthreads();
+    float2 S[16];
+#pragma unroll
+    for (int k1 = 0; k1 < 16; ++k1) S[k1] = X1[tid + 128 * k1];
+    __syncthreads();
+
+    // ---- template loop
+    const int64_t sV = s * p.V;
+    const int nvalid = (int)min((int64_t)p.V, p.nbins - sV);
+
+    if (PREC == FDAS_FP32) {
+        const float4* bank = reinterpret_cast<const float4*>(p.bank) + (size_t)jbeg * 8 * 128 + tid;
+        float4 K[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) K[c] = __ldg(bank + c * 128);
+        for (int j = jbeg; j < jend; ++j) {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                x[2 * c] = cmul(S[2 * c], make_float2(K[c].x, K[c].y));
+                x[2 * c + 1] = cmul(S[2 * c + 1], make_float2(K[c].z, K[c].w));
+            }
+            bank += 8 * 128;
+            if (j + 1 < jend) {
+#pragma unroll
+                for (int c = 0; c < 8; ++c) K[c] = __ldg(bank + c * 128);
+            }
+            ifft2048(x, X1, X2, tid, tw1, tw2);
+            float* row = reinterpret_cast<float*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                if (2 * tid + 256 * q < nvalid) {
+                    const float p0 = x[q].x * x[q].x + x[q].y * x[q].y;
+                    const float p1 = x[8 + q].x * x[8 + q].x + x[8 + q].y * x[8 + q].y;
+                    __stcs(reinterpret_cast<float2*>(row + 256 * q), make_float2(p0, p1));
+                }
+            }
+        }
+    } else {
+        const uint4* bank = reinterpret_cast<const uint4*>(p.bank) + (size_t)jbeg * 4 * 128 + tid;
+        uint4 K[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) K[c] = __ldg(bank + c * 128);
+        for (int j = jbeg; j < jend; ++j) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                x[4 * c + 0] = cmul(S[4 * c + 0], unpack_bf16x2(K[c].x));
+                x[4 * c + 1] = cmul(S[4 * c + 1], unpack_bf16x2(K[c].y));
+                x[4 * c + 2] = cmul(S[4 * c + 2], unpack_bf16x2(K[c].z));
+                x[4 * c + 3] = cmul(S[4 * c + 3], unpack_bf16x2(K[c].w));
+            }
+            bank += 4 * 128;
+            if (j + 1 < jend) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) K[c] = __ldg(bank + c * 128);
+            }
+            ifft2048(x, X1, X2, tid, tw1, tw2);
+            if (PREC == FDAS_BF16) {
+                float* row = reinterpret_cast<float*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    if (2 * tid + 256 * q < nvalid) {
+                        const float p0 = x[q].x * x[q].x + x[q].y * x[q].y;
+                        const float p1 = x[8 + q].x * x[8 + q].x + x[8 + q].y * x[8 + q].y;
+                        __stcs(reinterpret_cast<float2*>(row + 256 * q), make_float2(p0, p1));
+                    }
+                }
+            } else {
+                __nv_bfloat16* row =
+                    reinterpret_cast<__nv_bfloat16*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    if (2 * tid + 256 * q < nvalid) {
+                        const float p0 = x[q].x * x[q].x + x[q].y * x[q].y;
+                        const float p1 = x[8 + q].x * x[8 + q].x + x[8 + q].y * x[8 + q].y;
+                        const __nv_bfloat162 pk = __floats2bfloat162_rn(p0, p1);
+                        __stcs(reinterpret_cast<unsigned int*>(row + 256 * q),
+                               *reinterpret_cast<const unsigned int*>(&pk));
+                    }
+                }
+            }
+        }
+    }
+}
+
+cudaError_t launch_convolve(int precision, const ConvParams& p, int64_t nseg, int nsplit,
+                            cudaStream_t st) {
+    dim3 grid((unsigned)nseg, (unsigned)nsplit), block(kThreads);
+    switch (precision) {
+        case FDAS_FP32: convolve_kernel<FDAS_FP32><<<grid, block, 0, st>>>(p); break;
+        case FDAS_BF16: convolve_kernel<FDAS_BF16><<<grid, block, 0, st>>>(p); break;
+        case FDAS_BF16_PLANE16: convolve_kernel<FDAS_BF16_PLANE16><<<grid, block, 0, st>>>(p); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace fdas

@@ -1,0 +1,175 @@
+// fdas_fft_core.cuh -- per-thread building blocks of the 2048-point segment FFT used by the fused
+// convolution kernel (fdas_convolve.cu).  Every function is __host__ __device__ so that the exact
+// index arithmetic and exchange-buffer layouts can also be stepped on the CPU, thread by thread, by
+// the test-only emulator (fdas_emu.cu) -- there is no GPU on the development box.
+//
+// Inverse transform y[n] = sum_p Y[p] exp(+2 pi i n p / 2048) (unnormalised), 128 threads x 16 points,
+// three register passes (16 x 16 x 8) with two shared-memory exchanges:
+//   p = k0 + 128 k1            k0 = 8 k0a + k0b in [0,128), k1 in [0,16)
+//   n = n1 + 16 n2a + 256 n2b  n1, n2a in [0,16), n2b in [0,8)
+//   pass 1 (thread k0)        A[n1]  = w2048^(n1 k0) * sum_k1 Y[k0+128 k1] w16^(n1 k1)
+//   pass 2 (thread n1*8+k0b)  C[n2a] = sum_k0a A[n1][8 k0a+k0b] w16^(n2a k0a)
+//   pass 3 (thread t, m = 2t+e, n1 = m%16, n2a = m/16 = t/8)
+//                             y[m + 256 n2b] = sum_k0b w128^(n2a k0b) C[m][k0b] w8^(n2b k0b)
+// with wN^(x) = exp(+2 pi i x / N).  Convolution stage of PAPER.md:23 (section 2.2).
+#pragma once
+#include <cuda_runtime.h>
+
+#define FDAS_HD __host__ __device__ __forceinline__
+
+namespace fdas {
+
+constexpr int kL = 2048;        // segment length (complex bins)
+constexpr int kThreads = 128;   // threads per segment
+constexpr int kPts = 16;        // points per thread
+constexpr int kRowStride = 18;  // float2 per exchange-buffer row: 16 data + 2 pad (144 B: LDS.128 conflict-free)
+constexpr int kXbufElems = kThreads * kRowStride;  // float2 elements per exchange buffer (18,432 B)
+
+FDAS_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+FDAS_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+FDAS_HD float2 cmul(float2 a, float2 b) {
+    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+FDAS_HD float2 cconj(float2 a) { return make_float2(a.x, -a.y); }
+FDAS_HD float2 cmul_i(float2 a) { return make_float2(-a.y, a.x); }  // a * (+i)
+
+// y_d = sum_a x_a (+i)^(a d), in place.
+FDAS_HD void bfly4_inv(float2& x0, float2& x1, float2& x2, float2& x3) {
+    float2 t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), t3 = cmul_i(csub(x1, x3));
+    x0 = cadd(t0, t2);
+    x1 = cadd(t1, t3);
+    x2 = csub(t0, t2);
+    x3 = csub(t1, t3);
+}
+
+// 16-point inverse DFT, natural order in and out: x[n] <- sum_k x[k] exp(+2 pi i n k / 16).
+// k = b + 4a, n = d + 4c: radix-4 over a, twiddle w16^(b d), radix-4 over b.
+FDAS_HD void dft16_inv(float2 (&x)[16]) {
+    const float C1 = 0.92387953251128673848f;  // cos(pi/8)
+    const float S1 = 0.38268343236508978178f;  // sin(pi/8)
+    const float R = 0.70710678118654752440f;   // sqrt(1/2)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) bfly4_inv(x[b], x[b + 4], x[b + 8], x[b + 12]);  // -> E_b[d] at x[b+4d]
+    // b = 1: d = 1,2,3 -> w16^1, w16^2, w16^3
+    x[1 + 4] = cmul(x[1 + 4], make_float2(C1, S1));
+    x[1 + 8] = make_float2((x[1 + 8].x - x[1 + 8].y) * R, (x[1 + 8].x + x[1 + 8].y) * R);
+    x[1 + 12] = cmul(x[1 + 12], make_float2(S1, C1));
+    // b = 2: w16^2, w16^4 = i, w16^6
+    x[2 + 4] = make_float2((x[2 + 4].x - x[2 + 4].y) * R, (x[2 + 4].x + x[2 + 4].y) * R);
+    x[2 + 8] = cmul_i(x[2 + 8]);
+    x[2 + 12] = make_float2((-x[2 + 12].x - x[2 + 12].y) * R, (x[2 + 12].x - x[2 + 12].y) * R);
+    // b = 3: w16^3, w16^6, w16^9 = -w16^1
+    x[3 + 4] = cmul(x[3 + 4], make_float2(S1, C1));
+    x[3 + 8] = make_float2((-x[3 + 8].x - x[3 + 8].y) * R, (x[3 + 8].x - x[3 + 8].y) * R);
+    x[3 + 12] = cmul(x[3 + 12], make_float2(-C1, -S1));
+#pragma unroll
+    for (int d = 0; d < 4; ++d) bfly4_inv(x[4 * d], x[4 * d + 1], x[4 * d + 2], x[4 * d + 3]);  // F_d[c] at x[c+4d]
+    float2 y[16];
+#pragma unroll
+    for (int d = 0; d < 4; ++d)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) y[d + 4 * c] = x[c + 4 * d];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = y[i];
+}
+
+// 8-point inverse DFT on x[o..o+7], natural order in and out.  k = b + 4a, n = d + 2c.
+FDAS_HD void dft8_inv(float2 (&x)[16], const int o) {
+    const float R = 0.70710678118654752440f;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+        float2 s = cadd(x[o + b], x[o + b + 4]), t = csub(x[o + b], x[o + b + 4]);
+        x[o + b] = s;        // E_b[0]
+        x[o + b + 4] = t;    // E_b[1]
+    }
+    // twiddle w8^(b) on E_b[1]: b = 1 -> (1+i)/sqrt2, b = 2 -> i, b = 3 -> (-1+i)/sqrt2
+    x[o + 5] = make_float2((x[o + 5].x - x[o + 5].y) * R, (x[o + 5].x + x[o + 5].y) * R);
+    x[o + 6] = cmul_i(x[o + 6]);
+    x[o + 7] = make_float2((-x[o + 7].x - x[o + 7].y) * R, (x[o + 7].x - x[o + 7].y) * R);
+    bfly4_inv(x[o + 0], x[o + 1], x[o + 2], x[o + 3]);  // d = 0: F_0[c] at x[o+c]
+    bfly4_inv(x[o + 4], x[o + 5], x[o + 6], x[o + 7]);  // d = 1: F_1[c] at x[o+4+c]
+    float2 y[8];
+#pragma unroll
+    for (int d = 0; d < 2; ++d)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) y[d + 2 * c] = x[o + c + 4 * d];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[o + i] = y[i];
+}
+
+// ---- pass 1: thread k0 = tid holds x[k1] = Y[tid + 128 k1];  tw1[n1-1] = w2048^(n1 * tid)
+FDAS_HD void pass1(float2 (&x)[16], const float2 (&tw1)[15]) {
+    dft16_inv(x);
+#pragma unroll
+    for (int n1 = 1; n1 < 16; ++n1) x[n1] = cmul(x[n1], tw1[n1 - 1]);
+}
+
+// Exchange 1 write: element (n1, k0) goes to row n1*8 + k0b, column k0a (16 x 64-bit stores;
+// a half-warp covers all 32 banks exactly once).
+FDAS_HD void x1_store(float2* X1, const int tid, const float2 (&x)[16]) {
+    const int base = (tid & 7) * kRowStride + (tid >> 3);
+#pragma unroll
+    for (int n1 = 0; n1 < 16; ++n1) X1[base + n1 * 8 * kRowStride] = x[n1];
+}
+
+// Row read used after both exchanges: thread tid reads its own 16-element row with 8 x 128-bit
+// loads (row pitch 144 B rotates consecutive threads over the eight 16-byte bank groups).
+FDAS_HD void xrow_load(const float2* X, const int tid, float2 (&x)[16]) {
+    const float4* p = reinterpret_cast<const float4*>(X + tid * kRowStride);
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+        float4 v = p[c];
+        x[2 * c] = make_float2(v.x, v.y);
+        x[2 * c + 1] = make_float2(v.z, v.w);
+    }
+}
+
+// ---- pass 2: thread tid = n1*8 + k0b holds x[k0a]; result x[n2a]
+FDAS_HD void pass2(float2 (&x)[16]) { dft16_inv(x); }
+
+// Exchange 2 write: element (m = n1 + 16 n2a, k0b) goes to row m/2, column (m%2)*8 + k0b
+// (a half-warp writes one contiguous 128-byte row segment).
+FDAS_HD void x2_store(float2* X2, const int tid, const float2 (&x)[16]) {
+    const int n1 = tid >> 3, k0b = tid & 7;
+    const int base = (n1 >> 1) * kRowStride + (n1 & 1) * 8 + k0b;
+#pragma unroll
+    for (int n2a = 0; n2a < 16; ++n2a) X2[base + n2a * 8 * kRowStride] = x[n2a];
+}
+
+// ---- pass 3: thread tid holds x[e*8 + k0b] for m = 2 tid + e;  tw2[k0b-1] = w128^((tid/8) * k0b)
+// result x[e*8 + n2b] = y[2 tid + e + 256 n2b]
+FDAS_HD void pass3(float2 (&x)[16], const float2 (&tw2)[7]) {
+#pragma unroll
+    for (int k = 1; k < 8; ++k) {
+        x[k] = cmul(x[k], tw2[k - 1]);
+        x[8 + k] = cmul(x[8 + k], tw2[k - 1]);
+    }
+    dft8_inv(x, 0);
+    dft8_inv(x, 8);
+}
+
+// Round-to-nearest-even float -> bfloat16 bits and back (storage format of the bf16 path,
+// PAPER.md:23; reading A10).
+FDAS_HD unsigned short f32_to_bf16_rne(float f) {
+    union { float f; unsigned int u; } v;
+    v.f = f;
+    unsigned int u = v.u;
+    u += 0x7fffu + ((u >> 16) & 1u);
+    return (unsigned short)(u >> 16);
+}
+FDAS_HD float bf16_bits_to_f32(unsigned int hi16) {
+    union { float f; unsigned int u; } v;
+    v.u = hi16 << 16;
+    return v.f;
+}
+FDAS_HD unsigned int pack_bf16x2(float re, float im) {  // low half = re, high half = im
+    return (unsigned int)f32_to_bf16_rne(re) | ((unsigned int)f32_to_bf16_rne(im) << 16);
+}
+FDAS_HD float2 unpack_bf16x2(unsigned int v) {
+    union { float f; unsigned int u; } lo, hi;
+    lo.u = v << 16;
+    hi.u = v & 0xffff0000u;
+    return make_float2(lo.f, hi.f);
+}
+
+}  // namespace fdas

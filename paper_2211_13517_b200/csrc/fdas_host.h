@@ -1,0 +1,50 @@
+// fdas_host.h -- host-side (plan-time) mathematics of libfdas: template bank, twiddle tables,
+// whitening block schedule, thresholds.  Pure C++ (no CUDA calls) so it also links into the
+// test-only emulator.  Shares nothing with oracle/.
+#pragma once
+#include <complex>
+#include <cstdint>
+#include <vector>
+
+namespace fdas {
+
+typedef std::complex<double> cd;
+
+// Fresnel integrals C(t) = int_0^t cos(pi s^2/2) ds, S(t) = int_0^t sin(pi s^2/2) ds.
+void fresnel_cs(double t, double* C, double* S);
+
+// Half-width rule (reading A5): h = round-up-to-multiple-of-32(ceil(zmax/2) + 16).
+int template_halfwidth(double zmax);
+
+// Closed-form response of a constant-fdot signal (Ransom et al. 2002; reading A4):
+// T_z[m], m = -h..h, truncated and scaled to unit L2 norm.  out has 2h+1 entries.
+void template_response(double z, int h, cd* out);
+
+struct Bank {
+    int nz = 0, h = 0, L = 0;
+    std::vector<cd> time;      // nz x (2h+1): unit-norm T_j[m]
+    std::vector<cd> freq;      // nz x L: Khat_j[p] = conj(FFT_L(c_j))[p] / L, c_j[i] = T_j[i-h]
+};
+void build_bank(double zmax, double zstep, int nz, int h, int L, Bank* bank);
+
+// In-place iterative radix-2 FFT (sign = -1 forward, +1 inverse, unnormalised).
+void host_fft(cd* a, int n, int sign);
+
+// Kernel register order (see fdas_fft_core.cuh): thread k0 holds Khat[k0 + 128 k1], k1 = 0..15.
+// fp32: float4 words [nz][8][128] = {K[k0+128(2c)], K[k0+128(2c+1)]}  (re, im, re, im)
+// bf16: uint4  words [nz][4][128] = 4 complex k1 = 4c..4c+3, each (bf16 im << 16) | bf16 re
+void pack_bank_fp32(const Bank& bank, std::vector<float>* out);
+void pack_bank_bf16(const Bank& bank, std::vector<uint32_t>* out);
+
+// tw1[k0][n1-1] = exp(+2 pi i n1 k0 / 2048), n1 = 1..15 (128 x 15 complex fp32)
+// tw2[q][k-1]   = exp(+2 pi i q k / 128), q = 0..15, k = 1..7 (16 x 7 complex fp32)
+void build_twiddles(std::vector<float>* tw1, std::vector<float>* tw2);
+
+// Whitening block schedule (reading A3): s_0 = 1, len = clamp(2^(floor(log2 s) - 2), 32, 4096),
+// truncated at nb.
+void whitening_blocks(int64_t nb, std::vector<int32_t>* start, std::vector<int32_t>* len);
+
+// T_h with Q(h, T_h) = erfc(nsigma/sqrt 2)/2 (reading A13).
+int thresholds_from_sigma(int H, double nsigma, float* out);
+
+}  // namespace fdas

@@ -1,0 +1,50 @@
+// fdas_kernels.h -- launchers of the three sm_100a kernels behind the C ABI (internal).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "../../include/fdas.h"
+
+namespace fdas {
+
+struct ConvParams {
+    const void* spec;    // nbins complex: float2 (FDAS_FP32) or packed bf16x2 (re low, im high)
+    void* plane;         // nz x pitch: float or bf16
+    const void* bank;    // packed Khat, register order (fdas_host.h)
+    const float2* tw1;   // [128][15]
+    const float2* tw2;   // [16][7]
+    int64_t nbins;
+    int64_t pitch;
+    int nz, h, V;
+};
+
+// K2: one CTA of 128 threads per (segment, template chunk); grid = (nseg, nsplit).
+cudaError_t launch_convolve(int precision, const ConvParams& p, int64_t nseg, int nsplit,
+                            cudaStream_t st);
+
+struct WhitenParams {
+    const float2* X;         // nfft/2 + 1 complex from cuFFT R2C
+    void* spec;              // nbins complex fp32 or bf16x2
+    const int32_t* blk_start;
+    const int32_t* blk_len;
+    float* blk_med;          // nblk (scratch)
+    int nblk;
+    int64_t nbins;
+};
+// K1a (block medians) + K1b (interpolate, scale, cast).  Two launches.
+cudaError_t launch_whiten(int precision, const WhitenParams& p, cudaStream_t st);
+
+struct HarmParams {
+    const void* plane;
+    int64_t nbins, pitch;
+    int nz, H;
+    int64_t r_lo;
+    float thr[32];
+    fdas_cand_t* cands;
+    int64_t capacity;
+    unsigned long long* count;
+};
+// K3: harmonic sums, thresholds, warp-aggregated compaction.  One launch (+ a memset of *count).
+cudaError_t launch_harmonic(int plane_is_bf16, const HarmParams& p, cudaStream_t st);
+
+}  // namespace fdas

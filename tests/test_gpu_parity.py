@@ -1,0 +1,337 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle on the same seeded
+inputs.  Tolerances are BASELINE.json north_star's:
+    fp32 path   |GPU - oracle| <= 1e-4 x plane maximum
+    bf16 path   <= 2e-2 x plane maximum, candidate powers within 3 %
+    candidate (r, z, h) lists identical except entries within that tolerance of the threshold.
+Run with `pytest -m gpu` on the B200 box.
+"""
+import numpy as np
+import pytest
+
+from paper_2211_13517_b200 import inputs
+from helpers import compare_candidates, gpu_cand_dict, oracle_margin_fn
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"fp32": 1e-4, "bf16": 2e-2, "bf16_plane16": 2e-2}
+REL_POW = {"fp32": None, "bf16": 0.03, "bf16_plane16": 0.03}
+
+
+@pytest.fixture(scope="module")
+def fdas():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2211_13517_b200 import fdas as F   # raises if libfdas.so is missing (no fallback)
+    return F
+
+
+@pytest.fixture(scope="module")
+def torch_():
+    import torch
+    return torch
+
+
+def spec_to_complex(torch, d_spec):
+    a = d_spec.float().cpu().numpy().astype(np.float64)
+    return a[:, 0] + 1j * a[:, 1]
+
+
+def spec_from_complex(torch, w, precision):
+    a = np.stack([w.real, w.imag], axis=1).astype(np.float32)
+    t = torch.from_numpy(a).cuda()
+    return t if precision == "fp32" else t.to(torch.bfloat16)
+
+
+def run_gpu(fdas, torch, wl, x, precision, capacity=1 << 16, thr=None):
+    plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, precision)
+    d_x = torch.from_numpy(x).cuda()
+    d_spec, d_plane = plan.alloc_spec(), plan.alloc_plane()
+    d_plane.fill_(float("nan"))
+    d_c, d_n = plan.alloc_cands(capacity)
+    if thr is None:
+        thr = fdas.thresholds_from_sigma(wl.nharm, wl.nsigma)
+    plan.prepare_spectrum(d_x, d_spec)
+    plan.convolve_plane(d_spec, d_plane)
+    plan.harmonic_sum_peaks(d_plane, wl.nharm, thr, wl.r_lo, d_c, d_n)
+    torch.cuda.synchronize()
+    res = plan.read_cands(d_c, d_n)
+    return plan, d_spec, d_plane, res, thr
+
+
+# ------------------------------------------------------------------------------------ configs[0]
+def test_tiny_fp32_full_parity(fdas, torch_, oracle):
+    torch = torch_
+    wl = inputs.tiny()
+    x = inputs.series_for(wl)
+    plan, d_spec, d_plane, res, thr = run_gpu(fdas, torch, wl, x, "fp32")
+    info = plan.info
+    assert (info.nfft, info.nbins, info.nz, info.halfwidth, info.valid, info.nseg) == \
+        (1 << 17, 1 << 16, 33, 32, 1984, 34)
+    orc = oracle.run(x, wl.nfft, wl.zmax, wl.zstep, wl.nharm, wl.nsigma, wl.r_lo, want_candidates=False)
+    # library templates = oracle templates (closed form vs quadrature)
+    assert np.abs(plan.templates_host() - orc.bank).max() < 1e-12
+    # whitened spectrum
+    w_gpu = spec_to_complex(torch, d_spec)
+    assert w_gpu[0] == 0
+    assert np.abs(w_gpu - orc.w).max() <= 2e-5 * np.abs(orc.w).max()
+    # plane: every element, fp32 tolerance
+    P_gpu = d_plane.cpu().numpy().astype(np.float64)
+    assert not np.isnan(P_gpu).any()
+    err = np.abs(P_gpu - orc.P).max()
+    assert err <= TOL["fp32"] * orc.P.max(), err / orc.P.max()
+    # candidates (oracle gets the same float32 thresholds)
+    oc = oracle.candidates(orc.P, wl.nharm, thr.astype(np.float64), wl.r_lo)
+    s_at, margin = oracle_margin_fn(oracle, orc.P, wl.nharm, wl.r_lo)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, TOL["fp32"] * orc.P.max(),
+                               None, s_at, margin)
+    assert res.count == len(res.cands) and stats["common"] >= 1
+    keys = set(gpu_cand_dict(res.cands))
+    assert (20000, 23, 1) in keys or (20000, 24, 1) in keys     # the injected signal (z0 = 7.5)
+    assert plan.launch_count() == 4
+
+
+# ------------------------------------------------------------------------------------ configs[1]
+@pytest.fixture(scope="module")
+def medium_oracle(oracle):
+    wl = inputs.medium()
+    x = inputs.series_for(wl)
+    orc = oracle.run(x, wl.nfft, wl.zmax, wl.zstep, wl.nharm, wl.nsigma, wl.r_lo, want_candidates=False)
+    return wl, x, orc
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16", "bf16_plane16"])
+def test_medium_full_parity(fdas, torch_, oracle, medium_oracle, precision):
+    torch = torch_
+    wl, x, orc = medium_oracle
+    plan, d_spec, d_plane, res, thr = run_gpu(fdas, torch, wl, x, precision)
+    assert (plan.info.nbins, plan.info.nz, plan.info.halfwidth, plan.info.nseg) == (1 << 20, 193, 64, 547)
+    pmax = orc.P.max()
+    tol = TOL[precision] * pmax
+    # plane, element by element, in row chunks to bound host memory
+    worst = 0.0
+    for j0 in range(0, plan.info.nz, 16):
+        Pg = d_plane[j0:j0 + 16].float().cpu().numpy().astype(np.float64)
+        assert not np.isnan(Pg).any()
+        worst = max(worst, np.abs(Pg - orc.P[j0:j0 + 16]).max())
+    assert worst <= tol, (precision, worst / pmax)
+    oc = oracle.candidates(orc.P, wl.nharm, thr.astype(np.float64), wl.r_lo)
+    s_at, margin = oracle_margin_fn(oracle, orc.P, wl.nharm, wl.r_lo)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, tol, REL_POW[precision],
+                               s_at, margin)
+    # the four injected chirps are recovered at (round(r_c), nearest z)
+    keys = set(gpu_cand_dict(res.cands))
+    for s in wl.signals:
+        if s.amp ** 2 * wl.nfft / 4 < 60:
+            continue
+        r0, j0 = int(round(s.r_c)), int(round(s.z + wl.zmax))
+        assert any((r0 + dr, j0 + dj, 1) in keys for dr in (-1, 0, 1) for dj in (-1, 0, 1)), s
+    assert stats["common"] >= 4
+    print(precision, "worst/max", worst / pmax, stats)
+
+
+# --------------------------------------------------------------- K2 alone, fed a chosen spectrum
+@pytest.mark.parametrize("precision", ["fp32", "bf16", "bf16_plane16"])
+def test_convolve_alone_seams_tail_and_invariants(fdas, torch_, oracle, precision):
+    torch = torch_
+    n = 1 << 15                      # nbins = 16384: 9 segments of V = 1984 + ragged tail
+    plan = fdas.Plan(n, 64e-6, 16.0, 1.0, 2048, precision)
+    nb, nz = plan.info.nbins, plan.info.nz
+    rng = np.random.default_rng(8)
+    w = (rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)
+    for k in (0, 1, 1983, 1984, 1985, 3968, nb - 1):      # lines on and around segment seams
+        w[k] += 12.0
+    d_spec = spec_from_complex(torch, w, precision)
+    wq = spec_to_complex(torch, d_spec)                   # what the kernel actually reads
+    d_plane = plan.alloc_plane(); d_plane.fill_(float("nan"))
+    plan.convolve_plane(d_spec, d_plane)
+    torch.cuda.synchronize()
+    Pg = d_plane.float().cpu().numpy().astype(np.float64)
+    assert not np.isnan(Pg).any()
+    bank = oracle.template_bank(16.0, 1.0)
+    P = oracle.plane(w, bank)
+    assert np.abs(Pg - P).max() <= TOL[precision] * P.max()
+    if precision == "fp32":
+        # z = 0 row is the power spectrum; conj(w) flips the z axis; a shift by d bins (not a
+        # multiple of V) shifts every row
+        assert np.abs(Pg[16] - np.abs(wq) ** 2).max() <= 1e-5 * P.max()
+        d_spec_c = spec_from_complex(torch, np.conj(w), precision)
+        d_plane_c = plan.alloc_plane()
+        plan.convolve_plane(d_spec_c, d_plane_c)
+        Pc = d_plane_c.cpu().numpy()
+        assert np.abs(Pc - Pg[::-1]).max() <= 1e-5 * P.max()
+        d = 777
+        ws = np.concatenate([np.zeros(d), w[:-d]])
+        d_plane_s = plan.alloc_plane()
+        plan.convolve_plane(spec_from_complex(torch, ws, precision), d_plane_s)
+        Ps = d_plane_s.cpu().numpy()
+        assert np.abs(Ps[:, d + 32: nb - 32] - Pg[:, 32: nb - d - 32]).max() <= 1e-5 * P.max()
+    else:
+        # quantised oracle (reading A11): bf16-rounded spectrum, double arithmetic -- the kernel's
+        # remaining error is template quantisation + fp32 arithmetic (+ plane rounding)
+        Pq = oracle.plane(wq, bank)
+        assert np.abs(Pg - Pq).max() <= 1e-2 * P.max()
+
+
+def test_smallest_plan_and_zmax0(fdas, torch_, oracle):
+    torch = torch_
+    plan = fdas.Plan(4096, 64e-6, 0.0, 1.0, 2048, "fp32")   # N = 2 * seg_len, one template (delta)
+    assert (plan.info.nbins, plan.info.nz, plan.info.halfwidth, plan.info.nseg) == (2048, 1, 32, 2)
+    x = np.random.default_rng(1).standard_normal(4096).astype(np.float32)
+    d_spec, d_plane = plan.alloc_spec(), plan.alloc_plane()
+    plan.prepare_spectrum(torch.from_numpy(x).cuda(), d_spec)
+    plan.convolve_plane(d_spec, d_plane)
+    torch.cuda.synchronize()
+    w = spec_to_complex(torch, d_spec)
+    worc = oracle.whiten(oracle.spectrum(x, 4096))
+    assert np.abs(w - worc).max() <= 2e-5 * np.abs(worc).max()
+    assert np.abs(d_plane.cpu().numpy()[0] - np.abs(w) ** 2).max() <= 1e-5 * (np.abs(w) ** 2).max()
+
+
+def test_non_power_of_two_series_uses_largest_pow2(fdas, torch_, oracle):
+    torch = torch_
+    n = 100_000                                # nfft = 65536 (reading A1); the tail is ignored
+    plan = fdas.Plan(n, 64e-6, 16.0, 1.0, 2048, "fp32")
+    assert plan.info.n_in == n and plan.info.nfft == 65536
+    x = np.random.default_rng(12).standard_normal(n).astype(np.float32)
+    d_spec = plan.alloc_spec()
+    plan.prepare_spectrum(torch.from_numpy(x).cuda(), d_spec)
+    torch.cuda.synchronize()
+    worc = oracle.whiten(oracle.spectrum(x, 65536))
+    assert np.abs(spec_to_complex(torch, d_spec) - worc).max() <= 2e-5 * np.abs(worc).max()
+
+
+# ----------------------------------------------------------------- K3 alone on hand-made planes
+@pytest.mark.parametrize("precision", ["fp32", "bf16_plane16"])
+def test_harmonic_sum_alone_many_candidates(fdas, torch_, oracle, precision):
+    torch = torch_
+    plan = fdas.Plan(1 << 15, 64e-6, 16.0, 1.0, 2048, precision)
+    nb, nz = plan.info.nbins, plan.info.nz
+    rng = np.random.default_rng(17)
+    P32 = rng.exponential(1.0, size=(nz, nb)).astype(np.float32)
+    d_plane = torch.from_numpy(P32).cuda()
+    if precision == "bf16_plane16":
+        d_plane = d_plane.to(torch.bfloat16)
+    P = d_plane.float().cpu().numpy().astype(np.float64)     # the values the kernel reads
+    H = 16
+    thr = fdas.thresholds_from_sigma(H, 3.0)                 # ~1e-3 of the points pass
+    d_c, d_n = plan.alloc_cands(1 << 18)
+    plan.harmonic_sum_peaks(d_plane, H, thr, 5, d_c, d_n)
+    torch.cuda.synchronize()
+    res = plan.read_cands(d_c, d_n)
+    oc = oracle.candidates(P, H, thr.astype(np.float64), 5)
+    assert oc.count > 500
+    s_at, margin = oracle_margin_fn(oracle, P, H, 5)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * P.max(), None, s_at, margin)
+    assert stats["only_gpu"] + stats["only_orc"] <= 3 and stats["flags_checked"] > 100
+    # H = 1, r_lo beyond the plane, capacity overflow
+    plan.harmonic_sum_peaks(d_plane, 1, thr, nb, d_c, d_n)
+    assert plan.read_cands(d_c, d_n).count == 0
+    d_small, _ = plan.alloc_cands(10)
+    plan.harmonic_sum_peaks(d_plane, H, thr, 5, d_small, d_n)
+    small = plan.read_cands(d_small, d_n)
+    assert small.count == res.count and len(small.cands) == 10
+    assert set(gpu_cand_dict(small.cands)) <= set(gpu_cand_dict(res.cands))
+
+
+def test_abi_errors_on_device(fdas, torch_):
+    import ctypes as C
+    torch = torch_
+    plan = fdas.Plan(1 << 15, 64e-6, 16.0, 1.0, 2048, "fp32")
+    lib = fdas.lib()
+    d_plane = plan.alloc_plane()
+    thr = np.ones(32, dtype=np.float32)
+    thr_c = thr.ctypes.data_as(C.POINTER(C.c_float))
+    d_c, d_n = plan.alloc_cands(16)
+    assert lib.fdas_harmonic_sum_peaks(plan._h, d_plane.data_ptr(), 0, thr_c, 0, d_c.data_ptr(), 16, d_n.data_ptr(), None) == fdas.FDAS_EARG
+    assert lib.fdas_harmonic_sum_peaks(plan._h, d_plane.data_ptr(), 33, thr_c, 0, d_c.data_ptr(), 16, d_n.data_ptr(), None) == fdas.FDAS_EARG
+    assert lib.fdas_harmonic_sum_peaks(plan._h, d_plane.data_ptr(), 4, thr_c, -1, d_c.data_ptr(), 16, d_n.data_ptr(), None) == fdas.FDAS_EARG
+    assert lib.fdas_harmonic_sum_peaks(plan._h, None, 4, thr_c, 0, d_c.data_ptr(), 16, d_n.data_ptr(), None) == fdas.FDAS_EARG
+    assert lib.fdas_convolve_plane(plan._h, None, d_plane.data_ptr(), None) == fdas.FDAS_EARG
+    assert lib.fdas_prepare_spectrum(plan._h, None, None, None) == fdas.FDAS_EARG
+
+
+# ------------------------------------------------------------------ end-to-end host entry point
+def test_search_host_equals_device_calls(fdas, torch_):
+    torch = torch_
+    wl = inputs.tiny()
+    x = inputs.series_for(wl)
+    plan, _, _, res, thr = run_gpu(fdas, torch, wl, x, "fp32")
+    out = plan.search_host(x, wl.nharm, thr, wl.r_lo, capacity=4096)
+    assert out.count == res.count
+    assert gpu_cand_dict(out.cands) == gpu_cand_dict(res.cands)
+    tiny_cap = plan.search_host(x, wl.nharm, thr, wl.r_lo, capacity=1)
+    assert tiny_cap.count == res.count and len(tiny_cap.cands) == 1
+
+
+# ------------------------------------------------------- configs[2] at full size: sampled parity
+@pytest.mark.parametrize("precision", ["bf16", "fp32"])
+def test_ska_full_size_sampled_parity(fdas, torch_, oracle, precision):
+    """SKA-like single DM trial in the launch configuration bench.py times.  The oracle computes
+    sampled plane points and sampled harmonic sums one by one from its own whitened spectrum."""
+    torch = torch_
+    wl = inputs.ska()
+    x = inputs.series_for(wl)
+    plan, d_spec, d_plane, res, thr = run_gpu(fdas, torch, wl, x, precision)
+    info = plan.info
+    assert (info.n_in, info.nfft, info.nbins, info.nz, info.nseg) == (9_375_000, 1 << 23, 1 << 22, 193, 2185)
+    w = oracle.whiten(oracle.spectrum(x, wl.nfft))
+    w_gpu = spec_to_complex(torch, d_spec)
+    stol = 2e-5 if precision == "fp32" else 1e-2
+    assert np.abs(w_gpu - w).max() <= stol * np.abs(w).max()
+    bank = oracle.template_bank(wl.zmax, wl.zstep)
+    nb, nz, V = info.nbins, info.nz, info.valid
+    rng = np.random.default_rng(99)
+    rr = [rng.integers(0, nb, 30000)]
+    jj = [rng.integers(0, nz, 30000)]
+    # segment seams, the first bins, the ragged tail, and the injected signals' neighbourhoods
+    seams = np.array([s * V + d for s in (1, 2, 1000, 2184) for d in (-2, -1, 0, 1, 2)])
+    for cols in (seams, np.arange(0, 70), np.arange(nb - 70, nb)):
+        for j in (0, 56, 96, 136, 192):
+            rr.append(cols); jj.append(np.full(cols.size, j))
+    for s in wl.signals:
+        for k in (1, 2):
+            r0, j0 = int(round(k * s.r_c)), int(round(k * s.z + wl.zmax))
+            g_r, g_j = np.meshgrid(np.arange(r0 - 6, r0 + 7), np.arange(j0 - 3, j0 + 4))
+            rr.append(g_r.ravel()); jj.append(g_j.ravel())
+    rr = np.concatenate(rr).astype(np.int64); jj = np.concatenate(jj).astype(np.int32)
+    Po = oracle.plane_points(w, bank, rr, jj)
+    Pg = d_plane[torch.from_numpy(jj.astype(np.int64)).cuda(), torch.from_numpy(rr).cuda()].float().cpu().numpy()
+    # plane maximum: taken from the GPU plane, cross-checked against the oracle at that point
+    flat = int(torch.argmax(d_plane.float()).item())
+    jm, rm = flat // info.plane_pitch, flat % info.plane_pitch
+    pmax = float(oracle.plane_points(w, bank, [rm], [jm])[0])
+    assert abs(float(d_plane[jm, rm]) - pmax) <= TOL[precision] * pmax and pmax > 100
+    worst = np.abs(Pg - Po).max()
+    assert worst <= TOL[precision] * pmax, worst / pmax
+    assert not torch.isnan(d_plane.float().sum()).item()      # every element was written
+    # candidates: every GPU candidate is valid in the oracle; sampled fundamentals agree both ways
+    gd = gpu_cand_dict(res.cands)
+    assert res.count == len(gd) and res.count < 20000
+    tol = TOL[precision] * pmax
+    if gd:
+        keys = sorted(gd)
+        kr = np.array([k[0] for k in keys]); kj = np.array([k[1] for k in keys], dtype=np.int32)
+        S, hmax = oracle.harmonic_sums_sampled(w, bank, wl.nharm, kr, kj)
+        for i, (r, j, h) in enumerate(keys):
+            assert h <= hmax[i]
+            so = S[i, h - 1]
+            assert so > thr[h - 1] - h * tol, ((r, j, h), so)
+            assert abs(gd[(r, j, h)][0] - so) <= h * tol
+            if REL_POW[precision] is not None:
+                assert abs(gd[(r, j, h)][0] - so) <= REL_POW[precision] * so
+    sr = np.concatenate([rng.integers(wl.r_lo, nb, 4000)] +
+                        [np.arange(int(round(s.r_c)) - 3, int(round(s.r_c)) + 4) for s in wl.signals])
+    sj = np.concatenate([rng.integers(0, nz, 4000)] +
+                        [np.full(7, int(round(s.z + wl.zmax))) for s in wl.signals]).astype(np.int32)
+    S, hmax = oracle.harmonic_sums_sampled(w, bank, wl.nharm, sr, sj)
+    found = 0
+    for i in range(sr.size):
+        for h in range(1, hmax[i] + 1):
+            key = (int(sr[i]), int(sj[i]), h)
+            if S[i, h - 1] > thr[h - 1] + h * tol:
+                assert key in gd, key
+                found += 1
+            elif S[i, h - 1] < thr[h - 1] - h * tol:
+                assert key not in gd, key
+    assert found >= 2          # both injected fundamentals
+    print(precision, "sampled worst/max", worst / pmax, "pmax", pmax, "cands", res.count, "found", found)

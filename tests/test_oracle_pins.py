@@ -391,3 +391,18 @@ def test_p12_tiny_config_recovers_the_injected_signal(oracle):
     assert 1 <= res.cands.count < 200
     # noise part of the plane has unit mean
     assert abs(res.P[:, 30000:60000].mean() - 1.0) < 0.02
+
+
+def test_p9_sampled_harmonic_sums_equal_the_full_plane_route(oracle):
+    nb = 3000
+    w = _noise_w(nb, 31)
+    bank = oracle.template_bank(16.0, 1.0)
+    P = oracle.plane(w, bank)
+    rng = np.random.default_rng(2)
+    rr = rng.integers(1, nb, 200); jj = rng.integers(0, 33, 200).astype(np.int32)
+    S, hmax = oracle.harmonic_sums_sampled(w, bank, 16, rr, jj)
+    for i in range(200):
+        ref = oracle.harmonic_sums_at(P, 16, rr[i], jj[i])
+        assert hmax[i] == len(ref)
+        assert np.allclose(S[i, :hmax[i]], ref, rtol=1e-13)
+        assert np.all(np.isnan(S[i, hmax[i]:]))
