@@ -150,7 +150,7 @@ static int build_plan(fdas_plan_s* p) {
     int dev = 0, nsm = 148;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-    const int64_t slots = 3LL * nsm;  // K2 runs 3 CTAs per SM
+    const int64_t slots = (int64_t)convolve_ctas_per_sm() * nsm;
     int nsplit = 1;
     if (in.nseg < 4 * slots) nsplit = (int)std::min<int64_t>(in.nz, (4 * slots + in.nseg - 1) / in.nseg);
     if (const char* e = std::getenv("FDAS_NSPLIT")) {

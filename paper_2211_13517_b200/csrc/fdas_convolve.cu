@@ -12,10 +12,14 @@
 // variants only change the storage format of w, Khat (and optionally P) -- reading A10.
 #include <cuda_bf16.h>
 
+#include <cstdlib>
+
 #include "fdas_fft_core.cuh"
 #include "fdas_kernels.h"
 
 namespace fdas {
+
+constexpr int kDefaultOcc = 3;  // resident CTAs per SM the kernel is compiled for (FDAS_K2_OCC=3|4 overrides)
 
 __device__ __forceinline__ void ifft2048(float2 (&x)[16], float2* X1, float2* X2, const int tid,
                                          const float2 (&tw1)[15], const float2 (&tw2)[7]) {
@@ -30,8 +34,8 @@ __device__ __forceinline__ void ifft2048(float2 (&x)[16], float2* X1, float2* X2
     pass3(x, tw2);
 }
 
-template <int PREC>
-__global__ void __launch_bounds__(kThreads, 3) convolve_kernel(const ConvParams p) {
+template <int PREC, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvParams p) {
     __shared__ __align__(16) float2 X1[kXbufElems];
     __shared__ __align__(16) float2 X2[kXbufElems];
     const int tid = threadIdx.x;
@@ -152,16 +156,32 @@ __global__ void __launch_bounds__(kThreads, 3) convolve_kernel(const ConvParams 
     }
 }
 
-cudaError_t launch_convolve(int precision, const ConvParams& p, int64_t nseg, int nsplit,
-                            cudaStream_t st) {
-    dim3 grid((unsigned)nseg, (unsigned)nsplit), block(kThreads);
+int convolve_ctas_per_sm() {
+    static int occ = [] {
+        const char* e = std::getenv("FDAS_K2_OCC");
+        const int v = e ? std::atoi(e) : 0;
+        return (v == 3 || v == 4) ? v : kDefaultOcc;
+    }();
+    return occ;
+}
+
+template <int MINB>
+static cudaError_t launch_occ(int precision, const ConvParams& p, dim3 grid, cudaStream_t st) {
+    const dim3 block(kThreads);
     switch (precision) {
-        case FDAS_FP32: convolve_kernel<FDAS_FP32><<<grid, block, 0, st>>>(p); break;
-        case FDAS_BF16: convolve_kernel<FDAS_BF16><<<grid, block, 0, st>>>(p); break;
-        case FDAS_BF16_PLANE16: convolve_kernel<FDAS_BF16_PLANE16><<<grid, block, 0, st>>>(p); break;
+        case FDAS_FP32: convolve_kernel<FDAS_FP32, MINB><<<grid, block, 0, st>>>(p); break;
+        case FDAS_BF16: convolve_kernel<FDAS_BF16, MINB><<<grid, block, 0, st>>>(p); break;
+        case FDAS_BF16_PLANE16: convolve_kernel<FDAS_BF16_PLANE16, MINB><<<grid, block, 0, st>>>(p); break;
         default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
+}
+
+cudaError_t launch_convolve(int precision, const ConvParams& p, int64_t nseg, int nsplit,
+                            cudaStream_t st) {
+    const dim3 grid((unsigned)nseg, (unsigned)nsplit);
+    return convolve_ctas_per_sm() == 4 ? launch_occ<4>(precision, p, grid, st)
+                                       : launch_occ<3>(precision, p, grid, st);
 }
 
 }  // namespace fdas

@@ -21,6 +21,7 @@ struct ConvParams {
 // K2: one CTA of 128 threads per (segment, template chunk); grid = (nseg, nsplit).
 cudaError_t launch_convolve(int precision, const ConvParams& p, int64_t nseg, int nsplit,
                             cudaStream_t st);
+int convolve_ctas_per_sm();  // resident CTAs per SM K2 is launched for (sizes the template split)
 
 struct WhitenParams {
     const float2* X;         // nfft/2 + 1 complex from cuFFT R2C

@@ -10,7 +10,7 @@
 
 namespace fdas {
 
-constexpr int kMedThreads = 256;
+constexpr int kMedThreads = 1024;
 constexpr int kMedMax = 4096;
 
 __global__ void __launch_bounds__(kMedThreads) block_median_kernel(const WhitenParams p) {
