@@ -25,9 +25,18 @@ template <> __device__ __forceinline__ float ldp<__nv_bfloat16>(const __nv_bfloa
     return __bfloat162float(__ldg(p));
 }
 
+// Geometry handed BY VALUE to the rare emission path (a reference to the kernel parameter struct
+// would force every thread to spill all of it to local memory at kernel entry).
+struct HarmGeom {
+    int64_t nbins, pitch, r_lo, capacity;
+    fdas_cand_t* cands;
+    unsigned long long* count;
+    int nz;
+};
+
 // S_h at (r, j) if defined (r in [r_lo, Nb), all h harmonics inside the plane); summed k = 1..h.
 template <typename T>
-__device__ bool harmonic_sum_at(const T* P, const HarmParams& p, int64_t r, int j, int h, float* out) {
+__device__ bool harmonic_sum_at(const T* P, const HarmGeom p, int64_t r, int j, int h, float* out) {
     if (j < 0 || j >= p.nz || r < p.r_lo || r >= p.nbins) return false;
     const int c2 = p.nz - 1;
     float S = 0.f;
@@ -42,7 +51,7 @@ __device__ bool harmonic_sum_at(const T* P, const HarmParams& p, int64_t r, int 
 }
 
 template <typename T>
-__device__ __noinline__ void emit_candidate(const T* P, const HarmParams& p, int64_t r, int j, int h) {
+__device__ __noinline__ void emit_candidate(const T* P, const HarmGeom p, int64_t r, int j, int h) {
     float S;
     if (!harmonic_sum_at(P, p, r, j, h, &S)) return;
     const unsigned long long slot = atomicAdd(p.count, 1ULL);
@@ -108,13 +117,16 @@ __global__ void __launch_bounds__(kHarmThreads) harmonic_kernel(const HarmParams
         any |= hits[i];
     }
     if (any) {
+        HarmGeom g;
+        g.nbins = p.nbins; g.pitch = p.pitch; g.r_lo = p.r_lo; g.capacity = p.capacity;
+        g.cands = p.cands; g.count = p.count; g.nz = p.nz;
 #pragma unroll 1
         for (int i = 0; i < kRpt; ++i) {
             unsigned m = hits[i];
             while (m) {
                 const int k = __ffs(m);
                 m &= m - 1;
-                emit_candidate(P, p, rb + 256 * i, j, k);
+                emit_candidate(P, g, rb + 256 * i, j, k);
             }
         }
     }
