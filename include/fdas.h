@@ -16,7 +16,8 @@
  *   - returns an int status (FDAS_OK = 0); nothing throws or aborts across this boundary;
  *   - pointers named d_* are DEVICE pointers owned by the caller (allocate them with the sizes
  *     fdas_plan_info reports); pointers named h_* are HOST pointers; the plan owns its templates,
- *     twiddle tables, cuFFT plan + workspace and whitening scratch;
+ *     twiddle tables, cuFFT plan + workspace, whitening scratch and the harmonic-sum scratch
+ *     (block-maximum plane of nz x nbins/8 floats, prefilter list);
  *   - the three per-trial calls only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
  *     void*, NULL = legacy default stream) and return; they never synchronise, allocate or free;
  *   - a plan may be used from one stream at a time (its scratch is not duplicated).
@@ -124,6 +125,10 @@ int fdas_convolve_plane(fdas_plan_t plan, const void* d_spec, void* d_plane, voi
  *   d_cands       device, capacity records, filled in unspecified order
  *   d_count       device; set to 0 by this call, then receives the TRUE number of candidates found
  *                 (it may exceed capacity; only the first `capacity` claimed slots are stored)
+ * The search is exact (identical to evaluating every fundamental) but proceeds branch-and-bound on
+ * a plan-owned block-maximum plane that fdas_convolve_plane writes beside d_plane.  If d_plane is the
+ * buffer this plan's fdas_convolve_plane wrote last, its contents must not have been modified since;
+ * for any other d_plane the block maxima are rebuilt from it first (one extra pass over the plane).
  * FDAS_EARG: NULL pointers, H out of range, r_lo < 0, capacity < 0.
  */
 int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const float* h_thresholds,
@@ -152,6 +157,13 @@ int fdas_thresholds_from_sigma(int H, double nsigma, float* h_thresholds_out);
  * (nz x (2h+1) complex doubles, interleaved re/im, unit L2 norm) to h_out.  Host only.
  */
 int fdas_plan_templates_host(fdas_plan_t plan, double* h_out);
+
+/*
+ * fdas_plan_debug_maxplane -- diagnostic: device pointer and row pitch (elements) of the plan-owned
+ * block-maximum plane M[j][b] = max(P[j][8b..8b+7]) that fdas_convolve_plane writes for the
+ * harmonic-sum prefilter.  The buffer stays owned by the plan.
+ */
+int fdas_plan_debug_maxplane(fdas_plan_t plan, const float** d_out, int64_t* pitch_out);
 
 /* Number of kernels the library launched on behalf of this plan since it was created. */
 int64_t fdas_plan_launch_count(fdas_plan_t plan);

@@ -36,6 +36,10 @@ struct fdas_plan_s {
     int nblk = 0;
     int nsplit = 1;
     int64_t launches = 0;
+    float* d_maxplane = nullptr;             // block-max plane M (nz x nbins/8), written by K2
+    const void* max_valid_for = nullptr;     // the plane M currently describes (nullptr: none)
+    uint2* d_maybe = nullptr;                // K3 maybe list (kMaybeCapacity records)
+    unsigned long long* d_maybe_count = nullptr;
     // workspace of fdas_search_host (lazy)
     float* ws_series = nullptr;
     void* ws_spec = nullptr;
@@ -64,8 +68,11 @@ struct fdas_plan_s {
         }                                                                               \
     } while (0)
 
+static const int64_t kMaybeCapacity = 1 << 22;  // K3 prefilter survivors listed per call (more: evaluated in place)
+
 static void free_plan(fdas_plan_s* p) {
     if (!p) return;
+    cudaFree(p->d_maxplane); cudaFree(p->d_maybe); cudaFree(p->d_maybe_count);
     cudaFree(p->d_bank); cudaFree(p->d_tw1); cudaFree(p->d_tw2); cudaFree(p->d_fft_work);
     cudaFree(p->d_X); cudaFree(p->d_blk_start); cudaFree(p->d_blk_len); cudaFree(p->d_blk_med);
     cudaFree(p->ws_series); cudaFree(p->ws_spec); cudaFree(p->ws_plane); cudaFree(p->ws_cands);
@@ -138,6 +145,9 @@ static int build_plan(fdas_plan_s* p) {
     CU(cudaMemcpy(p->d_blk_start, bs.data(), bs.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
     CU(cudaMemcpy(p->d_blk_len, bl.data(), bl.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
 
+    CU(cudaMalloc(&p->d_maxplane, (size_t)in.nz * (size_t)(in.nbins / 8) * sizeof(float)));
+    CU(cudaMalloc(&p->d_maybe, (size_t)kMaybeCapacity * sizeof(uint2)));
+    CU(cudaMalloc(&p->d_maybe_count, sizeof(unsigned long long)));
     CU(cudaMalloc(&p->d_X, (size_t)(in.nfft / 2 + 1) * sizeof(float2)));
     size_t ws = 0;
     CF(cufftCreate(&p->fft));
@@ -216,7 +226,10 @@ int fdas_convolve_plane(fdas_plan_t plan, const void* d_spec, void* d_plane, voi
     c.spec = d_spec; c.plane = d_plane; c.bank = plan->d_bank; c.tw1 = plan->d_tw1; c.tw2 = plan->d_tw2;
     c.nbins = plan->info.nbins; c.pitch = plan->info.plane_pitch;
     c.nz = plan->info.nz; c.h = plan->info.halfwidth; c.V = plan->info.valid;
+    c.maxplane = plan->d_maxplane; c.mpitch = plan->info.nbins / 8;
+    plan->max_valid_for = nullptr;
     CU(launch_convolve(plan->info.precision, c, plan->info.nseg, plan->nsplit, (cudaStream_t)cuda_stream));
+    plan->max_valid_for = d_plane;
     plan->launches += 1;
     return FDAS_OK;
 }
@@ -231,8 +244,14 @@ int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const 
     hp.nz = plan->info.nz; hp.H = H; hp.r_lo = r_lo;
     for (int i = 0; i < 32; ++i) hp.thr[i] = (i < H) ? h_thresholds[i] : INFINITY;
     hp.cands = d_cands; hp.capacity = capacity; hp.count = d_count;
-    CU(launch_harmonic(plan->info.precision == FDAS_BF16_PLANE16, hp, (cudaStream_t)cuda_stream));
-    plan->launches += 1;
+    hp.maxplane = plan->d_maxplane; hp.mpitch = plan->info.nbins / 8;
+    hp.maybe = plan->d_maybe; hp.maybe_capacity = kMaybeCapacity; hp.maybe_count = plan->d_maybe_count;
+    // M describes the plane fdas_convolve_plane last wrote; any other plane gets its own M first
+    const bool build_max = (plan->max_valid_for != d_plane);
+    int nl = 0;
+    CU(launch_harmonic(plan->info.precision == FDAS_BF16_PLANE16, build_max, hp, (cudaStream_t)cuda_stream, &nl));
+    if (build_max && nl > 0) plan->max_valid_for = d_plane;
+    plan->launches += nl;
     return FDAS_OK;
 }
 
@@ -285,6 +304,13 @@ int fdas_thresholds_from_sigma(int H, double nsigma, float* h_thresholds_out) {
 int fdas_plan_templates_host(fdas_plan_t plan, double* h_out) {
     if (!plan || !h_out) return FDAS_EARG;
     std::memcpy(h_out, plan->bank_time.data(), plan->bank_time.size() * sizeof(cd));
+    return FDAS_OK;
+}
+
+int fdas_plan_debug_maxplane(fdas_plan_t plan, const float** d_out, int64_t* pitch_out) {
+    if (!plan || !d_out || !pitch_out) return FDAS_EARG;
+    *d_out = plan->d_maxplane;
+    *pitch_out = plan->info.nbins / 8;
     return FDAS_OK;
 }
 

@@ -34,6 +34,38 @@ __device__ __forceinline__ void ifft2048(float2 (&x)[16], float2* X1, float2* X2
     pass3(x, tw2);
 }
 
+
+// Epilogue of one (segment, template): thread t holds y[2t + e + 256 q] in x[e*8 + q].  Writes the
+// powers of the valid samples with streaming stores and, for K3's prefilter, the maximum of every
+// aligned block of 8 plane columns (= 4 consecutive lanes) of the values AS STORED.
+template <int PREC>
+__device__ __forceinline__ void store_powers(const float2 (&x)[16], const ConvParams& p, const int j,
+                                             const int64_t sV, const int nvalid, const int tid) {
+    float* mrow = p.maxplane + (size_t)j * p.mpitch + ((sV + 2 * tid) >> 3);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        float p0 = x[q].x * x[q].x + x[q].y * x[q].y;
+        float p1 = x[8 + q].x * x[8 + q].x + x[8 + q].y * x[8 + q].y;
+        const bool ok = 2 * tid + 256 * q < nvalid;
+        if (PREC == FDAS_BF16_PLANE16) {
+            const __nv_bfloat162 pk = __floats2bfloat162_rn(p0, p1);
+            if (ok) {
+                __nv_bfloat16* row = reinterpret_cast<__nv_bfloat16*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
+                __stcs(reinterpret_cast<unsigned int*>(row + 256 * q), *reinterpret_cast<const unsigned int*>(&pk));
+            }
+            p0 = __low2float(pk);
+            p1 = __high2float(pk);
+        } else if (ok) {
+            float* row = reinterpret_cast<float*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
+            __stcs(reinterpret_cast<float2*>(row + 256 * q), make_float2(p0, p1));
+        }
+        float m = fmaxf(p0, p1);
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+        if (ok && (tid & 3) == 0) mrow[32 * q] = m;
+    }
+}
+
 template <int PREC, int MINB>
 __global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvParams p) {
     __shared__ __align__(16) float2 X1[kXbufElems];
@@ -99,15 +131,7 @@ __global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvPara
                 for (int c = 0; c < 8; ++c) K[c] = __ldg(bank + c * 128);
             }
             ifft2048(x, X1, X2, tid, tw1, tw2);
-            float* row = reinterpret_cast<float*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
-#pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                if (2 * tid + 256 * q < nvalid) {
-                    const float p0 = x[q].x * x[q].x + x[q].y * x[q].y;
-                    const float p1 = x[8 + q].x * x[8 + q].x + x[8 + q].y * x[8 + q].y;
-                    __stcs(reinterpret_cast<float2*>(row + 256 * q), make_float2(p0, p1));
-                }
-            }
+            store_powers<PREC>(x, p, j, sV, nvalid, tid);
         }
     } else {
         const uint4* bank = reinterpret_cast<const uint4*>(p.bank) + (size_t)jbeg * 4 * 128 + tid;
@@ -128,30 +152,7 @@ __global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvPara
                 for (int c = 0; c < 4; ++c) K[c] = __ldg(bank + c * 128);
             }
             ifft2048(x, X1, X2, tid, tw1, tw2);
-            if (PREC == FDAS_BF16) {
-                float* row = reinterpret_cast<float*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    if (2 * tid + 256 * q < nvalid) {
-                        const float p0 = x[q].x * x[q].x + x[q].y * x[q].y;
-                        const float p1 = x[8 + q].x * x[8 + q].x + x[8 + q].y * x[8 + q].y;
-                        __stcs(reinterpret_cast<float2*>(row + 256 * q), make_float2(p0, p1));
-                    }
-                }
-            } else {
-                __nv_bfloat16* row =
-                    reinterpret_cast<__nv_bfloat16*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
-#pragma unroll
-                for (int q = 0; q < 8; ++q) {
-                    if (2 * tid + 256 * q < nvalid) {
-                        const float p0 = x[q].x * x[q].x + x[q].y * x[q].y;
-                        const float p1 = x[8 + q].x * x[8 + q].x + x[8 + q].y * x[8 + q].y;
-                        const __nv_bfloat162 pk = __floats2bfloat162_rn(p0, p1);
-                        __stcs(reinterpret_cast<unsigned int*>(row + 256 * q),
-                               *reinterpret_cast<const unsigned int*>(&pk));
-                    }
-                }
-            }
+            store_powers<PREC>(x, p, j, sV, nvalid, tid);
         }
     }
 }

@@ -16,6 +16,8 @@ struct ConvParams {
     int64_t nbins;
     int64_t pitch;
     int nz, h, V;
+    float* maxplane;     // nz x mpitch: max of every aligned block of 8 plane columns (as stored)
+    int64_t mpitch;      // nbins / 8
 };
 
 // K2: one CTA of 128 threads per (segment, template chunk); grid = (nseg, nsplit).
@@ -43,9 +45,15 @@ struct HarmParams {
     float thr[32];
     fdas_cand_t* cands;
     int64_t capacity;
-    unsigned long long* count;
+    unsigned long long* count;        // caller's: true number of candidates
+    float* maxplane;                  // plan-owned block-max plane, nz x mpitch
+    int64_t mpitch;                   // nbins / 8
+    uint2* maybe;                     // plan-owned list of (r, j) that failed the prefilter
+    int64_t maybe_capacity;
+    unsigned long long* maybe_count;  // plan-owned
 };
-// K3: harmonic sums, thresholds, warp-aggregated compaction.  One launch (+ a memset of *count).
-cudaError_t launch_harmonic(int plane_is_bf16, const HarmParams& p, cudaStream_t st);
+// K3: [build_max] + prefilter (pass A) + exact (pass B); `launches` receives the kernels launched.
+cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams& p, cudaStream_t st,
+                            int* launches);
 
 }  // namespace fdas

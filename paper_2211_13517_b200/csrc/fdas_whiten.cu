@@ -1,6 +1,6 @@
 // fdas_whiten.cu -- K1, running-median power whitening (BASELINE.json north_star; DESIGN.md step a2,
 // reading A3).
-//   K1a  one CTA per block of the A3 schedule: |X|^2 into shared memory, bitonic sort, exact median
+//   K1a  one CTA per block of the A3 schedule: |X|^2 in registers, exact median by radix selection
 //        (even count: mean of the two middle values)
 //   K1b  per bin: linear interpolation of the block medians between block centres (constant outside
 //        the first/last centre), w[k] = X[k] sqrt(ln2 / m(k)), w[0] = 0, stored fp32 or bf16 (RNE)
@@ -10,38 +10,87 @@
 
 namespace fdas {
 
-constexpr int kMedThreads = 1024;
+constexpr int kMedThreads = 256;
 constexpr int kMedMax = 4096;
+constexpr int kMedPer = kMedMax / kMedThreads;  // powers held in registers per thread
 
+// Exact order statistics by radix selection on the bit patterns of the (non-negative) powers:
+// four 8-bit passes, each a shared-memory histogram of the keys that still match the selected
+// prefix, then the bin holding rank k.  The second middle value (even count) is either the same
+// key (duplicates) or the smallest key above it.
 __global__ void __launch_bounds__(kMedThreads) block_median_kernel(const WhitenParams p) {
-    __shared__ float v[kMedMax];
+    __shared__ unsigned hist[256];
+    __shared__ unsigned sel_bin, sel_below, s_cnt_le, s_min_gt;
     const int b = blockIdx.x;
     const int start = p.blk_start[b], n = p.blk_len[b];
-    int npad = 1;
-    while (npad < n) npad <<= 1;
-    for (int i = threadIdx.x; i < npad; i += kMedThreads) {
-        float pw = __int_as_float(0x7f800000);  // +inf padding sorts to the end
+    unsigned key[kMedPer];
+#pragma unroll
+    for (int q = 0; q < kMedPer; ++q) {
+        const int i = threadIdx.x + q * kMedThreads;
+        key[q] = 0xffffffffu;
         if (i < n) {
             const float2 x = __ldg(p.X + start + i);
-            pw = x.x * x.x + x.y * x.y;
+            key[q] = __float_as_uint(x.x * x.x + x.y * x.y);
         }
-        v[i] = pw;
     }
-    __syncthreads();
-    for (int k = 2; k <= npad; k <<= 1) {
-        for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int i = threadIdx.x; i < npad; i += kMedThreads) {
-                const int ixj = i ^ j;
-                if (ixj > i) {
-                    const float a = v[i], c = v[ixj];
-                    const bool up = ((i & k) == 0);
-                    if ((a > c) == up) { v[i] = c; v[ixj] = a; }
+    unsigned k = (unsigned)((n - 1) / 2);  // 0-based rank of the lower middle value
+    unsigned prefix = 0u, mask = 0u;
+    for (int shift = 24; shift >= 0; shift -= 8) {
+        hist[threadIdx.x] = 0u;  // kMedThreads == 256 bins
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < kMedPer; ++q) {
+            const int i = threadIdx.x + q * kMedThreads;
+            if (i < n && (key[q] & mask) == prefix) atomicAdd(&hist[(key[q] >> shift) & 255u], 1u);
+        }
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            unsigned c[8], local = 0u;
+#pragma unroll
+            for (int t = 0; t < 8; ++t) { c[t] = hist[threadIdx.x * 8 + t]; local += c[t]; }
+            unsigned incl = local;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned v = __shfl_up_sync(0xffffffffu, incl, d);
+                if (threadIdx.x >= d) incl += v;
+            }
+            unsigned below = incl - local;  // keys in lower bins
+            if (k >= below && k < incl) {   // exactly one lane
+#pragma unroll
+                for (int t = 0; t < 8; ++t) {
+                    if (k < below + c[t]) { sel_bin = threadIdx.x * 8 + t; sel_below = below; break; }
+                    below += c[t];
                 }
             }
-            __syncthreads();
+        }
+        __syncthreads();
+        k -= sel_below;
+        prefix |= sel_bin << shift;
+        mask |= 255u << shift;
+    }
+    // prefix = key of rank (n-1)/2.  Rank n/2: same key if enough keys <= prefix, else the next key up.
+    if (threadIdx.x == 0) { s_cnt_le = 0u; s_min_gt = 0xffffffffu; }
+    __syncthreads();
+    unsigned cnt = 0u, mn = 0xffffffffu;
+#pragma unroll
+    for (int q = 0; q < kMedPer; ++q) {
+        const int i = threadIdx.x + q * kMedThreads;
+        if (i < n) {
+            if (key[q] <= prefix) ++cnt; else mn = min(mn, key[q]);
         }
     }
-    if (threadIdx.x == 0) p.blk_med[b] = 0.5f * (v[(n - 1) / 2] + v[n / 2]);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        cnt += __shfl_xor_sync(0xffffffffu, cnt, d);
+        mn = min(mn, __shfl_xor_sync(0xffffffffu, mn, d));
+    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&s_cnt_le, cnt); atomicMin(&s_min_gt, mn); }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned hi_rank = (unsigned)(n / 2);
+        const unsigned hi_key = (s_cnt_le > hi_rank) ? prefix : s_min_gt;
+        p.blk_med[b] = 0.5f * (__uint_as_float(prefix) + __uint_as_float(hi_key));
+    }
 }
 
 template <bool BF16>

@@ -23,7 +23,7 @@ FDAS_OK, FDAS_EARG, FDAS_EALLOC, FDAS_ECUDA, FDAS_ECUFFT, FDAS_EOVERFLOW, FDAS_E
 EXPORTS = (
     "fdas_plan", "fdas_plan_info", "fdas_prepare_spectrum", "fdas_convolve_plane",
     "fdas_harmonic_sum_peaks", "fdas_search_host", "fdas_thresholds_from_sigma",
-    "fdas_plan_templates_host", "fdas_plan_launch_count", "fdas_destroy", "fdas_strerror",
+    "fdas_plan_templates_host", "fdas_plan_debug_maxplane", "fdas_plan_launch_count", "fdas_destroy", "fdas_strerror",
     "fdas_last_error_detail",
 )
 
@@ -63,6 +63,7 @@ def _load():
     L.fdas_search_host.argtypes = [vp, vp, ci, C.POINTER(C.c_float), i64, vp, i64, C.POINTER(i64), vp]
     L.fdas_thresholds_from_sigma.argtypes = [ci, dbl, C.POINTER(C.c_float)]
     L.fdas_plan_templates_host.argtypes = [vp, vp]
+    L.fdas_plan_debug_maxplane.argtypes = [vp, C.POINTER(vp), C.POINTER(i64)]
     L.fdas_plan_launch_count.argtypes = [vp]
     L.fdas_plan_launch_count.restype = i64
     L.fdas_destroy.argtypes = [vp]
@@ -197,6 +198,12 @@ class Plan:
         out = np.empty((self.info.nz, taps), dtype=np.complex128)
         _check(_lib.fdas_plan_templates_host(self._h, out.ctypes.data), "fdas_plan_templates_host")
         return out
+
+    def debug_maxplane(self):
+        """(device pointer, pitch) of the plan-owned block-maximum plane (diagnostic)."""
+        ptr, pitch = C.c_void_p(), C.c_int64()
+        _check(_lib.fdas_plan_debug_maxplane(self._h, C.byref(ptr), C.byref(pitch)), "fdas_plan_debug_maxplane")
+        return int(ptr.value), int(pitch.value)
 
     def launch_count(self) -> int:
         return int(_lib.fdas_plan_launch_count(self._h))

@@ -87,7 +87,7 @@ def test_tiny_fp32_full_parity(fdas, torch_, oracle):
     assert res.count == len(res.cands) and stats["common"] >= 1
     keys = set(gpu_cand_dict(res.cands))
     assert (20000, 23, 1) in keys or (20000, 24, 1) in keys     # the injected signal (z0 = 7.5)
-    assert plan.launch_count() == 4
+    assert plan.launch_count() == 5
 
 
 # ------------------------------------------------------------------------------------ configs[1]
@@ -335,3 +335,42 @@ def test_ska_full_size_sampled_parity(fdas, torch_, oracle, precision):
                 assert key not in gd, key
     assert found >= 2          # both injected fundamentals
     print(precision, "sampled worst/max", worst / pmax, "pmax", pmax, "cands", res.count, "found", found)
+
+
+# ---------------------------------------------- K2's block-max side plane and the K3 prefilter
+@pytest.mark.parametrize("precision", ["fp32", "bf16_plane16"])
+def test_blockmax_plane_and_prefilter_equivalence(fdas, torch_, precision):
+    """M[j][b] written by K2 equals the maximum of the 8 stored plane values of block b exactly, and
+    the branch-and-bound search gives the same candidates whether M comes from K2 or is rebuilt from
+    a copy of the plane."""
+    torch = torch_
+    wl = inputs.medium()
+    x = inputs.series_for(wl)
+    plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, precision)
+    d_spec, d_plane = plan.alloc_spec(), plan.alloc_plane()
+    plan.prepare_spectrum(torch.from_numpy(x).cuda(), d_spec)
+    plan.convolve_plane(d_spec, d_plane)
+    torch.cuda.synchronize()
+    ptr, pitch = plan.debug_maxplane()
+    nz, nb = plan.info.nz, plan.info.nbins
+    assert pitch == nb // 8
+    M = _device_view(torch, ptr, nz * pitch).view(nz, pitch).clone()
+    ref = d_plane.float().view(nz, pitch, 8).amax(dim=2)
+    assert torch.equal(M, ref)
+    H = wl.nharm
+    thr = fdas.thresholds_from_sigma(H, 4.0)      # lower threshold: more work for the exact pass
+    d_c, d_n = plan.alloc_cands(1 << 18)
+    plan.harmonic_sum_peaks(d_plane, H, thr, wl.r_lo, d_c, d_n)
+    a = plan.read_cands(d_c, d_n)
+    clone = d_plane.clone()
+    plan.harmonic_sum_peaks(clone, H, thr, wl.r_lo, d_c, d_n)
+    b = plan.read_cands(d_c, d_n)
+    assert a.count == b.count and a.count > 1000
+    assert gpu_cand_dict(a.cands) == gpu_cand_dict(b.cands)
+
+
+def _device_view(torch, ptr, numel):
+    """float32 tensor aliasing `numel` floats of device memory at `ptr` (no copy)."""
+    class _Iface:
+        __cuda_array_interface__ = {"shape": (numel,), "typestr": "<f4", "data": (ptr, False), "version": 3}
+    return torch.as_tensor(_Iface(), device="cuda")
