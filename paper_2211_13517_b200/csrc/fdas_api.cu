@@ -68,7 +68,7 @@ struct fdas_plan_s {
         }                                                                               \
     } while (0)
 
-static const int64_t kMaybeCapacity = 1 << 22;  // K3 prefilter survivors listed per call (more: evaluated in place)
+static const int64_t kMaybeCapacity = 1 << 22;  // K3 prefilter survivors (blocks of 8 fundamentals) listed per call
 
 static void free_plan(fdas_plan_s* p) {
     if (!p) return;
@@ -147,7 +147,7 @@ static int build_plan(fdas_plan_s* p) {
 
     CU(cudaMalloc(&p->d_maxplane, (size_t)in.nz * (size_t)(in.nbins / 8) * sizeof(float)));
     CU(cudaMalloc(&p->d_maybe, (size_t)kMaybeCapacity * sizeof(uint2)));
-    CU(cudaMalloc(&p->d_maybe_count, sizeof(unsigned long long)));
+    CU(cudaMalloc(&p->d_maybe_count, 2 * sizeof(unsigned long long)));
     CU(cudaMalloc(&p->d_X, (size_t)(in.nfft / 2 + 1) * sizeof(float2)));
     size_t ws = 0;
     CF(cufftCreate(&p->fft));
@@ -246,6 +246,7 @@ int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const 
     hp.cands = d_cands; hp.capacity = capacity; hp.count = d_count;
     hp.maxplane = plan->d_maxplane; hp.mpitch = plan->info.nbins / 8;
     hp.maybe = plan->d_maybe; hp.maybe_capacity = kMaybeCapacity; hp.maybe_count = plan->d_maybe_count;
+    hp.overflow = reinterpret_cast<unsigned*>(plan->d_maybe_count + 1);
     // M describes the plane fdas_convolve_plane last wrote; any other plane gets its own M first
     const bool build_max = (plan->max_valid_for != d_plane);
     int nl = 0;

@@ -21,17 +21,39 @@ namespace fdas {
 
 constexpr int kDefaultOcc = 3;  // resident CTAs per SM the kernel is compiled for (FDAS_K2_OCC=3|4 overrides)
 
-__device__ __forceinline__ void ifft2048(float2 (&x)[16], float2* X1, float2* X2, const int tid,
-                                         const float2 (&tw1)[15], const float2 (&tw2)[7]) {
+// First half of the inverse FFT: up to the write of exchange 2 (x is dead afterwards).
+__device__ __forceinline__ void ifft2048_head(float2 (&x)[16], float2* X1, float2* X2, const int tid,
+                                              const float2 (&tw1)[15]) {
     pass1(x, tw1);
     x1_store(X1, tid, x);
     __syncthreads();
     xrow_load(X1, tid, x);
     pass2(x);
     x2_store(X2, tid, x);
+}
+// Second half: barrier, read of exchange 2, last pass.
+__device__ __forceinline__ void ifft2048_tail(float2 (&x)[16], const float2* X2, const int tid,
+                                              const float2 (&tw2)[7]) {
     __syncthreads();
     xrow_load(X2, tid, x);
     pass3(x, tw2);
+}
+__device__ __forceinline__ void ifft2048(float2 (&x)[16], float2* X1, float2* X2, const int tid,
+                                         const float2 (&tw1)[15], const float2 (&tw2)[7]) {
+    ifft2048_head(x, X1, X2, tid, tw1);
+    ifft2048_tail(x, X2, tid, tw2);
+}
+
+// 128-bit read-only loads of the next template, issued as volatile asm between the exchange-2
+// stores and the barrier (where the 32 x registers are dead): the compiler can neither sink them to
+// the point of use nor hoist them into the register-heavy passes, so the L2 latency is hidden by
+// pass 3 and the epilogue at the cost of 16 (bf16) / 32 (fp32) registers over that span only.
+__device__ __forceinline__ uint4 ldg_nc_v4(const void* ptr) {
+    uint4 v;
+    // plain ld.global (not .nc): a non-coherent load may legally be moved across bar.sync
+    asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(ptr) : "memory");
+    return v;
 }
 
 
@@ -115,29 +137,30 @@ __global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvPara
     const int nvalid = (int)min((int64_t)p.V, p.nbins - sV);
 
     if (PREC == FDAS_FP32) {
-        const float4* bank = reinterpret_cast<const float4*>(p.bank) + (size_t)jbeg * 8 * 128 + tid;
-        float4 K[8];
+        const uint4* bank = reinterpret_cast<const uint4*>(p.bank) + (size_t)jbeg * 8 * 128 + tid;
+        uint4 K[8];
 #pragma unroll
-        for (int c = 0; c < 8; ++c) K[c] = __ldg(bank + c * 128);
+        for (int c = 0; c < 8; ++c) K[c] = ldg_nc_v4(bank + c * 128);
         for (int j = jbeg; j < jend; ++j) {
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
-                x[2 * c] = cmul(S[2 * c], make_float2(K[c].x, K[c].y));
-                x[2 * c + 1] = cmul(S[2 * c + 1], make_float2(K[c].z, K[c].w));
+                x[2 * c] = cmul(S[2 * c], make_float2(__uint_as_float(K[c].x), __uint_as_float(K[c].y)));
+                x[2 * c + 1] = cmul(S[2 * c + 1], make_float2(__uint_as_float(K[c].z), __uint_as_float(K[c].w)));
             }
+            ifft2048_head(x, X1, X2, tid, tw1);
             bank += 8 * 128;
             if (j + 1 < jend) {
 #pragma unroll
-                for (int c = 0; c < 8; ++c) K[c] = __ldg(bank + c * 128);
+                for (int c = 0; c < 8; ++c) K[c] = ldg_nc_v4(bank + c * 128);
             }
-            ifft2048(x, X1, X2, tid, tw1, tw2);
+            ifft2048_tail(x, X2, tid, tw2);
             store_powers<PREC>(x, p, j, sV, nvalid, tid);
         }
     } else {
         const uint4* bank = reinterpret_cast<const uint4*>(p.bank) + (size_t)jbeg * 4 * 128 + tid;
         uint4 K[4];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) K[c] = __ldg(bank + c * 128);
+        for (int c = 0; c < 4; ++c) K[c] = ldg_nc_v4(bank + c * 128);
         for (int j = jbeg; j < jend; ++j) {
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
@@ -146,12 +169,13 @@ __global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvPara
                 x[4 * c + 2] = cmul(S[4 * c + 2], unpack_bf16x2(K[c].z));
                 x[4 * c + 3] = cmul(S[4 * c + 3], unpack_bf16x2(K[c].w));
             }
+            ifft2048_head(x, X1, X2, tid, tw1);
             bank += 4 * 128;
             if (j + 1 < jend) {
 #pragma unroll
-                for (int c = 0; c < 4; ++c) K[c] = __ldg(bank + c * 128);
+                for (int c = 0; c < 4; ++c) K[c] = ldg_nc_v4(bank + c * 128);
             }
-            ifft2048(x, X1, X2, tid, tw1, tw2);
+            ifft2048_tail(x, X2, tid, tw2);
             store_powers<PREC>(x, p, j, sV, nvalid, tid);
         }
     }

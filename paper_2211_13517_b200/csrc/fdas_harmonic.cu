@@ -9,10 +9,10 @@
 // writes beside the plane (1/8 of its size):
 //   pass A (prefilter)  U_h(r,j) = sum_{k<=h} M[row_k][(k r) >> 3] >= S_h(r,j) term by term, in the
 //                       same summation order, and fp32 addition is monotone -- so U_h <= T_h for all
-//                       h proves that (r, j) has no candidate without touching the plane.  The few
-//                       fundamentals that fail the test go to a "maybe" list.
-//   pass B (exact)      one thread per maybe entry: the plain definition above on the real plane,
-//                       thresholds, local-maximum attribute, atomic slot claim.
+//                       h proves that (r, j) has no candidate without touching the plane.  Blocks of
+//                       8 fundamentals in which some bound fails go to a "maybe" list.
+//   pass B (exact)      one thread per listed fundamental: the plain definition above on the real
+//                       plane, thresholds, local-maximum attribute, atomic slot claim.
 // Results are identical to evaluating every fundamental exactly.  When the plane was not produced by
 // fdas_convolve_plane of this plan (hand-made planes), M is first rebuilt from it (build_max_kernel).
 #include <cuda_bf16.h>
@@ -22,9 +22,7 @@
 namespace fdas {
 
 constexpr int kHarmThreads = 256;
-constexpr int kRpt = 4;
-constexpr int kTile = kHarmThreads * kRpt;
-constexpr int kExactBlocks = 592;
+constexpr int kExactBlocks = 148 * 16;
 
 template <typename T> __device__ __forceinline__ float ldp(const T* p);
 template <> __device__ __forceinline__ float ldp<float>(const float* p) { return __ldg(p); }
@@ -112,70 +110,90 @@ __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
     p.maxplane[(size_t)j * p.mpitch + b] = m;
 }
 
-// ---- pass A: upper bounds from the block-max plane.  A CTA owns one row j and a tile of kTile
-// fundamentals; thread t handles r = tile + t + 256 i, so the row arithmetic is CTA-uniform and the
-// lanes of a warp read runs of (32 k)/8 consecutive elements of M.
-template <typename T>
-__global__ void __launch_bounds__(kHarmThreads) prefilter_kernel(const HarmParams p) {
-    __shared__ float sthr[32];   // thresholds for the (rare) out-of-line exact path
-    if (threadIdx.x < 32) sthr[threadIdx.x] = p.thr[threadIdx.x];
-    __syncthreads();
-    const int j = blockIdx.y;
-    const int c2 = p.nz - 1;
-    const int64_t rb = (int64_t)blockIdx.x * kTile + threadIdx.x;
-    const int64_t last = p.nbins - 1;
-    float U[kRpt];
-    bool flagged[kRpt];
+// ---- pass A: upper bounds from the block-max plane.  Thread <-> one block B of 8 consecutive
+// fundamentals r = 8B + i of row j (CTA = 256 blocks of one row), so harmonic k needs the min(k, 8)
+// elements M[row_k][kB + ((k i) >> 3)]: with k unrolled every index is a compile-time offset and the
+// whole test costs one FADD + one FSETP per (fundamental, harmonic).  A block with any U_h > T_h is
+// appended to the maybe list as (B, j).
+template <int K>
+__device__ __forceinline__ void prefilter_step(const float* __restrict__ mrow, const unsigned B,
+                                               const float thr, const int nv, float (&U)[8], bool& any) {
+    const float* src = mrow + (size_t)K * B;
+    constexpr int NL = K < 8 ? K : 8;
+    float m[NL];
+    if (nv == 8) {
 #pragma unroll
-    for (int i = 0; i < kRpt; ++i) { U[i] = 0.f; flagged[i] = false; }
-
-    for (int k = 1; k <= p.H; ++k) {
-        const int v2 = 2 * k * j - (k - 1) * c2;          // CTA-uniform
-        if (v2 < 0 || v2 > 2 * c2) break;
-        if ((int64_t)k * ((int64_t)blockIdx.x * kTile) > last) break;   // whole tile beyond Nb/k
-        const int row = min((v2 + 1) >> 1, c2);
-        const float* __restrict__ mrow = p.maxplane + (size_t)row * p.mpitch;
-        const float thr = p.thr[k - 1];
-        float v[kRpt];
+        for (int q = 0; q < NL; ++q) m[q] = __ldg(src + (K <= 8 ? q : ((K * q) >> 3)));
 #pragma unroll
-        for (int i = 0; i < kRpt; ++i) {
-            const int64_t c = (int64_t)k * (rb + 256 * i);
-            v[i] = (c <= last) ? __ldg(mrow + (c >> 3)) : 0.f;
+        for (int i = 0; i < 8; ++i) {
+            U[i] += m[K <= 8 ? ((K * i) >> 3) : i];
+            any = any || (U[i] > thr);
         }
+    } else {   // the one block per row that straddles r = (Nb-1)/K
 #pragma unroll
-        for (int i = 0; i < kRpt; ++i) {
-            const int64_t c = (int64_t)k * (rb + 256 * i);
-            U[i] += v[i];
-            flagged[i] = flagged[i] || (c <= last && U[i] > thr);
-        }
-    }
-#pragma unroll
-    for (int i = 0; i < kRpt; ++i) {
-        const int64_t r = rb + 256 * i;
-        if (flagged[i] && r >= p.r_lo) {
-            const unsigned long long slot = atomicAdd(p.maybe_count, 1ULL);
-            if (slot < (unsigned long long)p.maybe_capacity) {
-                p.maybe[slot] = make_uint2((unsigned)r, (unsigned)j);
-            } else {   // list full: evaluate here so that nothing is ever dropped
-                exact_fundamental(reinterpret_cast<const T*>(p.plane), geom_of(p), sthr, r, j);
+        for (int i = 0; i < 8; ++i) {
+            if (i < nv) {
+                U[i] += __ldg(src + ((K * i) >> 3));
+                any = any || (U[i] > thr);
             }
         }
     }
 }
 
-// ---- pass B: one thread per maybe entry.
+template <int K>
+__device__ __forceinline__ void prefilter_from(const HarmParams& p, const int j, const int c2,
+                                               const unsigned B, float (&U)[8], bool& any) {
+    if constexpr (K <= 32) {
+        if (K > p.H) return;
+        const int v2 = 2 * K * j - (K - 1) * c2;          // CTA-uniform
+        if (v2 < 0 || v2 > 2 * c2) return;
+        const unsigned rmax = (unsigned)((p.nbins - 1) / K);   // last fundamental with harmonic K inside
+        if (8u * (blockIdx.x * (unsigned)kHarmThreads) > rmax) return;   // whole CTA beyond Nb/K
+        const int row = min((v2 + 1) >> 1, c2);
+        const int nv = (8u * B > rmax) ? 0 : (int)min(8u, rmax - 8u * B + 1u);
+        if (nv > 0) prefilter_step<K>(p.maxplane + (size_t)row * p.mpitch, B, p.thr[K - 1], nv, U, any);
+        prefilter_from<K + 1>(p, j, c2, B, U, any);
+    }
+}
+
+__global__ void __launch_bounds__(kHarmThreads) prefilter_kernel(const HarmParams p) {
+    const int j = blockIdx.y;
+    const unsigned B = blockIdx.x * (unsigned)kHarmThreads + threadIdx.x;
+    if ((int64_t)B >= p.mpitch) return;
+    float U[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) U[i] = 0.f;
+    bool any = false;
+    prefilter_from<1>(p, j, p.nz - 1, B, U, any);
+    if (any && (int64_t)(8u * B + 7u) >= p.r_lo) {
+        const unsigned long long slot = atomicAdd(p.maybe_count, 1ULL);
+        if (slot < (unsigned long long)p.maybe_capacity) p.maybe[slot] = make_uint2(B, (unsigned)j);
+        else atomicExch(p.overflow, 1u);   // handled by pass B (falls back to the full scan)
+    }
+}
+
+// ---- pass B: 8 lanes per maybe record (B, j), lane i evaluates r = 8B + i by the plain definition.
+// If the maybe list overflowed (pathological thresholds), every fundamental is evaluated instead.
 template <typename T>
 __global__ void __launch_bounds__(128) exact_kernel(const HarmParams p) {
     __shared__ float sthr[32];
     if (threadIdx.x < 32) sthr[threadIdx.x] = p.thr[threadIdx.x];
     __syncthreads();
     const T* P = reinterpret_cast<const T*>(p.plane);
-    const unsigned long long n = min(*p.maybe_count, (unsigned long long)p.maybe_capacity);
     const HarmGeom g = geom_of(p);
-    for (unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; q < n;
-         q += (unsigned long long)gridDim.x * blockDim.x) {
-        const uint2 rec = p.maybe[q];
-        exact_fundamental(P, g, sthr, (int64_t)rec.x, (int)rec.y);
+    const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned long long nthr = (unsigned long long)gridDim.x * blockDim.x;
+    if (*p.overflow == 0u) {
+        const unsigned long long n = *p.maybe_count * 8ULL;
+        for (unsigned long long q = tid; q < n; q += nthr) {
+            const uint2 rec = p.maybe[q >> 3];
+            exact_fundamental(P, g, sthr, (int64_t)rec.x * 8 + (int64_t)(q & 7), (int)rec.y);
+        }
+    } else {
+        const unsigned long long n = (unsigned long long)p.nbins * (unsigned long long)p.nz;
+        for (unsigned long long q = tid; q < n; q += nthr)
+            exact_fundamental(P, g, sthr, (int64_t)(q % (unsigned long long)p.nbins),
+                              (int)(q / (unsigned long long)p.nbins));
     }
 }
 
@@ -184,7 +202,7 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
     *launches = 0;
     cudaError_t e = cudaMemsetAsync(p.count, 0, sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(p.maybe_count, 0, sizeof(unsigned long long), st);
+    e = cudaMemsetAsync(p.maybe_count, 0, 2 * sizeof(unsigned long long), st);   // + overflow flag
     if (e != cudaSuccess) return e;
     if (p.r_lo >= p.nbins) return cudaSuccess;
     if (build_max) {
@@ -194,9 +212,8 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
     }
-    dim3 grid((unsigned)((p.nbins + kTile - 1) / kTile), (unsigned)p.nz), block(kHarmThreads);
-    if (plane_is_bf16) prefilter_kernel<__nv_bfloat16><<<grid, block, 0, st>>>(p);
-    else prefilter_kernel<float><<<grid, block, 0, st>>>(p);
+    dim3 grid((unsigned)((p.mpitch + kHarmThreads - 1) / kHarmThreads), (unsigned)p.nz), block(kHarmThreads);
+    prefilter_kernel<<<grid, block, 0, st>>>(p);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     ++*launches;
     if (plane_is_bf16) exact_kernel<__nv_bfloat16><<<kExactBlocks, 128, 0, st>>>(p);
