@@ -68,7 +68,7 @@ struct fdas_plan_s {
         }                                                                               \
     } while (0)
 
-static const int64_t kMaybeCapacity = 1 << 22;  // K3 prefilter survivors (blocks of 8 fundamentals) listed per call
+static const int64_t kMaybeCapacity = 1 << 22;  // K3 prefilter survivors (fundamentals) listed per call
 
 static void free_plan(fdas_plan_s* p) {
     if (!p) return;

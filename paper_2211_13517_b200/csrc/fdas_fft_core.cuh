@@ -42,6 +42,29 @@ FDAS_HD void bfly4_inv(float2& x0, float2& x1, float2& x2, float2& x3) {
     x3 = csub(t1, t3);
 }
 
+// Same butterfly with x1 = R*u1 and x3 = R*u3 still unscaled: the 1/sqrt2 of the w8-type twiddles
+// is folded into the final adds (FMAs), saving the four multiplies.
+FDAS_HD void bfly4_inv_s13(float2& x0, float2& u1, float2& x2, float2& u3, const float R) {
+    float2 t0 = cadd(x0, x2), t1 = csub(x0, x2), w = cadd(u1, u3), v = cmul_i(csub(u1, u3));
+    x0 = make_float2(fmaf(R, w.x, t0.x), fmaf(R, w.y, t0.y));
+    u1 = make_float2(fmaf(R, v.x, t1.x), fmaf(R, v.y, t1.y));
+    x2 = make_float2(fmaf(-R, w.x, t0.x), fmaf(-R, w.y, t0.y));
+    u3 = make_float2(fmaf(-R, v.x, t1.x), fmaf(-R, v.y, t1.y));
+}
+// ... and with only x2 = R*u2 unscaled.
+FDAS_HD void bfly4_inv_s2(float2& x0, float2& x1, float2& u2, float2& x3, const float R) {
+    float2 t0 = make_float2(fmaf(R, u2.x, x0.x), fmaf(R, u2.y, x0.y));
+    float2 t1 = make_float2(fmaf(-R, u2.x, x0.x), fmaf(-R, u2.y, x0.y));
+    float2 t2 = cadd(x1, x3), t3 = cmul_i(csub(x1, x3));
+    x0 = cadd(t0, t2);
+    x1 = cadd(t1, t3);
+    u2 = csub(t0, t2);
+    x3 = csub(t1, t3);
+}
+// (a + ib)(1 + i) and (a + ib)(-1 + i): the w8-type twiddles without their 1/sqrt2.
+FDAS_HD float2 rot45(float2 a) { return make_float2(a.x - a.y, a.x + a.y); }
+FDAS_HD float2 rot135(float2 a) { return make_float2(-a.x - a.y, a.x - a.y); }
+
 // 16-point inverse DFT, natural order in and out: x[n] <- sum_k x[k] exp(+2 pi i n k / 16).
 // k = b + 4a, n = d + 4c: radix-4 over a, twiddle w16^(b d), radix-4 over b.
 FDAS_HD void dft16_inv(float2 (&x)[16]) {
@@ -50,20 +73,20 @@ FDAS_HD void dft16_inv(float2 (&x)[16]) {
     const float R = 0.70710678118654752440f;   // sqrt(1/2)
 #pragma unroll
     for (int b = 0; b < 4; ++b) bfly4_inv(x[b], x[b + 4], x[b + 8], x[b + 12]);  // -> E_b[d] at x[b+4d]
-    // b = 1: d = 1,2,3 -> w16^1, w16^2, w16^3
-    x[1 + 4] = cmul(x[1 + 4], make_float2(C1, S1));
-    x[1 + 8] = make_float2((x[1 + 8].x - x[1 + 8].y) * R, (x[1 + 8].x + x[1 + 8].y) * R);
-    x[1 + 12] = cmul(x[1 + 12], make_float2(S1, C1));
-    // b = 2: w16^2, w16^4 = i, w16^6
-    x[2 + 4] = make_float2((x[2 + 4].x - x[2 + 4].y) * R, (x[2 + 4].x + x[2 + 4].y) * R);
-    x[2 + 8] = cmul_i(x[2 + 8]);
-    x[2 + 12] = make_float2((-x[2 + 12].x - x[2 + 12].y) * R, (x[2 + 12].x - x[2 + 12].y) * R);
-    // b = 3: w16^3, w16^6, w16^9 = -w16^1
-    x[3 + 4] = cmul(x[3 + 4], make_float2(S1, C1));
-    x[3 + 8] = make_float2((-x[3 + 8].x - x[3 + 8].y) * R, (x[3 + 8].x - x[3 + 8].y) * R);
-    x[3 + 12] = cmul(x[3 + 12], make_float2(-C1, -S1));
-#pragma unroll
-    for (int d = 0; d < 4; ++d) bfly4_inv(x[4 * d], x[4 * d + 1], x[4 * d + 2], x[4 * d + 3]);  // F_d[c] at x[c+4d]
+    // twiddles w16^(b d); the four of w8 type (b d = 2 or 6) keep their 1/sqrt2 for the next stage
+    x[1 + 4] = cmul(x[1 + 4], make_float2(C1, S1));      // b=1 d=1: w16^1
+    x[1 + 8] = rot45(x[1 + 8]);                          // b=1 d=2: w16^2 (x R later)
+    x[1 + 12] = cmul(x[1 + 12], make_float2(S1, C1));    // b=1 d=3: w16^3
+    x[2 + 4] = rot45(x[2 + 4]);                          // b=2 d=1: w16^2 (x R later)
+    x[2 + 8] = cmul_i(x[2 + 8]);                         // b=2 d=2: w16^4 = i
+    x[2 + 12] = rot135(x[2 + 12]);                       // b=2 d=3: w16^6 (x R later)
+    x[3 + 4] = cmul(x[3 + 4], make_float2(S1, C1));      // b=3 d=1: w16^3
+    x[3 + 8] = rot135(x[3 + 8]);                         // b=3 d=2: w16^6 (x R later)
+    x[3 + 12] = cmul(x[3 + 12], make_float2(-C1, -S1));  // b=3 d=3: w16^9 = -w16^1
+    bfly4_inv(x[0], x[1], x[2], x[3]);                   // d = 0: F_0[c] at x[c]
+    bfly4_inv_s2(x[4], x[5], x[6], x[7], R);             // d = 1: b = 2 unscaled
+    bfly4_inv_s13(x[8], x[9], x[10], x[11], R);          // d = 2: b = 1, 3 unscaled
+    bfly4_inv_s2(x[12], x[13], x[14], x[15], R);         // d = 3: b = 2 unscaled
     float2 y[16];
 #pragma unroll
     for (int d = 0; d < 4; ++d)
@@ -82,12 +105,12 @@ FDAS_HD void dft8_inv(float2 (&x)[16], const int o) {
         x[o + b] = s;        // E_b[0]
         x[o + b + 4] = t;    // E_b[1]
     }
-    // twiddle w8^(b) on E_b[1]: b = 1 -> (1+i)/sqrt2, b = 2 -> i, b = 3 -> (-1+i)/sqrt2
-    x[o + 5] = make_float2((x[o + 5].x - x[o + 5].y) * R, (x[o + 5].x + x[o + 5].y) * R);
+    // twiddle w8^(b) on E_b[1]: b = 1 -> (1+i)/sqrt2, b = 2 -> i, b = 3 -> (-1+i)/sqrt2 (R folded below)
+    x[o + 5] = rot45(x[o + 5]);
     x[o + 6] = cmul_i(x[o + 6]);
-    x[o + 7] = make_float2((-x[o + 7].x - x[o + 7].y) * R, (x[o + 7].x - x[o + 7].y) * R);
-    bfly4_inv(x[o + 0], x[o + 1], x[o + 2], x[o + 3]);  // d = 0: F_0[c] at x[o+c]
-    bfly4_inv(x[o + 4], x[o + 5], x[o + 6], x[o + 7]);  // d = 1: F_1[c] at x[o+4+c]
+    x[o + 7] = rot135(x[o + 7]);
+    bfly4_inv(x[o + 0], x[o + 1], x[o + 2], x[o + 3]);          // d = 0: F_0[c] at x[o+c]
+    bfly4_inv_s13(x[o + 4], x[o + 5], x[o + 6], x[o + 7], R);   // d = 1: F_1[c] at x[o+4+c]
     float2 y[8];
 #pragma unroll
     for (int d = 0; d < 2; ++d)

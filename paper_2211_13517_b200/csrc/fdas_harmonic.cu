@@ -9,10 +9,11 @@
 // writes beside the plane (1/8 of its size):
 //   pass A (prefilter)  U_h(r,j) = sum_{k<=h} M[row_k][(k r) >> 3] >= S_h(r,j) term by term, in the
 //                       same summation order, and fp32 addition is monotone -- so U_h <= T_h for all
-//                       h proves that (r, j) has no candidate without touching the plane.  Blocks of
-//                       8 fundamentals in which some bound fails go to a "maybe" list.
+//                       h proves that (r, j) has no candidate without touching the plane.  The few
+//                       fundamentals for which some bound fails go to a "maybe" list.
 //   pass B (exact)      one thread per listed fundamental: the plain definition above on the real
-//                       plane, thresholds, local-maximum attribute, atomic slot claim.
+//                       plane, thresholds, atomic slot claim.
+//   pass C (flags)      one thread per (stored candidate, neighbour): local-maximum attribute.
 // Results are identical to evaluating every fundamental exactly.  When the plane was not produced by
 // fdas_convolve_plane of this plan (hand-made planes), M is first rebuilt from it (build_max_kernel).
 #include <cuda_bf16.h>
@@ -21,8 +22,8 @@
 
 namespace fdas {
 
-constexpr int kHarmThreads = 256;
 constexpr int kExactBlocks = 148 * 16;
+constexpr int kFlagBlocks = 148 * 4;
 
 template <typename T> __device__ __forceinline__ float ldp(const T* p);
 template <> __device__ __forceinline__ float ldp<float>(const float* p) { return __ldg(p); }
@@ -46,54 +47,77 @@ __device__ __forceinline__ HarmGeom geom_of(const HarmParams& p) {
     return g;
 }
 
-// S_h at (r, j) if defined (r in [r_lo, Nb), all h harmonics inside the plane); summed k = 1..h.
+// S_h at (r, j) if defined (r in [r_lo, Nb), all h harmonics inside the plane); summed k = 1..h,
+// the gathers issued eight at a time.
 template <typename T>
 __device__ bool harmonic_sum_at(const T* P, const HarmGeom& g, int64_t r, int j, int h, float* out) {
     if (j < 0 || j >= g.nz || r < g.r_lo || r >= g.nbins) return false;
     const int c2 = g.nz - 1;
+    {   // validity is monotone in k: test the deepest harmonic only
+        const int v2 = 2 * h * j - (h - 1) * c2;
+        if (v2 < 0 || v2 > 2 * c2 || (int64_t)h * r > g.nbins - 1) return false;
+    }
     float S = 0.f;
-    for (int k = 1; k <= h; ++k) {
-        const int v2 = 2 * k * j - (k - 1) * c2;
-        if (v2 < 0 || v2 > 2 * c2 || (int64_t)k * r > g.nbins - 1) return false;
-        const int row = min((v2 + 1) >> 1, c2);
-        S += ldp(P + (size_t)row * g.pitch + (size_t)k * r);
+    for (int k0 = 1; k0 <= h; k0 += 8) {
+        float v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int k = k0 + q;
+            v[q] = 0.f;
+            if (k <= h) {
+                const int row = min((2 * k * j - (k - 1) * c2 + 1) >> 1, c2);
+                v[q] = ldp(P + (size_t)row * g.pitch + (size_t)k * r);
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+            if (k0 + q <= h) S += v[q];
     }
     *out = S;
     return true;
 }
 
-// The plain definition for one fundamental: all h, thresholds, local-maximum attribute (8 neighbours
-// for which S_h is defined; strict against those preceding (j, r) lexicographically), slot claim.
+// The plain definition for one fundamental: all h, thresholds, slot claim.  The gathers of 8
+// harmonics are issued together (independent addresses); sums stay in k order.
 template <typename T>
 __device__ __noinline__ void exact_fundamental(const T* P, const HarmGeom g, const float* thr,
                                                int64_t r, int j) {
     if (r < g.r_lo || r >= g.nbins) return;
     const int c2 = g.nz - 1;
-    float S = 0.f;
+    int hmax = 0;   // number of defined harmonics
     for (int h = 1; h <= g.H; ++h) {
         const int v2 = 2 * h * j - (h - 1) * c2;
         if (v2 < 0 || v2 > 2 * c2 || (int64_t)h * r > g.nbins - 1) break;
-        const int row = min((v2 + 1) >> 1, c2);
-        S += ldp(P + (size_t)row * g.pitch + (size_t)h * r);
-        if (!(S > thr[h - 1])) continue;
-        const unsigned long long slot = atomicAdd(g.count, 1ULL);   // the true count
-        if ((int64_t)slot >= g.capacity) continue;
-        unsigned flag = 1;
-        for (int dj = -1; dj <= 1 && flag; ++dj)
-            for (int dr = -1; dr <= 1 && flag; ++dr) {
-                if (dj == 0 && dr == 0) continue;
-                float nv;
-                if (!harmonic_sum_at(P, g, r + dr, j + dj, h, &nv)) continue;
-                const bool precedes = (dj < 0) || (dj == 0 && dr < 0);
-                if (precedes ? !(S > nv) : !(S >= nv)) flag = 0;
+        hmax = h;
+    }
+    float S = 0.f;
+    for (int h0 = 1; h0 <= hmax; h0 += 8) {
+        float v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int h = h0 + q;
+            v[q] = 0.f;
+            if (h <= hmax) {
+                const int row = min((2 * h * j - (h - 1) * c2 + 1) >> 1, c2);
+                v[q] = ldp(P + (size_t)row * g.pitch + (size_t)h * r);
             }
-        fdas_cand_t c;
-        c.r = (uint32_t)r;
-        c.zidx = (int16_t)j;
-        c.h = (uint16_t)h;
-        c.power = S;
-        c.flags = flag;
-        g.cands[slot] = c;
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int h = h0 + q;
+            if (h > hmax) break;
+            S += v[q];
+            if (!(S > thr[h - 1])) continue;
+            const unsigned long long slot = atomicAdd(g.count, 1ULL);   // the true count
+            if ((int64_t)slot >= g.capacity) continue;
+            fdas_cand_t c;
+            c.r = (uint32_t)r;
+            c.zidx = (int16_t)j;
+            c.h = (uint16_t)h;
+            c.power = S;
+            c.flags = 1u;   // local-maximum attribute: cleared by flag_kernel if a neighbour beats it
+            g.cands[slot] = c;
+        }
     }
 }
 
@@ -110,69 +134,159 @@ __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
     p.maxplane[(size_t)j * p.mpitch + b] = m;
 }
 
-// ---- pass A: upper bounds from the block-max plane.  Thread <-> one block B of 8 consecutive
-// fundamentals r = 8B + i of row j (CTA = 256 blocks of one row), so harmonic k needs the min(k, 8)
-// elements M[row_k][kB + ((k i) >> 3)]: with k unrolled every index is a compile-time offset and the
-// whole test costs one FADD + one FSETP per (fundamental, harmonic).  A block with any U_h > T_h is
-// appended to the maybe list as (B, j).
-template <int K>
-__device__ __forceinline__ void prefilter_step(const float* __restrict__ mrow, const unsigned B,
-                                               const float thr, const int nv, float (&U)[8], bool& any) {
-    const float* src = mrow + (size_t)K * B;
-    constexpr int NL = K < 8 ? K : 8;
-    float m[NL];
-    if (nv == 8) {
+// ---- pass A: upper bounds from the block-max plane.
+// Thread <-> 4 consecutive blocks of M = 32 consecutive fundamentals r = 32 Q + i of row j, so that
+// harmonic k <= 8 is k contiguous 128-bit loads (M[row_k][4kQ .. 4kQ+4k-1]) and every fundamental
+// picks element (k i) >> 3 of them -- a compile-time register choice once k and i are unrolled.  The
+// loads of harmonics 1..4 (then 5-6, 7-8, then one harmonic at a time) are all issued before the
+// first add: the kernel moves < 1 GB and would otherwise be bound by DRAM latency, not bandwidth.
+// One FADD, one FSETP and one predicated OR per (fundamental, harmonic); fundamentals with any
+// U_h > T_h go to the maybe list as (r, j).
+constexpr int kPfThreads = 128;
+
+// Harmonic K for the 32 fundamentals of quad-block Q, all of them valid (K (32Q+31) <= Nb-1).
+template <int K, int NV>
+__device__ __forceinline__ void pf_load(const float* __restrict__ mrow, const unsigned Q, const bool on,
+                                        float (&m)[NV]) {
+    if constexpr (K <= 8) {
+        static_assert(NV == 4 * K, "k <= 8 loads 4k contiguous elements");
+        const float4* src = reinterpret_cast<const float4*>(mrow + (size_t)4 * K * Q);
 #pragma unroll
-        for (int q = 0; q < NL; ++q) m[q] = __ldg(src + (K <= 8 ? q : ((K * q) >> 3)));
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            U[i] += m[K <= 8 ? ((K * i) >> 3) : i];
-            any = any || (U[i] > thr);
+        for (int q = 0; q < K; ++q) {
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (on) v = __ldg(src + q);
+            m[4 * q] = v.x; m[4 * q + 1] = v.y; m[4 * q + 2] = v.z; m[4 * q + 3] = v.w;
         }
-    } else {   // the one block per row that straddles r = (Nb-1)/K
+    } else {
+        static_assert(NV == 32, "k > 8 gathers one element per fundamental");
+        const float* src = mrow + (size_t)4 * K * Q;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
+        for (int i = 0; i < 32; ++i) m[i] = on ? __ldg(src + ((K * i) >> 3)) : 0.f;
+    }
+}
+
+template <int K, int NV>
+__device__ __forceinline__ void pf_add(const float (&m)[NV], const float thr, const bool on,
+                                       float (&U)[32], unsigned& flagged) {
+    if (on) {
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+            U[i] += m[K <= 8 ? ((K * i) >> 3) : i];
+            if (U[i] > thr) flagged |= 1u << i;
+        }
+    }
+}
+
+struct PfRow { const float* mrow; float thr; };
+
+__device__ __forceinline__ PfRow pf_row(const HarmParams& p, const int j, const int k) {
+    const int c2 = p.nz - 1;
+    const int v2 = 2 * k * j - (k - 1) * c2;   // only called for k <= hz: v2 is in range
+    PfRow r;
+    r.mrow = p.maxplane + (size_t)min((v2 + 1) >> 1, c2) * p.mpitch;
+    r.thr = p.thr[k - 1];
+    return r;
+}
+
+template <int K>
+__device__ __forceinline__ void pf_single_from(const HarmParams& p, const int j, const unsigned Q,
+                                               const int he_max, const int he, float (&U)[32],
+                                               unsigned& flagged) {
+    if constexpr (K <= 32) {
+        if (K > he_max) return;                 // CTA-uniform: no thread of this CTA goes deeper
+        const PfRow r = pf_row(p, j, K);
+        float m[K <= 8 ? 4 * K : 32];
+        pf_load<K>(r.mrow, Q, he >= K, m);
+        pf_add<K>(m, r.thr, he >= K, U, flagged);
+        pf_single_from<K + 1>(p, j, Q, he_max, he, U, flagged);
+    }
+}
+
+__global__ void __launch_bounds__(kPfThreads) prefilter_kernel(const HarmParams p) {
+    const int j = blockIdx.y;
+    const int c2 = p.nz - 1;
+    const unsigned Q0 = blockIdx.x * (unsigned)kPfThreads;
+    const unsigned Q = Q0 + threadIdx.x;
+    const unsigned nquad = (unsigned)(p.mpitch >> 2);   // nbins / 32
+    if (Q >= nquad) return;
+    const unsigned last = (unsigned)(p.nbins - 1);
+    // hz: harmonics inside the plane in z for this row (CTA-uniform, monotone in k)
+    int hz = 0;
+    for (int k = 1; k <= p.H; ++k) {
+        const int v2 = 2 * k * j - (k - 1) * c2;
+        if (v2 < 0 || v2 > 2 * c2) break;
+        hz = k;
+    }
+    // he: harmonics for which all 32 fundamentals of this thread are inside the plane in r
+    const int he = (int)min((unsigned)hz, last / (32u * Q + 31u));
+    const int he_max = (int)min((unsigned)hz, last / (32u * Q0 + 31u));   // deepest in this CTA
+    float U[32];
+    unsigned flagged = 0u;   // bit i: some U_h of fundamental 32 Q + i exceeds T_h
+#pragma unroll
+    for (int i = 0; i < 32; ++i) U[i] = 0.f;
+
+    {   // harmonics 1..4: ten 128-bit loads in flight
+        const PfRow r1 = pf_row(p, j, 1);
+        float m1[4], m2[8], m3[12], m4[16];
+        pf_load<1>(r1.mrow, Q, true, m1);
+        PfRow r2 = r1, r3 = r1, r4 = r1;
+        if (he_max >= 2) { r2 = pf_row(p, j, 2); pf_load<2>(r2.mrow, Q, he >= 2, m2); }
+        if (he_max >= 3) { r3 = pf_row(p, j, 3); pf_load<3>(r3.mrow, Q, he >= 3, m3); }
+        if (he_max >= 4) { r4 = pf_row(p, j, 4); pf_load<4>(r4.mrow, Q, he >= 4, m4); }
+        pf_add<1>(m1, r1.thr, true, U, flagged);
+        if (he_max >= 2) pf_add<2>(m2, r2.thr, he >= 2, U, flagged);
+        if (he_max >= 3) pf_add<3>(m3, r3.thr, he >= 3, U, flagged);
+        if (he_max >= 4) pf_add<4>(m4, r4.thr, he >= 4, U, flagged);
+    }
+    if (he_max >= 5) {   // harmonics 5, 6: eleven loads in flight
+        const PfRow r5 = pf_row(p, j, 5);
+        float m5[20], m6[24];
+        pf_load<5>(r5.mrow, Q, he >= 5, m5);
+        PfRow r6 = r5;
+        if (he_max >= 6) { r6 = pf_row(p, j, 6); pf_load<6>(r6.mrow, Q, he >= 6, m6); }
+        pf_add<5>(m5, r5.thr, he >= 5, U, flagged);
+        if (he_max >= 6) pf_add<6>(m6, r6.thr, he >= 6, U, flagged);
+    }
+    pf_single_from<7>(p, j, Q, he_max, he, U, flagged);
+
+    // the (at most a few) harmonics for which only some of the 32 fundamentals are inside the plane
+    for (int k = he + 1; k <= hz; ++k) {
+        const unsigned rmax = last / (unsigned)k;
+        if (32u * Q > rmax) break;
+        const int nv = (int)min(32u, rmax - 32u * Q + 1u);
+        const PfRow r = pf_row(p, j, k);
+        const float* src = r.mrow + (size_t)k * 4 * Q;
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
             if (i < nv) {
-                U[i] += __ldg(src + ((K * i) >> 3));
-                any = any || (U[i] > thr);
+                U[i] += __ldg(src + ((k * i) >> 3));
+                if (U[i] > r.thr) flagged |= 1u << i;
             }
         }
     }
-}
 
-template <int K>
-__device__ __forceinline__ void prefilter_from(const HarmParams& p, const int j, const int c2,
-                                               const unsigned B, float (&U)[8], bool& any) {
-    if constexpr (K <= 32) {
-        if (K > p.H) return;
-        const int v2 = 2 * K * j - (K - 1) * c2;          // CTA-uniform
-        if (v2 < 0 || v2 > 2 * c2) return;
-        const unsigned rmax = (unsigned)((p.nbins - 1) / K);   // last fundamental with harmonic K inside
-        if (8u * (blockIdx.x * (unsigned)kHarmThreads) > rmax) return;   // whole CTA beyond Nb/K
-        const int row = min((v2 + 1) >> 1, c2);
-        const int nv = (8u * B > rmax) ? 0 : (int)min(8u, rmax - 8u * B + 1u);
-        if (nv > 0) prefilter_step<K>(p.maxplane + (size_t)row * p.mpitch, B, p.thr[K - 1], nv, U, any);
-        prefilter_from<K + 1>(p, j, c2, B, U, any);
+    // r < r_lo never yields candidates
+    if (32 * (int64_t)Q < p.r_lo) {
+        const int64_t cut = p.r_lo - 32 * (int64_t)Q;
+        flagged = (cut >= 32) ? 0u : (flagged & ~((1u << (int)cut) - 1u));
+    }
+    if (flagged) {
+        const int n = __popc(flagged);
+        const unsigned long long base = atomicAdd(p.maybe_count, (unsigned long long)n);
+        if (base + (unsigned long long)n <= (unsigned long long)p.maybe_capacity) {
+            unsigned long long slot = base;
+            while (flagged) {
+                const int i = __ffs(flagged) - 1;
+                flagged &= flagged - 1;
+                p.maybe[slot++] = make_uint2(32u * Q + (unsigned)i, (unsigned)j);
+            }
+        } else {
+            atomicExch(p.overflow, 1u);   // pass B then falls back to the full scan
+        }
     }
 }
 
-__global__ void __launch_bounds__(kHarmThreads) prefilter_kernel(const HarmParams p) {
-    const int j = blockIdx.y;
-    const unsigned B = blockIdx.x * (unsigned)kHarmThreads + threadIdx.x;
-    if ((int64_t)B >= p.mpitch) return;
-    float U[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) U[i] = 0.f;
-    bool any = false;
-    prefilter_from<1>(p, j, p.nz - 1, B, U, any);
-    if (any && (int64_t)(8u * B + 7u) >= p.r_lo) {
-        const unsigned long long slot = atomicAdd(p.maybe_count, 1ULL);
-        if (slot < (unsigned long long)p.maybe_capacity) p.maybe[slot] = make_uint2(B, (unsigned)j);
-        else atomicExch(p.overflow, 1u);   // handled by pass B (falls back to the full scan)
-    }
-}
-
-// ---- pass B: 8 lanes per maybe record (B, j), lane i evaluates r = 8B + i by the plain definition.
+// ---- pass B: one thread per maybe record (r, j): the plain definition on the real plane.
 // If the maybe list overflowed (pathological thresholds), every fundamental is evaluated instead.
 template <typename T>
 __global__ void __launch_bounds__(128) exact_kernel(const HarmParams p) {
@@ -184,16 +298,38 @@ __global__ void __launch_bounds__(128) exact_kernel(const HarmParams p) {
     const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
     const unsigned long long nthr = (unsigned long long)gridDim.x * blockDim.x;
     if (*p.overflow == 0u) {
-        const unsigned long long n = *p.maybe_count * 8ULL;
+        const unsigned long long n = *p.maybe_count;
         for (unsigned long long q = tid; q < n; q += nthr) {
-            const uint2 rec = p.maybe[q >> 3];
-            exact_fundamental(P, g, sthr, (int64_t)rec.x * 8 + (int64_t)(q & 7), (int)rec.y);
+            const uint2 rec = p.maybe[q];
+            exact_fundamental(P, g, sthr, (int64_t)rec.x, (int)rec.y);
         }
     } else {
         const unsigned long long n = (unsigned long long)p.nbins * (unsigned long long)p.nz;
         for (unsigned long long q = tid; q < n; q += nthr)
             exact_fundamental(P, g, sthr, (int64_t)(q % (unsigned long long)p.nbins),
                               (int)(q / (unsigned long long)p.nbins));
+    }
+}
+
+// ---- pass C: local-maximum attribute, one thread per (stored candidate, neighbour): the flag is
+// cleared unless S_h(r,j) >= S_h at the neighbour (r+dr, j+dj) where that is defined, strictly >
+// for the neighbours that precede (j, r) lexicographically (reading A14).
+template <typename T>
+__global__ void __launch_bounds__(128) flag_kernel(const HarmParams p) {
+    const T* P = reinterpret_cast<const T*>(p.plane);
+    const HarmGeom g = geom_of(p);
+    const unsigned long long stored = min(*p.count, (unsigned long long)p.capacity);
+    const unsigned long long n = stored * 8ULL;
+    for (unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; q < n;
+         q += (unsigned long long)gridDim.x * blockDim.x) {
+        const fdas_cand_t c = p.cands[q >> 3];
+        const int nb = (int)(q & 7);
+        const int idx = nb < 4 ? nb : nb + 1;          // skip the centre of the 3 x 3 stencil
+        const int dj = idx / 3 - 1, dr = idx % 3 - 1;
+        float nv;
+        if (!harmonic_sum_at(P, g, (int64_t)c.r + dr, (int)c.zidx + dj, (int)c.h, &nv)) continue;
+        const bool precedes = (dj < 0) || (dj == 0 && dr < 0);
+        if (precedes ? !(c.power > nv) : !(c.power >= nv)) atomicAnd(&p.cands[q >> 3].flags, ~1u);
     }
 }
 
@@ -212,7 +348,7 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
     }
-    dim3 grid((unsigned)((p.mpitch + kHarmThreads - 1) / kHarmThreads), (unsigned)p.nz), block(kHarmThreads);
+    dim3 grid((unsigned)((p.mpitch / 4 + kPfThreads - 1) / kPfThreads), (unsigned)p.nz), block(kPfThreads);
     prefilter_kernel<<<grid, block, 0, st>>>(p);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     ++*launches;
@@ -220,6 +356,12 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
     else exact_kernel<float><<<kExactBlocks, 128, 0, st>>>(p);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     ++*launches;
+    if (p.capacity > 0) {
+        if (plane_is_bf16) flag_kernel<__nv_bfloat16><<<kFlagBlocks, 128, 0, st>>>(p);
+        else flag_kernel<float><<<kFlagBlocks, 128, 0, st>>>(p);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        ++*launches;
+    }
     return cudaSuccess;
 }
 

@@ -48,12 +48,13 @@ struct HarmParams {
     unsigned long long* count;        // caller's: true number of candidates
     float* maxplane;                  // plan-owned block-max plane, nz x mpitch
     int64_t mpitch;                   // nbins / 8
-    uint2* maybe;                     // plan-owned list of (B, j): blocks of 8 fundamentals that failed the prefilter
+    uint2* maybe;                     // plan-owned list of (r, j): fundamentals that failed the prefilter
     int64_t maybe_capacity;
     unsigned long long* maybe_count;  // plan-owned; followed by the overflow flag
     unsigned* overflow;               // plan-owned: set if the maybe list was too small
 };
-// K3: [build_max] + prefilter (pass A) + exact (pass B); `launches` receives the kernels launched.
+// K3: [build_max] + prefilter (pass A) + exact (pass B) + flags (pass C); `launches` receives the
+// number of kernels launched.
 cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams& p, cudaStream_t st,
                             int* launches);
 
