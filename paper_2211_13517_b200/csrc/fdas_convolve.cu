@@ -19,7 +19,13 @@
 
 namespace fdas {
 
-constexpr int kDefaultOcc = 3;  // resident CTAs per SM the kernel is compiled for (FDAS_K2_OCC=3|4 overrides)
+constexpr int kDefaultOcc = 3;
+// Where the next template is prefetched: 0 = between the exchange-2 stores and their barrier (the x
+// registers are dead there), 1 = after pass 3 (keeps the 16/32 K registers out of pass 3).
+#ifndef FDAS_K2_PREFETCH_AT
+#define FDAS_K2_PREFETCH_AT 1
+#endif
+constexpr int kPrefetchAt = FDAS_K2_PREFETCH_AT;  // resident CTAs per SM the kernel is compiled for (FDAS_K2_OCC=3|4 overrides)
 
 // First half of the inverse FFT: up to the write of exchange 2 (x is dead afterwards).
 __device__ __forceinline__ void ifft2048_head(float2 (&x)[16], float2* X1, float2* X2, const int tid,
@@ -48,7 +54,7 @@ __device__ __forceinline__ void ifft2048(float2 (&x)[16], float2* X1, float2* X2
 // stores and the barrier (where the 32 x registers are dead): the compiler can neither sink them to
 // the point of use nor hoist them into the register-heavy passes, so the L2 latency is hidden by
 // pass 3 and the epilogue at the cost of 16 (bf16) / 32 (fp32) registers over that span only.
-__device__ __forceinline__ uint4 ldg_nc_v4(const void* ptr) {
+__device__ __forceinline__ uint4 ldg_v4(const void* ptr) {
     uint4 v;
     // plain ld.global (not .nc): a non-coherent load may legally be moved across bar.sync
     asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];"
@@ -57,35 +63,41 @@ __device__ __forceinline__ uint4 ldg_nc_v4(const void* ptr) {
 }
 
 
+// S K for a stored template value (fp32 pair, or bf16 re in the low half and im in the high half).
+__device__ __forceinline__ float2 cmul_k32(float2 s, unsigned kx, unsigned ky) {
+    return cmul(s, make_float2(__uint_as_float(kx), __uint_as_float(ky)));
+}
+__device__ __forceinline__ float2 cmul_k16(float2 s, unsigned v) {
+    return cmul(s, make_float2(__uint_as_float(v << 16), __uint_as_float(v & 0xffff0000u)));
+}
+
 // Epilogue of one (segment, template): thread t holds y[2t + e + 256 q] in x[e*8 + q].  Writes the
 // powers of the valid samples with streaming stores and, for K3's prefilter, the maximum of every
-// aligned block of 8 plane columns (= 4 consecutive lanes) of the values AS STORED.
+// aligned block of 8 plane columns (= 4 consecutive lanes) of the values AS STORED.  `prow` / `mrow`
+// already point at this thread's first column of row j, so every store has an immediate offset;
+// q < qmax <=> the sample is valid (r < Nb and t < V), q < qmax_m <=> this lane also writes the max.
 template <int PREC>
-__device__ __forceinline__ void store_powers(const float2 (&x)[16], const ConvParams& p, const int j,
-                                             const int64_t sV, const int nvalid, const int tid) {
-    float* mrow = p.maxplane + (size_t)j * p.mpitch + ((sV + 2 * tid) >> 3);
+__device__ __forceinline__ void store_powers(const float2 (&x)[16], void* prow, float* mrow,
+                                             const int qmax, const int qmax_m) {
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
-        float p0 = x[q].x * x[q].x + x[q].y * x[q].y;
-        float p1 = x[8 + q].x * x[8 + q].x + x[8 + q].y * x[8 + q].y;
-        const bool ok = 2 * tid + 256 * q < nvalid;
+        float p0 = fmaf(x[q].x, x[q].x, x[q].y * x[q].y);
+        float p1 = fmaf(x[8 + q].x, x[8 + q].x, x[8 + q].y * x[8 + q].y);
         if (PREC == FDAS_BF16_PLANE16) {
             const __nv_bfloat162 pk = __floats2bfloat162_rn(p0, p1);
-            if (ok) {
-                __nv_bfloat16* row = reinterpret_cast<__nv_bfloat16*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
-                __stcs(reinterpret_cast<unsigned int*>(row + 256 * q), *reinterpret_cast<const unsigned int*>(&pk));
-            }
+            if (q < qmax)
+                __stcs(reinterpret_cast<unsigned int*>(reinterpret_cast<__nv_bfloat16*>(prow) + 256 * q),
+                       *reinterpret_cast<const unsigned int*>(&pk));
             p0 = __low2float(pk);
             p1 = __high2float(pk);
-        } else if (ok) {
-            float* row = reinterpret_cast<float*>(p.plane) + (size_t)j * p.pitch + sV + 2 * tid;
-            __stcs(reinterpret_cast<float2*>(row + 256 * q), make_float2(p0, p1));
+        } else {
+            if (q < qmax) __stcs(reinterpret_cast<float2*>(reinterpret_cast<float*>(prow) + 256 * q), make_float2(p0, p1));
         }
         // (a REDUX.MAX over 4-lane sub-masks was measured 2.5x slower for the whole kernel)
         float m = fmaxf(p0, p1);
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
         m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
-        if (ok && (tid & 3) == 0) mrow[32 * q] = m;
+        if (q < qmax_m) mrow[32 * q] = m;
     }
 }
 
@@ -136,49 +148,47 @@ __global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvPara
     // ---- template loop
     const int64_t sV = s * p.V;
     const int nvalid = (int)min((int64_t)p.V, p.nbins - sV);
-
-    if (PREC == FDAS_FP32) {
-        const uint4* bank = reinterpret_cast<const uint4*>(p.bank) + (size_t)jbeg * 8 * 128 + tid;
-        uint4 K[8];
+    const int qmax = max(0, min(8, (nvalid - 2 * tid + 255) >> 8));
+    const int qmax_m = (tid & 3) == 0 ? qmax : 0;
+    constexpr int kPlaneElem = (PREC == FDAS_BF16_PLANE16) ? 2 : 4;
+    char* prow = reinterpret_cast<char*>(p.plane) + ((size_t)jbeg * p.pitch + sV + 2 * tid) * kPlaneElem;
+    const size_t prow_step = (size_t)p.pitch * kPlaneElem;
+    float* mrow = p.maxplane + (size_t)jbeg * p.mpitch + ((sV + 2 * tid) >> 3);
+    constexpr int NK = (PREC == FDAS_FP32) ? 8 : 4;    // 128-bit words of one template per thread
+    const uint4* bank = reinterpret_cast<const uint4*>(p.bank) + (size_t)jbeg * NK * 128 + tid;
+    uint4 K[NK];
 #pragma unroll
-        for (int c = 0; c < 8; ++c) K[c] = ldg_nc_v4(bank + c * 128);
-        for (int j = jbeg; j < jend; ++j) {
+    for (int c = 0; c < NK; ++c) K[c] = ldg_v4(bank + c * 128);
+    for (int j = jbeg; j < jend; ++j) {
+        if (PREC == FDAS_FP32) {
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                x[2 * c] = cmul(S[2 * c], make_float2(__uint_as_float(K[c].x), __uint_as_float(K[c].y)));
-                x[2 * c + 1] = cmul(S[2 * c + 1], make_float2(__uint_as_float(K[c].z), __uint_as_float(K[c].w)));
+            for (int c = 0; c < NK; ++c) {
+                x[2 * c] = cmul_k32(S[2 * c], K[c].x, K[c].y);
+                x[2 * c + 1] = cmul_k32(S[2 * c + 1], K[c].z, K[c].w);
             }
-            ifft2048_head(x, X1, X2, tid, tw1);
-            bank += 8 * 128;
-            if (j + 1 < jend) {
+        } else {
 #pragma unroll
-                for (int c = 0; c < 8; ++c) K[c] = ldg_nc_v4(bank + c * 128);
+            for (int c = 0; c < NK; ++c) {
+                x[4 * c + 0] = cmul_k16(S[4 * c + 0], K[c].x);
+                x[4 * c + 1] = cmul_k16(S[4 * c + 1], K[c].y);
+                x[4 * c + 2] = cmul_k16(S[4 * c + 2], K[c].z);
+                x[4 * c + 3] = cmul_k16(S[4 * c + 3], K[c].w);
             }
-            ifft2048_tail(x, X2, tid, tw2);
-            store_powers<PREC>(x, p, j, sV, nvalid, tid);
         }
-    } else {
-        const uint4* bank = reinterpret_cast<const uint4*>(p.bank) + (size_t)jbeg * 4 * 128 + tid;
-        uint4 K[4];
+        ifft2048_head(x, X1, X2, tid, tw1);
+        bank += NK * 128;
+        if (kPrefetchAt == 0 && j + 1 < jend) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) K[c] = ldg_nc_v4(bank + c * 128);
-        for (int j = jbeg; j < jend; ++j) {
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                x[4 * c + 0] = cmul(S[4 * c + 0], unpack_bf16x2(K[c].x));
-                x[4 * c + 1] = cmul(S[4 * c + 1], unpack_bf16x2(K[c].y));
-                x[4 * c + 2] = cmul(S[4 * c + 2], unpack_bf16x2(K[c].z));
-                x[4 * c + 3] = cmul(S[4 * c + 3], unpack_bf16x2(K[c].w));
-            }
-            ifft2048_head(x, X1, X2, tid, tw1);
-            bank += 4 * 128;
-            if (j + 1 < jend) {
-#pragma unroll
-                for (int c = 0; c < 4; ++c) K[c] = ldg_nc_v4(bank + c * 128);
-            }
-            ifft2048_tail(x, X2, tid, tw2);
-            store_powers<PREC>(x, p, j, sV, nvalid, tid);
+            for (int c = 0; c < NK; ++c) K[c] = ldg_v4(bank + c * 128);
         }
+        ifft2048_tail(x, X2, tid, tw2);
+        if (kPrefetchAt == 1 && j + 1 < jend) {
+#pragma unroll
+            for (int c = 0; c < NK; ++c) K[c] = ldg_v4(bank + c * 128);
+        }
+        store_powers<PREC>(x, prow, mrow, qmax, qmax_m);
+        prow += prow_step;
+        mrow += p.mpitch;
     }
 }
 

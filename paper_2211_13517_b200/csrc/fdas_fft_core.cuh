@@ -25,67 +25,155 @@ constexpr int kPts = 16;        // points per thread
 constexpr int kRowStride = 18;  // float2 per exchange-buffer row: 16 data + 2 pad (144 B: LDS.128 conflict-free)
 constexpr int kXbufElems = kThreads * kRowStride;  // float2 elements per exchange buffer (18,432 B)
 
-FDAS_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-FDAS_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-FDAS_HD float2 cmul(float2 a, float2 b) {
-    return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+// ---- complex arithmetic on (re, im) register pairs.
+// On sm_100a every operation below is ONE packed instruction (FADD2 / FMUL2 / FFMA2, PTX *.f32x2):
+// two IEEE fp32 results per issue slot, rounding identical to the scalar forms.  ptxas folds the
+// mov.b64 pack/unpack of the operands into SASS operand modifiers (.F32 broadcast, .LO_HI swap,
+// per-half negation on FADD2), so multiplying by +-i never costs an instruction.  The host forms
+// (test-only emulator) spell out the same arithmetic.
+#ifdef __CUDA_ARCH__
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk2(float lo, float hi) {
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
 }
+__device__ __forceinline__ float2 up2(u64 v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+__device__ __forceinline__ u64 add2(u64 a, u64 b) {
+    u64 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
+    u64 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
+    u64 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+#endif
+
 FDAS_HD float2 cconj(float2 a) { return make_float2(a.x, -a.y); }
-FDAS_HD float2 cmul_i(float2 a) { return make_float2(-a.y, a.x); }  // a * (+i)
+FDAS_HD float2 cadd(float2 a, float2 b) {   // a + b
+#ifdef __CUDA_ARCH__
+    return up2(add2(pk2(a.x, a.y), pk2(b.x, b.y)));
+#else
+    return make_float2(a.x + b.x, a.y + b.y);
+#endif
+}
+FDAS_HD float2 csub(float2 a, float2 b) {   // a - b
+#ifdef __CUDA_ARCH__
+    return up2(add2(pk2(a.x, a.y), pk2(-b.x, -b.y)));
+#else
+    return make_float2(a.x - b.x, a.y - b.y);
+#endif
+}
+FDAS_HD float2 cadd_i(float2 a, float2 b) {  // a + i b
+#ifdef __CUDA_ARCH__
+    return up2(add2(pk2(a.x, a.y), pk2(-b.y, b.x)));
+#else
+    return make_float2(a.x - b.y, a.y + b.x);
+#endif
+}
+FDAS_HD float2 csub_i(float2 a, float2 b) {  // a - i b
+#ifdef __CUDA_ARCH__
+    return up2(add2(pk2(a.x, a.y), pk2(b.y, -b.x)));
+#else
+    return make_float2(a.x + b.y, a.y - b.x);
+#endif
+}
+FDAS_HD float2 rot45(float2 a) { return cadd_i(a, a); }     // a (1 + i):  sqrt2 w8^1 a
+FDAS_HD float2 rot135(float2 a) {                           // a (-1 + i): sqrt2 w8^3 a
+#ifdef __CUDA_ARCH__
+    return up2(add2(pk2(-a.x, -a.y), pk2(-a.y, a.x)));
+#else
+    return make_float2(-a.x - a.y, a.x - a.y);
+#endif
+}
+FDAS_HD float2 cscale(float2 a, const float r) {            // r a, r real
+#ifdef __CUDA_ARCH__
+    return up2(mul2(pk2(a.x, a.y), pk2(r, r)));
+#else
+    return make_float2(a.x * r, a.y * r);
+#endif
+}
+FDAS_HD float2 caxpy(const float r, float2 a, float2 c) {   // c + r a, r real
+#ifdef __CUDA_ARCH__
+    return up2(fma2(pk2(a.x, a.y), pk2(r, r), pk2(c.x, c.y)));
+#else
+    return make_float2(fmaf(r, a.x, c.x), fmaf(r, a.y, c.y));
+#endif
+}
+FDAS_HD float2 caxpy_i(const float r, float2 a, float2 c) {  // c + r (i a), r real
+#ifdef __CUDA_ARCH__
+    return up2(fma2(pk2(-a.y, a.x), pk2(r, r), pk2(c.x, c.y)));
+#else
+    return make_float2(fmaf(r, -a.y, c.x), fmaf(r, a.x, c.y));
+#endif
+}
+// a w = w.x a + w.y (i a): FMUL2 + FFMA2.  The swapped, half-negated pair (-a.y, a.x) must be the
+// FIRST multiplicand: only operands A and C of FFMA2 take the per-half sign, B takes the broadcast.
+FDAS_HD float2 cmul(float2 a, float2 w) {
+#ifdef __CUDA_ARCH__
+    return up2(fma2(pk2(-a.y, a.x), pk2(w.y, w.y), mul2(pk2(a.x, a.y), pk2(w.x, w.x))));
+#else
+    return make_float2(fmaf(-a.y, w.y, a.x * w.x), fmaf(a.x, w.y, a.y * w.x));
+#endif
+}
 
 // y_d = sum_a x_a (+i)^(a d), in place.
 FDAS_HD void bfly4_inv(float2& x0, float2& x1, float2& x2, float2& x3) {
-    float2 t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), t3 = cmul_i(csub(x1, x3));
+    const float2 t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), d = csub(x1, x3);
     x0 = cadd(t0, t2);
-    x1 = cadd(t1, t3);
+    x1 = cadd_i(t1, d);
     x2 = csub(t0, t2);
-    x3 = csub(t1, t3);
+    x3 = csub_i(t1, d);
 }
-
-// Same butterfly with x1 = R*u1 and x3 = R*u3 still unscaled: the 1/sqrt2 of the w8-type twiddles
-// is folded into the final adds (FMAs), saving the four multiplies.
-FDAS_HD void bfly4_inv_s13(float2& x0, float2& u1, float2& x2, float2& u3, const float R) {
-    float2 t0 = cadd(x0, x2), t1 = csub(x0, x2), w = cadd(u1, u3), v = cmul_i(csub(u1, u3));
-    x0 = make_float2(fmaf(R, w.x, t0.x), fmaf(R, w.y, t0.y));
-    u1 = make_float2(fmaf(R, v.x, t1.x), fmaf(R, v.y, t1.y));
-    x2 = make_float2(fmaf(-R, w.x, t0.x), fmaf(-R, w.y, t0.y));
-    u3 = make_float2(fmaf(-R, v.x, t1.x), fmaf(-R, v.y, t1.y));
-}
-// ... and with only x2 = R*u2 unscaled.
+// Same butterfly with x2 = R u2 still unscaled (the 1/sqrt2 of a w8-type twiddle folded into FMAs).
 FDAS_HD void bfly4_inv_s2(float2& x0, float2& x1, float2& u2, float2& x3, const float R) {
-    float2 t0 = make_float2(fmaf(R, u2.x, x0.x), fmaf(R, u2.y, x0.y));
-    float2 t1 = make_float2(fmaf(-R, u2.x, x0.x), fmaf(-R, u2.y, x0.y));
-    float2 t2 = cadd(x1, x3), t3 = cmul_i(csub(x1, x3));
+    const float2 t0 = caxpy(R, u2, x0), t1 = caxpy(-R, u2, x0), t2 = cadd(x1, x3), d = csub(x1, x3);
     x0 = cadd(t0, t2);
-    x1 = cadd(t1, t3);
+    x1 = cadd_i(t1, d);
     u2 = csub(t0, t2);
-    x3 = csub(t1, t3);
+    x3 = csub_i(t1, d);
 }
-// (a + ib)(1 + i) and (a + ib)(-1 + i): the w8-type twiddles without their 1/sqrt2.
-FDAS_HD float2 rot45(float2 a) { return make_float2(a.x - a.y, a.x + a.y); }
-FDAS_HD float2 rot135(float2 a) { return make_float2(-a.x - a.y, a.x - a.y); }
+// ... with x1 = R u1, x3 = R u3 unscaled and x2 = i v2 (v2 not yet rotated).
+FDAS_HD void bfly4_inv_s13_i2(float2& x0, float2& u1, float2& v2, float2& u3, const float R) {
+    const float2 t0 = cadd_i(x0, v2), t1 = csub_i(x0, v2), w = cadd(u1, u3), d = csub(u1, u3);
+    x0 = caxpy(R, w, t0);
+    u1 = caxpy_i(R, d, t1);
+    v2 = caxpy(-R, w, t0);
+    u3 = caxpy_i(-R, d, t1);
+}
 
 // 16-point inverse DFT, natural order in and out: x[n] <- sum_k x[k] exp(+2 pi i n k / 16).
-// k = b + 4a, n = d + 4c: radix-4 over a, twiddle w16^(b d), radix-4 over b.
+// k = b + 4a, n = d + 4c: radix-4 over a, twiddle w16^(b d), radix-4 over b.  76 packed instructions.
 FDAS_HD void dft16_inv(float2 (&x)[16]) {
     const float C1 = 0.92387953251128673848f;  // cos(pi/8)
     const float S1 = 0.38268343236508978178f;  // sin(pi/8)
     const float R = 0.70710678118654752440f;   // sqrt(1/2)
 #pragma unroll
     for (int b = 0; b < 4; ++b) bfly4_inv(x[b], x[b + 4], x[b + 8], x[b + 12]);  // -> E_b[d] at x[b+4d]
-    // twiddles w16^(b d); the four of w8 type (b d = 2 or 6) keep their 1/sqrt2 for the next stage
+    // twiddles w16^(b d); the w8-type ones (b d = 2 or 6) keep their 1/sqrt2 for the next stage and
+    // w16^4 = i is absorbed by the butterfly of d = 2
     x[1 + 4] = cmul(x[1 + 4], make_float2(C1, S1));      // b=1 d=1: w16^1
     x[1 + 8] = rot45(x[1 + 8]);                          // b=1 d=2: w16^2 (x R later)
     x[1 + 12] = cmul(x[1 + 12], make_float2(S1, C1));    // b=1 d=3: w16^3
     x[2 + 4] = rot45(x[2 + 4]);                          // b=2 d=1: w16^2 (x R later)
-    x[2 + 8] = cmul_i(x[2 + 8]);                         // b=2 d=2: w16^4 = i
     x[2 + 12] = rot135(x[2 + 12]);                       // b=2 d=3: w16^6 (x R later)
     x[3 + 4] = cmul(x[3 + 4], make_float2(S1, C1));      // b=3 d=1: w16^3
     x[3 + 8] = rot135(x[3 + 8]);                         // b=3 d=2: w16^6 (x R later)
     x[3 + 12] = cmul(x[3 + 12], make_float2(-C1, -S1));  // b=3 d=3: w16^9 = -w16^1
     bfly4_inv(x[0], x[1], x[2], x[3]);                   // d = 0: F_0[c] at x[c]
     bfly4_inv_s2(x[4], x[5], x[6], x[7], R);             // d = 1: b = 2 unscaled
-    bfly4_inv_s13(x[8], x[9], x[10], x[11], R);          // d = 2: b = 1, 3 unscaled
+    bfly4_inv_s13_i2(x[8], x[9], x[10], x[11], R);       // d = 2: b = 1, 3 unscaled, b = 2 times i
     bfly4_inv_s2(x[12], x[13], x[14], x[15], R);         // d = 3: b = 2 unscaled
     float2 y[16];
 #pragma unroll
@@ -101,16 +189,15 @@ FDAS_HD void dft8_inv(float2 (&x)[16], const int o) {
     const float R = 0.70710678118654752440f;
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
-        float2 s = cadd(x[o + b], x[o + b + 4]), t = csub(x[o + b], x[o + b + 4]);
+        const float2 s = cadd(x[o + b], x[o + b + 4]), t = csub(x[o + b], x[o + b + 4]);
         x[o + b] = s;        // E_b[0]
         x[o + b + 4] = t;    // E_b[1]
     }
-    // twiddle w8^(b) on E_b[1]: b = 1 -> (1+i)/sqrt2, b = 2 -> i, b = 3 -> (-1+i)/sqrt2 (R folded below)
+    // twiddle w8^(b) on E_b[1]: b = 1 -> (1+i)/sqrt2, b = 2 -> i, b = 3 -> (-1+i)/sqrt2 (R and i folded below)
     x[o + 5] = rot45(x[o + 5]);
-    x[o + 6] = cmul_i(x[o + 6]);
     x[o + 7] = rot135(x[o + 7]);
-    bfly4_inv(x[o + 0], x[o + 1], x[o + 2], x[o + 3]);          // d = 0: F_0[c] at x[o+c]
-    bfly4_inv_s13(x[o + 4], x[o + 5], x[o + 6], x[o + 7], R);   // d = 1: F_1[c] at x[o+4+c]
+    bfly4_inv(x[o + 0], x[o + 1], x[o + 2], x[o + 3]);             // d = 0: F_0[c] at x[o+c]
+    bfly4_inv_s13_i2(x[o + 4], x[o + 5], x[o + 6], x[o + 7], R);   // d = 1: F_1[c] at x[o+4+c]
     float2 y[8];
 #pragma unroll
     for (int d = 0; d < 2; ++d)
