@@ -160,10 +160,11 @@ int fdas_plan_templates_host(fdas_plan_t plan, double* h_out);
 
 /*
  * fdas_plan_debug_maxplane -- diagnostic: device pointer and row pitch (elements) of the plan-owned
- * block-maximum plane M[j][b] = max(P[j][8b..8b+7]) that fdas_convolve_plane writes for the
- * harmonic-sum prefilter.  The buffer stays owned by the plan.
+ * block-maximum plane that fdas_convolve_plane writes for the harmonic-sum prefilter:
+ * M[j][b] = bfloat16 bit pattern of max(P[j][8b..8b+7]) rounded toward +infinity (an upper bound;
+ * the prefilter only needs M >= P).  The buffer stays owned by the plan.
  */
-int fdas_plan_debug_maxplane(fdas_plan_t plan, const float** d_out, int64_t* pitch_out);
+int fdas_plan_debug_maxplane(fdas_plan_t plan, const uint16_t** d_out, int64_t* pitch_out);
 
 /* Number of kernels the library launched on behalf of this plan since it was created. */
 int64_t fdas_plan_launch_count(fdas_plan_t plan);

@@ -43,7 +43,8 @@ def _run(cmd, verbose):
 
 def build_lib(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> str:
     if force or _stale(LIB, LIB_SOURCES):
-        cmd = [NVCC] + ARCH + COMMON + (["-Xptxas", "-v"] if ptxas_v else []) + [
+        extra = os.environ.get("FDAS_NVCC_FLAGS", "").split()   # experiments: -DFDAS_K2_...=n
+        cmd = [NVCC] + ARCH + COMMON + extra + (["-Xptxas", "-v"] if ptxas_v else []) + [
             "-shared", "-o", LIB] + LIB_SOURCES + [
             "-L" + os.path.join(CUDA_HOME, "lib64"), "-lcufft",
             "-Xlinker", "-rpath," + os.path.join(CUDA_HOME, "lib64")]

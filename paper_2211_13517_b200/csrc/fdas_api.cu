@@ -36,7 +36,7 @@ struct fdas_plan_s {
     int nblk = 0;
     int nsplit = 1;
     int64_t launches = 0;
-    float* d_maxplane = nullptr;             // block-max plane M (nz x nbins/8), written by K2
+    unsigned short* d_maxplane = nullptr;    // block-max plane M (nz x nbins/8, bf16 bits), written by K2
     const void* max_valid_for = nullptr;     // the plane M currently describes (nullptr: none)
     uint2* d_maybe = nullptr;                // K3 maybe list (kMaybeCapacity records)
     unsigned long long* d_maybe_count = nullptr;
@@ -145,7 +145,7 @@ static int build_plan(fdas_plan_s* p) {
     CU(cudaMemcpy(p->d_blk_start, bs.data(), bs.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
     CU(cudaMemcpy(p->d_blk_len, bl.data(), bl.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
 
-    CU(cudaMalloc(&p->d_maxplane, (size_t)in.nz * (size_t)(in.nbins / 8) * sizeof(float)));
+    CU(cudaMalloc(&p->d_maxplane, (size_t)in.nz * (size_t)(in.nbins / 8) * sizeof(unsigned short)));
     CU(cudaMalloc(&p->d_maybe, (size_t)kMaybeCapacity * sizeof(uint2)));
     CU(cudaMalloc(&p->d_maybe_count, 2 * sizeof(unsigned long long)));
     CU(cudaMalloc(&p->d_X, (size_t)(in.nfft / 2 + 1) * sizeof(float2)));
@@ -308,7 +308,7 @@ int fdas_plan_templates_host(fdas_plan_t plan, double* h_out) {
     return FDAS_OK;
 }
 
-int fdas_plan_debug_maxplane(fdas_plan_t plan, const float** d_out, int64_t* pitch_out) {
+int fdas_plan_debug_maxplane(fdas_plan_t plan, const uint16_t** d_out, int64_t* pitch_out) {
     if (!plan || !d_out || !pitch_out) return FDAS_EARG;
     *d_out = plan->d_maxplane;
     *pitch_out = plan->info.nbins / 8;

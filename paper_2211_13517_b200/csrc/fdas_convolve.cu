@@ -72,32 +72,43 @@ __device__ __forceinline__ float2 cmul_k16(float2 s, unsigned v) {
 }
 
 // Epilogue of one (segment, template): thread t holds y[2t + e + 256 q] in x[e*8 + q].  Writes the
-// powers of the valid samples with streaming stores and, for K3's prefilter, the maximum of every
-// aligned block of 8 plane columns (= 4 consecutive lanes) of the values AS STORED.  `prow` / `mrow`
-// already point at this thread's first column of row j, so every store has an immediate offset;
-// q < qmax <=> the sample is valid (r < Nb and t < V), q < qmax_m <=> this lane also writes the max.
+// powers of the valid samples with streaming stores and, for K3's prefilter, an upper bound of the
+// maximum of every aligned block of 8 plane columns (= 4 consecutive lanes) of the values AS STORED:
+// bf16 rounded toward +inf (powers are >= 0, so adding 0xffff to the bit pattern and truncating
+// rounds up; for non-negative values the bf16 order is the order of the bit patterns).  Two blocks
+// (q, q+1) share one 32-bit word through the two shuffles.  `prow` / `mrow` already point at this
+// thread's first column of row j, so every store has an immediate offset; q < qmax <=> the sample is
+// valid (r < Nb and t < V), q < qmax_m <=> this lane also writes the block maximum.
 template <int PREC>
-__device__ __forceinline__ void store_powers(const float2 (&x)[16], void* prow, float* mrow,
+__device__ __forceinline__ void store_powers(const float2 (&x)[16], void* prow, unsigned short* mrow,
                                              const int qmax, const int qmax_m) {
 #pragma unroll
-    for (int q = 0; q < 8; ++q) {
-        float p0 = fmaf(x[q].x, x[q].x, x[q].y * x[q].y);
-        float p1 = fmaf(x[8 + q].x, x[8 + q].x, x[8 + q].y * x[8 + q].y);
-        if (PREC == FDAS_BF16_PLANE16) {
-            const __nv_bfloat162 pk = __floats2bfloat162_rn(p0, p1);
-            if (q < qmax)
-                __stcs(reinterpret_cast<unsigned int*>(reinterpret_cast<__nv_bfloat16*>(prow) + 256 * q),
-                       *reinterpret_cast<const unsigned int*>(&pk));
-            p0 = __low2float(pk);
-            p1 = __high2float(pk);
-        } else {
-            if (q < qmax) __stcs(reinterpret_cast<float2*>(reinterpret_cast<float*>(prow) + 256 * q), make_float2(p0, p1));
+    for (int q2 = 0; q2 < 8; q2 += 2) {
+        float mx[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            const int q = q2 + u;
+            float p0 = fmaf(x[q].x, x[q].x, x[q].y * x[q].y);
+            float p1 = fmaf(x[8 + q].x, x[8 + q].x, x[8 + q].y * x[8 + q].y);
+            if (PREC == FDAS_BF16_PLANE16) {
+                const __nv_bfloat162 pk = __floats2bfloat162_rn(p0, p1);
+                if (q < qmax)
+                    __stcs(reinterpret_cast<unsigned int*>(reinterpret_cast<__nv_bfloat16*>(prow) + 256 * q),
+                           *reinterpret_cast<const unsigned int*>(&pk));
+                p0 = __low2float(pk);
+                p1 = __high2float(pk);
+            } else {
+                if (q < qmax)
+                    __stcs(reinterpret_cast<float2*>(reinterpret_cast<float*>(prow) + 256 * q), make_float2(p0, p1));
+            }
+            mx[u] = fmaxf(p0, p1);
         }
-        // (a REDUX.MAX over 4-lane sub-masks was measured 2.5x slower for the whole kernel)
-        float m = fmaxf(p0, p1);
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
-        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
-        if (q < qmax_m) mrow[32 * q] = m;
+        // bytes 2,3 of each rounded-up pattern: low half = block q2, high half = block q2 + 1
+        unsigned w = __byte_perm(__float_as_uint(mx[0]) + 0xffffu, __float_as_uint(mx[1]) + 0xffffu, 0x7632);
+        w = __vmaxu2(w, __shfl_xor_sync(0xffffffffu, w, 1));
+        w = __vmaxu2(w, __shfl_xor_sync(0xffffffffu, w, 2));
+        if (q2 < qmax_m) mrow[32 * q2] = (unsigned short)w;
+        if (q2 + 1 < qmax_m) mrow[32 * (q2 + 1)] = (unsigned short)(w >> 16);
     }
 }
 
@@ -153,7 +164,7 @@ __global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvPara
     constexpr int kPlaneElem = (PREC == FDAS_BF16_PLANE16) ? 2 : 4;
     char* prow = reinterpret_cast<char*>(p.plane) + ((size_t)jbeg * p.pitch + sV + 2 * tid) * kPlaneElem;
     const size_t prow_step = (size_t)p.pitch * kPlaneElem;
-    float* mrow = p.maxplane + (size_t)jbeg * p.mpitch + ((sV + 2 * tid) >> 3);
+    unsigned short* mrow = p.maxplane + (size_t)jbeg * p.mpitch + ((sV + 2 * tid) >> 3);
     constexpr int NK = (PREC == FDAS_FP32) ? 8 : 4;    // 128-bit words of one template per thread
     const uint4* bank = reinterpret_cast<const uint4*>(p.bank) + (size_t)jbeg * NK * 128 + tid;
     uint4 K[NK];

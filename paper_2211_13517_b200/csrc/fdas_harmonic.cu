@@ -5,8 +5,8 @@
 //   (half-integers round away from zero).  A candidate (r, j, h) is emitted for every S_h > T_h.
 //
 // The direct evaluation is HBM-bound: the stride-k gathers touch 3.2x the plane in 32-byte sectors.
-// K3 therefore works branch-and-bound on the block-max plane M[j][b] = max P[j][8b..8b+7] that K2
-// writes beside the plane (1/8 of its size):
+// K3 therefore works branch-and-bound on the block-max plane M[j][b] >= max P[j][8b..8b+7] (bf16, rounded
+// toward +inf) that K2 writes beside the plane (1/16 of its bytes):
 //   pass A (prefilter)  U_h(r,j) = sum_{k<=h} M[row_k][(k r) >> 3] >= S_h(r,j) term by term, in the
 //                       same summation order, and fp32 addition is monotone -- so U_h <= T_h for all
 //                       h proves that (r, j) has no candidate without touching the plane.  The few
@@ -121,6 +121,13 @@ __device__ __noinline__ void exact_fundamental(const T* P, const HarmGeom g, con
     }
 }
 
+// bf16 bit pattern of a non-negative power rounded toward +inf, and back.
+__device__ __forceinline__ unsigned short bf16_up(float v) {
+    return (unsigned short)((__float_as_uint(v) + 0xffffu) >> 16);
+}
+__device__ __forceinline__ float bf16_lo(unsigned w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16_hi(unsigned w) { return __uint_as_float(w & 0xffff0000u); }
+
 // ---- M from an arbitrary plane (only when K2 did not just write it): one thread per block of 8.
 template <typename T>
 __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
@@ -131,7 +138,7 @@ __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
     float m = ldp(src);
 #pragma unroll
     for (int i = 1; i < 8; ++i) m = fmaxf(m, ldp(src + i));
-    p.maxplane[(size_t)j * p.mpitch + b] = m;
+    p.maxplane[(size_t)j * p.mpitch + b] = bf16_up(m);
 }
 
 // ---- pass A: upper bounds from the block-max plane.
@@ -146,22 +153,23 @@ constexpr int kPfThreads = 128;
 
 // Harmonic K for the 32 fundamentals of quad-block Q, all of them valid (K (32Q+31) <= Nb-1).
 template <int K, int NV>
-__device__ __forceinline__ void pf_load(const float* __restrict__ mrow, const unsigned Q, const bool on,
-                                        float (&m)[NV]) {
+__device__ __forceinline__ void pf_load(const unsigned short* __restrict__ mrow, const unsigned Q,
+                                        const bool on, float (&m)[NV]) {
     if constexpr (K <= 8) {
         static_assert(NV == 4 * K, "k <= 8 loads 4k contiguous elements");
-        const float4* src = reinterpret_cast<const float4*>(mrow + (size_t)4 * K * Q);
+        const uint2* src = reinterpret_cast<const uint2*>(mrow + (size_t)4 * K * Q);   // 8K bytes, 8-byte aligned
 #pragma unroll
         for (int q = 0; q < K; ++q) {
-            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            uint2 v = make_uint2(0u, 0u);
             if (on) v = __ldg(src + q);
-            m[4 * q] = v.x; m[4 * q + 1] = v.y; m[4 * q + 2] = v.z; m[4 * q + 3] = v.w;
+            m[4 * q] = bf16_lo(v.x); m[4 * q + 1] = bf16_hi(v.x);
+            m[4 * q + 2] = bf16_lo(v.y); m[4 * q + 3] = bf16_hi(v.y);
         }
     } else {
         static_assert(NV == 32, "k > 8 gathers one element per fundamental");
-        const float* src = mrow + (size_t)4 * K * Q;
+        const unsigned short* src = mrow + (size_t)4 * K * Q;
 #pragma unroll
-        for (int i = 0; i < 32; ++i) m[i] = on ? __ldg(src + ((K * i) >> 3)) : 0.f;
+        for (int i = 0; i < 32; ++i) m[i] = on ? bf16_lo(__ldg(src + ((K * i) >> 3))) : 0.f;
     }
 }
 
@@ -177,7 +185,7 @@ __device__ __forceinline__ void pf_add(const float (&m)[NV], const float thr, co
     }
 }
 
-struct PfRow { const float* mrow; float thr; };
+struct PfRow { const unsigned short* mrow; float thr; };
 
 __device__ __forceinline__ PfRow pf_row(const HarmParams& p, const int j, const int k) {
     const int c2 = p.nz - 1;
@@ -255,11 +263,11 @@ __global__ void __launch_bounds__(kPfThreads) prefilter_kernel(const HarmParams 
         if (32u * Q > rmax) break;
         const int nv = (int)min(32u, rmax - 32u * Q + 1u);
         const PfRow r = pf_row(p, j, k);
-        const float* src = r.mrow + (size_t)k * 4 * Q;
+        const unsigned short* src = r.mrow + (size_t)k * 4 * Q;
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
             if (i < nv) {
-                U[i] += __ldg(src + ((k * i) >> 3));
+                U[i] += bf16_lo(__ldg(src + ((k * i) >> 3)));
                 if (U[i] > r.thr) flagged |= 1u << i;
             }
         }

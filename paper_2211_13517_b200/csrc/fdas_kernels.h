@@ -16,7 +16,8 @@ struct ConvParams {
     int64_t nbins;
     int64_t pitch;
     int nz, h, V;
-    float* maxplane;     // nz x mpitch: max of every aligned block of 8 plane columns (as stored)
+    unsigned short* maxplane;  // nz x mpitch bf16 bit patterns: max of every aligned block of 8 plane
+                               // columns (as stored), rounded toward +inf (an upper bound)
     int64_t mpitch;      // nbins / 8
 };
 
@@ -46,7 +47,7 @@ struct HarmParams {
     fdas_cand_t* cands;
     int64_t capacity;
     unsigned long long* count;        // caller's: true number of candidates
-    float* maxplane;                  // plan-owned block-max plane, nz x mpitch
+    unsigned short* maxplane;         // plan-owned block-max plane (bf16 bits, rounded up), nz x mpitch
     int64_t mpitch;                   // nbins / 8
     uint2* maybe;                     // plan-owned list of (r, j): fundamentals that failed the prefilter
     int64_t maybe_capacity;
