@@ -40,7 +40,7 @@ N_SM, LANES, SM_MAX_GHZ = 148, 128, 1.965
 ALU_PEAK_TFLOPS = N_SM * LANES * 2 * SM_MAX_GHZ / 1e3
 # dram__bytes_read.sum + dram__bytes_write.sum of one K2 launch from `ncu --set full`
 # (profiles/); None until captured for that (workload, precision).
-NCU_K2_TRAFFIC_BYTES = {}
+NCU_K2_TRAFFIC_BYTES = {("ska", "bf16"): 18.5e6 + 3.381e9}   # profiles/r01c_packed_fp32x2.md
 
 
 def measured_peaks():
