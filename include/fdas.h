@@ -147,6 +147,28 @@ int fdas_search_host(fdas_plan_t plan, const float* h_series, int H, const float
                      void* cuda_stream);
 
 /*
+ * fdas_search_batch -- many independent DM trials through one plan ("5925 DM trials";
+ * BASELINE.json configs[3] "streamed through one GPU with double-buffered planes", configs[4]).
+ * Trial t is series[t]: n_in float32 samples, all DEVICE pointers (series_on_host = 0) or all HOST
+ * pointers (series_on_host = 1, pinned memory for full-speed copies); `series` itself is a host array
+ * of ntrials pointers.  The trials run through three plan-owned streams with two slots of every
+ * per-trial buffer (series, spectrum, plane, block-max plane, candidates): the host-to-device copy of
+ * trial t+1 and the harmonic sum of trial t-1 overlap the convolution of trial t.  Results are those
+ * of calling prepare -> convolve -> harmonic_sum_peaks per trial:
+ *   h_counts  host, ntrials: TRUE number of candidates of each trial
+ *   h_cands   host, ntrials x capacity records; trial t's first min(h_counts[t], capacity) candidates
+ *             start at h_cands + t*capacity (unspecified order)
+ * Work already queued on `cuda_stream` is waited for first, and `cuda_stream` is ordered after all of
+ * the batch's work (so events recorded on it before and after the call time the batch on the device);
+ * the call returns after the last copy has landed.  The device workspace (2 planes etc.) is allocated on first use and owned by the plan.
+ * FDAS_EOVERFLOW if some h_counts[t] > capacity (everything else is still valid); FDAS_EARG for NULL
+ * pointers, ntrials < 0, H outside 1..32, r_lo < 0, capacity < 0.
+ */
+int fdas_search_batch(fdas_plan_t plan, const float* const* series, int series_on_host, int ntrials,
+                      int H, const float* h_thresholds, int64_t r_lo, fdas_cand_t* h_cands,
+                      int64_t capacity, int64_t* h_counts, void* cuda_stream);
+
+/*
  * fdas_thresholds_from_sigma -- host helper (reading A13): h_thresholds_out[h-1] = T_h with
  * Q(h, T_h) = erfc(nsigma/sqrt2)/2, Q the survival function of a sum of h unit exponentials.
  */

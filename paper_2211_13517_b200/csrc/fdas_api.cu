@@ -15,63 +15,17 @@
 #include "fdas_fft_core.cuh"
 #include "fdas_host.h"
 #include "fdas_kernels.h"
+#include "fdas_plan_priv.h"
 
 using namespace fdas;
 
-static thread_local std::string g_detail;
-
-struct fdas_plan_s {
-    fdas_info_t info;
-    std::vector<cd> bank_time;  // nz x (2h+1), kept for diagnostics
-    void* d_bank = nullptr;
-    float2* d_tw1 = nullptr;
-    float2* d_tw2 = nullptr;
-    cufftHandle fft = 0;
-    bool fft_made = false;
-    void* d_fft_work = nullptr;
-    float2* d_X = nullptr;  // nfft/2 + 1
-    int32_t* d_blk_start = nullptr;
-    int32_t* d_blk_len = nullptr;
-    float* d_blk_med = nullptr;
-    int nblk = 0;
-    int nsplit = 1;
-    int64_t launches = 0;
-    unsigned short* d_maxplane = nullptr;    // block-max plane M (nz x nbins/8, bf16 bits), written by K2
-    const void* max_valid_for = nullptr;     // the plane M currently describes (nullptr: none)
-    uint2* d_maybe = nullptr;                // K3 maybe list (kMaybeCapacity records)
-    unsigned long long* d_maybe_count = nullptr;
-    // workspace of fdas_search_host (lazy)
-    float* ws_series = nullptr;
-    void* ws_spec = nullptr;
-    void* ws_plane = nullptr;
-    fdas_cand_t* ws_cands = nullptr;
-    int64_t ws_cap = 0;
-    unsigned long long* ws_count = nullptr;
-    unsigned long long* h_count = nullptr;  // pinned
-};
-
-#define CU(call)                                                                        \
-    do {                                                                                \
-        cudaError_t e_ = (call);                                                        \
-        if (e_ != cudaSuccess) {                                                        \
-            g_detail = std::string(#call) + ": " + cudaGetErrorString(e_);              \
-            return (e_ == cudaErrorMemoryAllocation) ? FDAS_EALLOC : FDAS_ECUDA;        \
-        }                                                                               \
-    } while (0)
-
-#define CF(call)                                                                        \
-    do {                                                                                \
-        cufftResult r_ = (call);                                                        \
-        if (r_ != CUFFT_SUCCESS) {                                                      \
-            g_detail = std::string(#call) + ": cufft status " + std::to_string((int)r_); \
-            return (r_ == CUFFT_ALLOC_FAILED) ? FDAS_EALLOC : FDAS_ECUFFT;              \
-        }                                                                               \
-    } while (0)
+thread_local std::string g_detail;
 
 static const int64_t kMaybeCapacity = 1 << 22;  // K3 prefilter survivors (fundamentals) listed per call
 
 static void free_plan(fdas_plan_s* p) {
     if (!p) return;
+    free_batch_state(p->batch);
     cudaFree(p->d_maxplane); cudaFree(p->d_maybe); cudaFree(p->d_maybe_count);
     cudaFree(p->d_bank); cudaFree(p->d_tw1); cudaFree(p->d_tw2); cudaFree(p->d_fft_work);
     cudaFree(p->d_X); cudaFree(p->d_blk_start); cudaFree(p->d_blk_len); cudaFree(p->d_blk_med);
@@ -171,6 +125,48 @@ static int build_plan(fdas_plan_s* p) {
     return FDAS_OK;
 }
 
+int fdas_enqueue_prepare(fdas_plan_s* plan, const float* d_series, void* d_spec, cudaStream_t st) {
+    CF(cufftSetStream(plan->fft, st));
+    CF(cufftExecR2C(plan->fft, const_cast<float*>(d_series), reinterpret_cast<cufftComplex*>(plan->d_X)));
+    WhitenParams w;
+    w.X = plan->d_X; w.spec = d_spec;
+    w.blk_start = plan->d_blk_start; w.blk_len = plan->d_blk_len; w.blk_med = plan->d_blk_med;
+    w.nblk = plan->nblk; w.nbins = plan->info.nbins;
+    CU(launch_whiten(plan->info.precision, w, st));
+    plan->launches += 2;
+    return FDAS_OK;
+}
+
+int fdas_enqueue_convolve(fdas_plan_s* plan, const void* d_spec, void* d_plane,
+                          unsigned short* d_maxplane, cudaStream_t st) {
+    ConvParams c;
+    c.spec = d_spec; c.plane = d_plane; c.bank = plan->d_bank; c.tw1 = plan->d_tw1; c.tw2 = plan->d_tw2;
+    c.nbins = plan->info.nbins; c.pitch = plan->info.plane_pitch;
+    c.nz = plan->info.nz; c.h = plan->info.halfwidth; c.V = plan->info.valid;
+    c.maxplane = d_maxplane; c.mpitch = plan->info.nbins / 8;
+    CU(launch_convolve(plan->info.precision, c, plan->info.nseg, plan->nsplit, st));
+    plan->launches += 1;
+    return FDAS_OK;
+}
+
+int fdas_enqueue_harmonic(fdas_plan_s* plan, const void* d_plane, unsigned short* d_maxplane,
+                          bool build_max, int H, const float* h_thresholds, int64_t r_lo,
+                          fdas_cand_t* d_cands, int64_t capacity, unsigned long long* d_count,
+                          cudaStream_t st) {
+    HarmParams hp;
+    hp.plane = d_plane; hp.nbins = plan->info.nbins; hp.pitch = plan->info.plane_pitch;
+    hp.nz = plan->info.nz; hp.H = H; hp.r_lo = r_lo;
+    for (int i = 0; i < 32; ++i) hp.thr[i] = (i < H) ? h_thresholds[i] : INFINITY;
+    hp.cands = d_cands; hp.capacity = capacity; hp.count = d_count;
+    hp.maxplane = d_maxplane; hp.mpitch = plan->info.nbins / 8;
+    hp.maybe = plan->d_maybe; hp.maybe_capacity = kMaybeCapacity; hp.maybe_count = plan->d_maybe_count;
+    hp.overflow = reinterpret_cast<unsigned*>(plan->d_maybe_count + 1);
+    int nl = 0;
+    CU(launch_harmonic(plan->info.precision == FDAS_BF16_PLANE16, build_max, hp, st, &nl));
+    plan->launches += nl;
+    return FDAS_OK;
+}
+
 extern "C" {
 
 int fdas_plan(fdas_plan_t* out, int64_t N, double tsamp, double zmax, double zstep, int seg_len,
@@ -207,31 +203,16 @@ int fdas_plan_info(fdas_plan_t plan, fdas_info_t* out) {
 
 int fdas_prepare_spectrum(fdas_plan_t plan, const float* d_series, void* d_spec, void* cuda_stream) {
     if (!plan || !d_series || !d_spec) return FDAS_EARG;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    CF(cufftSetStream(plan->fft, st));
-    CF(cufftExecR2C(plan->fft, const_cast<float*>(d_series), reinterpret_cast<cufftComplex*>(plan->d_X)));
-    WhitenParams w;
-    w.X = plan->d_X; w.spec = d_spec;
-    w.blk_start = plan->d_blk_start; w.blk_len = plan->d_blk_len; w.blk_med = plan->d_blk_med;
-    w.nblk = plan->nblk; w.nbins = plan->info.nbins;
-    CU(launch_whiten(plan->info.precision, w, st));
-    plan->launches += 2;
-    return FDAS_OK;
+    return fdas_enqueue_prepare(plan, d_series, d_spec, (cudaStream_t)cuda_stream);
 }
 
 int fdas_convolve_plane(fdas_plan_t plan, const void* d_spec, void* d_plane, void* cuda_stream) {
     if (!plan || !d_spec || !d_plane) return FDAS_EARG;
     if ((reinterpret_cast<uintptr_t>(d_plane) & 15u) != 0) return FDAS_EARG;
-    ConvParams c;
-    c.spec = d_spec; c.plane = d_plane; c.bank = plan->d_bank; c.tw1 = plan->d_tw1; c.tw2 = plan->d_tw2;
-    c.nbins = plan->info.nbins; c.pitch = plan->info.plane_pitch;
-    c.nz = plan->info.nz; c.h = plan->info.halfwidth; c.V = plan->info.valid;
-    c.maxplane = plan->d_maxplane; c.mpitch = plan->info.nbins / 8;
     plan->max_valid_for = nullptr;
-    CU(launch_convolve(plan->info.precision, c, plan->info.nseg, plan->nsplit, (cudaStream_t)cuda_stream));
-    plan->max_valid_for = d_plane;
-    plan->launches += 1;
-    return FDAS_OK;
+    const int rc = fdas_enqueue_convolve(plan, d_spec, d_plane, plan->d_maxplane, (cudaStream_t)cuda_stream);
+    if (rc == FDAS_OK) plan->max_valid_for = d_plane;
+    return rc;
 }
 
 int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const float* h_thresholds,
@@ -239,21 +220,12 @@ int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const 
                             unsigned long long* d_count, void* cuda_stream) {
     if (!plan || !d_plane || !h_thresholds || !d_count) return FDAS_EARG;
     if (H < 1 || H > 32 || r_lo < 0 || capacity < 0 || (capacity > 0 && !d_cands)) return FDAS_EARG;
-    HarmParams hp;
-    hp.plane = d_plane; hp.nbins = plan->info.nbins; hp.pitch = plan->info.plane_pitch;
-    hp.nz = plan->info.nz; hp.H = H; hp.r_lo = r_lo;
-    for (int i = 0; i < 32; ++i) hp.thr[i] = (i < H) ? h_thresholds[i] : INFINITY;
-    hp.cands = d_cands; hp.capacity = capacity; hp.count = d_count;
-    hp.maxplane = plan->d_maxplane; hp.mpitch = plan->info.nbins / 8;
-    hp.maybe = plan->d_maybe; hp.maybe_capacity = kMaybeCapacity; hp.maybe_count = plan->d_maybe_count;
-    hp.overflow = reinterpret_cast<unsigned*>(plan->d_maybe_count + 1);
     // M describes the plane fdas_convolve_plane last wrote; any other plane gets its own M first
     const bool build_max = (plan->max_valid_for != d_plane);
-    int nl = 0;
-    CU(launch_harmonic(plan->info.precision == FDAS_BF16_PLANE16, build_max, hp, (cudaStream_t)cuda_stream, &nl));
-    if (build_max && nl > 0) plan->max_valid_for = d_plane;
-    plan->launches += nl;
-    return FDAS_OK;
+    const int rc = fdas_enqueue_harmonic(plan, d_plane, plan->d_maxplane, build_max, H, h_thresholds, r_lo,
+                                         d_cands, capacity, d_count, (cudaStream_t)cuda_stream);
+    if (rc == FDAS_OK && build_max && r_lo < plan->info.nbins) plan->max_valid_for = d_plane;
+    return rc;
 }
 
 int fdas_search_host(fdas_plan_t plan, const float* h_series, int H, const float* h_thresholds,

@@ -22,7 +22,7 @@ FDAS_OK, FDAS_EARG, FDAS_EALLOC, FDAS_ECUDA, FDAS_ECUFFT, FDAS_EOVERFLOW, FDAS_E
 
 EXPORTS = (
     "fdas_plan", "fdas_plan_info", "fdas_prepare_spectrum", "fdas_convolve_plane",
-    "fdas_harmonic_sum_peaks", "fdas_search_host", "fdas_thresholds_from_sigma",
+    "fdas_harmonic_sum_peaks", "fdas_search_host", "fdas_search_batch", "fdas_thresholds_from_sigma",
     "fdas_plan_templates_host", "fdas_plan_debug_maxplane", "fdas_plan_launch_count", "fdas_destroy", "fdas_strerror",
     "fdas_last_error_detail",
 )
@@ -61,6 +61,8 @@ def _load():
     L.fdas_convolve_plane.argtypes = [vp, vp, vp, vp]
     L.fdas_harmonic_sum_peaks.argtypes = [vp, vp, ci, C.POINTER(C.c_float), i64, vp, i64, vp, vp]
     L.fdas_search_host.argtypes = [vp, vp, ci, C.POINTER(C.c_float), i64, vp, i64, C.POINTER(i64), vp]
+    L.fdas_search_batch.argtypes = [vp, C.POINTER(vp), ci, ci, ci, C.POINTER(C.c_float), i64, vp, i64,
+                                    C.POINTER(i64), vp]
     L.fdas_thresholds_from_sigma.argtypes = [ci, dbl, C.POINTER(C.c_float)]
     L.fdas_plan_templates_host.argtypes = [vp, vp]
     L.fdas_plan_debug_maxplane.argtypes = [vp, C.POINTER(vp), C.POINTER(i64)]
@@ -191,6 +193,34 @@ class Plan:
         st = _lib.fdas_search_host(self._h, h_ptr, int(H), thr_c, int(r_lo), out_ptr, int(capacity),
                                    C.byref(cnt), stream_ptr)
         return st, cnt.value
+
+    # ---- many trials, pipelined (configs[3], configs[4]) -------------------------------------
+    def search_batch(self, series, H, thresholds, r_lo, capacity=1 << 16, out=None, stream=None):
+        """series: list of device tensors (all) or of float32 numpy arrays / pinned CPU tensors (all),
+        n_in samples each.  Returns (counts[int64 ntrials], cands[ntrials, capacity] CAND_DTYPE, status);
+        status is FDAS_OK or FDAS_EOVERFLOW."""
+        n = len(series)
+        on_host = n == 0 or not (hasattr(series[0], "is_cuda") and series[0].is_cuda)
+        ptrs = (C.c_void_p * max(n, 1))()
+        for i, x in enumerate(series):
+            if hasattr(x, "data_ptr"):
+                assert x.is_cuda != on_host and x.numel() >= self.info.n_in and x.element_size() == 4
+                ptrs[i] = x.data_ptr()
+            else:
+                assert on_host and x.dtype == np.float32 and x.size >= self.info.n_in
+                ptrs[i] = x.ctypes.data
+        thr = np.ascontiguousarray(thresholds, dtype=np.float32)
+        if out is None:
+            out = np.empty((max(n, 1), capacity), dtype=CAND_DTYPE)
+        assert out.shape[0] >= n and out.flags.c_contiguous
+        counts = np.zeros(max(n, 1), dtype=np.int64)
+        st = _lib.fdas_search_batch(self._h, ptrs, 1 if on_host else 0, n, int(H),
+                                    thr.ctypes.data_as(C.POINTER(C.c_float)), int(r_lo), out.ctypes.data,
+                                    int(out.shape[1]), counts.ctypes.data_as(C.POINTER(C.c_int64)),
+                                    _stream_ptr(stream))
+        if st not in (FDAS_OK, FDAS_EOVERFLOW):
+            raise FdasError(st, "fdas_search_batch")
+        return counts[:n], out, st
 
     # ---- diagnostics -----------------------------------------------------------------------
     def templates_host(self) -> np.ndarray:

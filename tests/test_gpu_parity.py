@@ -378,3 +378,97 @@ def _device_view(torch, ptr, numel):
     class _Iface:
         __cuda_array_interface__ = {"shape": (numel,), "typestr": "<i2", "data": (ptr, False), "version": 3}
     return torch.as_tensor(_Iface(), device="cuda")
+
+
+# ------------------------------------- configs[3] / configs[4]: pipelined batch of DM trials
+def _sequential(fdas, torch, plan, x, wl, thr, capacity=1 << 16):
+    d_x = torch.from_numpy(x).cuda()
+    d_spec, d_plane = plan.alloc_spec(), plan.alloc_plane()
+    d_c, d_n = plan.alloc_cands(capacity)
+    plan.prepare_spectrum(d_x, d_spec)
+    plan.convolve_plane(d_spec, d_plane)
+    plan.harmonic_sum_peaks(d_plane, wl.nharm, thr, wl.r_lo, d_c, d_n)
+    torch.cuda.synchronize()
+    return plan.read_cands(d_c, d_n), d_spec, d_plane
+
+
+def test_batch_small_trial_counts_and_overflow(fdas, torch_):
+    """fdas_search_batch == the three calls per trial, for 0, 1, 2 and 5 trials (slot reuse), device
+    and host inputs, and with a capacity that overflows."""
+    torch = torch_
+    wl = inputs.tiny()
+    plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, "fp32")
+    thr = fdas.thresholds_from_sigma(wl.nharm, 4.5)        # lower threshold: tens of candidates per trial
+    xs = [inputs.make_series(wl.n, 500 + i, wl.signals if i % 2 == 0 else ()) for i in range(5)]
+    want = [gpu_cand_dict(_sequential(fdas, torch, plan, x, wl, thr)[0].cands) for x in xs]
+    assert all(len(w) > 3 for w in want) and len(want[0]) != len(want[1])
+    counts, _, st = plan.search_batch([], wl.nharm, thr, wl.r_lo, capacity=16)
+    assert st == fdas.FDAS_OK and counts.size == 0
+    for n in (1, 2, 5):
+        for on_host in (False, True):
+            series = xs[:n] if on_host else [torch.from_numpy(x).cuda() for x in xs[:n]]
+            counts, cands, st = plan.search_batch(series, wl.nharm, thr, wl.r_lo, capacity=4096)
+            assert st == fdas.FDAS_OK
+            for t in range(n):
+                assert counts[t] == len(want[t])
+                assert gpu_cand_dict(cands[t, :counts[t]]) == want[t], (n, on_host, t)
+    counts, cands, st = plan.search_batch(xs, wl.nharm, thr, wl.r_lo, capacity=2)
+    assert st == fdas.FDAS_EOVERFLOW
+    for t in range(5):
+        assert counts[t] == len(want[t])
+        assert set(gpu_cand_dict(cands[t, :2])) <= set(want[t])
+    # the plan still serves single calls afterwards (its own block-max plane is rebuilt or rewritten)
+    again = gpu_cand_dict(_sequential(fdas, torch, plan, xs[3], wl, thr)[0].cands)
+    assert again == want[3]
+
+
+@pytest.mark.parametrize("half_res", [False, True])
+def test_batch_ska_members_full_size(fdas, torch_, oracle, half_res):
+    """Members 5, 6, 7 of configs[3] (6 carries an injected accelerated signal), and the 128 us shape
+    of configs[4], through the pipelined batch in the configuration bench.py times: equal to the
+    per-trial calls, signal recovered at its (r, z), sampled oracle parity on the signal's trial."""
+    torch = torch_
+    members = [inputs.batched_member(i, half_res=half_res) for i in (5, 6, 7)]
+    wl = members[1]
+    assert len(wl.signals) == 1 and not members[0].signals
+    plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, "bf16")
+    assert plan.info.nfft == (1 << 22 if half_res else 1 << 23)
+    thr = fdas.thresholds_from_sigma(wl.nharm, wl.nsigma)
+    xs = [inputs.series_for(m) for m in members]
+    pinned = [torch.from_numpy(x).pin_memory() for x in xs]
+    counts, cands, st = plan.search_batch(pinned, wl.nharm, thr, wl.r_lo, capacity=1 << 14)
+    assert st == fdas.FDAS_OK
+    dev = [torch.from_numpy(x).cuda() for x in xs]
+    counts_d, cands_d, st = plan.search_batch(dev, wl.nharm, thr, wl.r_lo, capacity=1 << 14)
+    assert st == fdas.FDAS_OK and list(counts_d) == list(counts)
+    seq = None
+    for t in range(3):
+        res, d_spec, d_plane = _sequential(fdas, torch, plan, xs[t], wl, thr)
+        got = gpu_cand_dict(cands[t, :counts[t]])
+        assert got == gpu_cand_dict(res.cands) == gpu_cand_dict(cands_d[t, :counts_d[t]])
+        if t == 1:
+            seq = (got, d_spec, d_plane)
+        else:
+            del d_spec, d_plane
+    got, d_spec, d_plane = seq
+    s = wl.signals[0]
+    r0, j0 = int(round(s.r_c)), int(round(s.z + wl.zmax))
+    assert any(abs(k[0] - r0) <= 1 and abs(k[1] - j0) <= 1 and k[2] == 1 for k in got), (r0, j0)
+    # sampled oracle parity on the signal's trial
+    w = oracle.whiten(oracle.spectrum(xs[1], wl.nfft))
+    bank = oracle.template_bank(wl.zmax, wl.zstep)
+    g_r, g_j = np.meshgrid(np.arange(r0 - 8, r0 + 9), np.arange(max(0, j0 - 4), min(plan.info.nz, j0 + 5)))
+    rng = np.random.default_rng(7)
+    rr = np.concatenate([g_r.ravel(), rng.integers(0, plan.info.nbins, 5000)]).astype(np.int64)
+    jj = np.concatenate([g_j.ravel(), rng.integers(0, plan.info.nz, 5000)]).astype(np.int32)
+    Po = oracle.plane_points(w, bank, rr, jj)
+    Pg = d_plane[torch.from_numpy(jj.astype(np.int64)).cuda(), torch.from_numpy(rr).cuda()].float().cpu().numpy()
+    pmax = float(Po.max())
+    assert pmax > 50 and np.abs(Pg - Po).max() <= TOL["bf16"] * pmax
+    keys = sorted(got)
+    S, hmax = oracle.harmonic_sums_sampled(w, bank, wl.nharm, np.array([k[0] for k in keys]),
+                                           np.array([k[1] for k in keys], dtype=np.int32))
+    for i, (r, j, h) in enumerate(keys):
+        so = S[i, h - 1]
+        assert h <= hmax[i] and so > thr[h - 1] - h * TOL["bf16"] * pmax
+        assert abs(got[(r, j, h)][0] - so) <= min(h * TOL["bf16"] * pmax, REL_POW["bf16"] * so)
