@@ -34,7 +34,7 @@ UNIT = "points/s"
 L_SEG = 2048
 FLOP_IFFT = 5 * L_SEG * 11          # 5 L log2 L
 FLOP_MUL = 6 * L_SEG
-HBM_BYTES_PER_POINT = {"fp32": 4.05, "bf16": 4.02, "bf16_plane16": 2.02}
+HBM_BYTES_PER_POINT = {"fp32": 4.05, "bf16": 4.02, "bf16_plane16": 2.02, "bf16_tc": 4.02, "bf16_tc_plane16": 2.02}
 # ALU peak: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (B200_PROFILING.md unit counts/clocks)
 N_SM, LANES, SM_MAX_GHZ = 148, 128, 1.965
 ALU_PEAK_TFLOPS = N_SM * LANES * 2 * SM_MAX_GHZ / 1e3
@@ -523,7 +523,7 @@ def main():
                     help="length of the separate energy loop (0 = off)")
     ap.add_argument("--trials", type=int, default=0,
                     help="batched/survey: trials per rank (0 = 64 for batched, 3050+2875 for survey)")
-    ap.add_argument("--precision", default="bf16", choices=["fp32", "bf16", "bf16_plane16"])
+    ap.add_argument("--precision", default="bf16", choices=["fp32", "bf16", "bf16_plane16", "bf16_tc", "bf16_tc_plane16"])
     ap.add_argument("--pool", type=int, default=4, help="distinct series cycled per rank")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle plane work")

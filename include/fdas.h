@@ -35,8 +35,13 @@ typedef struct fdas_plan_s* fdas_plan_t; /* opaque, library-owned */
 
 /* Storage precision of the convolution stage (reading A10).  Arithmetic is
  * always fp32.  FP32: spectrum, templates and plane in fp32.  BF16: whitened spectrum and templates
- * stored as bfloat16 (round-to-nearest-even), plane fp32.  BF16_PLANE16: plane stored bf16 too. */
-enum { FDAS_FP32 = 0, FDAS_BF16 = 1, FDAS_BF16_PLANE16 = 2 };
+ * stored as bfloat16 (round-to-nearest-even), plane fp32.  BF16_PLANE16: plane stored bf16 too.
+ * BF16_TC / BF16_TC_PLANE16 (a separate labelled path): the same bf16 storage
+ * contract, but the matched filter is evaluated as the direct tap-domain contraction
+ * y_j(r) = sum_m w[r+m] conj(T_j[m]) on the tensor cores (bf16 spectrum x bf16 tap-domain templates,
+ * exact products, fp32 accumulation) instead of through segment FFTs on the fp32 ALUs.  seg_len is
+ * accepted and reported but does not enter this path (no overlap-save segmentation). */
+enum { FDAS_FP32 = 0, FDAS_BF16 = 1, FDAS_BF16_PLANE16 = 2, FDAS_BF16_TC = 3, FDAS_BF16_TC_PLANE16 = 4 };
 
 enum {
     FDAS_OK = 0,
@@ -87,7 +92,7 @@ typedef struct {
  *   zstep    template spacing in z (> 0); 2*zmax/zstep must be an integer (nz = that + 1 <= 32767)
  *   seg_len  L; this build supports 2048 only (FDAS_EUNSUPPORTED otherwise; FDAS_EARG if not a
  *            power of two or if V = L - 2h <= 0)
- *   precision  FDAS_FP32 | FDAS_BF16 | FDAS_BF16_PLANE16
+ *   precision  FDAS_FP32 | FDAS_BF16 | FDAS_BF16_PLANE16 | FDAS_BF16_TC | FDAS_BF16_TC_PLANE16
  * On success *out receives the handle (release with fdas_destroy).
  */
 int fdas_plan(fdas_plan_t* out, int64_t N, double tsamp, double zmax, double zstep, int seg_len,

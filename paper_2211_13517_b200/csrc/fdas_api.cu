@@ -39,7 +39,7 @@ static void free_plan(fdas_plan_s* p) {
 static int derive_info(int64_t N, double tsamp, double zmax, double zstep, int seg_len, int precision,
                        fdas_info_t* o) {
     if (N < 2 || !(tsamp > 0.0) || !(zmax >= 0.0) || !(zstep > 0.0) || seg_len < 2) return FDAS_EARG;
-    if (precision != FDAS_FP32 && precision != FDAS_BF16 && precision != FDAS_BF16_PLANE16) return FDAS_EARG;
+    if (precision < FDAS_FP32 || precision > FDAS_BF16_TC_PLANE16) return FDAS_EARG;
     if ((seg_len & (seg_len - 1)) != 0) return FDAS_EARG;
     if (N < 2 * (int64_t)seg_len) return FDAS_EARG;
     const double cnt = 2.0 * zmax / zstep;
@@ -60,7 +60,7 @@ static int derive_info(int64_t N, double tsamp, double zmax, double zstep, int s
     o->nseg = (o->nbins + o->valid - 1) / o->valid;
     o->plane_pitch = o->nbins;
     o->spec_elem_bytes = (precision == FDAS_FP32) ? 8 : 4;
-    o->plane_elem_bytes = (precision == FDAS_BF16_PLANE16) ? 2 : 4;
+    o->plane_elem_bytes = fdas_plane16(precision) ? 2 : 4;
     o->precision = precision;
     o->zmax = zmax; o->zstep = zstep; o->tsamp = tsamp; o->tobs = (double)nfft * tsamp;
     if (seg_len != kL) return FDAS_EUNSUPPORTED;
@@ -72,7 +72,21 @@ static int build_plan(fdas_plan_s* p) {
     Bank bank;
     build_bank(in.zmax, in.zstep, in.nz, in.halfwidth, in.seg_len, &bank);
     p->bank_time = bank.time;
-    if (in.precision == FDAS_FP32) {
+    if (fdas_is_tc(in.precision)) {
+        if (!tc_geometry(in.nz, in.halfwidth, &p->tc) || in.nbins % 128 != 0) {
+            g_detail = "FDAS_BF16_TC: template bank does not fit the tensor-core kernel";
+            return FDAS_EUNSUPPORTED;
+        }
+        std::vector<uint16_t> img;
+        double asym = 0.0;
+        pack_bank_tc(bank, p->tc, &img, &asym);
+        if (asym > 1e-12) {
+            g_detail = "FDAS_BF16_TC: bank is not conjugate-symmetric in z";
+            return FDAS_EUNSUPPORTED;
+        }
+        CU(cudaMalloc(&p->d_bank, img.size() * sizeof(uint16_t)));
+        CU(cudaMemcpy(p->d_bank, img.data(), img.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+    } else if (in.precision == FDAS_FP32) {
         std::vector<float> packed;
         pack_bank_fp32(bank, &packed);
         CU(cudaMalloc(&p->d_bank, packed.size() * sizeof(float)));
@@ -114,6 +128,7 @@ static int build_plan(fdas_plan_s* p) {
     int dev = 0, nsm = 148;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    p->nsm = nsm;
     const int64_t slots = (int64_t)convolve_ctas_per_sm() * nsm;
     int nsplit = 1;
     if (in.nseg < 4 * slots) nsplit = (int)std::min<int64_t>(in.nz, (4 * slots + in.nseg - 1) / in.nseg);
@@ -132,13 +147,24 @@ int fdas_enqueue_prepare(fdas_plan_s* plan, const float* d_series, void* d_spec,
     w.X = plan->d_X; w.spec = d_spec;
     w.blk_start = plan->d_blk_start; w.blk_len = plan->d_blk_len; w.blk_med = plan->d_blk_med;
     w.nblk = plan->nblk; w.nbins = plan->info.nbins;
-    CU(launch_whiten(plan->info.precision, w, st));
+    CU(launch_whiten(plan->info.precision == FDAS_FP32 ? FDAS_FP32 : FDAS_BF16, w, st));
     plan->launches += 2;
     return FDAS_OK;
 }
 
 int fdas_enqueue_convolve(fdas_plan_s* plan, const void* d_spec, void* d_plane,
                           unsigned short* d_maxplane, cudaStream_t st) {
+    if (fdas_is_tc(plan->info.precision)) {
+        ConvTcParams t;
+        t.spec = reinterpret_cast<const unsigned*>(d_spec); t.plane = d_plane; t.bimg = plan->d_bank;
+        t.bimg_bytes = plan->tc.bytes; t.nbins = plan->info.nbins; t.pitch = plan->info.plane_pitch;
+        t.nz = plan->info.nz; t.h = plan->info.halfwidth; t.kp = plan->tc.kp;
+        t.ngroups = plan->tc.ngroups; t.gch = plan->tc.gch;
+        t.maxplane = d_maxplane; t.mpitch = plan->info.nbins / 8;
+        CU(launch_convolve_tc(fdas_plane16(plan->info.precision), t, plan->nsm, st));
+        plan->launches += 1;
+        return FDAS_OK;
+    }
     ConvParams c;
     c.spec = d_spec; c.plane = d_plane; c.bank = plan->d_bank; c.tw1 = plan->d_tw1; c.tw2 = plan->d_tw2;
     c.nbins = plan->info.nbins; c.pitch = plan->info.plane_pitch;
@@ -162,7 +188,7 @@ int fdas_enqueue_harmonic(fdas_plan_s* plan, const void* d_plane, unsigned short
     hp.maybe = plan->d_maybe; hp.maybe_capacity = kMaybeCapacity; hp.maybe_count = plan->d_maybe_count;
     hp.overflow = reinterpret_cast<unsigned*>(plan->d_maybe_count + 1);
     int nl = 0;
-    CU(launch_harmonic(plan->info.precision == FDAS_BF16_PLANE16, build_max, hp, st, &nl));
+    CU(launch_harmonic(fdas_plane16(plan->info.precision), build_max, hp, st, &nl));
     plan->launches += nl;
     return FDAS_OK;
 }

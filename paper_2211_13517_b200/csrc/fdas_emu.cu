@@ -6,12 +6,14 @@
 // the CPU test-suite (tests/test_host_logic.py) on a box without a GPU.  It also exposes the
 // plan-time host mathematics (templates, Fresnel integrals, thresholds, whitening blocks) for the
 // same purpose.
+#include <algorithm>
 #include <cstring>
 #include <vector>
 
 #include "../../include/fdas.h"
 #include "fdas_fft_core.cuh"
 #include "fdas_host.h"
+#include "fdas_tc_common.h"
 
 using namespace fdas;
 
@@ -162,6 +164,142 @@ int fdas_emu_convolve(const float* spec, int64_t nb, double zmax, double zstep, 
         }
     }
     delete c;
+    return FDAS_OK;
+}
+
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// K2-TC stepped on the host: the same shared-memory image, descriptor encodings, producer row
+// builder, MMA issue order, TMEM column map and epilogue as fdas_convolve_tc.cu; only tcgen05.mma is
+// replaced by `emu_umma`, which decodes the two shared-memory descriptors and the instruction
+// descriptor as the hardware is documented to (K-major, no swizzle, M = 128, K = 16).
+namespace {
+
+inline float bf16_to_f(uint16_t b) { return bf16_bits_to_f32(b); }
+
+void emu_umma(const std::vector<unsigned char>& smem, float (*D)[256], int dcol, uint64_t adesc,
+              uint64_t bdesc, uint32_t idesc, bool accumulate) {
+    const uint32_t a0 = (uint32_t)(adesc & 0x3fff) << 4, alb = (uint32_t)((adesc >> 16) & 0x3fff) << 4,
+                   asb = (uint32_t)((adesc >> 32) & 0x3fff) << 4;
+    const uint32_t b0 = (uint32_t)(bdesc & 0x3fff) << 4, blb = (uint32_t)((bdesc >> 16) & 0x3fff) << 4,
+                   bsb = (uint32_t)((bdesc >> 32) & 0x3fff) << 4;
+    const int N = (int)((idesc >> 17) & 0x3f) << 3, M = (int)((idesc >> 24) & 0x1f) << 4;
+    for (int i = 0; i < M; ++i)
+        for (int n = 0; n < N; ++n) {
+            float acc = accumulate ? D[i][dcol + n] : 0.0f;
+            for (int k = 0; k < 16; ++k) {
+                const uint32_t ao = a0 + (i % 8) * 16 + (i / 8) * asb + (k / 8) * alb + (k % 8) * 2;
+                const uint32_t bo = b0 + (n % 8) * 16 + (n / 8) * bsb + (k / 8) * blb + (k % 8) * 2;
+                uint16_t av, bv;
+                std::memcpy(&av, &smem[ao], 2);
+                std::memcpy(&bv, &smem[bo], 2);
+                acc += bf16_to_f(av) * bf16_to_f(bv);
+            }
+            D[i][dcol + n] = acc;
+        }
+}
+
+}  // namespace
+
+extern "C" {
+// spec: nb complex fp32 (rounded here to bf16 as K1b stores it); plane: nz x nb float (plane16: the
+// bf16-rounded value as float); maxplane: nz x nb/8 bf16 bit patterns.  nb must be a multiple of 128.
+int fdas_emu_convolve_tc(const float* spec, int64_t nb, double zmax, double zstep, int plane16,
+                         float* plane, uint16_t* maxplane) {
+    using namespace fdas::tc;
+    const int nz = (int)(2.0 * zmax / zstep + 0.5) + 1;
+    const int h = template_halfwidth(zmax);
+    if (nb % kTileR != 0) return FDAS_EARG;
+    Bank bank;
+    build_bank(zmax, zstep, nz, h, kL, &bank);
+    TcGeom g;
+    if (!tc_geometry(nz, h, &g)) return FDAS_EUNSUPPORTED;
+    std::vector<uint16_t> img;
+    double asym = 0.0;
+    pack_bank_tc(bank, g, &img, &asym);
+    if (asym > 1e-12) return FDAS_EUNSUPPORTED;
+    const Layout L = make_layout(g.bytes, g.kp);
+    std::vector<unsigned char> smem((size_t)L.total, 0xff);   // 0xff: unwritten bf16 reads as NaN
+    std::memcpy(&smem[L.b_off], img.data(), (size_t)g.bytes);
+    std::vector<uint32_t> specq((size_t)nb);
+    for (int64_t k = 0; k < nb; ++k) specq[k] = pack_bf16x2(spec[2 * k], spec[2 * k + 1]);
+    const int npair = (nz - 1) / 2, mid = npair, ksteps = g.kp / 16;
+    const int64_t mpitch = nb / 8, ntiles = nb / kTileR;
+    auto D = new float[2][128][256];
+    uint32_t item = 0;
+    int it = 0;
+    for (int64_t tile = 0; tile < ntiles; ++tile, ++it) {
+        // producer
+        const int hs = it % kHStages;
+        uint16_t* sre = reinterpret_cast<uint16_t*>(&smem[L.st_off]);
+        uint16_t* sim = reinterpret_cast<uint16_t*>(&smem[L.st_off + L.st_part]);
+        const int nrows = g.kp + 120, nsrc = g.kp + 130;
+        const int64_t base = tile * kTileR - h;
+        for (int i = 0; i < nsrc; ++i) {
+            const int64_t idx = base + i;
+            const uint32_t v = (idx >= 0 && idx < nb) ? specq[idx] : 0u;
+            sre[i] = (uint16_t)v;
+            sim[i] = (uint16_t)(v >> 16);
+        }
+        unsigned char* hst = &smem[L.h_off + hs * L.h_stage];
+        for (int rho = 0; rho < nrows; ++rho)
+            for (int part = 0; part < 2; ++part) {
+                const uint32_t* w32 = reinterpret_cast<const uint32_t*>(part ? sim : sre) + (rho >> 1);
+                const uint4 o = window_row(w32, rho);
+                std::memcpy(hst + part * L.h_part + rho * 16, &o, 16);
+            }
+        // MMA issuer + epilogue, one accumulator stage at a time
+        const uint32_t idesc = instr_desc(16 * g.gch);
+        const uint32_t lbo = (uint32_t)(g.ngroups * g.gch * 2) * 128u;
+        const uint32_t a_re = (uint32_t)(L.h_off + hs * L.h_stage), a_im = a_re + L.h_part;
+        for (int grp = 0; grp < g.ngroups; ++grp, ++item) {
+            const uint32_t st = item & 1u;
+            const uint32_t bbase = (uint32_t)L.b_off + (uint32_t)(grp * g.gch * 2) * 128u;
+            for (int ks = 0; ks < ksteps; ++ks) {
+                const uint64_t bd = smem_desc(bbase + (uint32_t)ks * 2u * lbo, lbo, 128u);
+                emu_umma(smem, D[st], 0, smem_desc(a_re + ks * 256u, 128u, 128u), bd, idesc, ks > 0);
+                emu_umma(smem, D[st], 128, smem_desc(a_im + ks * 256u, 128u, 128u), bd, idesc, ks > 0);
+            }
+            for (int lane_r = 0; lane_r < 128; ++lane_r) {
+                const int64_t r = tile * kTileR + lane_r;
+                if (grp == 0) {
+                    const float2 w = unpack_bf16x2(specq[r]);
+                    float P = fmaf(w.x, w.x, w.y * w.y);
+                    if (plane16) P = bf16_bits_to_f32(f32_to_bf16_rne(P));
+                    plane[(size_t)mid * nb + r] = P;
+                }
+                for (int c = 0; c < g.gch; ++c)
+                    for (int pp = 0; pp < 8; ++pp) {
+                        const int pr = (grp * g.gch + c) * 8 + pp;
+                        if (pr >= npair) continue;
+                        float Pp, Pm;
+                        pair_powers(D[st][lane_r][16 * c + 2 * pp], D[st][lane_r][16 * c + 2 * pp + 1],
+                                    D[st][lane_r][128 + 16 * c + 2 * pp], D[st][lane_r][128 + 16 * c + 2 * pp + 1],
+                                    &Pp, &Pm);
+                        if (plane16) {
+                            Pp = bf16_bits_to_f32(f32_to_bf16_rne(Pp));
+                            Pm = bf16_bits_to_f32(f32_to_bf16_rne(Pm));
+                        }
+                        plane[(size_t)(mid + 1 + pr) * nb + r] = Pp;
+                        plane[(size_t)(mid - 1 - pr) * nb + r] = Pm;
+                    }
+            }
+        }
+    }
+    delete[] D;
+    // block maxima of the values as stored, rounded toward +inf to bf16
+    for (int j = 0; j < nz; ++j)
+        for (int64_t b = 0; b < mpitch; ++b) {
+            uint32_t m = 0;
+            for (int e = 0; e < 8; ++e) {
+                uint32_t bits;
+                std::memcpy(&bits, &plane[(size_t)j * nb + 8 * b + e], 4);
+                m = std::max(m, (bits + 0xffffu) >> 16);
+            }
+            maxplane[(size_t)j * mpitch + b] = (uint16_t)m;
+        }
     return FDAS_OK;
 }
 

@@ -26,6 +26,26 @@ cudaError_t launch_convolve(int precision, const ConvParams& p, int64_t nseg, in
                             cudaStream_t st);
 int convolve_ctas_per_sm();  // resident CTAs per SM K2 is launched for (sizes the template split)
 
+// K2-TC: the convolution stage as a dense contraction on the tensor cores (fdas_convolve_tc.cu).
+// Direct correlation y_j(r) = sum_m w[r+m] conj(T_j[m]) written as D[r][n] = sum_k A[r][k] B[n][k]
+// with A the sliding-window (Hankel) matrix of the bf16 spectrum and B the bf16 tap-domain bank.
+struct ConvTcParams {
+    const unsigned* spec;      // nbins packed bf16x2 (re low, im high)
+    void* plane;               // nz x pitch: float or bf16
+    const void* bimg;          // B operand image in UMMA K-major no-swizzle order (fdas_host.h)
+    int bimg_bytes;
+    int64_t nbins, pitch;
+    int nz, h;
+    int kp;                    // taps 2h+1 padded to a multiple of 16
+    int ngroups, gch;          // template-pair groups per tile, chunks of 8 pairs per group (<= 6)
+    unsigned short* maxplane;  // as ConvParams
+    int64_t mpitch;
+    __host__ __device__ int ng_cols() const { return 16 * gch; }
+};
+// One persistent CTA per SM; `nsm` CTAs are launched.  plane16 != 0 stores the plane as bf16.
+cudaError_t launch_convolve_tc(int plane16, const ConvTcParams& p, int nsm, cudaStream_t st);
+int convolve_tc_smem_bytes(const ConvTcParams& p);
+
 struct WhitenParams {
     const float2* X;         // nfft/2 + 1 complex from cuFFT R2C
     void* spec;              // nbins complex fp32 or bf16x2

@@ -19,6 +19,9 @@ void free_batch_state(BatchState*);
 
 extern thread_local std::string g_detail;
 
+static inline bool fdas_is_tc(int precision) { return precision == FDAS_BF16_TC || precision == FDAS_BF16_TC_PLANE16; }
+static inline bool fdas_plane16(int precision) { return precision == FDAS_BF16_PLANE16 || precision == FDAS_BF16_TC_PLANE16; }
+
 struct fdas_plan_s {
     fdas_info_t info;
     std::vector<fdas::cd> bank_time;  // nz x (2h+1), kept for diagnostics
@@ -34,6 +37,8 @@ struct fdas_plan_s {
     float* d_blk_med = nullptr;
     int nblk = 0;
     int nsplit = 1;
+    fdas::TcGeom tc;                          // K2-TC operand geometry (FDAS_BF16_TC*)
+    int nsm = 148;
     int64_t launches = 0;
     unsigned short* d_maxplane = nullptr;    // block-max plane M (nz x nbins/8, bf16 bits), written by K2
     const void* max_valid_for = nullptr;     // the plane M currently describes (nullptr: none)

@@ -16,8 +16,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfdas.so")
 
-FDAS_FP32, FDAS_BF16, FDAS_BF16_PLANE16 = 0, 1, 2
-PRECISIONS = {"fp32": FDAS_FP32, "bf16": FDAS_BF16, "bf16_plane16": FDAS_BF16_PLANE16}
+FDAS_FP32, FDAS_BF16, FDAS_BF16_PLANE16, FDAS_BF16_TC, FDAS_BF16_TC_PLANE16 = 0, 1, 2, 3, 4
+PRECISIONS = {"fp32": FDAS_FP32, "bf16": FDAS_BF16, "bf16_plane16": FDAS_BF16_PLANE16,
+              "bf16_tc": FDAS_BF16_TC, "bf16_tc_plane16": FDAS_BF16_TC_PLANE16}
 FDAS_OK, FDAS_EARG, FDAS_EALLOC, FDAS_ECUDA, FDAS_ECUFFT, FDAS_EOVERFLOW, FDAS_EUNSUPPORTED = range(7)
 
 EXPORTS = (
@@ -135,7 +136,7 @@ class Plan:
 
     def alloc_plane(self, device="cuda"):
         import torch
-        dt = torch.bfloat16 if self.precision == FDAS_BF16_PLANE16 else torch.float32
+        dt = torch.bfloat16 if self.precision in (FDAS_BF16_PLANE16, FDAS_BF16_TC_PLANE16) else torch.float32
         return torch.empty((self.info.nz, self.info.plane_pitch), dtype=dt, device=device)
 
     def alloc_cands(self, capacity: int, device="cuda"):

@@ -13,8 +13,9 @@ from helpers import compare_candidates, gpu_cand_dict, oracle_margin_fn
 
 pytestmark = pytest.mark.gpu
 
-TOL = {"fp32": 1e-4, "bf16": 2e-2, "bf16_plane16": 2e-2}
-REL_POW = {"fp32": None, "bf16": 0.03, "bf16_plane16": 0.03}
+TOL = {"fp32": 1e-4, "bf16": 2e-2, "bf16_plane16": 2e-2, "bf16_tc": 2e-2, "bf16_tc_plane16": 2e-2}
+REL_POW = {"fp32": None, "bf16": 0.03, "bf16_plane16": 0.03, "bf16_tc": 0.03, "bf16_tc_plane16": 0.03}
+ALL_PREC = ["fp32", "bf16", "bf16_plane16", "bf16_tc", "bf16_tc_plane16"]
 
 
 @pytest.fixture(scope="module")
@@ -99,7 +100,7 @@ def medium_oracle(oracle):
     return wl, x, orc
 
 
-@pytest.mark.parametrize("precision", ["fp32", "bf16", "bf16_plane16"])
+@pytest.mark.parametrize("precision", ALL_PREC)
 def test_medium_full_parity(fdas, torch_, oracle, medium_oracle, precision):
     torch = torch_
     wl, x, orc = medium_oracle
@@ -130,7 +131,7 @@ def test_medium_full_parity(fdas, torch_, oracle, medium_oracle, precision):
 
 
 # --------------------------------------------------------------- K2 alone, fed a chosen spectrum
-@pytest.mark.parametrize("precision", ["fp32", "bf16", "bf16_plane16"])
+@pytest.mark.parametrize("precision", ALL_PREC)
 def test_convolve_alone_seams_tail_and_invariants(fdas, torch_, oracle, precision):
     torch = torch_
     n = 1 << 15                      # nbins = 16384: 9 segments of V = 1984 + ragged tail
@@ -170,6 +171,14 @@ def test_convolve_alone_seams_tail_and_invariants(fdas, torch_, oracle, precisio
         # remaining error is template quantisation + fp32 arithmetic (+ plane rounding)
         Pq = oracle.plane(wq, bank)
         assert np.abs(Pg - Pq).max() <= 1e-2 * P.max()
+    if precision.startswith("bf16_tc"):
+        # tensor-core contraction: the z = 0 row is |w|^2 of the stored spectrum (T_0 = delta), and
+        # conj(w) negates Im-part accumulators only, so the z axis flips bit-exactly
+        rel = 2.0 ** -8 if precision.endswith("plane16") else 1e-6
+        assert np.abs(Pg[16] - np.abs(wq) ** 2).max() <= rel * P.max()
+        d_plane_c = plan.alloc_plane()
+        plan.convolve_plane(spec_from_complex(torch, np.conj(w), precision), d_plane_c)
+        assert torch.equal(d_plane_c, torch.flip(d_plane, dims=[0]))
 
 
 def test_smallest_plan_and_zmax0(fdas, torch_, oracle):
@@ -264,7 +273,7 @@ def test_search_host_equals_device_calls(fdas, torch_):
 
 
 # ------------------------------------------------------- configs[2] at full size: sampled parity
-@pytest.mark.parametrize("precision", ["bf16", "fp32"])
+@pytest.mark.parametrize("precision", ["bf16", "fp32", "bf16_tc", "bf16_tc_plane16"])
 def test_ska_full_size_sampled_parity(fdas, torch_, oracle, precision):
     """SKA-like single DM trial in the launch configuration bench.py times.  The oracle computes
     sampled plane points and sampled harmonic sums one by one from its own whitened spectrum."""
@@ -285,7 +294,8 @@ def test_ska_full_size_sampled_parity(fdas, torch_, oracle, precision):
     jj = [rng.integers(0, nz, 30000)]
     # segment seams, the first bins, the ragged tail, and the injected signals' neighbourhoods
     seams = np.array([s * V + d for s in (1, 2, 1000, 2184) for d in (-2, -1, 0, 1, 2)])
-    for cols in (seams, np.arange(0, 70), np.arange(nb - 70, nb)):
+    tiles = np.array([t * 128 + d for t in (1, 147, 148, 149, 32767) for d in (-1, 0, 1)])   # K2-TC tile seams
+    for cols in (seams, tiles, np.arange(0, 70), np.arange(nb - 70, nb)):
         for j in (0, 56, 96, 136, 192):
             rr.append(cols); jj.append(np.full(cols.size, j))
     for s in wl.signals:
@@ -338,7 +348,7 @@ def test_ska_full_size_sampled_parity(fdas, torch_, oracle, precision):
 
 
 # ---------------------------------------------- K2's block-max side plane and the K3 prefilter
-@pytest.mark.parametrize("precision", ["fp32", "bf16_plane16"])
+@pytest.mark.parametrize("precision", ["fp32", "bf16_plane16", "bf16_tc", "bf16_tc_plane16"])
 def test_blockmax_plane_and_prefilter_equivalence(fdas, torch_, precision):
     """M[j][b] written by K2 equals the maximum of the 8 stored plane values of block b rounded up to
     bfloat16 (bit-exact), and

@@ -29,6 +29,7 @@ def emu():
     L.fdas_emu_whitening_blocks.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_int64]
     L.fdas_emu_whitening_blocks.restype = C.c_int64
     L.fdas_emu_halfwidth.argtypes = [C.c_double]
+    L.fdas_emu_convolve_tc.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
     return L
 
 
@@ -139,6 +140,41 @@ def test_emulated_k2_matches_the_oracle_plane(emu, oracle, zmax, nb):
         assert emu.fdas_emu_convolve(w.ctypes.data, nb, zmax, 1.0, prec, out.ctypes.data) == 0
         assert not np.isnan(out).any()                      # every r < nb written, nothing else
         assert np.abs(out - P).max() <= tol * P.max(), (prec, np.abs(out - P).max() / P.max())
+
+
+@pytest.mark.parametrize("zmax,nb", [(16.0, 1152), (96.0, 640)])
+def test_emulated_k2_tc_matches_the_oracle_plane(emu, oracle, zmax, nb):
+    """K2-TC (tensor-core contraction) stepped on the CPU: same shared-memory image, UMMA descriptor
+    encodings (sliding-window A operand with LBO = SBO = 128 B, packed bank B), issue order, TMEM
+    column map and pair epilogue as fdas_convolve_tc.cu; tcgen05.mma replaced by a descriptor walker.
+    Several tiles, both edges (zero fill below bin 0 and above nb), strong lines at the edges."""
+    rng = np.random.default_rng(5)
+    w = ((rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)).astype(np.complex64)
+    w[nb // 3] += 15.0
+    w[1] += 9.0
+    w[nb - 1] += 7.0
+    nz = int(2 * zmax) + 1
+    bank = oracle.template_bank(zmax, 1.0)
+    P = oracle.plane(w.astype(np.complex128), bank)
+
+    def bf16(a):   # round-to-nearest-even to bfloat16, returned as float32
+        u = np.ascontiguousarray(a, dtype=np.float32).view(np.uint32)
+        return ((u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000).astype(np.uint32).view(np.float32)
+
+    Pq = oracle.plane(bf16(w.real).astype(np.float64) + 1j * bf16(w.imag).astype(np.float64), bank)
+    for plane16 in (0, 1):
+        out = np.full((nz, nb), np.nan, dtype=np.float32)
+        mx = np.zeros((nz, nb // 8), dtype=np.uint16)
+        assert emu.fdas_emu_convolve_tc(w.ctypes.data, nb, zmax, 1.0, plane16, out.ctypes.data, mx.ctypes.data) == 0
+        assert not np.isnan(out).any()
+        assert np.abs(out - P).max() <= 2e-2 * P.max()
+        # against the oracle on the bf16-rounded spectrum (reading A11) only the bf16 rounding of the
+        # taps (2^-9 relative per tap) and, for plane16, of the stored power remains
+        assert np.abs(out - Pq).max() <= (5e-3 if not plane16 else 9e-3) * Pq.max(), np.abs(out - Pq).max() / Pq.max()
+        # block maxima bound the stored values from above, within one bf16 ulp
+        up = (mx.astype(np.uint32) << 16).view(np.float32)
+        blk = out.reshape(nz, nb // 8, 8).max(axis=2)
+        assert (up >= blk).all() and (up <= blk * (1 + 2.0 ** -7) + 1e-30).all()
 
 
 # --------------------------------------------------------------------------- sharding over ranks
