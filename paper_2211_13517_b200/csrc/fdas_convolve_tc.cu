@@ -22,8 +22,8 @@
 // * TMEM lane = r (128 per tile), column = operand column: a warp's store of one plane row is
 //   128 contiguous bytes; the thread that owns r has all four values of a pair in its own lane.
 //
-// Warp roles of the persistent CTA (one per SM, 320 threads): warp 0 builds H for tile i+1.. (3
-// stages), warp 1 allocates TMEM and issues the MMAs (one lane), warps 2..9 drain the two
+// Warp roles of the persistent CTA (one per SM, 448 threads): warp 0 builds H for tile i+1.. (3
+// stages), warp 1 allocates TMEM and issues the MMAs (one lane), warps 2..13 drain the two
 // accumulator stages (TMEM -> registers -> power -> plane + block-max side plane).
 #include <cuda_bf16.h>
 
@@ -35,6 +35,17 @@
 namespace fdas {
 namespace tc {
 
+// Timing experiments only (never set in the product build): 1 = epilogue skips its arithmetic and
+// stores, 2 = the MMA issuer skips the MMAs.
+#ifndef FDAS_TC_DIAG
+#define FDAS_TC_DIAG 0
+#endif
+#ifndef FDAS_TC_SLEEP_PROD
+#define FDAS_TC_SLEEP_PROD 2000
+#endif
+#ifndef FDAS_TC_SLEEP_MMA
+#define FDAS_TC_SLEEP_MMA 100
+#endif
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return (uint32_t)__cvta_generic_to_shared(p);
@@ -55,6 +66,22 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "bra WAIT_%=;\n\t"
         "DONE_%=:\n\t"
         "}" ::"r"(bar), "r"(parity) : "memory");
+}
+// Same, for the two single-warp roles that wait most of the time (producer, MMA issuer): back off
+// between polls so that the spinning warp does not take issue slots from the epilogue warps of its
+// scheduler.
+__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity, unsigned ns) {
+    for (;;) {
+        uint32_t ok;
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return;
+        __nanosleep(ns);
+    }
 }
 __device__ __forceinline__ void fence_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -111,54 +138,80 @@ __device__ __forceinline__ unsigned bf16_up_pair(float a, float b) {
     return __byte_perm(__float_as_uint(a) + 0xffffu, __float_as_uint(b) + 0xffffu, 0x7632);
 }
 
+// Block maxima are reduced one chunk late so that the shared-memory round trip and the dependent
+// max chain of chunk i-1 overlap the arithmetic of chunk i: this is what is still owed.
+struct PendingMax {
+    unsigned short* mup;
+    unsigned short* mdn;
+    int buf;     // scratch buffer (0/1) holding the packed powers
+    int nval;    // real pairs in that chunk (0: nothing pending)
+};
+
+// Lane (pp, blk) reduces pair pp over lanes 8 blk..+7 (two 128-bit rows of the scratch buffer).
+__device__ __forceinline__ void pending_load(const uint32_t* scratch, const PendingMax& pm, const int lane,
+                                             uint4* v0, uint4* v1) {
+    const uint32_t* row = scratch + pm.buf * 256 + (lane >> 2) * 32 + (lane & 3) * 8;
+    *v0 = *reinterpret_cast<const uint4*>(row);
+    *v1 = *reinterpret_cast<const uint4*>(row + 4);
+}
+template <int TAIL>
+__device__ __forceinline__ void pending_store(const PendingMax& pm, const int lane, const uint4& v0,
+                                              const uint4& v1) {
+    unsigned m = __vmaxu2(__vmaxu2(v0.x, v0.y), __vmaxu2(v0.z, v0.w));
+    m = __vmaxu2(m, __vmaxu2(__vmaxu2(v1.x, v1.y), __vmaxu2(v1.z, v1.w)));
+    if (!TAIL || (lane >> 2) < pm.nval) {
+        *pm.mup = (unsigned short)m;
+        *pm.mdn = (unsigned short)(m >> 16);
+    }
+}
+
 // One chunk = 8 template pairs = 16 columns of D1 (Ar, Br interleaved) and D2 (Ai, Bi): powers of
-// the 16 plane rows at this thread's bin, coalesced row stores, and the block maxima over aligned
-// groups of 8 bins through the warp's scratch (lane (pp, blk) reduces pair pp over lanes 8 blk..+7).
-template <int PLANE16>
-__device__ __forceinline__ void chunk_out(const uint32_t (&a)[16], const uint32_t (&b)[16], const int p0,
-                                          const int npair, const int mid, const int64_t r,
-                                          const ConvTcParams& p, uint32_t* scratch, const int lane) {
+// the 16 plane rows at this thread's bin, coalesced row stores through two running row pointers
+// (`up`: row mid+1+p0 ascending, `dn`: row mid-1-p0 descending; `step` = row pitch in bytes); the
+// packed bf16 upper bounds go to the warp's scratch for the block maxima over aligned groups of 8
+// bins, which the NEXT call reduces and stores (`pm`).  nval = real pairs in the chunk (8 unless
+// TAIL, the bank's padded last chunk).
+template <int PLANE16, int TAIL>
+__device__ __forceinline__ void chunk_out(const uint32_t (&a)[16], const uint32_t (&b)[16], char* up,
+                                          char* dn, const int64_t step, unsigned short* mup,
+                                          unsigned short* mdn, const int nval, uint32_t* scratch,
+                                          const int lane, PendingMax& pm) {
+    uint4 v0 = make_uint4(0, 0, 0, 0), v1 = v0;
+    const bool owed = pm.nval > 0;
+    if (owed) pending_load(scratch, pm, lane, &v0, &v1);
+    const int buf = pm.buf ^ 1;
+    uint32_t* mine = scratch + buf * 256 + lane;
 #pragma unroll
     for (int pp = 0; pp < 8; ++pp) {
         const float Ar = __uint_as_float(a[2 * pp]), Br = __uint_as_float(a[2 * pp + 1]);
         const float Ai = __uint_as_float(b[2 * pp]), Bi = __uint_as_float(b[2 * pp + 1]);
         float Pp, Pm;
         pair_powers(Ar, Br, Ai, Bi, &Pp, &Pm);
-        const int pr = p0 + pp;
         unsigned packed;
         if (PLANE16) {
             const __nv_bfloat162 pk = __floats2bfloat162_rn(Pp, Pm);
             packed = *reinterpret_cast<const unsigned*>(&pk);
-            if (pr < npair) {
-                unsigned short* pl = reinterpret_cast<unsigned short*>(p.plane);
-                __stcs(pl + (int64_t)(mid + 1 + pr) * p.pitch + r, (unsigned short)packed);
-                __stcs(pl + (int64_t)(mid - 1 - pr) * p.pitch + r, (unsigned short)(packed >> 16));
+            if (!TAIL || pp < nval) {
+                __stcs(reinterpret_cast<unsigned short*>(up), (unsigned short)packed);
+                __stcs(reinterpret_cast<unsigned short*>(dn), (unsigned short)(packed >> 16));
             }
         } else {
             packed = bf16_up_pair(Pp, Pm);
-            if (pr < npair) {
-                float* pl = reinterpret_cast<float*>(p.plane);
-                __stcs(pl + (int64_t)(mid + 1 + pr) * p.pitch + r, Pp);
-                __stcs(pl + (int64_t)(mid - 1 - pr) * p.pitch + r, Pm);
+            if (!TAIL || pp < nval) {
+                __stcs(reinterpret_cast<float*>(up), Pp);
+                __stcs(reinterpret_cast<float*>(dn), Pm);
             }
         }
-        scratch[pp * 32 + lane] = packed;
+        up += step;
+        dn -= step;
+        mine[pp * 32] = packed;
     }
+    if (owed) pending_store<TAIL>(pm, lane, v0, v1);
     __syncwarp();
-    {
-        const int pp = lane >> 2, blk = lane & 3;
-        const uint4 v0 = *reinterpret_cast<const uint4*>(scratch + pp * 32 + blk * 8);
-        const uint4 v1 = *reinterpret_cast<const uint4*>(scratch + pp * 32 + blk * 8 + 4);
-        unsigned m = __vmaxu2(__vmaxu2(v0.x, v0.y), __vmaxu2(v0.z, v0.w));
-        m = __vmaxu2(m, __vmaxu2(__vmaxu2(v1.x, v1.y), __vmaxu2(v1.z, v1.w)));
-        const int pr = p0 + pp;
-        if (pr < npair) {
-            const int64_t col = ((r - lane) >> 3) + blk;
-            p.maxplane[(int64_t)(mid + 1 + pr) * p.mpitch + col] = (unsigned short)m;
-            p.maxplane[(int64_t)(mid - 1 - pr) * p.mpitch + col] = (unsigned short)(m >> 16);
-        }
-    }
-    __syncwarp();
+    pm.mup = mup;
+    pm.mdn = mdn;
+    pm.buf = buf;
+    pm.nval = nval;
 }
 
 // z = 0: T_0 = delta, so the row is |w[r]|^2 of the stored (bf16) spectrum.
@@ -184,8 +237,9 @@ __device__ __forceinline__ void zero_row_out(const int mid, const int64_t r, con
     if ((lane & 7) == 0) p.maxplane[(int64_t)mid * p.mpitch + (r >> 3)] = (unsigned short)w;
 }
 
-// MAXC = ceil(gch / 2): chunks one epilogue warp drains per accumulator stage.
-template <int PLANE16, int MAXC>
+// MAXC = ceil(gch / 3): chunks one epilogue warp drains per accumulator stage; TAIL: the bank's
+// last chunk has fewer than 8 real pairs.
+template <int PLANE16, int MAXC, int TAIL>
 __global__ void __launch_bounds__(kThreads, 1) convolve_tc_kernel(const ConvTcParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
     const Layout L = make_layout(p.bimg_bytes, p.kp);
@@ -240,7 +294,7 @@ __global__ void __launch_bounds__(kThreads, 1) convolve_tc_kernel(const ConvTcPa
         int it = 0;
         for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
             const int hs = it % kHStages;
-            mbar_wait(hempty(hs), ((it / kHStages) & 1) ^ 1);
+            mbar_wait_backoff(hempty(hs), ((it / kHStages) & 1) ^ 1, FDAS_TC_SLEEP_PROD);
             const int64_t base = tile * kTileR - p.h;
             for (int i = lane; i < nsrc; i += 32) {
                 const int64_t idx = base + i;
@@ -271,18 +325,19 @@ __global__ void __launch_bounds__(kThreads, 1) convolve_tc_kernel(const ConvTcPa
             uint32_t item = 0;
             for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
                 const int hs = it % kHStages;
-                mbar_wait(hfull(hs), (it / kHStages) & 1);
+                mbar_wait_backoff(hfull(hs), (it / kHStages) & 1, FDAS_TC_SLEEP_MMA);
                 tc_fence_after();
                 const uint32_t a_re = smem_u32(smem + L.h_off + hs * L.h_stage);
                 const uint32_t a_im = a_re + L.h_part;
                 for (int g = 0; g < p.ngroups; ++g, ++item) {
                     const uint32_t st = item & 1u;
-                    mbar_wait(tempty(st), ((item >> 1) & 1u) ^ 1u);
+                    mbar_wait_backoff(tempty(st), ((item >> 1) & 1u) ^ 1u, FDAS_TC_SLEEP_MMA);
                     tc_fence_after();
                     const uint32_t d1 = tmem_base + st * 256u, d2 = d1 + 128u;
                     const uint32_t bbase = smem_u32(smem + L.b_off) + (uint32_t)(g * p.gch * 2) * 128u;
                     for (int ks = 0; ks < ksteps; ++ks) {
                         const uint64_t bd = smem_desc(bbase + (uint32_t)ks * 2u * lbo, lbo, 128u);
+                        if (FDAS_TC_DIAG == 2) continue;
                         tc_mma(d1, smem_desc(a_re + ks * 256u, 128u, 128u), bd, idesc, ks > 0);
                         tc_mma(d2, smem_desc(a_im + ks * 256u, 128u, 128u), bd, idesc, ks > 0);
                     }
@@ -293,29 +348,38 @@ __global__ void __launch_bounds__(kThreads, 1) convolve_tc_kernel(const ConvTcPa
         }
     } else {
         // ===== epilogue warps: TMEM lane quarter = warp % 4, chunks c = hf, hf + 2, ...
-        const int q = warp & 3, hf = (warp - 2) >> 2;
-        uint32_t* scratch = reinterpret_cast<uint32_t*>(smem + L.sc_off) + (warp - 2) * 256;
-        const int nmine = (p.gch - hf + 1) / 2;
+        const int q = warp & 3, t3 = (warp - 2) >> 2;      // chunks c = t3, t3 + 3, ...
+        uint32_t* scratch = reinterpret_cast<uint32_t*>(smem + L.sc_off) + (warp - 2) * 512;
+        const int gch = p.gch, ngroups = p.ngroups;
+        const int nmine = (gch - t3 + 2) / 3;
+        constexpr int kElem = PLANE16 ? 2 : 4;
+        const int64_t step = p.pitch * kElem, mpitch = p.mpitch;
+        char* const plane = reinterpret_cast<char*>(p.plane);
+        unsigned short* const maxplane = p.maxplane;
+        const int rpp = lane >> 2;                     // the pair this lane reduces in every chunk
+        PendingMax pm = {nullptr, nullptr, 0, 0};
         uint32_t item = 0;
         for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
             const int64_t r = tile * kTileR + 32 * q + lane;
-            for (int g = 0; g < p.ngroups; ++g, ++item) {
+            char* const col = plane + r * kElem;                                    // this bin, row 0
+            unsigned short* const mcol = maxplane + ((r - lane) >> 3) + (lane & 3);    // its block
+            for (int g = 0; g < ngroups; ++g, ++item) {
                 const uint32_t st = item & 1u;
-                if (g == 0 && hf == 0) zero_row_out<PLANE16>(mid, r, p, lane);
+                if (g == 0 && t3 == 2) zero_row_out<PLANE16>(mid, r, p, lane);
                 mbar_wait(tfull(st), (item >> 1) & 1u);
                 tc_fence_after();
                 const uint32_t tb = tmem_base + ((uint32_t)(32 * q) << 16) + st * 256u;
                 uint32_t a[2][16], b[2][16];
                 if (nmine > 0) {
-                    tmem_ld16(tb + 16u * hf, a[0]);
-                    tmem_ld16(tb + 128u + 16u * hf, b[0]);
+                    tmem_ld16(tb + 16u * t3, a[0]);
+                    tmem_ld16(tb + 128u + 16u * t3, b[0]);
                 }
 #pragma unroll
                 for (int i = 0; i < MAXC; ++i) {
                     if (i < nmine) {
                         tmem_wait16(a[i & 1], b[i & 1]);
                         if (i + 1 < nmine) {
-                            const uint32_t c = (uint32_t)(hf + 2 * (i + 1));
+                            const uint32_t c = (uint32_t)(t3 + 3 * (i + 1));
                             tmem_ld16(tb + 16u * c, a[(i + 1) & 1]);
                             tmem_ld16(tb + 128u + 16u * c, b[(i + 1) & 1]);
                         } else {
@@ -324,8 +388,14 @@ __global__ void __launch_bounds__(kThreads, 1) convolve_tc_kernel(const ConvTcPa
                             __syncwarp();
                             if (lane == 0) mbar_arrive(tempty(st));
                         }
-                        const int p0 = (g * p.gch + hf + 2 * i) * 8;
-                        chunk_out<PLANE16>(a[i & 1], b[i & 1], p0, npair, mid, r, p, scratch, lane);
+                        const int p0 = (g * gch + t3 + 3 * i) * 8;
+                        const int nval = TAIL ? min(8, npair - p0) : 8;
+                        if ((!TAIL || nval > 0) && FDAS_TC_DIAG != 1)
+                            chunk_out<PLANE16, TAIL>(a[i & 1], b[i & 1], col + (int64_t)(mid + 1 + p0) * step,
+                                                     col + (int64_t)(mid - 1 - p0) * step, step,
+                                                     mcol + (int64_t)(mid + 1 + p0 + rpp) * mpitch,
+                                                     mcol + (int64_t)(mid - 1 - p0 - rpp) * mpitch, nval,
+                                                     scratch, lane, pm);
                     }
                 }
                 if (nmine == 0) {
@@ -334,6 +404,11 @@ __global__ void __launch_bounds__(kThreads, 1) convolve_tc_kernel(const ConvTcPa
                     if (lane == 0) mbar_arrive(tempty(st));
                 }
             }
+        }
+        if (pm.nval > 0) {
+            uint4 v0, v1;
+            pending_load(scratch, pm, lane, &v0, &v1);
+            pending_store<TAIL>(pm, lane, v0, v1);
         }
     }
 
@@ -358,7 +433,8 @@ int convolve_tc_smem_bytes(const ConvTcParams& p) {
 template <int PLANE16>
 static cudaError_t launch_tc_maxc(const ConvTcParams& p, int nsm, cudaStream_t st) {
     const int smem = convolve_tc_smem_bytes(p);
-    const int maxc = (p.gch + 1) / 2;
+    const int maxc = (p.gch + 2) / 3;
+    const bool tail = ((p.nz - 1) / 2) % 8 != 0;
     auto go = [&](auto kern) -> cudaError_t {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
@@ -367,12 +443,8 @@ static cudaError_t launch_tc_maxc(const ConvTcParams& p, int nsm, cudaStream_t s
         kern<<<grid, tc::kThreads, smem, st>>>(p);
         return cudaGetLastError();
     };
-    switch (maxc) {
-        case 1: return go(tc::convolve_tc_kernel<PLANE16, 1>);
-        case 2: return go(tc::convolve_tc_kernel<PLANE16, 2>);
-        case 3: return go(tc::convolve_tc_kernel<PLANE16, 3>);
-        default: return cudaErrorInvalidValue;
-    }
+    if (tail) return maxc == 1 ? go(tc::convolve_tc_kernel<PLANE16, 1, 1>) : go(tc::convolve_tc_kernel<PLANE16, 2, 1>);
+    return maxc == 1 ? go(tc::convolve_tc_kernel<PLANE16, 1, 0>) : go(tc::convolve_tc_kernel<PLANE16, 2, 0>);
 }
 
 cudaError_t launch_convolve_tc(int plane16, const ConvTcParams& p, int nsm, cudaStream_t st) {

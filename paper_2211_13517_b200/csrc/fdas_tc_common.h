@@ -9,10 +9,10 @@
 namespace fdas {
 namespace tc {
 
-constexpr int kThreads = 320;   // warp 0 producer, warp 1 MMA issuer, warps 2..9 epilogue
+constexpr int kThreads = 448;   // warp 0 producer, warp 1 MMA issuer, warps 2..13 epilogue
 constexpr int kHStages = 3;     // sliding-window (A operand) stages
 constexpr int kTileR = 128;     // Fourier bins per tile = MMA M = TMEM lanes
-constexpr int kEpiWarps = 8;
+constexpr int kEpiWarps = 12;
 
 // K-major, no-swizzle shared-memory matrix descriptor: start address, LBO (between the two 8-element
 // K halves of one MMA), SBO (between 8-row groups), all in 16-byte units; version 1 (sm_100).
@@ -40,7 +40,7 @@ __host__ __device__ inline Layout make_layout(int bimg_bytes, int kp) {
     l.st_off = l.h_off + kHStages * l.h_stage;
     l.st_part = ((kp + 136) * 2 + 127) & ~127;      // kp + 130 bf16 of the slice (incl. read slack)
     l.sc_off = l.st_off + 2 * l.st_part;
-    l.bar_off = l.sc_off + kEpiWarps * 1024;        // 8 pairs x 32 lanes x 4 bytes per epilogue warp
+    l.bar_off = l.sc_off + kEpiWarps * 2048;        // 2 buffers x 8 pairs x 32 lanes x 4 bytes per warp
     l.total = l.bar_off + 128;
     return l;
 }
@@ -56,17 +56,11 @@ __host__ __device__ inline uint4 window_row(const uint32_t* w32, int rho) {
 }
 
 // Powers of the rows +z and -z from A~ = w (*) Re T_z = Ar + i Ai and B~ = w (*) Im T_z = Br + i Bi:
-// y_{+z} = A~ - i B~, y_{-z} = A~ + i B~, so P_{+-z} = (Ar^2+Ai^2+Br^2+Bi^2) +- 2 (Ar Bi - Ai Br),
-// clamped at 0 (the difference can round a hair below zero).
+// y_{+z} = A~ - i B~ = (Ar + Bi) + i (Ai - Br),  y_{-z} = A~ + i B~ = (Ar - Bi) + i (Ai + Br).
 __host__ __device__ inline void pair_powers(float Ar, float Br, float Ai, float Bi, float* Pp, float* Pm) {
-    float S = Ar * Ar;
-    S = fmaf(Ai, Ai, S);
-    S = fmaf(Br, Br, S);
-    S = fmaf(Bi, Bi, S);
-    float X = Ar * Bi;
-    X = fmaf(-Ai, Br, X);
-    *Pp = fmaxf(fmaf(2.0f, X, S), 0.0f);
-    *Pm = fmaxf(fmaf(-2.0f, X, S), 0.0f);
+    const float rp = Ar + Bi, ip = Ai - Br, rm = Ar - Bi, im = Ai + Br;
+    *Pp = fmaf(rp, rp, ip * ip);
+    *Pm = fmaf(rm, rm, im * im);
 }
 
 }  // namespace tc
