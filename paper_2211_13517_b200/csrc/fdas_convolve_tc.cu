@@ -25,6 +25,7 @@
 // Warp roles of the persistent CTA (one per SM, 448 threads): warp 0 builds H for tile i+1.. (3
 // stages), warp 1 allocates TMEM and issues the MMAs (one lane), warps 2..13 drain the two
 // accumulator stages (TMEM -> registers -> power -> plane + block-max side plane).
+#include <cuda.h>
 #include <cuda_bf16.h>
 
 #include <cstdint>
@@ -83,6 +84,17 @@ __device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity,
         __nanosleep(ns);
     }
 }
+// One poll (the hardware may block for a short system-dependent time): true if the phase completed.
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void fence_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
@@ -138,80 +150,93 @@ __device__ __forceinline__ unsigned bf16_up_pair(float a, float b) {
     return __byte_perm(__float_as_uint(a) + 0xffffu, __float_as_uint(b) + 0xffffu, 0x7632);
 }
 
-// Block maxima are reduced one chunk late so that the shared-memory round trip and the dependent
-// max chain of chunk i-1 overlap the arithmetic of chunk i: this is what is still owed.
-struct PendingMax {
-    unsigned short* mup;
-    unsigned short* mdn;
-    int buf;     // scratch buffer (0/1) holding the packed powers
-    int nval;    // real pairs in that chunk (0: nothing pending)
-};
-
-// Lane (pp, blk) reduces pair pp over lanes 8 blk..+7 (two 128-bit rows of the scratch buffer).
-__device__ __forceinline__ void pending_load(const uint32_t* scratch, const PendingMax& pm, const int lane,
-                                             uint4* v0, uint4* v1) {
-    const uint32_t* row = scratch + pm.buf * 256 + (lane >> 2) * 32 + (lane & 3) * 8;
-    *v0 = *reinterpret_cast<const uint4*>(row);
-    *v1 = *reinterpret_cast<const uint4*>(row + 4);
+// ---- epilogue staging: a warpgroup (4 warps = the 128 bins of the tile) turns one chunk of 8
+// template pairs into a [16 rows][128 bins] tile of powers in shared memory -- local rows 0..7 are
+// plane rows mid+1+p0 .. +7, local rows 8..15 are plane rows mid-1-p0-7 .. mid-1-p0 (ascending) --
+// which two TMA tensor stores (8 rows x 128 bins each) write to the plane; the block maxima over
+// aligned groups of 8 bins are then read back from the same tile.
+__device__ __forceinline__ void bar_sync_wg(int id) {
+    asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory");
 }
-template <int TAIL>
-__device__ __forceinline__ void pending_store(const PendingMax& pm, const int lane, const uint4& v0,
-                                              const uint4& v1) {
-    unsigned m = __vmaxu2(__vmaxu2(v0.x, v0.y), __vmaxu2(v0.z, v0.w));
-    m = __vmaxu2(m, __vmaxu2(__vmaxu2(v1.x, v1.y), __vmaxu2(v1.z, v1.w)));
-    if (!TAIL || (lane >> 2) < pm.nval) {
-        *pm.mup = (unsigned short)m;
-        *pm.mdn = (unsigned short)(m >> 16);
-    }
+__device__ __forceinline__ void tma_store_2d(const void* tmap, uint32_t smem_src, int c0, int c1) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(tmap),
+                 "r"(smem_src), "r"(c0), "r"(c1)
+                 : "memory");
 }
+__device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// Returns once all but the newest kStageBufs - 2 committed store groups have finished READING shared
+// memory (their buffers may be overwritten).
+__device__ __forceinline__ void tma_wait_read_older() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(kStageBufs - 2) : "memory");
+}
+__device__ __forceinline__ void tma_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
-// One chunk = 8 template pairs = 16 columns of D1 (Ar, Br interleaved) and D2 (Ai, Bi): powers of
-// the 16 plane rows at this thread's bin, coalesced row stores through two running row pointers
-// (`up`: row mid+1+p0 ascending, `dn`: row mid-1-p0 descending; `step` = row pitch in bytes); the
-// packed bf16 upper bounds go to the warp's scratch for the block maxima over aligned groups of 8
-// bins, which the NEXT call reduces and stores (`pm`).  nval = real pairs in the chunk (8 unless
-// TAIL, the bank's padded last chunk).
-template <int PLANE16, int TAIL>
-__device__ __forceinline__ void chunk_out(const uint32_t (&a)[16], const uint32_t (&b)[16], char* up,
-                                          char* dn, const int64_t step, unsigned short* mup,
-                                          unsigned short* mdn, const int nval, uint32_t* scratch,
-                                          const int lane, PendingMax& pm) {
-    uint4 v0 = make_uint4(0, 0, 0, 0), v1 = v0;
-    const bool owed = pm.nval > 0;
-    if (owed) pending_load(scratch, pm, lane, &v0, &v1);
-    const int buf = pm.buf ^ 1;
-    uint32_t* mine = scratch + buf * 256 + lane;
+// Powers of one chunk from the accumulators of this thread's bin (column `col` of the tile) into the
+// staging tile.
+template <int PLANE16>
+__device__ __forceinline__ void chunk_to_smem(const uint32_t (&a)[16], const uint32_t (&b)[16], void* sbuf,
+                                              const int col) {
 #pragma unroll
     for (int pp = 0; pp < 8; ++pp) {
         const float Ar = __uint_as_float(a[2 * pp]), Br = __uint_as_float(a[2 * pp + 1]);
         const float Ai = __uint_as_float(b[2 * pp]), Bi = __uint_as_float(b[2 * pp + 1]);
         float Pp, Pm;
         pair_powers(Ar, Br, Ai, Bi, &Pp, &Pm);
-        unsigned packed;
         if (PLANE16) {
             const __nv_bfloat162 pk = __floats2bfloat162_rn(Pp, Pm);
-            packed = *reinterpret_cast<const unsigned*>(&pk);
-            if (!TAIL || pp < nval) {
-                __stcs(reinterpret_cast<unsigned short*>(up), (unsigned short)packed);
-                __stcs(reinterpret_cast<unsigned short*>(dn), (unsigned short)(packed >> 16));
-            }
+            const unsigned packed = *reinterpret_cast<const unsigned*>(&pk);
+            unsigned short* t = reinterpret_cast<unsigned short*>(sbuf) + col;
+            t[pp * 128] = (unsigned short)packed;
+            t[(15 - pp) * 128] = (unsigned short)(packed >> 16);
         } else {
-            packed = bf16_up_pair(Pp, Pm);
-            if (!TAIL || pp < nval) {
-                __stcs(reinterpret_cast<float*>(up), Pp);
-                __stcs(reinterpret_cast<float*>(dn), Pm);
-            }
+            float* t = reinterpret_cast<float*>(sbuf) + col;
+            t[pp * 128] = Pp;
+            t[(15 - pp) * 128] = Pm;
         }
-        up += step;
-        dn -= step;
-        mine[pp * 32] = packed;
     }
-    if (owed) pending_store<TAIL>(pm, lane, v0, v1);
-    __syncwarp();
-    pm.mup = mup;
-    pm.mdn = mdn;
-    pm.buf = buf;
-    pm.nval = nval;
+}
+
+// Block maxima of a staged tile, one chunk late (the loads overlap the next chunk's arithmetic):
+// thread tw of the warpgroup reduces block (tw & 15) of local rows tw >> 4 and 8 + (tw >> 4) and
+// writes the bf16 upper bound into the [16][16] side tile, which goes out with the next TMA group.
+// The two 16-byte halves of a block are read in lane-dependent order so that the 8 lanes of a
+// shared-memory phase touch 8 different 16-byte bank groups.
+struct MaxRegs {
+    uint4 u[2], v[2];
+};
+template <int PLANE16>
+__device__ __forceinline__ void block_max_load(const void* sbuf, const int tw, MaxRegs* m) {
+    const int lr0 = tw >> 4, blk = tw & 15;
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        const int lr = lr0 + 8 * t;
+        if (PLANE16) {
+            m->u[t] = *reinterpret_cast<const uint4*>(reinterpret_cast<const unsigned short*>(sbuf) + lr * 128 + blk * 8);
+        } else {
+            const float* row = reinterpret_cast<const float*>(sbuf) + lr * 128 + blk * 8;
+            const int sw = (blk >> 2) & 1;
+            m->u[t] = *reinterpret_cast<const uint4*>(row + 4 * sw);
+            m->v[t] = *reinterpret_cast<const uint4*>(row + 4 * (sw ^ 1));
+        }
+    }
+}
+template <int PLANE16>
+__device__ __forceinline__ void block_max_finish(const MaxRegs& m, unsigned short* mtile, const int tw) {
+    const int lr0 = tw >> 4, blk = tw & 15;
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        unsigned bits;
+        if (PLANE16) {
+            const unsigned x = __vmaxu2(__vmaxu2(m.u[t].x, m.u[t].y), __vmaxu2(m.u[t].z, m.u[t].w));
+            bits = max(x & 0xffffu, x >> 16);
+        } else {
+            // powers are >= 0: the order of the bit patterns is the order of the values
+            const unsigned x = max(max(max(m.u[t].x, m.u[t].y), max(m.u[t].z, m.u[t].w)),
+                                   max(max(m.v[t].x, m.v[t].y), max(m.v[t].z, m.v[t].w)));
+            bits = (x + 0xffffu) >> 16;
+        }
+        mtile[(lr0 + 8 * t) * 16 + blk] = (unsigned short)bits;
+    }
 }
 
 // z = 0: T_0 = delta, so the row is |w[r]|^2 of the stored (bf16) spectrum.
@@ -237,10 +262,10 @@ __device__ __forceinline__ void zero_row_out(const int mid, const int64_t r, con
     if ((lane & 7) == 0) p.maxplane[(int64_t)mid * p.mpitch + (r >> 3)] = (unsigned short)w;
 }
 
-// MAXC = ceil(gch / 3): chunks one epilogue warp drains per accumulator stage; TAIL: the bank's
-// last chunk has fewer than 8 real pairs.
-template <int PLANE16, int MAXC, int TAIL>
-__global__ void __launch_bounds__(kThreads, 1) convolve_tc_kernel(const ConvTcParams p) {
+template <int PLANE16>
+__global__ void __launch_bounds__(kThreads, 1)
+convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tmap,
+                   const __grid_constant__ CUtensorMap mmap) {
     extern __shared__ __align__(128) unsigned char smem[];
     const Layout L = make_layout(p.bimg_bytes, p.kp);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -348,67 +373,132 @@ __global__ void __launch_bounds__(kThreads, 1) convolve_tc_kernel(const ConvTcPa
         }
     } else {
         // ===== epilogue warps: TMEM lane quarter = warp % 4, chunks c = hf, hf + 2, ...
-        const int q = warp & 3, t3 = (warp - 2) >> 2;      // chunks c = t3, t3 + 3, ...
-        uint32_t* scratch = reinterpret_cast<uint32_t*>(smem + L.sc_off) + (warp - 2) * 512;
+        const int q = warp & 3, wg = (warp - 2) >> 2;      // warpgroup wg drains chunks wg, wg+3, ..
+        const int tw = ((warp - 2) & 3) * 32 + lane;        // thread index inside the warpgroup
+        const bool elected = (tw == 0);
         const int gch = p.gch, ngroups = p.ngroups;
-        const int nmine = (gch - t3 + 2) / 3;
-        constexpr int kElem = PLANE16 ? 2 : 4;
-        const int64_t step = p.pitch * kElem, mpitch = p.mpitch;
-        char* const plane = reinterpret_cast<char*>(p.plane);
-        unsigned short* const maxplane = p.maxplane;
-        const int rpp = lane >> 2;                     // the pair this lane reduces in every chunk
-        PendingMax pm = {nullptr, nullptr, 0, 0};
-        uint32_t item = 0;
-        for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-            const int64_t r = tile * kTileR + 32 * q + lane;
-            char* const col = plane + r * kElem;                                    // this bin, row 0
-            unsigned short* const mcol = maxplane + ((r - lane) >> 3) + (lane & 3);    // its block
-            for (int g = 0; g < ngroups; ++g, ++item) {
-                const uint32_t st = item & 1u;
-                if (g == 0 && t3 == 2) zero_row_out<PLANE16>(mid, r, p, lane);
-                mbar_wait(tfull(st), (item >> 1) & 1u);
-                tc_fence_after();
-                const uint32_t tb = tmem_base + ((uint32_t)(32 * q) << 16) + st * 256u;
-                uint32_t a[2][16], b[2][16];
-                if (nmine > 0) {
-                    tmem_ld16(tb + 16u * t3, a[0]);
-                    tmem_ld16(tb + 128u + 16u * t3, b[0]);
-                }
-#pragma unroll
-                for (int i = 0; i < MAXC; ++i) {
-                    if (i < nmine) {
-                        tmem_wait16(a[i & 1], b[i & 1]);
-                        if (i + 1 < nmine) {
-                            const uint32_t c = (uint32_t)(t3 + 3 * (i + 1));
-                            tmem_ld16(tb + 16u * c, a[(i + 1) & 1]);
-                            tmem_ld16(tb + 128u + 16u * c, b[(i + 1) & 1]);
-                        } else {
-                            // every load of this stage has landed in registers: hand it back
-                            tc_fence_before();
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(tempty(st));
-                        }
-                        const int p0 = (g * gch + t3 + 3 * i) * 8;
-                        const int nval = TAIL ? min(8, npair - p0) : 8;
-                        if ((!TAIL || nval > 0) && FDAS_TC_DIAG != 1)
-                            chunk_out<PLANE16, TAIL>(a[i & 1], b[i & 1], col + (int64_t)(mid + 1 + p0) * step,
-                                                     col + (int64_t)(mid - 1 - p0) * step, step,
-                                                     mcol + (int64_t)(mid + 1 + p0 + rpp) * mpitch,
-                                                     mcol + (int64_t)(mid - 1 - p0 - rpp) * mpitch, nval,
-                                                     scratch, lane, pm);
-                    }
-                }
-                if (nmine == 0) {
+        const int nmine = (gch - wg + 2) / 3;
+        unsigned char* const stage0 = smem + L.sc_off + wg * (kStageBufs * kStageBufBytes);
+        const int col = 32 * q + lane;
+        const uint32_t lane_base = tmem_base + ((uint32_t)(32 * q) << 16);
+        const int64_t tstep = gridDim.x;
+        if (nmine == 0) {
+            // nothing to drain (small banks): hand every stage straight back, keep the z = 0 duty
+            uint32_t item = 0;
+            for (int64_t tile = blockIdx.x; tile < ntiles; tile += tstep)
+                for (int g = 0; g < ngroups; ++g, ++item) {
+                    if (g == 0 && wg == 2) zero_row_out<PLANE16>(mid, tile * kTileR + col, p, lane);
+                    mbar_wait(tfull(item & 1u), (item >> 1) & 1u);
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(tempty(st));
+                    if (lane == 0) mbar_arrive(tempty(item & 1u));
+                }
+        } else {
+            // flat software pipeline over this warp's chunks (tile, group g, i-th own chunk): the
+            // TMEM loads of chunk n+1 are issued before the arithmetic of chunk n, across stages too;
+            // chunk n's powers leave through TMA group n together with the block maxima of chunk n-1
+            int64_t tile = blockIdx.x;
+            int g = 0, i = 0;
+            uint32_t item = 0, n = 0;
+            int prev_c0 = 0, prev_p0 = 0;
+            uint32_t ra[16], rb[16], sa[16], sb[16];
+            auto issue_ld = [&](uint32_t it_, int i_, uint32_t (&x)[16], uint32_t (&y)[16]) {
+                const uint32_t tb = lane_base + (it_ & 1u) * 256u + 16u * (uint32_t)(wg + 3 * i_);
+                tmem_ld16(tb, x);
+                tmem_ld16(tb + 128u, y);
+            };
+            auto buf_of = [&](uint32_t k) { return stage0 + (k % kStageBufs) * kStageBufBytes; };
+            auto store_maxes = [&](uint32_t k, int c0, int p0) {      // elected thread: side tile of chunk k
+                const uint32_t src = smem_u32(buf_of(k) + kStageTileBytes);
+                tma_store_2d(&mmap, src, c0 >> 3, mid + 1 + p0);
+                tma_store_2d(&mmap, src + 8 * 16 * 2, c0 >> 3, mid - 1 - p0 - 7);
+            };
+            // one pipeline step: consume (x, y) = chunk (tile, g, i), prefetch the next into (nx, ny)
+            auto step = [&](uint32_t (&x)[16], uint32_t (&y)[16], uint32_t (&nx)[16], uint32_t (&ny)[16]) {
+                int64_t ntile = tile;
+                int ng = g, ni = i + 1;
+                uint32_t nitem = item;
+                if (ni == nmine) {
+                    ni = 0;
+                    ++nitem;
+                    if (++ng == ngroups) {
+                        ng = 0;
+                        ntile += tstep;
+                    }
+                }
+                const bool have_next = ntile < ntiles;
+                tmem_wait16(x, y);
+                bool fetched = false;
+                if (have_next && (nitem == item || mbar_test(tfull(nitem & 1u), (nitem >> 1) & 1u))) {
+                    if (nitem != item) tc_fence_after();
+                    issue_ld(nitem, ni, nx, ny);
+                    fetched = true;
+                }
+                if (nitem != item) {
+                    // every load of this stage has landed in registers: hand it back to the MMA warp
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(tempty(item & 1u));
+                }
+                if (g == 0 && i == 0 && wg == 2) zero_row_out<PLANE16>(mid, tile * kTileR + col, p, lane);
+                const int p0 = (g * gch + wg + 3 * i) * 8;
+                const int c0 = (int)(tile * kTileR);
+                if (FDAS_TC_DIAG != 1) {
+                    MaxRegs mr;
+                    if (n > 0) block_max_load<PLANE16>(buf_of(n - 1), tw, &mr);
+                    unsigned char* sbuf = buf_of(n);
+                    chunk_to_smem<PLANE16>(x, y, sbuf, col);
+                    if (n > 0)
+                        block_max_finish<PLANE16>(mr, reinterpret_cast<unsigned short*>(buf_of(n - 1) + kStageTileBytes), tw);
+                    if (elected) tma_wait_read_older();      // buffer n+1 (chunk n+1-kStageBufs) is free
+                    fence_async_smem();
+                    bar_sync_wg(1 + wg);
+                    if (elected) {
+                        if (p0 < npair) {
+                            const uint32_t src = smem_u32(sbuf);
+                            tma_store_2d(&tmap, src, c0, mid + 1 + p0);
+                            tma_store_2d(&tmap, src + 8 * 128 * (PLANE16 ? 2 : 4), c0, mid - 1 - p0 - 7);
+                        }
+                        if (n > 0 && prev_p0 < npair) store_maxes(n - 1, prev_c0, prev_p0);
+                        tma_commit();
+                    }
+                }
+                if (have_next && !fetched) {
+                    mbar_wait(tfull(nitem & 1u), (nitem >> 1) & 1u);
+                    tc_fence_after();
+                    issue_ld(nitem, ni, nx, ny);
+                }
+                prev_c0 = c0;
+                prev_p0 = p0;
+                tile = ntile;
+                g = ng;
+                i = ni;
+                item = nitem;
+                ++n;
+            };
+            if (tile < ntiles) {
+                mbar_wait(tfull(0), 0);
+                tc_fence_after();
+                issue_ld(0, 0, ra, rb);
+            }
+            while (tile < ntiles) {
+                step(ra, rb, sa, sb);
+                if (tile >= ntiles) break;
+                step(sa, sb, ra, rb);
+            }
+            if (n > 0 && FDAS_TC_DIAG != 1) {
+                // the last chunk's block maxima
+                MaxRegs mr;
+                block_max_load<PLANE16>(buf_of(n - 1), tw, &mr);
+                block_max_finish<PLANE16>(mr, reinterpret_cast<unsigned short*>(buf_of(n - 1) + kStageTileBytes), tw);
+                fence_async_smem();
+                bar_sync_wg(1 + wg);
+                if (elected) {
+                    if (prev_p0 < npair) store_maxes(n - 1, prev_c0, prev_p0);
+                    tma_commit();
                 }
             }
-        }
-        if (pm.nval > 0) {
-            uint4 v0, v1;
-            pending_load(scratch, pm, lane, &v0, &v1);
-            pending_store<TAIL>(pm, lane, v0, v1);
+            if (elected) tma_wait_all();
         }
     }
 
@@ -430,27 +520,62 @@ int convolve_tc_smem_bytes(const ConvTcParams& p) {
     return need < 120 * 1024 ? 120 * 1024 : need;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libfdas.so does not link libcuda).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qr) != cudaSuccess ||
+            qr != cudaDriverEntryPointSuccess)
+            f = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(f);
+    }();
+    return fn;
+}
+
+// A row-major [rows][cols] array (row pitch `pitch` elements) as a 2-D tensor stored in boxes of
+// 8 rows x `box_cols`; rows outside [0, rows) (the padded tail of the bank) are clipped by the hardware.
+static cudaError_t make_map(void* base, int elem_bytes, bool is_float, int64_t cols, int64_t rows,
+                            int64_t pitch, int box_cols, CUtensorMap* map) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return cudaErrorNotSupported;
+    const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)pitch * elem_bytes};
+    const cuuint32_t box[2] = {(cuuint32_t)box_cols, 8u};
+    const cuuint32_t estr[2] = {1u, 1u};
+    const CUresult r = enc(map, is_float ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT16, 2,
+                           base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 template <int PLANE16>
-static cudaError_t launch_tc_maxc(const ConvTcParams& p, int nsm, cudaStream_t st) {
+static cudaError_t launch_tc(const ConvTcParams& p, int nsm, cudaStream_t st) {
     const int smem = convolve_tc_smem_bytes(p);
-    const int maxc = (p.gch + 2) / 3;
-    const bool tail = ((p.nz - 1) / 2) % 8 != 0;
-    auto go = [&](auto kern) -> cudaError_t {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        const int64_t ntiles = p.nbins / tc::kTileR;
-        const unsigned grid = (unsigned)(ntiles < nsm ? ntiles : nsm);
-        kern<<<grid, tc::kThreads, smem, st>>>(p);
-        return cudaGetLastError();
-    };
-    if (tail) return maxc == 1 ? go(tc::convolve_tc_kernel<PLANE16, 1, 1>) : go(tc::convolve_tc_kernel<PLANE16, 2, 1>);
-    return maxc == 1 ? go(tc::convolve_tc_kernel<PLANE16, 1, 0>) : go(tc::convolve_tc_kernel<PLANE16, 2, 0>);
+    CUtensorMap pmap, mmap;
+    cudaError_t e = make_map(p.plane, PLANE16 ? 2 : 4, !PLANE16, p.nbins, p.nz, p.pitch, tc::kTileR, &pmap);
+    if (e != cudaSuccess) return e;
+    e = make_map(p.maxplane, 2, false, p.nbins / 8, p.nz, p.mpitch, tc::kTileR / 8, &mmap);
+    if (e != cudaSuccess) return e;
+    auto kern = tc::convolve_tc_kernel<PLANE16>;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    const int64_t ntiles = p.nbins / tc::kTileR;
+    const unsigned grid = (unsigned)(ntiles < nsm ? ntiles : nsm);
+    kern<<<grid, tc::kThreads, smem, st>>>(p, pmap, mmap);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_convolve_tc(int plane16, const ConvTcParams& p, int nsm, cudaStream_t st) {
-    if (p.nbins % tc::kTileR != 0 || p.kp % 16 != 0 || p.gch < 1 || p.gch > 6 || (p.bimg_bytes & 15))
+    if (p.nbins % tc::kTileR != 0 || p.kp % 16 != 0 || p.gch < 1 || p.gch > 6 || (p.bimg_bytes & 15) ||
+        (reinterpret_cast<uintptr_t>(p.plane) & 15u) || ((p.pitch * (plane16 ? 2 : 4)) & 15))
         return cudaErrorInvalidValue;
-    return plane16 ? launch_tc_maxc<1>(p, nsm, st) : launch_tc_maxc<0>(p, nsm, st);
+    return plane16 ? launch_tc<1>(p, nsm, st) : launch_tc<0>(p, nsm, st);
 }
 
 }  // namespace fdas

@@ -12,7 +12,10 @@ namespace tc {
 constexpr int kThreads = 448;   // warp 0 producer, warp 1 MMA issuer, warps 2..13 epilogue
 constexpr int kHStages = 3;     // sliding-window (A operand) stages
 constexpr int kTileR = 128;     // Fourier bins per tile = MMA M = TMEM lanes
-constexpr int kEpiWarps = 12;
+constexpr int kEpiWarps = 12;   // three warpgroups
+constexpr int kStageTileBytes = 16 * 128 * 4;   // one staged chunk: 16 plane rows x 128 bins (fp32)
+constexpr int kStageBufBytes = kStageTileBytes + 16 * 16 * 2;   // + its [16][16] bf16 block-max tile
+constexpr int kStageBufs = 4;                   // staged chunks in flight per warpgroup
 
 // K-major, no-swizzle shared-memory matrix descriptor: start address, LBO (between the two 8-element
 // K halves of one MMA), SBO (between 8-row groups), all in 16-byte units; version 1 (sm_100).
@@ -26,8 +29,8 @@ __host__ __device__ constexpr uint32_t instr_desc(int n) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 }
 
-// Shared-memory carve-up (dynamic, 128-byte aligned): B image | H stages (re, im) | staging | epilogue
-// scratch | barriers.
+// Shared-memory carve-up (dynamic, 128-byte aligned): B image | H stages (re, im) | slice staging |
+// epilogue tiles | barriers.
 struct Layout {
     int b_off, h_off, h_part, h_stage, st_off, st_part, sc_off, bar_off, total;
 };
@@ -40,7 +43,7 @@ __host__ __device__ inline Layout make_layout(int bimg_bytes, int kp) {
     l.st_off = l.h_off + kHStages * l.h_stage;
     l.st_part = ((kp + 136) * 2 + 127) & ~127;      // kp + 130 bf16 of the slice (incl. read slack)
     l.sc_off = l.st_off + 2 * l.st_part;
-    l.bar_off = l.sc_off + kEpiWarps * 2048;        // 2 buffers x 8 pairs x 32 lanes x 4 bytes per warp
+    l.bar_off = l.sc_off + (kEpiWarps / 4) * kStageBufs * kStageBufBytes;
     l.total = l.bar_off + 128;
     return l;
 }
