@@ -40,7 +40,9 @@ N_SM, LANES, SM_MAX_GHZ = 148, 128, 1.965
 ALU_PEAK_TFLOPS = N_SM * LANES * 2 * SM_MAX_GHZ / 1e3
 # dram__bytes_read.sum + dram__bytes_write.sum of one K2 launch from `ncu --set full`
 # (profiles/); None until captured for that (workload, precision).
-NCU_K2_TRAFFIC_BYTES = {("ska", "bf16"): 18.5e6 + 3.381e9}   # profiles/r01c_packed_fp32x2.md
+NCU_K2_TRAFFIC_BYTES = {("ska", "bf16"): 18.5e6 + 3.381e9,       # profiles/r01c_packed_fp32x2.md
+                        ("ska", "bf16_tc"): 17.4e6 + 3.383e9}   # profiles/r01d_tensor_core_k2.md
+TC_PRECISIONS = ("bf16_tc", "bf16_tc_plane16")
 
 
 def measured_peaks():
@@ -52,6 +54,30 @@ def measured_peaks():
         except Exception:
             pass
     return 6650.0, "fallback"
+
+
+def measured_tensor_peak():
+    """Dense bf16 TFLOP/s (cuBLAS burst figure: K2 is timed alone per launch), else the guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["bf16_tflops"]), "measured"
+        except Exception:
+            pass
+    return 1590.0, "fallback"
+
+
+def tc_mma_flops(info):
+    """Tensor-core flops one K2-TC launch issues (padded operand shapes, K2-TC): per tile of
+    128 bins, per group of gch chunks: ceil((2h+1)/16) K-steps x 2 parts (Re w, Im w) of a
+    128 x (16 gch) x 16 MMA."""
+    npair = (int(info.nz) - 1) // 2
+    kp = (2 * int(info.halfwidth) + 1 + 15) // 16 * 16
+    nch = (npair + 7) // 8
+    ngroups = (nch + 5) // 6
+    gch = (nch + ngroups - 1) // ngroups
+    ntiles = int(info.nbins) // 128
+    return ntiles * ngroups * (kp // 16) * 2 * (2 * 128 * 16 * gch * 16)
 
 
 def workload_for(name: str, inputs):
@@ -323,16 +349,40 @@ def run_cuda(args):
     k2_tflops = k2_flops / (t_conv * 1e-3) / 1e12
     k2_gbs = HBM_BYTES_PER_POINT[precision] * points / (t_conv * 1e-3) / 1e9
     plane_bytes = points * int(info.plane_elem_bytes)
-    k3_gbs = plane_bytes / (t_harm * 1e-3) / 1e9
+    k3_gbs = int(info.nz) * (int(info.nbins) // 8) * 2 / (t_harm * 1e-3) / 1e9
+    is_tc = precision in TC_PRECISIONS
+    k2_name = "K2-TC convolve_tc_kernel" if is_tc else "K2 convolve_kernel"
+    if is_tc:
+        # dense contraction on the tensor cores: the plane write is the binding roof (K2-TC)
+        tpeak, tkind = measured_tensor_peak()
+        tflops = tc_mma_flops(info) / (t_conv * 1e-3) / 1e12
+        roofline = {
+            "kernel": k2_name, "bound": "hbm", "achieved": k2_gbs, "peak": hbm_peak, "unit": "GB/s",
+            "frac": k2_gbs / hbm_peak, "traffic": NCU_K2_TRAFFIC_BYTES.get((args.workload, precision)),
+            "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json)",
+            "bytes_per_launch": HBM_BYTES_PER_POINT[precision] * points,
+            "tensor": {"achieved": tflops, "peak": tpeak, "unit": "TFLOP/s", "frac": tflops / tpeak,
+                       "peak_kind": f"{tkind} cuBLAS bf16 burst", "flops_per_launch": tc_mma_flops(info)},
+        }
+    else:
+        roofline = {
+            "kernel": k2_name, "bound": "alu", "achieved": k2_tflops, "peak": ALU_PEAK_TFLOPS,
+            "unit": "TFLOP/s", "frac": k2_tflops / ALU_PEAK_TFLOPS,
+            "traffic": NCU_K2_TRAFFIC_BYTES.get((args.workload, precision)),
+            "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz",
+            "flops_per_launch": k2_flops,
+        }
 
+    arith = "bf16 operands, fp32 accumulation on the tensor cores" if is_tc else "fp32 arithmetic"
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ctx.world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": t_max_ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16 x bf16 -> f32 (tensor cores)" if is_tc else "f32", "data": "synthetic",
         "config": {
             "workload": f"{wl.name}: N={wl.n} samples at {wl.tsamp * 1e6:.0f} us, nfft={info.nfft}, nz={info.nz} "
                         f"(zmax={wl.zmax:g}), seg_len={info.seg_len}, h={info.halfwidth}, S={info.nseg}, H={wl.nharm}, "
-                        f"{wl.nsigma:g} sigma, storage={precision} (fp32 arithmetic)",
+                        f"{wl.nsigma:g} sigma, storage={precision} ({arith})",
             "precision": precision, "plane_points_per_step": points,
             "parallelism": f"dm-trial replicas x{ctx.world} (no data-path collective)",
             "l2": f"plane of {plane_bytes / 1e9:.2f} GB per step exceeds the 126 MB L2; input pool of "
@@ -345,22 +395,18 @@ def run_cuda(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": wl.n * 4,
                 "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps,
                 "api": "fdas_search_host (pinned host series -> candidates on host), wall clock"},
-        "roofline": {
-            "kernel": "K2 convolve_kernel", "bound": "alu", "achieved": k2_tflops, "peak": ALU_PEAK_TFLOPS,
-            "unit": "TFLOP/s", "frac": k2_tflops / ALU_PEAK_TFLOPS,
-            "traffic": NCU_K2_TRAFFIC_BYTES.get((args.workload, precision)),
-            "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz",
-            "flops_per_launch": k2_flops,
-        },
+        "roofline": roofline,
         "roofline_hbm": {
-            "kernel": "K2 convolve_kernel", "bound": "hbm", "achieved": k2_gbs, "peak": hbm_peak, "unit": "GB/s",
+            "kernel": k2_name, "bound": "hbm", "achieved": k2_gbs, "peak": hbm_peak, "unit": "GB/s",
             "frac": k2_gbs / hbm_peak, "peak_kind": f"{peak_kind} copy bandwidth",
             "bytes_per_point": HBM_BYTES_PER_POINT[precision], "frac_of_8TBs_nominal": k2_gbs / 8000.0,
         },
         "roofline_k3": {
-            "kernel": "K3 harmonic_kernel", "bound": "hbm", "achieved": k3_gbs, "peak": hbm_peak, "unit": "GB/s",
-            "frac": k3_gbs / hbm_peak, "note": "algorithmic bytes = one read of the plane; the stride-k gathers "
-                                               "touch ~3.2x that in 32-byte sectors (DESIGN.md)",
+            "kernel": "K3 prefilter_kernel + exact_kernel + flag_kernel", "bound": "hbm", "achieved": k3_gbs,
+            "peak": hbm_peak, "unit": "GB/s", "frac": k3_gbs / hbm_peak,
+            "note": "algorithmic bytes = one read of the bf16 block-max side plane (nz x Nb/8) that the "
+                    "branch-and-bound prefilter scans; K3 is bound by its own select arithmetic, not by DRAM "
+                    "(profiles/r01c: ALU pipe 45 %, 0.22 GB read per launch)",
         },
         "clocks": sampler.summary(),
     }
@@ -468,14 +514,29 @@ def run_batch(args):
     hbm_peak, peak_kind = measured_peaks()
     k2_flops = sum(p["ntr"] * int(p["plan"].info.nseg) * (int(p["plan"].info.nz) * (
         FLOP_IFFT + FLOP_MUL + 3 * int(p["plan"].info.valid)) + FLOP_IFFT) for p in parts)
+    is_tc = precision in TC_PRECISIONS
+    arith = "bf16 operands, fp32 accumulation on the tensor cores" if is_tc else "fp32 arithmetic"
+    hbm_gbs = HBM_BYTES_PER_POINT[precision] * points / (t_max_ms * 1e-3) / 1e9
+    if is_tc:
+        batch_roofline = {"kernel": "K2-TC convolve_tc_kernel's algorithmic bytes of all trials over the whole pipelined time",
+                          "bound": "hbm", "achieved": hbm_gbs, "peak": hbm_peak, "unit": "GB/s",
+                          "frac": hbm_gbs / hbm_peak, "traffic": None,
+                          "note": "per-kernel rooflines are reported by the single-trial workload (--workload ska)"}
+    else:
+        batch_roofline = {"kernel": "K2 convolve_kernel's algorithmic flops of all trials over the whole pipelined time",
+                          "bound": "alu", "achieved": k2_flops / (t_max_ms * 1e-3) / 1e12, "peak": ALU_PEAK_TFLOPS,
+                          "unit": "TFLOP/s", "frac": k2_flops / (t_max_ms * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+                          "traffic": None,
+                          "note": "per-kernel rooflines are reported by the single-trial workload (--workload ska)"}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ctx.world, "steps": trials,
         "warmup": args.warmup, "ms_per_step": t_max_ms / trials, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16 x bf16 -> f32 (tensor cores)" if is_tc else "f32", "data": "synthetic",
         "config": {
             "workload": (f"{args.workload}: " + " + ".join(
                 f"{p['ntr']} trials of N={p['wl'].n} at {p['wl'].tsamp * 1e6:.0f} us (nfft={p['plan'].info.nfft})"
-                for p in parts) + f", nz=193, seg_len=2048, H=16, 6 sigma, storage={precision} (fp32 arithmetic)"),
+                for p in parts) + f", nz=193, seg_len=2048, H=16, 6 sigma, storage={precision} ({arith})"),
             "precision": precision, "plane_points_total": points,
             "parallelism": f"dm-trial replicas x{ctx.world} (no data-path collective)",
             "pipeline": "fdas_search_batch: copy / prepare+K2 / K3+D2H streams, two slots of every per-trial buffer",
@@ -489,10 +550,7 @@ def run_batch(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "steps": trials, "seconds": t_e2e,
                 "api": "fdas_search_batch (pinned host series -> candidates on host), wall clock"},
-        "roofline": {"kernel": "K2 convolve_kernel's algorithmic flops of all trials over the whole pipelined time",
-                     "bound": "alu", "achieved": k2_flops / (t_max_ms * 1e-3) / 1e12, "peak": ALU_PEAK_TFLOPS,
-                     "unit": "TFLOP/s", "frac": k2_flops / (t_max_ms * 1e-3) / 1e12 / ALU_PEAK_TFLOPS, "traffic": None,
-                     "note": "per-kernel rooflines are reported by the single-trial workload (--workload ska)"},
+        "roofline": batch_roofline,
         "roofline_hbm": {"bound": "hbm", "achieved": HBM_BYTES_PER_POINT[precision] * points / (t_max_ms * 1e-3) / 1e9,
                          "peak": hbm_peak, "unit": "GB/s", "peak_kind": f"{peak_kind} copy bandwidth",
                          "note": "K2's algorithmic bytes of all trials over the whole pipelined time"},
@@ -523,7 +581,7 @@ def main():
                     help="length of the separate energy loop (0 = off)")
     ap.add_argument("--trials", type=int, default=0,
                     help="batched/survey: trials per rank (0 = 64 for batched, 3050+2875 for survey)")
-    ap.add_argument("--precision", default="bf16", choices=["fp32", "bf16", "bf16_plane16", "bf16_tc", "bf16_tc_plane16"])
+    ap.add_argument("--precision", default="bf16_tc", choices=["fp32", "bf16", "bf16_plane16", "bf16_tc", "bf16_tc_plane16"])
     ap.add_argument("--pool", type=int, default=4, help="distinct series cycled per rank")
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle plane work")

@@ -37,15 +37,12 @@ namespace fdas {
 namespace tc {
 
 // Timing experiments only (never set in the product build): 1 = epilogue skips its arithmetic and
-// stores, 2 = the MMA issuer skips the MMAs.
+// stores, 2 = the MMA issuer skips the MMAs, 3 = no block maxima, 4 = no TMA stores.
 #ifndef FDAS_TC_DIAG
 #define FDAS_TC_DIAG 0
 #endif
-#ifndef FDAS_TC_SLEEP_PROD
-#define FDAS_TC_SLEEP_PROD 2000
-#endif
-#ifndef FDAS_TC_SLEEP_MMA
-#define FDAS_TC_SLEEP_MMA 100
+#ifndef FDAS_TC_WAIT_HINT
+#define FDAS_TC_WAIT_HINT 20000
 #endif
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
@@ -68,21 +65,19 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "DONE_%=:\n\t"
         "}" ::"r"(bar), "r"(parity) : "memory");
 }
-// Same, for the two single-warp roles that wait most of the time (producer, MMA issuer): back off
-// between polls so that the spinning warp does not take issue slots from the epilogue warps of its
-// scheduler.
-__device__ __forceinline__ void mbar_wait_backoff(uint32_t bar, uint32_t parity, unsigned ns) {
-    for (;;) {
-        uint32_t ok;
-        asm volatile(
-            "{\n\t"
-            ".reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t"
-            "}" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-        if (ok) return;
-        __nanosleep(ns);
-    }
+// Same for the two single-warp roles that wait most of the time (producer, MMA issuer): the thread
+// is suspended in hardware until the phase completes or the time hint (ns) runs out, so the waiting
+// warp does not take issue slots from the epilogue warps of its scheduler.
+__device__ __forceinline__ void mbar_wait_suspend(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "WAITH_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
+        "@p bra DONEH_%=;\n\t"
+        "bra WAITH_%=;\n\t"
+        "DONEH_%=:\n\t"
+        "}" ::"r"(bar), "r"(parity), "r"((unsigned)FDAS_TC_WAIT_HINT) : "memory");
 }
 // One poll (the hardware may block for a short system-dependent time): true if the phase completed.
 __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
@@ -319,7 +314,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
         int it = 0;
         for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
             const int hs = it % kHStages;
-            mbar_wait_backoff(hempty(hs), ((it / kHStages) & 1) ^ 1, FDAS_TC_SLEEP_PROD);
+            mbar_wait_suspend(hempty(hs), ((it / kHStages) & 1) ^ 1);
             const int64_t base = tile * kTileR - p.h;
             for (int i = lane; i < nsrc; i += 32) {
                 const int64_t idx = base + i;
@@ -350,13 +345,13 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
             uint32_t item = 0;
             for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
                 const int hs = it % kHStages;
-                mbar_wait_backoff(hfull(hs), (it / kHStages) & 1, FDAS_TC_SLEEP_MMA);
+                mbar_wait_suspend(hfull(hs), (it / kHStages) & 1);
                 tc_fence_after();
                 const uint32_t a_re = smem_u32(smem + L.h_off + hs * L.h_stage);
                 const uint32_t a_im = a_re + L.h_part;
                 for (int g = 0; g < p.ngroups; ++g, ++item) {
                     const uint32_t st = item & 1u;
-                    mbar_wait_backoff(tempty(st), ((item >> 1) & 1u) ^ 1u, FDAS_TC_SLEEP_MMA);
+                    mbar_wait_suspend(tempty(st), ((item >> 1) & 1u) ^ 1u);
                     tc_fence_after();
                     const uint32_t d1 = tmem_base + st * 256u, d2 = d1 + 128u;
                     const uint32_t bbase = smem_u32(smem + L.b_off) + (uint32_t)(g * p.gch * 2) * 128u;
@@ -445,15 +440,15 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
                 const int c0 = (int)(tile * kTileR);
                 if (FDAS_TC_DIAG != 1) {
                     MaxRegs mr;
-                    if (n > 0) block_max_load<PLANE16>(buf_of(n - 1), tw, &mr);
+                    if (n > 0 && FDAS_TC_DIAG != 3) block_max_load<PLANE16>(buf_of(n - 1), tw, &mr);
                     unsigned char* sbuf = buf_of(n);
                     chunk_to_smem<PLANE16>(x, y, sbuf, col);
-                    if (n > 0)
+                    if (n > 0 && FDAS_TC_DIAG != 3)
                         block_max_finish<PLANE16>(mr, reinterpret_cast<unsigned short*>(buf_of(n - 1) + kStageTileBytes), tw);
                     if (elected) tma_wait_read_older();      // buffer n+1 (chunk n+1-kStageBufs) is free
                     fence_async_smem();
                     bar_sync_wg(1 + wg);
-                    if (elected) {
+                    if (elected && FDAS_TC_DIAG != 4) {
                         if (p0 < npair) {
                             const uint32_t src = smem_u32(sbuf);
                             tma_store_2d(&tmap, src, c0, mid + 1 + p0);
