@@ -18,6 +18,8 @@
 // fdas_convolve_plane of this plan (hand-made planes), M is first rebuilt from it (build_max_kernel).
 #include <cuda_bf16.h>
 
+#include <algorithm>
+
 #include "fdas_kernels.h"
 
 namespace fdas {
@@ -147,8 +149,8 @@ __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
 // picks element (k i) >> 3 of them -- a compile-time register choice once k and i are unrolled.  The
 // loads of harmonics 1..4 (then 5-6, 7-8, then one harmonic at a time) are all issued before the
 // first add: the kernel moves < 1 GB and would otherwise be bound by DRAM latency, not bandwidth.
-// One FADD, one FSETP and one predicated OR per (fundamental, harmonic); fundamentals with any
-// U_h > T_h go to the maybe list as (r, j).
+// One FADD, one FSETP and one predicated OR per (fundamental, harmonic) for h >= 3 (h = 1, 2 are
+// evaluated once per block / half block); fundamentals with any U_h > T_h go to the maybe list as (r, j).
 constexpr int kPfThreads = 128;
 
 // Harmonic K for the 32 fundamentals of quad-block Q, all of them valid (K (32Q+31) <= Nb-1).
@@ -210,28 +212,103 @@ __device__ __forceinline__ void pf_single_from(const HarmParams& p, const int j,
     }
 }
 
-__global__ void __launch_bounds__(kPfThreads) prefilter_kernel(const HarmParams p) {
-    const int j = blockIdx.y;
+// Fundamentals of quad-block Q flagged by pass A go to the maybe list as (r, j).
+__device__ __forceinline__ void pf_emit(const HarmParams& p, const unsigned Q, const int j, unsigned flagged) {
+    // r < r_lo never yields candidates
+    if (32 * (int64_t)Q < p.r_lo) {
+        const int64_t cut = p.r_lo - 32 * (int64_t)Q;
+        flagged = (cut >= 32) ? 0u : (flagged & ~((1u << (int)cut) - 1u));
+    }
+    if (flagged) {
+        const int n = __popc(flagged);
+        const unsigned long long base = atomicAdd(p.maybe_count, (unsigned long long)n);
+        if (base + (unsigned long long)n <= (unsigned long long)p.maybe_capacity) {
+            unsigned long long slot = base;
+            while (flagged) {
+                const int i = __ffs(flagged) - 1;
+                flagged &= flagged - 1;
+                p.maybe[slot++] = make_uint2(32u * Q + (unsigned)i, (unsigned)j);
+            }
+        } else {
+            atomicExch(p.overflow, 1u);   // pass B then falls back to the full scan
+        }
+    }
+}
+
+// Rows with one or two harmonics only (|z| > zmax/3: the nlow first and the nlow last rows, two thirds
+// of the plane).  U_1 is the same for the 8 fundamentals of a block and U_2 for the 4 of a half block,
+// so nothing is evaluated per fundamental: a thread streams 8 blocks (64 fundamentals) of M[j] and, for
+// hz = 2, the 16 blocks of M[row_2] they map to.  Few registers, every load issued up front: this pass
+// is a plain scan of 0.15 GB.
+constexpr int kPfShallowThreads = 256;
+__global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(const HarmParams p, const int nlow) {
+    const int y = blockIdx.y;
+    const int j = y < nlow ? y : p.nz - 2 * nlow + y;
+    const int c2 = p.nz - 1;
+    const unsigned O = blockIdx.x * (unsigned)kPfShallowThreads + threadIdx.x;   // octet of blocks
+    if (O >= (unsigned)(p.mpitch >> 3)) return;
+    const unsigned last = (unsigned)(p.nbins - 1);
+    const int d = abs(2 * j - c2);
+    const int hz = d == 0 ? p.H : min(p.H, c2 / d);          // 1 or 2 here
+    const PfRow r1 = pf_row(p, j, 1);
+    const uint4 a = __ldg(reinterpret_cast<const uint4*>(r1.mrow) + O);
+    // harmonic 2 of all 64 fundamentals inside the plane?
+    const bool two = hz >= 2 && 2u * (64u * O + 63u) <= last;
+    PfRow r2 = r1;
+    uint4 b0 = make_uint4(0, 0, 0, 0), b1 = b0;
+    if (hz >= 2) {
+        r2 = pf_row(p, j, 2);
+        if (two) {
+            b0 = __ldg(reinterpret_cast<const uint4*>(r2.mrow) + 2 * O);
+            b1 = __ldg(reinterpret_cast<const uint4*>(r2.mrow) + 2 * O + 1);
+        }
+    }
+    const unsigned aw[4] = {a.x, a.y, a.z, a.w};
+    const unsigned bw[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+    unsigned f[2] = {0u, 0u};   // flags of fundamentals 64 O + 32 t + i
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {          // block q: fundamentals 8q..8q+7
+        const float m1 = (q & 1) ? bf16_hi(aw[q >> 1]) : bf16_lo(aw[q >> 1]);
+        if (m1 > r1.thr) f[q >> 2] |= 0xffu << (8 * (q & 3));
+        if (two) {
+            const float lo = bf16_lo(bw[q]), hi = bf16_hi(bw[q]);   // blocks 2q, 2q+1 of row_2
+            if (m1 + lo > r2.thr) f[q >> 2] |= 0x0fu << (8 * (q & 3));
+            if (m1 + hi > r2.thr) f[q >> 2] |= 0xf0u << (8 * (q & 3));
+        }
+    }
+    if (hz >= 2 && !two) {
+        // the thread that straddles r = (Nb-1)/2: harmonic 2 exists for its first fundamentals only
+        const unsigned rmax = last / 2u;
+        if (64u * O <= rmax) {
+            const int nv = (int)min(64u, rmax - 64u * O + 1u);
+            const unsigned short* src = r2.mrow + (size_t)16 * O;
+            const unsigned short* m1p = r1.mrow + (size_t)8 * O;
+            for (int i = 0; i < nv; ++i)
+                if (bf16_lo(__ldg(m1p + (i >> 3))) + bf16_lo(__ldg(src + (i >> 2))) > r2.thr)
+                    f[i >> 5] |= 1u << (i & 31);
+        }
+    }
+    pf_emit(p, 2u * O, j, f[0]);
+    pf_emit(p, 2u * O + 1u, j, f[1]);
+}
+
+__global__ void __launch_bounds__(kPfThreads) prefilter_kernel(const HarmParams p, const int nlow) {
+    const int j = nlow + blockIdx.y;   // the rows with three or more harmonics (|z| <= zmax/3)
     const int c2 = p.nz - 1;
     const unsigned Q0 = blockIdx.x * (unsigned)kPfThreads;
     const unsigned Q = Q0 + threadIdx.x;
     const unsigned nquad = (unsigned)(p.mpitch >> 2);   // nbins / 32
     if (Q >= nquad) return;
     const unsigned last = (unsigned)(p.nbins - 1);
-    // hz: harmonics inside the plane in z for this row (CTA-uniform, monotone in k)
-    int hz = 0;
-    for (int k = 1; k <= p.H; ++k) {
-        const int v2 = 2 * k * j - (k - 1) * c2;
-        if (v2 < 0 || v2 > 2 * c2) break;
-        hz = k;
-    }
+    // hz: harmonics inside the plane in z for this row (CTA-uniform): twice the row of harmonic k is
+    // v2 = k d + c2 with d = 2 j - c2, and 0 <= v2 <= 2 c2  <=>  k |d| <= c2
+    const int d = abs(2 * j - c2);
+    const int hz = d == 0 ? p.H : min(p.H, c2 / d);
     // he: harmonics for which all 32 fundamentals of this thread are inside the plane in r
     const int he = (int)min((unsigned)hz, last / (32u * Q + 31u));
     const int he_max = (int)min((unsigned)hz, last / (32u * Q0 + 31u));   // deepest in this CTA
     float U[32];
     unsigned flagged = 0u;   // bit i: some U_h of fundamental 32 Q + i exceeds T_h
-#pragma unroll
-    for (int i = 0; i < 32; ++i) U[i] = 0.f;
 
     {   // harmonics 1..4: ten 128-bit loads in flight
         const PfRow r1 = pf_row(p, j, 1);
@@ -241,8 +318,24 @@ __global__ void __launch_bounds__(kPfThreads) prefilter_kernel(const HarmParams 
         if (he_max >= 2) { r2 = pf_row(p, j, 2); pf_load<2>(r2.mrow, Q, he >= 2, m2); }
         if (he_max >= 3) { r3 = pf_row(p, j, 3); pf_load<3>(r3.mrow, Q, he >= 3, m3); }
         if (he_max >= 4) { r4 = pf_row(p, j, 4); pf_load<4>(r4.mrow, Q, he >= 4, m4); }
-        pf_add<1>(m1, r1.thr, true, U, flagged);
-        if (he_max >= 2) pf_add<2>(m2, r2.thr, he >= 2, U, flagged);
+        // U_1 is the same for the 8 fundamentals of a block and U_2 for the 4 fundamentals of a
+        // half block (harmonic k picks block (k i) >> 3): 4 + 8 sums and compares stand for 64 --
+        // h = 1, 2 are 79 % of all (r, j, h) triples of the SKA-like plane
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (m1[q] > r1.thr) flagged |= 0xffu << (8 * q);
+        if (he >= 2) {
+#pragma unroll
+            for (int gq = 0; gq < 8; ++gq) {
+                const float u2 = m1[gq >> 1] + m2[gq];
+                if (u2 > r2.thr) flagged |= 0xfu << (4 * gq);
+#pragma unroll
+                for (int e = 0; e < 4; ++e) U[4 * gq + e] = u2;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 32; ++i) U[i] = m1[i >> 3];
+        }
         if (he_max >= 3) pf_add<3>(m3, r3.thr, he >= 3, U, flagged);
         if (he_max >= 4) pf_add<4>(m4, r4.thr, he >= 4, U, flagged);
     }
@@ -273,25 +366,7 @@ __global__ void __launch_bounds__(kPfThreads) prefilter_kernel(const HarmParams 
         }
     }
 
-    // r < r_lo never yields candidates
-    if (32 * (int64_t)Q < p.r_lo) {
-        const int64_t cut = p.r_lo - 32 * (int64_t)Q;
-        flagged = (cut >= 32) ? 0u : (flagged & ~((1u << (int)cut) - 1u));
-    }
-    if (flagged) {
-        const int n = __popc(flagged);
-        const unsigned long long base = atomicAdd(p.maybe_count, (unsigned long long)n);
-        if (base + (unsigned long long)n <= (unsigned long long)p.maybe_capacity) {
-            unsigned long long slot = base;
-            while (flagged) {
-                const int i = __ffs(flagged) - 1;
-                flagged &= flagged - 1;
-                p.maybe[slot++] = make_uint2(32u * Q + (unsigned)i, (unsigned)j);
-            }
-        } else {
-            atomicExch(p.overflow, 1u);   // pass B then falls back to the full scan
-        }
-    }
+    pf_emit(p, Q, j, flagged);
 }
 
 // ---- pass B: one thread per maybe record (r, j): the plain definition on the real plane.
@@ -356,10 +431,29 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
     }
-    dim3 grid((unsigned)((p.mpitch / 4 + kPfThreads - 1) / kPfThreads), (unsigned)p.nz), block(kPfThreads);
-    prefilter_kernel<<<grid, block, 0, st>>>(p);
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    ++*launches;
+    // rows j < nlow and j >= nz - nlow have at most two harmonics inside the plane (reading A12)
+    int nlow = 0;
+    if ((p.mpitch & 7) == 0) {   // the shallow pass streams octets of blocks
+        const int c2 = p.nz - 1;
+        while (2 * nlow < p.nz - 1) {
+            const int d = c2 - 2 * nlow;                       // |2 j - c2| for j = nlow (< mid)
+            if ((d == 0 ? p.H : std::min(p.H, c2 / d)) > 2) break;
+            ++nlow;
+        }
+        if (p.H <= 2) nlow = p.nz / 2;                         // (nz odd: the z = 0 row goes to the general pass)
+    }
+    if (nlow > 0) {
+        dim3 grid((unsigned)((p.mpitch / 8 + kPfShallowThreads - 1) / kPfShallowThreads), (unsigned)(2 * nlow));
+        prefilter_shallow_kernel<<<grid, kPfShallowThreads, 0, st>>>(p, nlow);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        ++*launches;
+    }
+    if (p.nz - 2 * nlow > 0) {
+        dim3 grid((unsigned)((p.mpitch / 4 + kPfThreads - 1) / kPfThreads), (unsigned)(p.nz - 2 * nlow)), block(kPfThreads);
+        prefilter_kernel<<<grid, block, 0, st>>>(p, nlow);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        ++*launches;
+    }
     if (plane_is_bf16) exact_kernel<__nv_bfloat16><<<kExactBlocks, 128, 0, st>>>(p);
     else exact_kernel<float><<<kExactBlocks, 128, 0, st>>>(p);
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
