@@ -37,7 +37,8 @@ namespace fdas {
 namespace tc {
 
 // Timing experiments only (never set in the product build): 1 = epilogue skips its arithmetic and
-// stores, 2 = the MMA issuer skips the MMAs, 3 = no block maxima, 4 = no TMA stores.
+// stores, 2 = the MMA issuer skips the MMAs, 3 = no block maxima, 4 = no TMA stores,
+// 7 = every TMA store of a CTA goes to the same column block (no DRAM write stream).
 #ifndef FDAS_TC_DIAG
 #define FDAS_TC_DIAG 0
 #endif
@@ -437,7 +438,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
                 }
                 if (g == 0 && i == 0 && wg == 2) zero_row_out<PLANE16>(mid, tile * kTileR + col, p, lane);
                 const int p0 = (g * gch + wg + 3 * i) * 8;
-                const int c0 = (int)(tile * kTileR);
+                const int c0 = FDAS_TC_DIAG == 7 ? (int)(blockIdx.x * kTileR) : (int)(tile * kTileR);
                 if (FDAS_TC_DIAG != 1) {
                     MaxRegs mr;
                     if (n > 0 && FDAS_TC_DIAG != 3) block_max_load<PLANE16>(buf_of(n - 1), tw, &mr);

@@ -93,42 +93,61 @@ __global__ void __launch_bounds__(kMedThreads) block_median_kernel(const WhitenP
     }
 }
 
+// Twice the centre of block b (an integer): 2 c_b = 2 s_b + l_b - 1.
+__device__ __forceinline__ int64_t centre2(const WhitenParams& p, int b) {
+    return 2 * (int64_t)__ldg(p.blk_start + b) + __ldg(p.blk_len + b) - 1;
+}
+
+constexpr int kScaleThreads = 256;
+constexpr int kScalePer = 4;   // bins per thread, strided by the CTA width (coalesced)
+
+// One CTA scales kScaleThreads * kScalePer consecutive bins.  The bracketing pair of block centres is
+// found once per CTA by binary search for its first bin; every bin then walks forward from there (the
+// blocks are >= 32 bins long, usually 4096: a handful of steps at most).
 template <bool BF16>
-__global__ void __launch_bounds__(256) whiten_scale_kernel(const WhitenParams p) {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= p.nbins) return;
-    float2 w = make_float2(0.f, 0.f);
-    if (k > 0) {
-        // twice the block centres are integers: 2 c_b = 2 s_b + l_b - 1
-        const int64_t k2 = 2 * k;
-        const int last = p.nblk - 1;
-        const int64_t c2_first = 2 * (int64_t)p.blk_start[0] + p.blk_len[0] - 1;
-        const int64_t c2_last = 2 * (int64_t)p.blk_start[last] + p.blk_len[last] - 1;
-        float m;
-        if (k2 <= c2_first) m = p.blk_med[0];
-        else if (k2 >= c2_last) m = p.blk_med[last];
-        else {
-            int lo = 0, hi = last;  // c2[lo] <= k2 < c2[hi]
-            while (hi - lo > 1) {
-                const int mid = (lo + hi) >> 1;
-                const int64_t c2m = 2 * (int64_t)__ldg(p.blk_start + mid) + __ldg(p.blk_len + mid) - 1;
-                if (c2m <= k2) lo = mid; else hi = mid;
-            }
-            const int64_t c2lo = 2 * (int64_t)__ldg(p.blk_start + lo) + __ldg(p.blk_len + lo) - 1;
-            const int64_t c2hi = 2 * (int64_t)__ldg(p.blk_start + hi) + __ldg(p.blk_len + hi) - 1;
-            const float t = (float)(k2 - c2lo) / (float)(c2hi - c2lo);
-            const float mlo = p.blk_med[lo], mhi = p.blk_med[hi];
-            m = mlo + t * (mhi - mlo);
+__global__ void __launch_bounds__(kScaleThreads) whiten_scale_kernel(const WhitenParams p) {
+    __shared__ int s_lo;
+    const int64_t k0 = (int64_t)blockIdx.x * (kScaleThreads * kScalePer);
+    const int last = p.nblk - 1;
+    if (threadIdx.x == 0) {
+        int lo = 0, hi = last;   // largest lo with c2[lo] <= 2 k0 (0 if none)
+        const int64_t k2 = 2 * k0;
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (centre2(p, mid) <= k2) lo = mid; else hi = mid;
         }
-        const float sc = sqrtf(0.69314718055994530942f / m);
-        const float2 x = __ldg(p.X + k);
-        w = make_float2(x.x * sc, x.y * sc);
+        s_lo = lo;
     }
-    if (BF16) {
-        const __nv_bfloat162 pk = __floats2bfloat162_rn(w.x, w.y);  // .x (re) in the low half
-        reinterpret_cast<unsigned int*>(p.spec)[k] = *reinterpret_cast<const unsigned int*>(&pk);
-    } else {
-        reinterpret_cast<float2*>(p.spec)[k] = w;
+    __syncthreads();
+    const int64_t c2_first = centre2(p, 0), c2_last = centre2(p, last);
+    int lo = s_lo;
+#pragma unroll
+    for (int q = 0; q < kScalePer; ++q) {
+        const int64_t k = k0 + threadIdx.x + q * kScaleThreads;
+        if (k >= p.nbins) break;
+        float2 w = make_float2(0.f, 0.f);
+        if (k > 0) {
+            const int64_t k2 = 2 * k;
+            float m;
+            if (k2 <= c2_first) m = p.blk_med[0];
+            else if (k2 >= c2_last) m = p.blk_med[last];
+            else {
+                while (lo + 1 < last && centre2(p, lo + 1) <= k2) ++lo;   // c2[lo] <= k2 < c2[lo+1]
+                const int64_t c2lo = centre2(p, lo), c2hi = centre2(p, lo + 1);
+                const float t = (float)(k2 - c2lo) / (float)(c2hi - c2lo);
+                const float mlo = p.blk_med[lo], mhi = p.blk_med[lo + 1];
+                m = mlo + t * (mhi - mlo);
+            }
+            const float sc = sqrtf(0.69314718055994530942f / m);
+            const float2 x = __ldg(p.X + k);
+            w = make_float2(x.x * sc, x.y * sc);
+        }
+        if (BF16) {
+            const __nv_bfloat162 pk = __floats2bfloat162_rn(w.x, w.y);  // .x (re) in the low half
+            reinterpret_cast<unsigned int*>(p.spec)[k] = *reinterpret_cast<const unsigned int*>(&pk);
+        } else {
+            reinterpret_cast<float2*>(p.spec)[k] = w;
+        }
     }
 }
 
@@ -136,9 +155,10 @@ cudaError_t launch_whiten(int precision, const WhitenParams& p, cudaStream_t st)
     block_median_kernel<<<p.nblk, kMedThreads, 0, st>>>(p);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const unsigned grid = (unsigned)((p.nbins + 255) / 256);
-    if (precision == FDAS_FP32) whiten_scale_kernel<false><<<grid, 256, 0, st>>>(p);
-    else whiten_scale_kernel<true><<<grid, 256, 0, st>>>(p);
+    const int per_cta = kScaleThreads * kScalePer;
+    const unsigned grid = (unsigned)((p.nbins + per_cta - 1) / per_cta);
+    if (precision == FDAS_FP32) whiten_scale_kernel<false><<<grid, kScaleThreads, 0, st>>>(p);
+    else whiten_scale_kernel<true><<<grid, kScaleThreads, 0, st>>>(p);
     return cudaGetLastError();
 }
 
