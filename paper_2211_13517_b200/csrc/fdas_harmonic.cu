@@ -292,7 +292,10 @@ __global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(co
     pf_emit(p, 2u * O + 1u, j, f[1]);
 }
 
-__global__ void __launch_bounds__(kPfThreads) prefilter_kernel(const HarmParams p, const int nlow) {
+#ifndef FDAS_PF_MINB
+#define FDAS_PF_MINB 8
+#endif
+__global__ void __launch_bounds__(kPfThreads, FDAS_PF_MINB) prefilter_kernel(const HarmParams p, const int nlow) {
     const int j = nlow + blockIdx.y;   // the rows with three or more harmonics (|z| <= zmax/3)
     const int c2 = p.nz - 1;
     const unsigned Q0 = blockIdx.x * (unsigned)kPfThreads;
