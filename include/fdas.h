@@ -142,7 +142,8 @@ int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const 
 
 /*
  * fdas_search_host -- the same three steps for a HOST time series (the end-to-end entry point):
- * copies h_series (n_in floats) to the device, runs prepare -> convolve -> harmonic_sum_peaks on
+ * copies the first nfft of h_series' n_in floats (the samples the transform uses, reading A1) to the
+ * device, runs prepare -> convolve -> harmonic_sum_peaks on
  * `cuda_stream`, copies the count and the first min(count, capacity) candidates back and waits for
  * them.  Device workspace (series, spectrum, plane, candidates) is allocated on first use and owned
  * by the plan.  Returns FDAS_EOVERFLOW (after copying `capacity` records) if count > capacity.

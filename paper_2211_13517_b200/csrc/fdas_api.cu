@@ -275,7 +275,8 @@ int fdas_search_host(fdas_plan_t plan, const float* h_series, int H, const float
         CU(cudaMalloc(&plan->ws_cands, (size_t)capacity * sizeof(fdas_cand_t)));
         plan->ws_cap = capacity;
     }
-    CU(cudaMemcpyAsync(plan->ws_series, h_series, (size_t)in.n_in * sizeof(float), cudaMemcpyHostToDevice, st));
+    // only the first nfft samples enter the transform (reading A1): the tail is not copied
+    CU(cudaMemcpyAsync(plan->ws_series, h_series, (size_t)in.nfft * sizeof(float), cudaMemcpyHostToDevice, st));
     int rc = fdas_prepare_spectrum(plan, plan->ws_series, plan->ws_spec, cuda_stream);
     if (rc != FDAS_OK) return rc;
     rc = fdas_convolve_plane(plan, plan->ws_spec, plan->ws_plane, cuda_stream);

@@ -130,15 +130,23 @@ extern "C" int fdas_search_batch(fdas_plan_t plan, const float* const* series, i
     CU(cudaStreamWaitEvent(s->b, s->entry, 0));
 
     bool overflow = false;
+    // host series: the copies run two trials ahead of the kernels (both slots are filled up front;
+    // slot sl is refilled with trial t+2 as soon as the spectrum of trial t exists), so that a copy
+    // never waits for the host to come back from collecting an earlier trial's candidates
+    auto queue_copy = [&](int t) -> int {
+        const int sl = t & 1;
+        CU(cudaMemcpyAsync(s->series[sl], series[t], (size_t)in.nfft * sizeof(float),   // reading A1: nfft samples used
+                           cudaMemcpyHostToDevice, s->copy));
+        CU(cudaEventRecord(s->in_ready[sl], s->copy));
+        return FDAS_OK;
+    };
+    if (series_on_host)
+        for (int t = 0; t < std::min(2, ntrials); ++t)
+            if ((rc = queue_copy(t)) != FDAS_OK) return rc;
     for (int t = 0; t < ntrials; ++t) {
         const int sl = t & 1;
         const float* d_series = series[t];
         if (series_on_host) {
-            // slot's series buffer is free once the spectrum of trial t-2 exists
-            if (t >= 2) CU(cudaStreamWaitEvent(s->copy, s->spec_done[sl], 0));
-            CU(cudaMemcpyAsync(s->series[sl], series[t], (size_t)in.n_in * sizeof(float),
-                               cudaMemcpyHostToDevice, s->copy));
-            CU(cudaEventRecord(s->in_ready[sl], s->copy));
             CU(cudaStreamWaitEvent(s->a, s->in_ready[sl], 0));
             d_series = s->series[sl];
         }
@@ -146,6 +154,10 @@ extern "C" int fdas_search_batch(fdas_plan_t plan, const float* const* series, i
         rc = fdas_enqueue_prepare(plan, d_series, s->spec[sl], s->a);
         if (rc != FDAS_OK) return rc;
         CU(cudaEventRecord(s->spec_done[sl], s->a));
+        if (series_on_host && t + 2 < ntrials) {
+            CU(cudaStreamWaitEvent(s->copy, s->spec_done[sl], 0));   // the slot's series has been consumed
+            if ((rc = queue_copy(t + 2)) != FDAS_OK) return rc;
+        }
         // plane[sl] / maxplane[sl] are free once K3 (and its flag pass) of trial t-2 is done
         if (t >= 2) CU(cudaStreamWaitEvent(s->a, s->k3_done[sl], 0));
         rc = fdas_enqueue_convolve(plan, s->spec[sl], s->plane[sl], s->maxplane[sl], s->a);
