@@ -242,6 +242,40 @@ def test_harmonic_sum_alone_many_candidates(fdas, torch_, oracle, precision):
     assert set(gpu_cand_dict(small.cands)) <= set(gpu_cand_dict(res.cands))
 
 
+@pytest.mark.parametrize("H", [1, 2, 3, 5])
+def test_harmonic_sum_small_h_exact_sets(fdas, torch_, oracle, H):
+    """K3 on a hand-made plane for small harmonic counts: with H <= 2 every row but z = 0 goes
+    through the streaming shallow pass, H = 3, 5 mix both passes; the threads that straddle
+    r = (Nb-1)/k (harmonic k defined for their first fundamentals only) and an r_lo inside a block
+    are exercised.  fp32 plane, so the candidate set must be the oracle's exactly (up to rounding
+    at the threshold)."""
+    torch = torch_
+    plan = fdas.Plan(1 << 13, 64e-6, 16.0, 1.0, 2048, "fp32")      # nbins = 4096: few CTAs per row
+    nb, nz = plan.info.nbins, plan.info.nz
+    rng = np.random.default_rng(23 + H)
+    P32 = rng.exponential(1.0, size=(nz, nb)).astype(np.float32)
+    # spikes around the harmonic cut-offs r = (Nb-1)/k and at the plane's corners
+    for k in (1, 2, 3):
+        rc = (nb - 1) // k
+        for dr in (-33, -2, -1, 0):
+            P32[:, min(nb - 1, max(0, rc + dr))] += 9.0
+    P32[0, 0] += 50.0; P32[nz - 1, nb - 1] += 50.0; P32[nz // 2, 77] += 50.0
+    d_plane = torch.from_numpy(P32).cuda()
+    P = P32.astype(np.float64)
+    thr = fdas.thresholds_from_sigma(H, 2.5)
+    r_lo = 37
+    d_c, d_n = plan.alloc_cands(1 << 18)
+    plan.harmonic_sum_peaks(d_plane, H, thr, r_lo, d_c, d_n)
+    torch.cuda.synchronize()
+    res = plan.read_cands(d_c, d_n)
+    oc = oracle.candidates(P, H, thr.astype(np.float64), r_lo)
+    assert oc.count > 200 and res.count == len(res.cands)
+    s_at, margin = oracle_margin_fn(oracle, P, H, r_lo)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * P.max(), None, s_at, margin)
+    assert stats["only_gpu"] + stats["only_orc"] <= 2, stats
+    assert min(k[0] for k in gpu_cand_dict(res.cands)) >= r_lo
+
+
 def test_abi_errors_on_device(fdas, torch_):
     import ctypes as C
     torch = torch_
