@@ -73,7 +73,16 @@ static int build_plan(fdas_plan_s* p) {
     build_bank(in.zmax, in.zstep, in.nz, in.halfwidth, in.seg_len, &bank);
     p->bank_time = bank.time;
     if (fdas_is_tc(in.precision)) {
-        if (!tc_geometry(in.nz, in.halfwidth, &p->tc) || in.nbins % 128 != 0) {
+        bool fits = tc_geometry(in.nz, in.halfwidth, &p->tc) && in.nbins % 128 == 0;
+        if (fits) {   // bank image + window stages + epilogue tiles within the CTA's shared memory
+            ConvTcParams t{};
+            t.bimg_bytes = p->tc.bytes; t.kp = p->tc.kp;
+            int dev0 = 0, optin = 0;
+            CU(cudaGetDevice(&dev0));
+            CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev0));
+            fits = convolve_tc_smem_bytes(t) <= optin;
+        }
+        if (!fits) {
             g_detail = "FDAS_BF16_TC: template bank does not fit the tensor-core kernel";
             return FDAS_EUNSUPPORTED;
         }

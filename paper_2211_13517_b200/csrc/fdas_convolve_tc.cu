@@ -261,7 +261,7 @@ __device__ __forceinline__ void zero_row_out(const int mid, const int64_t r, con
 template <int PLANE16>
 __global__ void __launch_bounds__(kThreads, 1)
 convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tmap,
-                   const __grid_constant__ CUtensorMap mmap) {
+                   const __grid_constant__ CUtensorMap mmap, const __grid_constant__ CUtensorMap tmap1) {
     extern __shared__ __align__(128) unsigned char smem[];
     const Layout L = make_layout(p.bimg_bytes, p.kp);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -404,10 +404,38 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
                 tmem_ld16(tb + 128u, y);
             };
             auto buf_of = [&](uint32_t k) { return stage0 + (k % kStageBufs) * kStageBufBytes; };
-            auto store_maxes = [&](uint32_t k, int c0, int p0) {      // elected thread: side tile of chunk k
+            // elected thread: the staged rows of the chunk of pairs p0.. go out as two boxes of 8 rows;
+            // the bank's last chunk may hold fewer than 8 real pairs -- its rows go one by one (the
+            // other local rows belong to padded pairs, whose plane rows do not exist)
+            constexpr int kRowBytes = 128 * (PLANE16 ? 2 : 4);
+            auto store_tile = [&](uint32_t src, int c0, int p0) {
+                const int nval = npair - p0;
+                if (nval >= 8) {
+                    tma_store_2d(&tmap, src, c0, mid + 1 + p0);
+                    tma_store_2d(&tmap, src + 8 * kRowBytes, c0, mid - 1 - p0 - 7);
+                } else {
+                    for (int pp = 0; pp < nval; ++pp) {
+                        tma_store_2d(&tmap1, src + pp * kRowBytes, c0, mid + 1 + p0 + pp);
+                        tma_store_2d(&tmap1, src + (15 - pp) * kRowBytes, c0, mid - 1 - p0 - pp);
+                    }
+                }
+            };
+            auto store_maxes = [&](uint32_t k, int c0, int p0) {      // side tile of chunk k
                 const uint32_t src = smem_u32(buf_of(k) + kStageTileBytes);
-                tma_store_2d(&mmap, src, c0 >> 3, mid + 1 + p0);
-                tma_store_2d(&mmap, src + 8 * 16 * 2, c0 >> 3, mid - 1 - p0 - 7);
+                const int nval = npair - p0;
+                if (nval >= 8) {
+                    tma_store_2d(&mmap, src, c0 >> 3, mid + 1 + p0);
+                    tma_store_2d(&mmap, src + 8 * 16 * 2, c0 >> 3, mid - 1 - p0 - 7);
+                } else {
+                    // 32-byte rows are below the TMA's shared-memory alignment: plain 16-byte stores
+                    const uint4* t = reinterpret_cast<const uint4*>(buf_of(k) + kStageTileBytes);
+                    for (int pp = 0; pp < nval; ++pp) {
+                        uint4* up = reinterpret_cast<uint4*>(p.maxplane + (int64_t)(mid + 1 + p0 + pp) * p.mpitch + (c0 >> 3));
+                        uint4* dn = reinterpret_cast<uint4*>(p.maxplane + (int64_t)(mid - 1 - p0 - pp) * p.mpitch + (c0 >> 3));
+                        up[0] = t[2 * pp]; up[1] = t[2 * pp + 1];
+                        dn[0] = t[2 * (15 - pp)]; dn[1] = t[2 * (15 - pp) + 1];
+                    }
+                }
             };
             // one pipeline step: consume (x, y) = chunk (tile, g, i), prefetch the next into (nx, ny)
             auto step = [&](uint32_t (&x)[16], uint32_t (&y)[16], uint32_t (&nx)[16], uint32_t (&ny)[16]) {
@@ -450,11 +478,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
                     fence_async_smem();
                     bar_sync_wg(1 + wg);
                     if (elected && FDAS_TC_DIAG != 4) {
-                        if (p0 < npair) {
-                            const uint32_t src = smem_u32(sbuf);
-                            tma_store_2d(&tmap, src, c0, mid + 1 + p0);
-                            tma_store_2d(&tmap, src + 8 * 128 * (PLANE16 ? 2 : 4), c0, mid - 1 - p0 - 7);
-                        }
+                        if (p0 < npair) store_tile(smem_u32(sbuf), c0, p0);
                         if (n > 0 && prev_p0 < npair) store_maxes(n - 1, prev_c0, prev_p0);
                         tma_commit();
                     }
@@ -534,14 +558,14 @@ static EncodeTiledFn encode_tiled_fn() {
 }
 
 // A row-major [rows][cols] array (row pitch `pitch` elements) as a 2-D tensor stored in boxes of
-// 8 rows x `box_cols`; rows outside [0, rows) (the padded tail of the bank) are clipped by the hardware.
+// `box_rows` rows x `box_cols`.
 static cudaError_t make_map(void* base, int elem_bytes, bool is_float, int64_t cols, int64_t rows,
-                            int64_t pitch, int box_cols, CUtensorMap* map) {
+                            int64_t pitch, int box_cols, int box_rows, CUtensorMap* map) {
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return cudaErrorNotSupported;
     const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
     const cuuint64_t strides[1] = {(cuuint64_t)pitch * elem_bytes};
-    const cuuint32_t box[2] = {(cuuint32_t)box_cols, 8u};
+    const cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1u, 1u};
     const CUresult r = enc(map, is_float ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT16, 2,
                            base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -553,17 +577,19 @@ static cudaError_t make_map(void* base, int elem_bytes, bool is_float, int64_t c
 template <int PLANE16>
 static cudaError_t launch_tc(const ConvTcParams& p, int nsm, cudaStream_t st) {
     const int smem = convolve_tc_smem_bytes(p);
-    CUtensorMap pmap, mmap;
-    cudaError_t e = make_map(p.plane, PLANE16 ? 2 : 4, !PLANE16, p.nbins, p.nz, p.pitch, tc::kTileR, &pmap);
-    if (e != cudaSuccess) return e;
-    e = make_map(p.maxplane, 2, false, p.nbins / 8, p.nz, p.mpitch, tc::kTileR / 8, &mmap);
+    CUtensorMap pmap, mmap, pmap1;   // boxes of 8 rows; single plane rows for the bank's ragged last chunk
+    cudaError_t e = make_map(p.plane, PLANE16 ? 2 : 4, !PLANE16, p.nbins, p.nz, p.pitch, tc::kTileR, 8, &pmap);
+    if (e == cudaSuccess)
+        e = make_map(p.plane, PLANE16 ? 2 : 4, !PLANE16, p.nbins, p.nz, p.pitch, tc::kTileR, 1, &pmap1);
+    if (e == cudaSuccess)
+        e = make_map(p.maxplane, 2, false, p.nbins / 8, p.nz, p.mpitch, tc::kTileR / 8, 8, &mmap);
     if (e != cudaSuccess) return e;
     auto kern = tc::convolve_tc_kernel<PLANE16>;
     e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     const int64_t ntiles = p.nbins / tc::kTileR;
     const unsigned grid = (unsigned)(ntiles < nsm ? ntiles : nsm);
-    kern<<<grid, tc::kThreads, smem, st>>>(p, pmap, mmap);
+    kern<<<grid, tc::kThreads, smem, st>>>(p, pmap, mmap, pmap1);
     return cudaGetLastError();
 }
 

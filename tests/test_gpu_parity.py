@@ -417,6 +417,64 @@ def test_blockmax_plane_and_prefilter_equivalence(fdas, torch_, precision):
     assert gpu_cand_dict(a.cands) == gpu_cand_dict(b.cands)
 
 
+@pytest.mark.parametrize("precision", ["bf16_tc", "bf16_tc_plane16"])
+@pytest.mark.parametrize("zmax", [4.0, 10.0, 20.0, 52.0])
+def test_tensor_core_path_odd_banks(fdas, torch_, oracle, precision, zmax):
+    """K2-TC with banks whose pair count is not a multiple of 8 (4, 10, 20, 52 pairs: a chunk with
+    padded pairs, fewer chunks than epilogue warpgroups, two groups with a ragged last chunk): the rows
+    of the padded pairs lie outside the plane and must be clipped by the TMA stores (plane and
+    block-max side plane), every real row must be written, and the candidates must match."""
+    torch = torch_
+    n = 1 << 14                                   # nbins = 8192: 64 tiles over <= 148 CTAs
+    plan = fdas.Plan(n, 64e-6, zmax, 1.0, 2048, precision)
+    nb, nz = plan.info.nbins, plan.info.nz
+    rng = np.random.default_rng(int(zmax))
+    w = (rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)
+    for k in (0, 127, 128, 129, 5000, nb - 1):
+        w[k] += 10.0
+    d_spec = spec_from_complex(torch, w, precision)
+    wq = spec_to_complex(torch, d_spec)
+    # canaries around the plane: the rows before and after it must stay untouched
+    elem = torch.bfloat16 if precision.endswith("plane16") else torch.float32
+    big = torch.full((nz + 16, nb), -7.0, dtype=elem, device="cuda")
+    d_plane = big[8:8 + nz]
+    plan.convolve_plane(d_spec, d_plane)
+    torch.cuda.synchronize()
+    assert bool((big[:8] == -7.0).all()) and bool((big[8 + nz:] == -7.0).all())
+    Pg = d_plane.float().cpu().numpy().astype(np.float64)
+    assert (Pg >= 0).all()                        # every element written (canary is negative)
+    bank = oracle.template_bank(zmax, 1.0)
+    P = oracle.plane(w, bank)
+    assert np.abs(Pg - P).max() <= TOL[precision] * P.max()
+    assert np.abs(Pg - oracle.plane(wq, bank)).max() <= 1e-2 * P.max()
+    # block-max side plane: bit-exact upper bound of the stored values
+    ptr, pitch = plan.debug_maxplane()
+    M = _device_view(torch, ptr, nz * pitch).view(nz, pitch).clone()
+    ref = d_plane.float().contiguous().view(nz, pitch, 8).amax(dim=2)
+    assert torch.equal(M, ((ref.view(torch.int32) + 0xFFFF) >> 16).to(torch.int16))
+    # harmonic sums on that plane
+    H = 8
+    thr = fdas.thresholds_from_sigma(H, 3.0)
+    d_c, d_n = plan.alloc_cands(1 << 16)
+    plan.harmonic_sum_peaks(d_plane, H, thr, 16, d_c, d_n)
+    res = plan.read_cands(d_c, d_n)
+    oc = oracle.candidates(Pg, H, thr.astype(np.float64), 16)
+    s_at, margin = oracle_margin_fn(oracle, Pg, H, 16)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * Pg.max(), None, s_at, margin)
+    assert stats["only_gpu"] + stats["only_orc"] <= 2 and stats["common"] > 10, stats
+
+
+def test_tensor_core_path_unsupported_banks(fdas, torch_):
+    """Banks the tensor-core kernel cannot hold are refused at plan time (no silent fallback):
+    nz = 1 (no conjugate pairs) and a half-bin bank whose image does not fit the CTA's shared memory;
+    the FFT path takes the same plans."""
+    for zmax, zstep in ((0.0, 1.0), (96.0, 0.5)):
+        with pytest.raises(fdas.FdasError) as ei:
+            fdas.Plan(1 << 14, 64e-6, zmax, zstep, 2048, "bf16_tc")
+        assert ei.value.status == fdas.FDAS_EUNSUPPORTED
+        fdas.Plan(1 << 14, 64e-6, zmax, zstep, 2048, "bf16").close()
+
+
 def _device_view(torch, ptr, numel):
     """int16 tensor aliasing `numel` 16-bit words of device memory at `ptr` (no copy)."""
     class _Iface:
