@@ -258,7 +258,8 @@ __device__ __forceinline__ void zero_row_out(const int mid, const int64_t r, con
     if ((lane & 7) == 0) p.maxplane[(int64_t)mid * p.mpitch + (r >> 3)] = (unsigned short)w;
 }
 
-template <int PLANE16>
+// TAIL: the bank's pair count is not a multiple of 8 (its last chunk holds padded pairs).
+template <int PLANE16, int TAIL>
 __global__ void __launch_bounds__(kThreads, 1)
 convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tmap,
                    const __grid_constant__ CUtensorMap mmap, const __grid_constant__ CUtensorMap tmap1) {
@@ -367,11 +368,11 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
                 tc_commit(hempty(hs));
             }
         }
-    } else {
+    } else if (warp < 2 + kEpiWarps) {
         // ===== epilogue warps: TMEM lane quarter = warp % 4, chunks c = hf, hf + 2, ...
         const int q = warp & 3, wg = (warp - 2) >> 2;      // warpgroup wg drains chunks wg, wg+3, ..
         const int tw = ((warp - 2) & 3) * 32 + lane;        // thread index inside the warpgroup
-        const bool elected = (tw == 0);
+        const bool elected = (tw == 0);      // issues the warpgroup's TMA stores
         const int gch = p.gch, ngroups = p.ngroups;
         const int nmine = (gch - wg + 2) / 3;
         unsigned char* const stage0 = smem + L.sc_off + wg * (kStageBufs * kStageBufBytes);
@@ -410,7 +411,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
             constexpr int kRowBytes = 128 * (PLANE16 ? 2 : 4);
             auto store_tile = [&](uint32_t src, int c0, int p0) {
                 const int nval = npair - p0;
-                if (nval >= 8) {
+                if (!TAIL || nval >= 8) {
                     tma_store_2d(&tmap, src, c0, mid + 1 + p0);
                     tma_store_2d(&tmap, src + 8 * kRowBytes, c0, mid - 1 - p0 - 7);
                 } else {
@@ -423,7 +424,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
             auto store_maxes = [&](uint32_t k, int c0, int p0) {      // side tile of chunk k
                 const uint32_t src = smem_u32(buf_of(k) + kStageTileBytes);
                 const int nval = npair - p0;
-                if (nval >= 8) {
+                if (!TAIL || nval >= 8) {
                     tma_store_2d(&mmap, src, c0 >> 3, mid + 1 + p0);
                     tma_store_2d(&mmap, src + 8 * 16 * 2, c0 >> 3, mid - 1 - p0 - 7);
                 } else {
@@ -584,7 +585,8 @@ static cudaError_t launch_tc(const ConvTcParams& p, int nsm, cudaStream_t st) {
     if (e == cudaSuccess)
         e = make_map(p.maxplane, 2, false, p.nbins / 8, p.nz, p.mpitch, tc::kTileR / 8, 8, &mmap);
     if (e != cudaSuccess) return e;
-    auto kern = tc::convolve_tc_kernel<PLANE16>;
+    const bool tail = ((p.nz - 1) / 2) % 8 != 0;
+    auto kern = tail ? tc::convolve_tc_kernel<PLANE16, 1> : tc::convolve_tc_kernel<PLANE16, 0>;
     e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     const int64_t ntiles = p.nbins / tc::kTileR;
