@@ -23,8 +23,10 @@
 //   128 contiguous bytes; the thread that owns r has all four values of a pair in its own lane.
 //
 // Warp roles of the persistent CTA (one per SM, 448 threads): warp 0 builds H for tile i+1.. (3
-// stages), warp 1 allocates TMEM and issues the MMAs (one lane), warps 2..13 drain the two
-// accumulator stages (TMEM -> registers -> power -> plane + block-max side plane).
+// stages), warp 1 allocates TMEM and issues the MMAs (one lane), warps 2..13 (three warpgroups) drain
+// the two accumulator stages (TMEM -> registers -> power -> plane + block-max side plane).  Two
+// warpgroups are 14 % slower (too few warps to hide the drain's latencies), four do not fit the
+// register file (profiles/r01e).
 #include <cuda.h>
 #include <cuda_bf16.h>
 
@@ -370,11 +372,11 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
         }
     } else if (warp < 2 + kEpiWarps) {
         // ===== epilogue warps: TMEM lane quarter = warp % 4, chunks c = hf, hf + 2, ...
-        const int q = warp & 3, wg = (warp - 2) >> 2;      // warpgroup wg drains chunks wg, wg+3, ..
+        const int q = warp & 3, wg = (warp - 2) >> 2;      // warpgroup wg drains chunks wg, wg + kWarpGroups, ..
         const int tw = ((warp - 2) & 3) * 32 + lane;        // thread index inside the warpgroup
         const bool elected = (tw == 0);      // issues the warpgroup's TMA stores
         const int gch = p.gch, ngroups = p.ngroups;
-        const int nmine = (gch - wg + 2) / 3;
+        const int nmine = (gch - wg + kWarpGroups - 1) / kWarpGroups;
         unsigned char* const stage0 = smem + L.sc_off + wg * (kStageBufs * kStageBufBytes);
         const int col = 32 * q + lane;
         const uint32_t lane_base = tmem_base + ((uint32_t)(32 * q) << 16);
@@ -384,7 +386,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
             uint32_t item = 0;
             for (int64_t tile = blockIdx.x; tile < ntiles; tile += tstep)
                 for (int g = 0; g < ngroups; ++g, ++item) {
-                    if (g == 0 && wg == 2) zero_row_out<PLANE16>(mid, tile * kTileR + col, p, lane);
+                    if (g == 0 && wg == kWarpGroups - 1) zero_row_out<PLANE16>(mid, tile * kTileR + col, p, lane);
                     mbar_wait(tfull(item & 1u), (item >> 1) & 1u);
                     tc_fence_before();
                     __syncwarp();
@@ -400,7 +402,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
             int prev_c0 = 0, prev_p0 = 0;
             uint32_t ra[16], rb[16], sa[16], sb[16];
             auto issue_ld = [&](uint32_t it_, int i_, uint32_t (&x)[16], uint32_t (&y)[16]) {
-                const uint32_t tb = lane_base + (it_ & 1u) * 256u + 16u * (uint32_t)(wg + 3 * i_);
+                const uint32_t tb = lane_base + (it_ & 1u) * 256u + 16u * (uint32_t)(wg + kWarpGroups * i_);
                 tmem_ld16(tb, x);
                 tmem_ld16(tb + 128u, y);
             };
@@ -465,8 +467,8 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap tma
                     __syncwarp();
                     if (lane == 0) mbar_arrive(tempty(item & 1u));
                 }
-                if (g == 0 && i == 0 && wg == 2) zero_row_out<PLANE16>(mid, tile * kTileR + col, p, lane);
-                const int p0 = (g * gch + wg + 3 * i) * 8;
+                if (g == 0 && i == 0 && wg == kWarpGroups - 1) zero_row_out<PLANE16>(mid, tile * kTileR + col, p, lane);
+                const int p0 = (g * gch + wg + kWarpGroups * i) * 8;
                 const int c0 = FDAS_TC_DIAG == 7 ? (int)(blockIdx.x * kTileR) : (int)(tile * kTileR);
                 if (FDAS_TC_DIAG != 1) {
                     MaxRegs mr;

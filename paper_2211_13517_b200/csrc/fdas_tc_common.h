@@ -9,10 +9,14 @@
 namespace fdas {
 namespace tc {
 
-constexpr int kThreads = 448;   // warp 0 producer, warp 1 MMA issuer, warps 2..13 epilogue
+#ifndef FDAS_TC_WGS
+#define FDAS_TC_WGS 3
+#endif
+constexpr int kWarpGroups = FDAS_TC_WGS;               // epilogue warpgroups (4 warps = the tile's 128 bins)
+constexpr int kThreads = 64 + 128 * kWarpGroups;      // warp 0 producer, warp 1 MMA issuer, then the epilogue warps
 constexpr int kHStages = 3;     // sliding-window (A operand) stages
 constexpr int kTileR = 128;     // Fourier bins per tile = MMA M = TMEM lanes
-constexpr int kEpiWarps = 12;   // three warpgroups
+constexpr int kEpiWarps = 4 * kWarpGroups;
 constexpr int kStageTileBytes = 16 * 128 * 4;   // one staged chunk: 16 plane rows x 128 bins (fp32)
 constexpr int kStageBufBytes = kStageTileBytes + 16 * 16 * 2;   // + its [16][16] bf16 block-max tile
 constexpr int kStageBufs = 4;                   // staged chunks in flight per warpgroup
