@@ -252,6 +252,15 @@ __global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(co
     const int hz = d == 0 ? p.H : min(p.H, c2 / d);          // 1 or 2 here
     const PfRow r1 = pf_row(p, j, 1);
     const uint4 a = __ldg(reinterpret_cast<const uint4*>(r1.mrow) + O);
+    if (hz <= 1) {
+        // one harmonic only (half of the plane's rows): M > T_1 on the bf16 bit patterns.  For
+        // non-negative values the order of the patterns is the order of the values, and with
+        // tb = pattern of T_1 truncated to bf16, M > T_1 <=> pattern(M) > tb (M is a bf16 value).
+        const unsigned tb = __float_as_uint(fmaxf(r1.thr, 0.f)) >> 16;
+        const unsigned tb2 = tb | (tb << 16);
+        if ((__vcmpgtu2(a.x, tb2) | __vcmpgtu2(a.y, tb2) | __vcmpgtu2(a.z, tb2) | __vcmpgtu2(a.w, tb2)) == 0u)
+            return;                                   // nothing above threshold: almost every thread
+    }
     // harmonic 2 of all 64 fundamentals inside the plane?
     const bool two = hz >= 2 && 2u * (64u * O + 63u) <= last;
     PfRow r2 = r1;

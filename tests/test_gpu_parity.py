@@ -524,8 +524,9 @@ def test_batch_small_trial_counts_and_overflow(fdas, torch_):
     assert again == want[3]
 
 
+@pytest.mark.parametrize("precision", ["bf16_tc", "bf16"])
 @pytest.mark.parametrize("half_res", [False, True])
-def test_batch_ska_members_full_size(fdas, torch_, oracle, half_res):
+def test_batch_ska_members_full_size(fdas, torch_, oracle, half_res, precision):
     """Members 5, 6, 7 of configs[3] (6 carries an injected accelerated signal), and the 128 us shape
     of configs[4], through the pipelined batch in the configuration bench.py times: equal to the
     per-trial calls, signal recovered at its (r, z), sampled oracle parity on the signal's trial."""
@@ -533,7 +534,7 @@ def test_batch_ska_members_full_size(fdas, torch_, oracle, half_res):
     members = [inputs.batched_member(i, half_res=half_res) for i in (5, 6, 7)]
     wl = members[1]
     assert len(wl.signals) == 1 and not members[0].signals
-    plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, "bf16")
+    plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, precision)
     assert plan.info.nfft == (1 << 22 if half_res else 1 << 23)
     thr = fdas.thresholds_from_sigma(wl.nharm, wl.nsigma)
     xs = [inputs.series_for(m) for m in members]

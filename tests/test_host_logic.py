@@ -142,7 +142,7 @@ def test_emulated_k2_matches_the_oracle_plane(emu, oracle, zmax, nb):
         assert np.abs(out - P).max() <= tol * P.max(), (prec, np.abs(out - P).max() / P.max())
 
 
-@pytest.mark.parametrize("zmax,nb", [(16.0, 1152), (96.0, 640)])
+@pytest.mark.parametrize("zmax,nb", [(16.0, 1152), (96.0, 640), (10.0, 384), (52.0, 256)])
 def test_emulated_k2_tc_matches_the_oracle_plane(emu, oracle, zmax, nb):
     """K2-TC (tensor-core contraction) stepped on the CPU: same shared-memory image, UMMA descriptor
     encodings (sliding-window A operand with LBO = SBO = 128 B, packed bank B), issue order, TMEM
