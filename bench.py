@@ -85,6 +85,8 @@ def workload_for(name: str, inputs):
         return inputs.ska()
     if name == "ska_half":
         return inputs.ska(half_res=True)
+    if name == "ska_padded":
+        return inputs.ska_padded()
     if name == "medium":
         return inputs.medium()
     if name == "tiny":
@@ -100,6 +102,8 @@ def trial_series(wl_name, trial, inputs):
             w = workload_for(wl_name, inputs)      # trial 0 is configs[2] itself (2 injected pulsars)
         return inputs.series_for(w)
     w = workload_for(wl_name, inputs)
+    if wl_name == "ska_padded":
+        return inputs.series_for(inputs.ska_padded(seed=3 + 7919 * trial))
     return inputs.make_series(w.n, w.seed + 7919 * trial, w.signals, w.red_knee)
 
 
@@ -592,7 +596,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="ska",
-                    choices=["ska", "ska_half", "medium", "tiny", "batched", "survey"])
+                    choices=["ska", "ska_half", "ska_padded", "medium", "tiny", "batched", "survey"])
     ap.add_argument("--energy-seconds", type=float, default=2.5,
                     help="length of the separate energy loop (0 = off)")
     ap.add_argument("--trials", type=int, default=0,

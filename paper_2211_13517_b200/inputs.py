@@ -93,10 +93,11 @@ def red_noise(n: int, knee: float, rng: np.random.Generator) -> np.ndarray:
     return np.fft.irfft(spec, n=n)
 
 
-def make_series(n: int, seed: int, signals=(), red_knee: float = 0.0) -> np.ndarray:
-    """float32 time series: N(0,1) noise (+ optional red noise) + injected signals."""
+def make_series(n: int, seed: int, signals=(), red_knee: float = 0.0, nfft_ref: int = 0) -> np.ndarray:
+    """float32 time series: N(0,1) noise (+ optional red noise) + injected signals.  The signals'
+    (r_c, z) refer to a transform of nfft_ref samples (default: the largest power of two <= n)."""
     rng = np.random.default_rng(seed)
-    nfft = largest_pow2_le(n)
+    nfft = nfft_ref if nfft_ref > 0 else largest_pow2_le(n)
     x = rng.standard_normal(n)
     if red_knee > 0.0:
         x = x + red_noise(n, red_knee, rng)
@@ -142,6 +143,20 @@ def ska(seed: int = 3, half_res: bool = False, signals=None) -> Workload:
                     96.0, 1.0, 2048, 16, 6.0, 64, ("bf16",), seed, tuple(signals), red_knee=600.0)
 
 
+N_SKA_PADDED = 1 << 24
+
+
+def ska_padded(seed: int = 3) -> Workload:
+    """The secondary reading A1-B of configs[2] ("zero-padded ... for the real FFT"): all 9,375,000
+    samples, mean-subtracted and zero-padded to 2^24 by the caller -- for the library it is simply a
+    series of N = 2^24 samples (nfft 2^24, Nb 2^23, a 6.5 GB fp32 plane).  (r_c, z) of the injected
+    signals are in bins of the padded transform."""
+    signals = (Signal(r_c=246912.02, z=40.0, amp=0.012, phase=0.3, nharm=5),
+               Signal(r_c=1308642.02, z=-40.0, amp=0.012, phase=1.1, nharm=5))
+    return Workload("ska_padded", N_SKA_PADDED, TSAMP_FULL, 96.0, 1.0, 2048, 16, 6.0, 64, ("bf16",), seed,
+                    signals, red_knee=600.0)
+
+
 BATCH_SIGNAL_SERIES = (6, 17, 23, 38, 49, 60)   # ~10 % of 64 carry one injected signal
 
 
@@ -162,6 +177,11 @@ SURVEY_TRIALS_HALF = 2875   # BASELINE.json configs[4]
 
 
 def series_for(w: Workload) -> np.ndarray:
+    if w.name == "ska_padded":
+        x = make_series(N_SKA_FULL, w.seed, w.signals, w.red_knee, nfft_ref=w.n).astype(np.float64)
+        out = np.zeros(w.n, dtype=np.float32)
+        out[:N_SKA_FULL] = (x - x.mean()).astype(np.float32)
+        return out
     return make_series(w.n, w.seed, w.signals, w.red_knee)
 
 

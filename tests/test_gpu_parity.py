@@ -482,6 +482,52 @@ def _device_view(torch, ptr, numel):
     return torch.as_tensor(_Iface(), device="cuda")
 
 
+def test_ska_zero_padded_2p24_sampled_parity(fdas, torch_, oracle):
+    """Reading A1-B of configs[2]: all 9,375,000 samples, mean-subtracted and zero-padded to 2^24 by
+    the caller (Nb = 2^23, 1.6e9 plane points, a 6.5 GB fp32 plane, 65536 K2-TC tiles), tensor-core
+    path: sampled plane parity against the oracle's own spectrum, candidates valid in the oracle."""
+    torch = torch_
+    wl = inputs.ska_padded()
+    x = inputs.series_for(wl)
+    assert x.size == 1 << 24 and not x[9_375_000:].any() and abs(float(x[:9_375_000].mean())) < 1e-6
+    plan, d_spec, d_plane, res, thr = run_gpu(fdas, torch, wl, x, "bf16_tc")
+    info = plan.info
+    assert (info.nfft, info.nbins, info.nz) == (1 << 24, 1 << 23, 193)
+    w = oracle.whiten(oracle.spectrum(x, wl.nfft))
+    assert np.abs(spec_to_complex(torch, d_spec) - w).max() <= 1e-2 * np.abs(w).max()
+    bank = oracle.template_bank(wl.zmax, wl.zstep)
+    nb, nz = info.nbins, info.nz
+    rng = np.random.default_rng(5)
+    rr = [rng.integers(0, nb, 20000)]; jj = [rng.integers(0, nz, 20000)]
+    edge = np.concatenate([np.arange(0, 70), np.arange(nb - 70, nb),
+                           np.array([t * 128 + d for t in (1, 148, 32768, 65535) for d in (-1, 0, 1)])])
+    for j in (0, 96, 192):
+        rr.append(edge); jj.append(np.full(edge.size, j))
+    for s in wl.signals:
+        r0, j0 = int(round(s.r_c)), int(round(s.z + wl.zmax))
+        g_r, g_j = np.meshgrid(np.arange(r0 - 6, r0 + 7), np.arange(j0 - 3, j0 + 4))
+        rr.append(g_r.ravel()); jj.append(g_j.ravel())
+    rr = np.concatenate(rr).astype(np.int64); jj = np.concatenate(jj).astype(np.int32)
+    Po = oracle.plane_points(w, bank, rr, jj)
+    Pg = d_plane[torch.from_numpy(jj.astype(np.int64)).cuda(), torch.from_numpy(rr).cuda()].float().cpu().numpy()
+    flat = int(torch.argmax(d_plane).item())
+    jm, rm = flat // info.plane_pitch, flat % info.plane_pitch
+    pmax = float(oracle.plane_points(w, bank, [rm], [jm])[0])
+    assert abs(float(d_plane[jm, rm]) - pmax) <= TOL["bf16_tc"] * pmax and pmax > 30
+    assert np.abs(Pg - Po).max() <= TOL["bf16_tc"] * pmax
+    assert not torch.isnan(d_plane.sum()).item()
+    gd = gpu_cand_dict(res.cands)
+    assert res.count == len(gd) and 0 < res.count < 50000
+    keys = sorted(gd)
+    S, hmax = oracle.harmonic_sums_sampled(w, bank, wl.nharm, np.array([k[0] for k in keys]),
+                                           np.array([k[1] for k in keys], dtype=np.int32))
+    tol = TOL["bf16_tc"] * pmax
+    for i, (r, j, h) in enumerate(keys):
+        so = S[i, h - 1]
+        assert h <= hmax[i] and so > thr[h - 1] - h * tol
+        assert abs(gd[(r, j, h)][0] - so) <= min(h * tol, REL_POW["bf16_tc"] * so)
+
+
 # ------------------------------------- configs[3] / configs[4]: pipelined batch of DM trials
 def _sequential(fdas, torch, plan, x, wl, thr, capacity=1 << 16):
     d_x = torch.from_numpy(x).cuda()
