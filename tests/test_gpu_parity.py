@@ -242,7 +242,7 @@ def test_harmonic_sum_alone_many_candidates(fdas, torch_, oracle, precision):
     assert set(gpu_cand_dict(small.cands)) <= set(gpu_cand_dict(res.cands))
 
 
-@pytest.mark.parametrize("H", [1, 2, 3, 5])
+@pytest.mark.parametrize("H", [1, 2, 3, 5, 32])
 def test_harmonic_sum_small_h_exact_sets(fdas, torch_, oracle, H):
     """K3 on a hand-made plane for small harmonic counts: with H <= 2 every row but z = 0 goes
     through the streaming shallow pass, H = 3, 5 mix both passes; the threads that straddle
