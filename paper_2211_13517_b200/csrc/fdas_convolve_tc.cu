@@ -200,7 +200,7 @@ __device__ __forceinline__ void chunk_to_smem(const uint32_t (&a)[16], const uin
 // The two 16-byte halves of a block are read in lane-dependent order so that the 8 lanes of a
 // shared-memory phase touch 8 different 16-byte bank groups.
 struct MaxRegs {
-    uint4 u[2], v[2];
+    unsigned x[2];   // per task: the block's largest bit pattern (fp32) / packed bf16 pair maximum
 };
 template <int PLANE16>
 __device__ __forceinline__ void block_max_load(const void* sbuf, const int tw, MaxRegs* m) {
@@ -209,12 +209,15 @@ __device__ __forceinline__ void block_max_load(const void* sbuf, const int tw, M
     for (int t = 0; t < 2; ++t) {
         const int lr = lr0 + 8 * t;
         if (PLANE16) {
-            m->u[t] = *reinterpret_cast<const uint4*>(reinterpret_cast<const unsigned short*>(sbuf) + lr * 128 + blk * 8);
+            const uint4 u = *reinterpret_cast<const uint4*>(reinterpret_cast<const unsigned short*>(sbuf) + lr * 128 + blk * 8);
+            m->x[t] = __vmaxu2(__vmaxu2(u.x, u.y), __vmaxu2(u.z, u.w));
         } else {
+            // powers are >= 0: the order of the bit patterns is the order of the values
             const float* row = reinterpret_cast<const float*>(sbuf) + lr * 128 + blk * 8;
             const int sw = (blk >> 2) & 1;
-            m->u[t] = *reinterpret_cast<const uint4*>(row + 4 * sw);
-            m->v[t] = *reinterpret_cast<const uint4*>(row + 4 * (sw ^ 1));
+            const uint4 u = *reinterpret_cast<const uint4*>(row + 4 * sw);
+            const uint4 v = *reinterpret_cast<const uint4*>(row + 4 * (sw ^ 1));
+            m->x[t] = max(max(max(u.x, u.y), max(u.z, u.w)), max(max(v.x, v.y), max(v.z, v.w)));
         }
     }
 }
@@ -223,16 +226,7 @@ __device__ __forceinline__ void block_max_finish(const MaxRegs& m, unsigned shor
     const int lr0 = tw >> 4, blk = tw & 15;
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
-        unsigned bits;
-        if (PLANE16) {
-            const unsigned x = __vmaxu2(__vmaxu2(m.u[t].x, m.u[t].y), __vmaxu2(m.u[t].z, m.u[t].w));
-            bits = max(x & 0xffffu, x >> 16);
-        } else {
-            // powers are >= 0: the order of the bit patterns is the order of the values
-            const unsigned x = max(max(max(m.u[t].x, m.u[t].y), max(m.u[t].z, m.u[t].w)),
-                                   max(max(m.v[t].x, m.v[t].y), max(m.v[t].z, m.v[t].w)));
-            bits = (x + 0xffffu) >> 16;
-        }
+        const unsigned bits = PLANE16 ? max(m.x[t] & 0xffffu, m.x[t] >> 16) : (m.x[t] + 0xffffu) >> 16;
         mtile[(lr0 + 8 * t) * 16 + blk] = (unsigned short)bits;
     }
 }
