@@ -18,9 +18,10 @@
 // * T_{-z} = conj(T_z): with A~ = w (*) Re T_z and B~ = w (*) Im T_z (complex), y_{+z} = A~ - i B~ and
 //   y_{-z} = A~ + i B~, so one pair of rows costs 4 real correlations instead of 8:
 //   D1 = H_re x B, D2 = H_im x B with B's columns (Re T_z, Im T_z) interleaved, and
-//   P_{+-z} = (Ar^2 + Ai^2 + Br^2 + Bi^2) +- 2 (Ar Bi - Ai Br).   The z = 0 row is |w|^2 exactly.
-// * TMEM lane = r (128 per tile), column = operand column: a warp's store of one plane row is
-//   128 contiguous bytes; the thread that owns r has all four values of a pair in its own lane.
+//   P_{+z} = (Ar + Bi)^2 + (Ai - Br)^2,  P_{-z} = (Ar - Bi)^2 + (Ai + Br)^2.   The z = 0 row is |w|^2 exactly.
+// * TMEM lane = r (128 per tile), column = operand column: the thread that owns r has all four values
+//   of a pair in its own lane, and a plane row segment of the tile is 512 contiguous bytes, staged in
+//   shared memory and written with TMA tensor stores.
 //
 // Warp roles of the persistent CTA (one per SM, 448 threads): warp 0 builds H for tile i+1.. (3
 // stages), warp 1 allocates TMEM and issues the MMAs (one lane), warps 2..13 (three warpgroups) drain
@@ -141,11 +142,6 @@ __device__ __forceinline__ void tmem_wait16(uint32_t (&a)[16], uint32_t (&b)[16]
                    "+r"(b[14]), "+r"(b[15])
                  :
                  : "memory");
-}
-
-// bf16 bit pattern that bounds a non-negative power from above (as fdas_convolve.cu's block max).
-__device__ __forceinline__ unsigned bf16_up_pair(float a, float b) {
-    return __byte_perm(__float_as_uint(a) + 0xffffu, __float_as_uint(b) + 0xffffu, 0x7632);
 }
 
 // ---- epilogue staging: a warpgroup (4 warps = the 128 bins of the tile) turns one chunk of 8
