@@ -198,6 +198,44 @@ __device__ __forceinline__ PfRow pf_row(const HarmParams& p, const int j, const 
     return r;
 }
 
+// Harmonic K > 8 of the 32 fundamentals of quad-block Q: the thread's slice M[row_K][4KQ .. 4KQ+4K-1]
+// (8K bytes) is read with 64-bit loads in two halves -- fundamentals 0..15 pick elements
+// (K i) >> 3 < 2K (words 0..K-1), fundamentals 16..31 elements >= 2K (words K..2K-1) -- instead of one
+// 16-bit gather per fundamental: half the load instructions, K + 2 live registers instead of 32.
+template <int K>
+__device__ __forceinline__ void pf_deep(const unsigned short* __restrict__ mrow, const unsigned Q,
+                                        const float thr, float (&U)[32], unsigned& flagged) {
+    const unsigned* words = reinterpret_cast<const unsigned*>(mrow + (size_t)4 * K * Q);   // 8-byte aligned
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+        constexpr int kPairs = K / 2 + 1;                 // 64-bit loads covering the half's K words
+        const int w0 = half ? (K & ~1) : 0;               // first word loaded (even: aligned)
+        unsigned wv[2 * kPairs];
+#pragma unroll
+        for (int c = 0; c < kPairs; ++c) {
+            // the last pair of the second half may reach one word past the slice when K is even
+            if (w0 + 2 * c + 1 < 2 * K) {
+                const uint2 v = __ldg(reinterpret_cast<const uint2*>(words + w0) + c);
+                wv[2 * c] = v.x;
+                wv[2 * c + 1] = v.y;
+            } else if (w0 + 2 * c < 2 * K) {
+                wv[2 * c] = __ldg(words + w0 + 2 * c);
+                wv[2 * c + 1] = 0u;
+            } else {
+                wv[2 * c] = wv[2 * c + 1] = 0u;
+            }
+        }
+#pragma unroll
+        for (int ii = 0; ii < 16; ++ii) {
+            const int i = 16 * half + ii;
+            const int e = (K * i) >> 3;                   // element of the slice (compile time)
+            const unsigned w = wv[(e >> 1) - w0];
+            U[i] += (e & 1) ? bf16_hi(w) : bf16_lo(w);
+            if (U[i] > thr) flagged |= 1u << i;
+        }
+    }
+}
+
 template <int K>
 __device__ __forceinline__ void pf_single_from(const HarmParams& p, const int j, const unsigned Q,
                                                const int he_max, const int he, float (&U)[32],
@@ -205,9 +243,13 @@ __device__ __forceinline__ void pf_single_from(const HarmParams& p, const int j,
     if constexpr (K <= 32) {
         if (K > he_max) return;                 // CTA-uniform: no thread of this CTA goes deeper
         const PfRow r = pf_row(p, j, K);
-        float m[K <= 8 ? 4 * K : 32];
-        pf_load<K>(r.mrow, Q, he >= K, m);
-        pf_add<K>(m, r.thr, he >= K, U, flagged);
+        if constexpr (K <= 8) {
+            float m[4 * K];
+            pf_load<K>(r.mrow, Q, he >= K, m);
+            pf_add<K>(m, r.thr, he >= K, U, flagged);
+        } else {
+            if (he >= K) pf_deep<K>(r.mrow, Q, r.thr, U, flagged);
+        }
         pf_single_from<K + 1>(p, j, Q, he_max, he, U, flagged);
     }
 }
