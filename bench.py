@@ -361,6 +361,31 @@ def run_cuda(args):
     e2e_value = fd.sum_over_ranks(ctx, float(points * e2e_steps)) / t_e2e
     d2h = int(np.minimum(counts, bcap).sum()) * 16 + 8 * e2e_steps
 
+    # ---- beside the tensor-core K2: north_star's literal FFT kernel on the same spectrum, K2 alone
+    fft_path = None
+    if precision in TC_PRECISIONS and not args.no_fft_path:
+        fprec = "bf16_plane16" if precision.endswith("plane16") else "bf16"
+        plan_f = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, fprec)
+        for _ in range(3):
+            plan_f.convolve_plane(d_spec, d_plane, stream)
+        ev_a, ev_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nrep = 10
+        ev_a.record(stream)
+        for _ in range(nrep):
+            plan_f.convolve_plane(d_spec, d_plane, stream)
+        ev_b.record(stream)
+        torch.cuda.synchronize()
+        t_f = ev_a.elapsed_time(ev_b) / nrep
+        fi = plan_f.info
+        f_flops = int(fi.nseg) * (int(fi.nz) * (FLOP_IFFT + FLOP_MUL + 3 * int(fi.valid)) + FLOP_IFFT)
+        fft_path = {"precision": fprec, "kernel": "K2 convolve_kernel (overlap-save FFT, fp32 arithmetic, no tensor cores)",
+                    "convolve_plane_ms": t_f, "alu_frac": f_flops / (t_f * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+                    "hbm_frac": HBM_BYTES_PER_POINT[fprec] * points / (t_f * 1e-3) / 1e9 / measured_peaks()[0],
+                    "launches": nrep}
+        plan_f.close()
+        plan.convolve_plane(d_spec, d_plane, stream)      # leave the plane as the timed path wrote it
+        torch.cuda.synchronize()
+
     hbm_peak, peak_kind = measured_peaks()
     seg_flops = FLOP_IFFT + FLOP_MUL + 3 * int(info.valid)
     k2_flops = int(info.nseg) * (int(info.nz) * seg_flops + FLOP_IFFT)
@@ -430,6 +455,8 @@ def run_cuda(args):
         },
         "clocks": sampler.summary(),
     }
+    if fft_path is not None:
+        line["fft_path"] = fft_path
     if energy is not None:
         line["energy"] = energy
     elif e_short[0] is not None and e_short[1] is not None and e_short[1] > e_short[0]:
@@ -606,6 +633,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle plane work")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-fft-path", action="store_true", help="skip the side measurement of the FFT K2")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
