@@ -39,6 +39,8 @@ struct HarmGeom {
     int64_t nbins, pitch, r_lo, capacity;
     fdas_cand_t* cands;
     unsigned long long* count;
+    const unsigned short* maxplane;   // block-max side plane (bf16 bits, upper bounds), nz x mpitch
+    int64_t mpitch;
     int nz, H;
 };
 
@@ -46,6 +48,7 @@ __device__ __forceinline__ HarmGeom geom_of(const HarmParams& p) {
     HarmGeom g;
     g.nbins = p.nbins; g.pitch = p.pitch; g.r_lo = p.r_lo; g.capacity = p.capacity;
     g.cands = p.cands; g.count = p.count; g.nz = p.nz; g.H = p.H;
+    g.maxplane = p.maxplane; g.mpitch = p.mpitch;
     return g;
 }
 
@@ -79,8 +82,24 @@ __device__ bool harmonic_sum_at(const T* P, const HarmGeom& g, int64_t r, int j,
     return true;
 }
 
-// The plain definition for one fundamental: all h, thresholds, slot claim.  The gathers of 8
-// harmonics are issued together (independent addresses); sums stay in k order.
+__device__ __forceinline__ void emit_candidate(const HarmGeom& g, int64_t r, int j, int h, float S) {
+    const unsigned long long slot = atomicAdd(g.count, 1ULL);   // the true count
+    if ((int64_t)slot >= g.capacity) return;
+    fdas_cand_t c;
+    c.r = (uint32_t)r;
+    c.zidx = (int16_t)j;
+    c.h = (uint16_t)h;
+    c.power = S;
+    c.flags = 1u;   // local-maximum attribute: cleared by flag_kernel if a neighbour beats it
+    g.cands[slot] = c;
+}
+
+// The plain definition for one fundamental: all h, thresholds, slot claim; sums stay in k order.
+// Harmonics 1..4 are gathered first (4 DRAM sectors); the deeper sums are then bounded from above by
+// continuing the same running sum with the block maxima M (an L2-resident side plane) in place of the
+// plane values -- term by term M >= P and fp32 addition is monotone -- and only if such a bound exceeds
+// its threshold are harmonics 5.. gathered from the plane, 8 at a time (independent addresses).  Most
+// fundamentals the prefilter lets through are settled by the first four gathers.
 template <typename T>
 __device__ __noinline__ void exact_fundamental(const T* P, const HarmGeom g, const float* thr,
                                                int64_t r, int j) {
@@ -92,33 +111,57 @@ __device__ __noinline__ void exact_fundamental(const T* P, const HarmGeom g, con
         if (v2 < 0 || v2 > 2 * c2 || (int64_t)h * r > g.nbins - 1) break;
         hmax = h;
     }
+    auto row_of = [&](int h) { return min((2 * h * j - (h - 1) * c2 + 1) >> 1, c2); };
     float S = 0.f;
-    for (int h0 = 1; h0 <= hmax; h0 += 8) {
+    {
+        float v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int h = 1 + q;
+            v[q] = (h <= hmax) ? ldp(P + (size_t)row_of(h) * g.pitch + (size_t)h * r) : 0.f;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int h = 1 + q;
+            if (h > hmax) break;
+            S += v[q];
+            if (S > thr[h - 1]) emit_candidate(g, r, j, h, S);
+        }
+    }
+    if (hmax <= 4) return;
+    {   // can any deeper sum still exceed its threshold?
+        float U = S;
+        bool deeper = false;
+        for (int h0 = 5; h0 <= hmax && !deeper; h0 += 8) {
+            unsigned short m[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const int h = h0 + q;
+                m[q] = (h <= hmax) ? __ldg(g.maxplane + (size_t)row_of(h) * g.mpitch + (size_t)(((int64_t)h * r) >> 3)) : 0;
+            }
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const int h = h0 + q;
+                if (h > hmax) break;
+                U += __uint_as_float((unsigned)m[q] << 16);
+                if (U > thr[h - 1]) deeper = true;
+            }
+        }
+        if (!deeper) return;
+    }
+    for (int h0 = 5; h0 <= hmax; h0 += 8) {
         float v[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
             const int h = h0 + q;
-            v[q] = 0.f;
-            if (h <= hmax) {
-                const int row = min((2 * h * j - (h - 1) * c2 + 1) >> 1, c2);
-                v[q] = ldp(P + (size_t)row * g.pitch + (size_t)h * r);
-            }
+            v[q] = (h <= hmax) ? ldp(P + (size_t)row_of(h) * g.pitch + (size_t)h * r) : 0.f;
         }
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
             const int h = h0 + q;
             if (h > hmax) break;
             S += v[q];
-            if (!(S > thr[h - 1])) continue;
-            const unsigned long long slot = atomicAdd(g.count, 1ULL);   // the true count
-            if ((int64_t)slot >= g.capacity) continue;
-            fdas_cand_t c;
-            c.r = (uint32_t)r;
-            c.zidx = (int16_t)j;
-            c.h = (uint16_t)h;
-            c.power = S;
-            c.flags = 1u;   // local-maximum attribute: cleared by flag_kernel if a neighbour beats it
-            g.cands[slot] = c;
+            if (S > thr[h - 1]) emit_candidate(g, r, j, h, S);
         }
     }
 }
