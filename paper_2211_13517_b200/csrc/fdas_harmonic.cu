@@ -320,66 +320,112 @@ __device__ __forceinline__ void pf_emit(const HarmParams& p, const unsigned Q, c
     }
 }
 
-// Rows with one or two harmonics only (|z| > zmax/3: the nlow first and the nlow last rows, two thirds
-// of the plane).  U_1 is the same for the 8 fundamentals of a block and U_2 for the 4 of a half block,
-// so nothing is evaluated per fundamental: a thread streams 8 blocks (64 fundamentals) of M[j] and, for
-// hz = 2, the 16 blocks of M[row_2] they map to.  Few registers, every load issued up front: this pass
-// is a plain scan of 0.15 GB.
+// Rows with at most kShallowDepth = 4 harmonics inside the plane (|z| > zmax/5: the nlow first and the
+// nlow last rows, four fifths of the plane).  Harmonic k picks block (k i) >> 3 for fundamental i of a
+// block of 8, so U_1 is the same for all 8 fundamentals, U_2 for halves, U_3 takes 4 and U_4 5 distinct
+// values per block: 12 sums and compares stand for 32.  A thread streams 8 blocks (64 fundamentals) of
+// M[j] and the 8k blocks of M[row_k] they map to; few registers, every load issued up front.
 constexpr int kPfShallowThreads = 256;
-__global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(const HarmParams p, const int nlow) {
+constexpr int kShallowDepth = 4;
+
+__device__ __forceinline__ float bf16_at(const uint4 (&w)[4], const int e) {   // element e of up to 32 (static e)
+    const uint4 v = w[e >> 3];
+    const unsigned x = ((e >> 1) & 3) == 0 ? v.x : ((e >> 1) & 3) == 1 ? v.y : ((e >> 1) & 3) == 2 ? v.z : v.w;
+    return (e & 1) ? bf16_hi(x) : bf16_lo(x);
+}
+
+// DMAX = 2 | 4: deepest harmonic of the rows this instance scans, rows [ja, jb) and their mirror images
+// [nz - jb, nz - ja) (the two-harmonic instance needs a third of the registers of the four-harmonic one).
+template <int DMAX>
+__global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(const HarmParams p, const int ja,
+                                                                              const int jb) {
     const int y = blockIdx.y;
-    const int j = y < nlow ? y : p.nz - 2 * nlow + y;
+    const int j = y < jb - ja ? ja + y : p.nz - jb + (y - (jb - ja));
     const int c2 = p.nz - 1;
     const unsigned O = blockIdx.x * (unsigned)kPfShallowThreads + threadIdx.x;   // octet of blocks
     if (O >= (unsigned)(p.mpitch >> 3)) return;
     const unsigned last = (unsigned)(p.nbins - 1);
     const int d = abs(2 * j - c2);
-    const int hz = d == 0 ? p.H : min(p.H, c2 / d);          // 1 or 2 here
+    const int hz = min(DMAX, d == 0 ? p.H : min(p.H, c2 / d));   // 1 .. DMAX here (CTA-uniform)
     const PfRow r1 = pf_row(p, j, 1);
-    const uint4 a = __ldg(reinterpret_cast<const uint4*>(r1.mrow) + O);
+    uint4 m1[4], m2[4], m3[4], m4[4];   // (only the first DMAX arrays are live)
+    m1[0] = __ldg(reinterpret_cast<const uint4*>(r1.mrow) + O);
     if (hz <= 1) {
         // one harmonic only (half of the plane's rows): M > T_1 on the bf16 bit patterns.  For
         // non-negative values the order of the patterns is the order of the values, and with
         // tb = pattern of T_1 truncated to bf16, M > T_1 <=> pattern(M) > tb (M is a bf16 value).
         const unsigned tb = __float_as_uint(fmaxf(r1.thr, 0.f)) >> 16;
         const unsigned tb2 = tb | (tb << 16);
-        if ((__vcmpgtu2(a.x, tb2) | __vcmpgtu2(a.y, tb2) | __vcmpgtu2(a.z, tb2) | __vcmpgtu2(a.w, tb2)) == 0u)
+        if ((__vcmpgtu2(m1[0].x, tb2) | __vcmpgtu2(m1[0].y, tb2) | __vcmpgtu2(m1[0].z, tb2) |
+             __vcmpgtu2(m1[0].w, tb2)) == 0u)
             return;                                   // nothing above threshold: almost every thread
     }
-    // harmonic 2 of all 64 fundamentals inside the plane?
-    const bool two = hz >= 2 && 2u * (64u * O + 63u) <= last;
-    PfRow r2 = r1;
-    uint4 b0 = make_uint4(0, 0, 0, 0), b1 = b0;
-    if (hz >= 2) {
-        r2 = pf_row(p, j, 2);
-        if (two) {
-            b0 = __ldg(reinterpret_cast<const uint4*>(r2.mrow) + 2 * O);
-            b1 = __ldg(reinterpret_cast<const uint4*>(r2.mrow) + 2 * O + 1);
-        }
+    // dep: harmonics inside the plane for all 64 fundamentals of this thread
+    const int dep = (int)min((unsigned)hz, last / (64u * O + 63u));
+    PfRow r2 = r1, r3 = r1, r4 = r1;
+    if (hz >= 2) r2 = pf_row(p, j, 2);
+    if (DMAX >= 3 && hz >= 3) r3 = pf_row(p, j, 3);
+    if (DMAX >= 4 && hz >= 4) r4 = pf_row(p, j, 4);
+    if (dep >= 2) {
+#pragma unroll
+        for (int c = 0; c < 2; ++c) m2[c] = __ldg(reinterpret_cast<const uint4*>(r2.mrow) + 2 * O + c);
     }
-    const unsigned aw[4] = {a.x, a.y, a.z, a.w};
-    const unsigned bw[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+    if (DMAX >= 3 && dep >= 3) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) m3[c] = __ldg(reinterpret_cast<const uint4*>(r3.mrow) + 3 * O + c);
+    }
+    if (DMAX >= 4 && dep >= 4) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) m4[c] = __ldg(reinterpret_cast<const uint4*>(r4.mrow) + 4 * O + c);
+    }
     unsigned f[2] = {0u, 0u};   // flags of fundamentals 64 O + 32 t + i
 #pragma unroll
     for (int q = 0; q < 8; ++q) {          // block q: fundamentals 8q..8q+7
-        const float m1 = (q & 1) ? bf16_hi(aw[q >> 1]) : bf16_lo(aw[q >> 1]);
-        if (m1 > r1.thr) f[q >> 2] |= 0xffu << (8 * (q & 3));
-        if (two) {
-            const float lo = bf16_lo(bw[q]), hi = bf16_hi(bw[q]);   // blocks 2q, 2q+1 of row_2
-            if (m1 + lo > r2.thr) f[q >> 2] |= 0x0fu << (8 * (q & 3));
-            if (m1 + hi > r2.thr) f[q >> 2] |= 0xf0u << (8 * (q & 3));
+        const int sh = 8 * (q & 3);
+        unsigned fl = 0u;
+        const float u1 = bf16_at(m1, q);
+        if (u1 > r1.thr) fl |= 0xffu;
+        if (dep >= 2) {
+            // U_2: fundamentals 0..3 -> block 2q, 4..7 -> block 2q+1 of row_2
+            const float u2[2] = {u1 + bf16_at(m2, 2 * q), u1 + bf16_at(m2, 2 * q + 1)};
+            if (u2[0] > r2.thr) fl |= 0x0fu;
+            if (u2[1] > r2.thr) fl |= 0xf0u;
+            if (DMAX >= 3 && dep >= 3) {
+                // U_3: (i >> 2, (3 i) >> 3) = (0,0) for i = 0,1,2; (0,1) for 3; (1,1) for 4,5; (1,2) for 6,7
+                const float u3[4] = {u2[0] + bf16_at(m3, 3 * q), u2[0] + bf16_at(m3, 3 * q + 1),
+                                     u2[1] + bf16_at(m3, 3 * q + 1), u2[1] + bf16_at(m3, 3 * q + 2)};
+                if (u3[0] > r3.thr) fl |= 0x07u;
+                if (u3[1] > r3.thr) fl |= 0x08u;
+                if (u3[2] > r3.thr) fl |= 0x30u;
+                if (u3[3] > r3.thr) fl |= 0xc0u;
+                if (DMAX >= 4 && dep >= 4) {
+                    // U_4 adds block i >> 1 of row_4: i = 0,1 | 2 | 3 | 4,5 | 6,7
+                    if (u3[0] + bf16_at(m4, 4 * q) > r4.thr) fl |= 0x03u;
+                    if (u3[0] + bf16_at(m4, 4 * q + 1) > r4.thr) fl |= 0x04u;
+                    if (u3[1] + bf16_at(m4, 4 * q + 1) > r4.thr) fl |= 0x08u;
+                    if (u3[2] + bf16_at(m4, 4 * q + 2) > r4.thr) fl |= 0x30u;
+                    if (u3[3] + bf16_at(m4, 4 * q + 3) > r4.thr) fl |= 0xc0u;
+                }
+            }
         }
+        f[q >> 2] |= fl << sh;
     }
-    if (hz >= 2 && !two) {
-        // the thread that straddles r = (Nb-1)/2: harmonic 2 exists for its first fundamentals only
-        const unsigned rmax = last / 2u;
+    if (dep < hz) {
+        // the thread that straddles r = (Nb-1)/(dep+1): harmonic dep+1 exists for its first
+        // fundamentals only (no deeper one can: see DESIGN.md K3); U_dep is rebuilt in k order
+        const int k = dep + 1;
+        const unsigned rmax = last / (unsigned)k;
         if (64u * O <= rmax) {
             const int nv = (int)min(64u, rmax - 64u * O + 1u);
-            const unsigned short* src = r2.mrow + (size_t)16 * O;
-            const unsigned short* m1p = r1.mrow + (size_t)8 * O;
-            for (int i = 0; i < nv; ++i)
-                if (bf16_lo(__ldg(m1p + (i >> 3))) + bf16_lo(__ldg(src + (i >> 2))) > r2.thr)
-                    f[i >> 5] |= 1u << (i & 31);
+            const float thr_k = p.thr[k - 1];
+            for (int i = 0; i < nv; ++i) {
+                float u = 0.f;
+                for (int kk = 1; kk <= k; ++kk) {
+                    const PfRow rk = pf_row(p, j, kk);
+                    u += bf16_lo(__ldg(rk.mrow + (size_t)8 * kk * O + ((kk * i) >> 3)));
+                }
+                if (u > thr_k) f[i >> 5] |= 1u << (i & 31);
+            }
         }
     }
     pf_emit(p, 2u * O, j, f[0]);
@@ -390,7 +436,7 @@ __global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(co
 #define FDAS_PF_MINB 8
 #endif
 __global__ void __launch_bounds__(kPfThreads, FDAS_PF_MINB) prefilter_kernel(const HarmParams p, const int nlow) {
-    const int j = nlow + blockIdx.y;   // the rows with three or more harmonics (|z| <= zmax/3)
+    const int j = nlow + blockIdx.y;   // the rows with more than kShallowDepth harmonics (|z| <= zmax/5)
     const int c2 = p.nz - 1;
     const unsigned Q0 = blockIdx.x * (unsigned)kPfThreads;
     const unsigned Q = Q0 + threadIdx.x;
@@ -528,20 +574,24 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
     }
-    // rows j < nlow and j >= nz - nlow have at most two harmonics inside the plane (reading A12)
-    int nlow = 0;
-    if ((p.mpitch & 7) == 0) {   // the shallow pass streams octets of blocks
+    // rows j < nlow and j >= nz - nlow have at most kShallowDepth harmonics inside the plane (reading
+    // A12), rows j < nlow2 and j >= nz - nlow2 at most two
+    int nlow = 0, nlow2 = 0;
+    if ((p.mpitch & 7) == 0) {   // the shallow passes stream octets of blocks
         const int c2 = p.nz - 1;
-        while (2 * nlow < p.nz - 1) {
-            const int d = c2 - 2 * nlow;                       // |2 j - c2| for j = nlow (< mid)
-            if ((d == 0 ? p.H : std::min(p.H, c2 / d)) > 2) break;
-            ++nlow;
-        }
-        if (p.H <= 2) nlow = p.nz / 2;                         // (nz odd: the z = 0 row goes to the general pass)
+        auto hz_of = [&](int j) { const int d = c2 - 2 * j; return d == 0 ? p.H : std::min(p.H, c2 / d); };
+        while (2 * nlow2 < p.nz - 1 && hz_of(nlow2) <= 2) ++nlow2;
+        nlow = nlow2;
+        while (2 * nlow < p.nz - 1 && hz_of(nlow) <= kShallowDepth) ++nlow;
     }
-    if (nlow > 0) {
-        dim3 grid((unsigned)((p.mpitch / 8 + kPfShallowThreads - 1) / kPfShallowThreads), (unsigned)(2 * nlow));
-        prefilter_shallow_kernel<<<grid, kPfShallowThreads, 0, st>>>(p, nlow);
+    const unsigned sgx = (unsigned)((p.mpitch / 8 + kPfShallowThreads - 1) / kPfShallowThreads);
+    if (nlow2 > 0) {
+        prefilter_shallow_kernel<2><<<dim3(sgx, (unsigned)(2 * nlow2)), kPfShallowThreads, 0, st>>>(p, 0, nlow2);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        ++*launches;
+    }
+    if (nlow > nlow2) {
+        prefilter_shallow_kernel<4><<<dim3(sgx, (unsigned)(2 * (nlow - nlow2))), kPfShallowThreads, 0, st>>>(p, nlow2, nlow);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
     }

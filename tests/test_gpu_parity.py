@@ -88,7 +88,7 @@ def test_tiny_fp32_full_parity(fdas, torch_, oracle):
     assert res.count == len(res.cands) and stats["common"] >= 1
     keys = set(gpu_cand_dict(res.cands))
     assert (20000, 23, 1) in keys or (20000, 24, 1) in keys     # the injected signal (z0 = 7.5)
-    assert plan.launch_count() == 7      # K1a, K1b, K2, K3 shallow + general prefilter, exact, flags (cuFFT not counted)
+    assert plan.launch_count() == 8      # K1a, K1b, K2, K3 two shallow + general prefilter, exact, flags (cuFFT not counted)
 
 
 # ------------------------------------------------------------------------------------ configs[1]
