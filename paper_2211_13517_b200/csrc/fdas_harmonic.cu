@@ -461,26 +461,64 @@ __global__ void __launch_bounds__(kPfThreads, FDAS_PF_MINB) prefilter_kernel(con
         if (he_max >= 2) { r2 = pf_row(p, j, 2); pf_load<2>(r2.mrow, Q, he >= 2, m2); }
         if (he_max >= 3) { r3 = pf_row(p, j, 3); pf_load<3>(r3.mrow, Q, he >= 3, m3); }
         if (he_max >= 4) { r4 = pf_row(p, j, 4); pf_load<4>(r4.mrow, Q, he >= 4, m4); }
-        // U_1 is the same for the 8 fundamentals of a block and U_2 for the 4 fundamentals of a
-        // half block (harmonic k picks block (k i) >> 3): 4 + 8 sums and compares stand for 64 --
-        // h = 1, 2 are 79 % of all (r, j, h) triples of the SKA-like plane
+        // harmonic k picks block (k i) >> 3 for fundamental i of a block of 8: U_1 is the same for all
+        // 8, U_2 for the 4 of a half block, U_3 takes 4 and U_4 5 distinct values per block -- 12 sums
+        // and compares per block stand for 32 (h <= 4 are 90 % of all (r, j, h) triples of the plane)
 #pragma unroll
         for (int q = 0; q < 4; ++q)
             if (m1[q] > r1.thr) flagged |= 0xffu << (8 * q);
+        float u2[8];
+#pragma unroll
+        for (int gq = 0; gq < 8; ++gq) u2[gq] = m1[gq >> 1];
         if (he >= 2) {
 #pragma unroll
             for (int gq = 0; gq < 8; ++gq) {
-                const float u2 = m1[gq >> 1] + m2[gq];
-                if (u2 > r2.thr) flagged |= 0xfu << (4 * gq);
+                u2[gq] += m2[gq];
+                if (u2[gq] > r2.thr) flagged |= 0xfu << (4 * gq);
+            }
+        }
+        if (he >= 3) {
+            float u3[16];
 #pragma unroll
-                for (int e = 0; e < 4; ++e) U[4 * gq + e] = u2;
+            for (int b = 0; b < 4; ++b) {
+                // (i >> 2, (3 i) >> 3) = (0,0) for i = 0,1,2; (0,1) for 3; (1,1) for 4,5; (1,2) for 6,7
+                u3[4 * b + 0] = u2[2 * b] + m3[3 * b];
+                u3[4 * b + 1] = u2[2 * b] + m3[3 * b + 1];
+                u3[4 * b + 2] = u2[2 * b + 1] + m3[3 * b + 1];
+                u3[4 * b + 3] = u2[2 * b + 1] + m3[3 * b + 2];
+                if (u3[4 * b + 0] > r3.thr) flagged |= 0x07u << (8 * b);
+                if (u3[4 * b + 1] > r3.thr) flagged |= 0x08u << (8 * b);
+                if (u3[4 * b + 2] > r3.thr) flagged |= 0x30u << (8 * b);
+                if (u3[4 * b + 3] > r3.thr) flagged |= 0xc0u << (8 * b);
+            }
+            if (he >= 4) {
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    // U_4 adds block i >> 1 of row_4: i = 0,1 | 2 | 3 | 4,5 | 6,7
+                    const float v0 = u3[4 * b + 0] + m4[4 * b], v1 = u3[4 * b + 0] + m4[4 * b + 1];
+                    const float v2 = u3[4 * b + 1] + m4[4 * b + 1], v3 = u3[4 * b + 2] + m4[4 * b + 2];
+                    const float v4 = u3[4 * b + 3] + m4[4 * b + 3];
+                    if (v0 > r4.thr) flagged |= 0x03u << (8 * b);
+                    if (v1 > r4.thr) flagged |= 0x04u << (8 * b);
+                    if (v2 > r4.thr) flagged |= 0x08u << (8 * b);
+                    if (v3 > r4.thr) flagged |= 0x30u << (8 * b);
+                    if (v4 > r4.thr) flagged |= 0xc0u << (8 * b);
+                    U[8 * b + 0] = v0; U[8 * b + 1] = v0; U[8 * b + 2] = v1; U[8 * b + 3] = v2;
+                    U[8 * b + 4] = v3; U[8 * b + 5] = v3; U[8 * b + 6] = v4; U[8 * b + 7] = v4;
+                }
+            } else {
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    U[8 * b + 0] = u3[4 * b]; U[8 * b + 1] = u3[4 * b]; U[8 * b + 2] = u3[4 * b];
+                    U[8 * b + 3] = u3[4 * b + 1];
+                    U[8 * b + 4] = u3[4 * b + 2]; U[8 * b + 5] = u3[4 * b + 2];
+                    U[8 * b + 6] = u3[4 * b + 3]; U[8 * b + 7] = u3[4 * b + 3];
+                }
             }
         } else {
 #pragma unroll
-            for (int i = 0; i < 32; ++i) U[i] = m1[i >> 3];
+            for (int i = 0; i < 32; ++i) U[i] = u2[i >> 2];
         }
-        if (he_max >= 3) pf_add<3>(m3, r3.thr, he >= 3, U, flagged);
-        if (he_max >= 4) pf_add<4>(m4, r4.thr, he >= 4, U, flagged);
     }
     if (he_max >= 5) {   // harmonics 5, 6: eleven loads in flight
         const PfRow r5 = pf_row(p, j, 5);
