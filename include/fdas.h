@@ -20,7 +20,10 @@
  *     (block-maximum plane of nz x nbins/8 floats, prefilter list);
  *   - the three per-trial calls only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
  *     void*, NULL = legacy default stream) and return; they never synchronise, allocate or free;
- *   - a plan may be used from one stream at a time (its scratch is not duplicated).
+ *   - the plan's scratch is not duplicated, so the per-trial calls of one plan are ordered on the
+ *     device in the order they are issued: a call on a stream other than the previous call's first
+ *     waits (cudaStreamWaitEvent) for that call's work.  Independent trials overlap through
+ *     fdas_search_batch or through one plan per stream; one plan is for one host thread at a time.
  */
 #ifndef FDAS_H
 #define FDAS_H
@@ -50,7 +53,7 @@ enum {
     FDAS_ECUDA = 3,        /* a CUDA runtime call or kernel launch failed */
     FDAS_ECUFFT = 4,       /* a cuFFT call failed */
     FDAS_EOVERFLOW = 5,    /* more candidates than capacity (host-side helper only) */
-    FDAS_EUNSUPPORTED = 6  /* valid request this build does not implement (e.g. seg_len != 2048) */
+    FDAS_EUNSUPPORTED = 6  /* valid request this build does not implement (e.g. seg_len != 2048, nfft > 2^30) */
 };
 
 typedef struct {
@@ -131,14 +134,21 @@ int fdas_convolve_plane(fdas_plan_t plan, const void* d_spec, void* d_plane, voi
  *   d_count       device; set to 0 by this call, then receives the TRUE number of candidates found
  *                 (it may exceed capacity; only the first `capacity` claimed slots are stored)
  * The search is exact (identical to evaluating every fundamental) but proceeds branch-and-bound on
- * a plan-owned block-maximum plane that fdas_convolve_plane writes beside d_plane.  If d_plane is the
- * buffer this plan's fdas_convolve_plane wrote last, its contents must not have been modified since;
- * for any other d_plane the block maxima are rebuilt from it first (one extra pass over the plane).
- * FDAS_EARG: NULL pointers, H out of range, r_lo < 0, capacity < 0.
+ * a plan-owned block-maximum plane M that fdas_convolve_plane writes beside d_plane.  Contract: M is
+ * trusted only when d_plane is the buffer this plan's fdas_convolve_plane wrote last and
+ * fdas_plan_invalidate_plane has not been called since; a caller that changes that buffer in place
+ * calls fdas_plan_invalidate_plane first.  For every other d_plane M is rebuilt from the plane on
+ * EVERY call (one extra pass over it), so a caller-made plane may be refilled freely between calls.
+ * Plane values must be >= 0 (they are powers).
+ * FDAS_EARG: NULL pointers, H out of range, r_lo < 0, capacity < 0, a NaN threshold.
  */
 int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const float* h_thresholds,
                             int64_t r_lo, fdas_cand_t* d_cands, int64_t capacity,
                             unsigned long long* d_count, void* cuda_stream);
+
+/* Tells the plan that the plane fdas_convolve_plane wrote last has been modified (or its buffer reused)
+ * by the caller: the next fdas_harmonic_sum_peaks rebuilds the block maxima from the plane it is given. */
+int fdas_plan_invalidate_plane(fdas_plan_t plan);
 
 /*
  * fdas_search_host -- the same three steps for a HOST time series (the end-to-end entry point):
@@ -180,6 +190,15 @@ int fdas_search_batch(fdas_plan_t plan, const float* const* series, int series_o
  */
 int fdas_thresholds_from_sigma(int H, double nsigma, float* h_thresholds_out);
 
+int fdas_destroy(fdas_plan_t plan);
+const char* fdas_strerror(int status);
+const char* fdas_last_error_detail(void); /* thread-local text of the last CUDA/cuFFT failure */
+
+/* ---------------------------------------------------------------------------------------------
+ * FDAS_DIAGNOSTICS -- test and measurement hooks.  NOT part of the stable ABI: they expose plan
+ * internals (template bank, side plane, launch counter) and may change with the kernels.
+ * ------------------------------------------------------------------------------------------- */
+
 /*
  * fdas_plan_templates_host -- diagnostic: copies the plan's time-domain template bank
  * (nz x (2h+1) complex doubles, interleaved re/im, unit L2 norm) to h_out.  Host only.
@@ -196,10 +215,6 @@ int fdas_plan_debug_maxplane(fdas_plan_t plan, const uint16_t** d_out, int64_t* 
 
 /* Number of kernels the library launched on behalf of this plan since it was created. */
 int64_t fdas_plan_launch_count(fdas_plan_t plan);
-
-int fdas_destroy(fdas_plan_t plan);
-const char* fdas_strerror(int status);
-const char* fdas_last_error_detail(void); /* thread-local text of the last CUDA/cuFFT failure */
 
 #ifdef __cplusplus
 }

@@ -32,6 +32,7 @@ static void free_plan(fdas_plan_s* p) {
     cudaFree(p->ws_series); cudaFree(p->ws_spec); cudaFree(p->ws_plane); cudaFree(p->ws_cands);
     cudaFree(p->ws_count);
     if (p->h_count) cudaFreeHost(p->h_count);
+    if (p->ev_last) cudaEventDestroy(p->ev_last);
     if (p->fft_made) cufftDestroy(p->fft);
     delete p;
 }
@@ -49,7 +50,7 @@ static int derive_info(int64_t N, double tsamp, double zmax, double zstep, int s
     o->n_in = N;
     int64_t nfft = 1;
     while (nfft * 2 <= N) nfft *= 2;
-    if (nfft > ((int64_t)1 << 31)) return FDAS_EARG;  // candidate r is 32-bit
+    if (nfft > ((int64_t)1 << 30)) return FDAS_EUNSUPPORTED;  // cuFFT plan size and 32-bit bin indices
     o->nfft = nfft;
     o->nbins = nfft / 2;
     o->nz = (int)rc + 1;
@@ -141,11 +142,8 @@ static int build_plan(fdas_plan_s* p) {
     const int64_t slots = (int64_t)convolve_ctas_per_sm() * nsm;
     int nsplit = 1;
     if (in.nseg < 4 * slots) nsplit = (int)std::min<int64_t>(in.nz, (4 * slots + in.nseg - 1) / in.nseg);
-    if (const char* e = std::getenv("FDAS_NSPLIT")) {
-        const int v = std::atoi(e);
-        if (v >= 1) nsplit = std::min(v, (int)in.nz);
-    }
     p->nsplit = nsplit;
+    CU(cudaEventCreateWithFlags(&p->ev_last, cudaEventDisableTiming));
     return FDAS_OK;
 }
 
@@ -202,6 +200,20 @@ int fdas_enqueue_harmonic(fdas_plan_s* plan, const void* d_plane, unsigned short
     return FDAS_OK;
 }
 
+// The plan's scratch (cuFFT work area, median table, block-max plane, prefilter list) is shared by
+// every call, so calls on different streams are ordered in issue order: a call on a stream other than
+// the previous call's first waits (on the device) for that call's work.
+static int order_before(fdas_plan_s* p, cudaStream_t st) {
+    if (p->have_last && p->last_stream != st) CU(cudaStreamWaitEvent(st, p->ev_last, 0));
+    return FDAS_OK;
+}
+static int order_after(fdas_plan_s* p, cudaStream_t st) {
+    CU(cudaEventRecord(p->ev_last, st));
+    p->last_stream = st;
+    p->have_last = true;
+    return FDAS_OK;
+}
+
 extern "C" {
 
 int fdas_plan(fdas_plan_t* out, int64_t N, double tsamp, double zmax, double zstep, int seg_len,
@@ -238,16 +250,29 @@ int fdas_plan_info(fdas_plan_t plan, fdas_info_t* out) {
 
 int fdas_prepare_spectrum(fdas_plan_t plan, const float* d_series, void* d_spec, void* cuda_stream) {
     if (!plan || !d_series || !d_spec) return FDAS_EARG;
-    return fdas_enqueue_prepare(plan, d_series, d_spec, (cudaStream_t)cuda_stream);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = order_before(plan, st);
+    if (rc == FDAS_OK) rc = fdas_enqueue_prepare(plan, d_series, d_spec, st);
+    if (rc == FDAS_OK) rc = order_after(plan, st);
+    return rc;
 }
 
 int fdas_convolve_plane(fdas_plan_t plan, const void* d_spec, void* d_plane, void* cuda_stream) {
     if (!plan || !d_spec || !d_plane) return FDAS_EARG;
     if ((reinterpret_cast<uintptr_t>(d_plane) & 15u) != 0) return FDAS_EARG;
     plan->max_valid_for = nullptr;
-    const int rc = fdas_enqueue_convolve(plan, d_spec, d_plane, plan->d_maxplane, (cudaStream_t)cuda_stream);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = order_before(plan, st);
+    if (rc == FDAS_OK) rc = fdas_enqueue_convolve(plan, d_spec, d_plane, plan->d_maxplane, st);
+    if (rc == FDAS_OK) rc = order_after(plan, st);
     if (rc == FDAS_OK) plan->max_valid_for = d_plane;
     return rc;
+}
+
+int fdas_plan_invalidate_plane(fdas_plan_t plan) {
+    if (!plan) return FDAS_EARG;
+    plan->max_valid_for = nullptr;
+    return FDAS_OK;
 }
 
 int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const float* h_thresholds,
@@ -255,11 +280,18 @@ int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const 
                             unsigned long long* d_count, void* cuda_stream) {
     if (!plan || !d_plane || !h_thresholds || !d_count) return FDAS_EARG;
     if (H < 1 || H > 32 || r_lo < 0 || capacity < 0 || (capacity > 0 && !d_cands)) return FDAS_EARG;
-    // M describes the plane fdas_convolve_plane last wrote; any other plane gets its own M first
+    for (int i = 0; i < H; ++i)
+        if (std::isnan(h_thresholds[i])) return FDAS_EARG;
+    // M describes the plane fdas_convolve_plane last wrote (until fdas_plan_invalidate_plane); any
+    // other plane gets its own M first, on every call: its contents may have changed since the last one
     const bool build_max = (plan->max_valid_for != d_plane);
-    const int rc = fdas_enqueue_harmonic(plan, d_plane, plan->d_maxplane, build_max, H, h_thresholds, r_lo,
-                                         d_cands, capacity, d_count, (cudaStream_t)cuda_stream);
-    if (rc == FDAS_OK && build_max && r_lo < plan->info.nbins) plan->max_valid_for = d_plane;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = order_before(plan, st);
+    if (rc == FDAS_OK)
+        rc = fdas_enqueue_harmonic(plan, d_plane, plan->d_maxplane, build_max, H, h_thresholds, r_lo, d_cands,
+                                   capacity, d_count, st);
+    if (rc == FDAS_OK) rc = order_after(plan, st);
+    if (build_max) plan->max_valid_for = nullptr;   // M now belongs to a plane this plan did not write
     return rc;
 }
 

@@ -107,21 +107,13 @@ static int collect(fdas_plan_s* plan, int t, fdas_cand_t* h_cands, int64_t capac
 
 using namespace fdas;
 
-extern "C" int fdas_search_batch(fdas_plan_t plan, const float* const* series, int series_on_host,
-                                 int ntrials, int H, const float* h_thresholds, int64_t r_lo,
-                                 fdas_cand_t* h_cands, int64_t capacity, int64_t* h_counts,
-                                 void* cuda_stream) {
-    if (!plan || !series || ntrials < 0 || !h_thresholds || !h_counts || capacity < 0 ||
-        (capacity > 0 && !h_cands) || H < 1 || H > 32 || r_lo < 0)
-        return FDAS_EARG;
-    for (int t = 0; t < ntrials; ++t)
-        if (!series[t]) return FDAS_EARG;
-    if (ntrials == 0) return FDAS_OK;
+// Queues the whole batch; on an error it returns at once (fdas_search_batch then drains the streams).
+static int run_batch(fdas_plan_s* plan, const float* const* series, int series_on_host, int ntrials, int H,
+                     const float* h_thresholds, int64_t r_lo, fdas_cand_t* h_cands, int64_t capacity,
+                     int64_t* h_counts, cudaStream_t user) {
     const fdas_info_t& in = plan->info;
-    int rc = make_batch_state(plan, series_on_host != 0, capacity);
-    if (rc != FDAS_OK) return rc;
     BatchState* s = plan->batch;
-    cudaStream_t user = (cudaStream_t)cuda_stream;
+    int rc = FDAS_OK;
 
     // everything queued on the caller's stream so far (e.g. the upload of the series) comes first
     CU(cudaEventRecord(s->entry, user));
@@ -188,6 +180,39 @@ extern "C" int fdas_search_batch(fdas_plan_t plan, const float* const* series, i
         CU(cudaStreamWaitEvent(user, s->leave[i], 0));
     }
     for (int i = 0; i < 3; ++i) CU(cudaStreamSynchronize(all[i]));
-    plan->max_valid_for = nullptr;
     return overflow ? FDAS_EOVERFLOW : FDAS_OK;
+}
+
+extern "C" int fdas_search_batch(fdas_plan_t plan, const float* const* series, int series_on_host,
+                                 int ntrials, int H, const float* h_thresholds, int64_t r_lo,
+                                 fdas_cand_t* h_cands, int64_t capacity, int64_t* h_counts,
+                                 void* cuda_stream) {
+    if (!plan || !series || ntrials < 0 || !h_thresholds || !h_counts || capacity < 0 ||
+        (capacity > 0 && !h_cands) || H < 1 || H > 32 || r_lo < 0)
+        return FDAS_EARG;
+    for (int t = 0; t < ntrials; ++t)
+        if (!series[t]) return FDAS_EARG;
+    for (int i = 0; i < H; ++i)
+        if (h_thresholds[i] != h_thresholds[i]) return FDAS_EARG;   // NaN
+    if (ntrials == 0) return FDAS_OK;
+    int rc = make_batch_state(plan, series_on_host != 0, capacity);
+    if (rc != FDAS_OK) return rc;
+    cudaStream_t user = (cudaStream_t)cuda_stream;
+    if (plan->have_last) {   // work of earlier per-trial calls on other streams comes first
+        if (cudaStreamWaitEvent(user, plan->ev_last, 0) != cudaSuccess) return FDAS_ECUDA;
+    }
+    rc = run_batch(plan, series, series_on_host, ntrials, H, h_thresholds, r_lo, h_cands, capacity, h_counts,
+                   user);
+    if (rc != FDAS_OK && rc != FDAS_EOVERFLOW) {
+        // an enqueue failed mid-pipeline: work already queued still writes into h_cands and the pinned
+        // counters, so wait for it (best effort) before the caller may free or reuse them
+        BatchState* s = plan->batch;
+        cudaStreamSynchronize(s->copy);
+        cudaStreamSynchronize(s->a);
+        cudaStreamSynchronize(s->b);
+    }
+    // every stream of the batch has been waited for: nothing of this plan is in flight
+    plan->have_last = false;
+    plan->max_valid_for = nullptr;
+    return rc;
 }

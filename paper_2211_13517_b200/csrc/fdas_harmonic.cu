@@ -350,11 +350,12 @@ __global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(co
     const PfRow r1 = pf_row(p, j, 1);
     uint4 m1[4], m2[4], m3[4], m4[4];   // (only the first DMAX arrays are live)
     m1[0] = __ldg(reinterpret_cast<const uint4*>(r1.mrow) + O);
-    if (hz <= 1) {
+    if (hz <= 1 && r1.thr >= 0.f) {
         // one harmonic only (half of the plane's rows): M > T_1 on the bf16 bit patterns.  For
         // non-negative values the order of the patterns is the order of the values, and with
         // tb = pattern of T_1 truncated to bf16, M > T_1 <=> pattern(M) > tb (M is a bf16 value).
-        const unsigned tb = __float_as_uint(fmaxf(r1.thr, 0.f)) >> 16;
+        // (A negative T_1 passes every point, M = 0 included: no early exit then.)
+        const unsigned tb = __float_as_uint(r1.thr) >> 16;
         const unsigned tb2 = tb | (tb << 16);
         if ((__vcmpgtu2(m1[0].x, tb2) | __vcmpgtu2(m1[0].y, tb2) | __vcmpgtu2(m1[0].z, tb2) |
              __vcmpgtu2(m1[0].w, tb2)) == 0u)
@@ -432,10 +433,7 @@ __global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(co
     pf_emit(p, 2u * O + 1u, j, f[1]);
 }
 
-#ifndef FDAS_PF_MINB
-#define FDAS_PF_MINB 8
-#endif
-__global__ void __launch_bounds__(kPfThreads, FDAS_PF_MINB) prefilter_kernel(const HarmParams p, const int nlow) {
+__global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmParams p, const int nlow) {
     const int j = nlow + blockIdx.y;   // the rows with more than kShallowDepth harmonics (|z| <= zmax/5)
     const int c2 = p.nz - 1;
     const unsigned Q0 = blockIdx.x * (unsigned)kPfThreads;

@@ -42,6 +42,9 @@ struct fdas_plan_s {
     int64_t launches = 0;
     unsigned short* d_maxplane = nullptr;    // block-max plane M (nz x nbins/8, bf16 bits), written by K2
     const void* max_valid_for = nullptr;     // the plane M currently describes (nullptr: none)
+    cudaEvent_t ev_last = nullptr;           // end of the last public per-trial call (cross-stream ordering)
+    cudaStream_t last_stream = nullptr;
+    bool have_last = false;
     uint2* d_maybe = nullptr;                // K3 maybe list (kMaybeCapacity records)
     unsigned long long* d_maybe_count = nullptr;
     // workspace of fdas_search_host (lazy)

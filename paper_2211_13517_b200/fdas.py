@@ -23,7 +23,7 @@ FDAS_OK, FDAS_EARG, FDAS_EALLOC, FDAS_ECUDA, FDAS_ECUFFT, FDAS_EOVERFLOW, FDAS_E
 
 EXPORTS = (
     "fdas_plan", "fdas_plan_info", "fdas_prepare_spectrum", "fdas_convolve_plane",
-    "fdas_harmonic_sum_peaks", "fdas_search_host", "fdas_search_batch", "fdas_thresholds_from_sigma",
+    "fdas_harmonic_sum_peaks", "fdas_plan_invalidate_plane", "fdas_search_host", "fdas_search_batch", "fdas_thresholds_from_sigma",
     "fdas_plan_templates_host", "fdas_plan_debug_maxplane", "fdas_plan_launch_count", "fdas_destroy", "fdas_strerror",
     "fdas_last_error_detail",
 )
@@ -61,6 +61,7 @@ def _load():
     L.fdas_prepare_spectrum.argtypes = [vp, vp, vp, vp]
     L.fdas_convolve_plane.argtypes = [vp, vp, vp, vp]
     L.fdas_harmonic_sum_peaks.argtypes = [vp, vp, ci, C.POINTER(C.c_float), i64, vp, i64, vp, vp]
+    L.fdas_plan_invalidate_plane.argtypes = [vp]
     L.fdas_search_host.argtypes = [vp, vp, ci, C.POINTER(C.c_float), i64, vp, i64, C.POINTER(i64), vp]
     L.fdas_search_batch.argtypes = [vp, C.POINTER(vp), ci, ci, ci, C.POINTER(C.c_float), i64, vp, i64,
                                     C.POINTER(i64), vp]
@@ -163,6 +164,10 @@ class Plan:
             self._h, d_plane.data_ptr(), int(H), thr.ctypes.data_as(C.POINTER(C.c_float)), int(r_lo),
             d_cands.data_ptr() if d_cands is not None else None, cap, d_count.data_ptr(),
             _stream_ptr(stream)), "fdas_harmonic_sum_peaks")
+
+    def invalidate_plane(self):
+        """The plane convolve_plane wrote last was modified by the caller: rebuild the block maxima."""
+        _check(_lib.fdas_plan_invalidate_plane(self._h), "fdas_plan_invalidate_plane")
 
     @staticmethod
     def read_cands(d_cands, d_count) -> PeakResult:

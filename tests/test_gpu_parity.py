@@ -9,12 +9,11 @@ import numpy as np
 import pytest
 
 from paper_2211_13517_b200 import inputs
-from helpers import compare_candidates, gpu_cand_dict, oracle_margin_fn
+from helpers import (REL_POW, STRICT_REL, TOL, PlaneStats, compare_candidates, gpu_cand_dict,
+                     local_amplitude, membership_window, oracle_margin_fn, record_stats)
 
 pytestmark = pytest.mark.gpu
 
-TOL = {"fp32": 1e-4, "bf16": 2e-2, "bf16_plane16": 2e-2, "bf16_tc": 2e-2, "bf16_tc_plane16": 2e-2}
-REL_POW = {"fp32": None, "bf16": 0.03, "bf16_plane16": 0.03, "bf16_tc": 0.03, "bf16_tc_plane16": 0.03}
 ALL_PREC = ["fp32", "bf16", "bf16_plane16", "bf16_tc", "bf16_tc_plane16"]
 
 
@@ -78,14 +77,17 @@ def test_tiny_fp32_full_parity(fdas, torch_, oracle):
     # plane: every element, fp32 tolerance
     P_gpu = d_plane.cpu().numpy().astype(np.float64)
     assert not np.isnan(P_gpu).any()
-    err = np.abs(P_gpu - orc.P).max()
-    assert err <= TOL["fp32"] * orc.P.max(), err / orc.P.max()
+    ps = PlaneStats("fp32")
+    ps.add(P_gpu, orc.P, local_amplitude(orc.w))
+    ps.check(orc.P.max())
     # candidates (oracle gets the same float32 thresholds)
     oc = oracle.candidates(orc.P, wl.nharm, thr.astype(np.float64), wl.r_lo)
     s_at, margin = oracle_margin_fn(oracle, orc.P, wl.nharm, wl.r_lo)
     stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, TOL["fp32"] * orc.P.max(),
-                               None, s_at, margin)
+                               None, s_at, margin, strict_rel=STRICT_REL["fp32"])
     assert res.count == len(res.cands) and stats["common"] >= 1
+    assert stats["only_gpu"] + stats["only_orc"] == 0, stats
+    record_stats("tiny_fp32", {**ps.summary(orc.P.max()), **stats})
     keys = set(gpu_cand_dict(res.cands))
     assert (20000, 23, 1) in keys or (20000, 24, 1) in keys     # the injected signal (z0 = 7.5)
     assert plan.launch_count() == 8      # K1a, K1b, K2, K3 two shallow + general prefilter, exact, flags (cuFFT not counted)
@@ -109,16 +111,24 @@ def test_medium_full_parity(fdas, torch_, oracle, medium_oracle, precision):
     pmax = orc.P.max()
     tol = TOL[precision] * pmax
     # plane, element by element, in row chunks to bound host memory
-    worst = 0.0
+    ps = PlaneStats(precision)
+    W = local_amplitude(orc.w)
     for j0 in range(0, plan.info.nz, 16):
         Pg = d_plane[j0:j0 + 16].float().cpu().numpy().astype(np.float64)
         assert not np.isnan(Pg).any()
-        worst = max(worst, np.abs(Pg - orc.P[j0:j0 + 16]).max())
-    assert worst <= tol, (precision, worst / pmax)
+        ps.add(Pg, orc.P[j0:j0 + 16], W)
+    ps.check(pmax)
+    worst = ps.worst_abs
     oc = oracle.candidates(orc.P, wl.nharm, thr.astype(np.float64), wl.r_lo)
     s_at, margin = oracle_margin_fn(oracle, orc.P, wl.nharm, wl.r_lo)
     stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, tol, REL_POW[precision],
-                               s_at, margin)
+                               s_at, margin, strict_rel=STRICT_REL[precision])
+    if precision == "fp32":
+        assert stats["only_gpu"] + stats["only_orc"] == 0, stats
+    else:       # bf16 storage moves ~0.3 % of the 4e4 triples across their threshold, all within 3 % of it
+        assert stats["only_gpu"] + stats["only_orc"] <= 0.01 * stats["common"], stats
+    assert stats["flags_checked"] > 1000
+    record_stats("medium_" + precision, {**ps.summary(pmax), **stats})
     # the four injected chirps are recovered at (round(r_c), nearest z)
     keys = set(gpu_cand_dict(res.cands))
     for s in wl.signals:
@@ -127,7 +137,7 @@ def test_medium_full_parity(fdas, torch_, oracle, medium_oracle, precision):
         r0, j0 = int(round(s.r_c)), int(round(s.z + wl.zmax))
         assert any((r0 + dr, j0 + dj, 1) in keys for dr in (-1, 0, 1) for dj in (-1, 0, 1)), s
     assert stats["common"] >= 4
-    print(precision, "worst/max", worst / pmax, stats)
+    print(precision, ps.summary(pmax), stats)
 
 
 # --------------------------------------------------------------- K2 alone, fed a chosen spectrum
@@ -150,7 +160,9 @@ def test_convolve_alone_seams_tail_and_invariants(fdas, torch_, oracle, precisio
     assert not np.isnan(Pg).any()
     bank = oracle.template_bank(16.0, 1.0)
     P = oracle.plane(w, bank)
-    assert np.abs(Pg - P).max() <= TOL[precision] * P.max()
+    ps = PlaneStats(precision)
+    ps.add(Pg, P, local_amplitude(w))
+    ps.check(P.max())
     if precision == "fp32":
         # z = 0 row is the power spectrum; conj(w) flips the z axis; a shift by d bins (not a
         # multiple of V) shifts every row
@@ -230,7 +242,8 @@ def test_harmonic_sum_alone_many_candidates(fdas, torch_, oracle, precision):
     oc = oracle.candidates(P, H, thr.astype(np.float64), 5)
     assert oc.count > 500
     s_at, margin = oracle_margin_fn(oracle, P, H, 5)
-    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * P.max(), None, s_at, margin)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * P.max(), None, s_at, margin,
+                               strict_rel=1e-5)
     assert stats["only_gpu"] + stats["only_orc"] <= 3 and stats["flags_checked"] > 100
     # H = 1, r_lo beyond the plane, capacity overflow
     plan.harmonic_sum_peaks(d_plane, 1, thr, nb, d_c, d_n)
@@ -271,7 +284,8 @@ def test_harmonic_sum_small_h_exact_sets(fdas, torch_, oracle, H):
     oc = oracle.candidates(P, H, thr.astype(np.float64), r_lo)
     assert oc.count > 200 and res.count == len(res.cands)
     s_at, margin = oracle_margin_fn(oracle, P, H, r_lo)
-    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * P.max(), None, s_at, margin)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * P.max(), None, s_at, margin,
+                               strict_rel=1e-5)
     assert stats["only_gpu"] + stats["only_orc"] <= 2, stats
     assert min(k[0] for k in gpu_cand_dict(res.cands)) >= r_lo
 
@@ -359,7 +373,7 @@ def test_ska_full_size_sampled_parity(fdas, torch_, oracle, precision):
         for i, (r, j, h) in enumerate(keys):
             assert h <= hmax[i]
             so = S[i, h - 1]
-            assert so > thr[h - 1] - h * tol, ((r, j, h), so)
+            assert so > thr[h - 1] - membership_window(thr, h, tol, precision), ((r, j, h), so)
             assert abs(gd[(r, j, h)][0] - so) <= h * tol
             if REL_POW[precision] is not None:
                 assert abs(gd[(r, j, h)][0] - so) <= REL_POW[precision] * so
@@ -372,10 +386,11 @@ def test_ska_full_size_sampled_parity(fdas, torch_, oracle, precision):
     for i in range(sr.size):
         for h in range(1, hmax[i] + 1):
             key = (int(sr[i]), int(sj[i]), h)
-            if S[i, h - 1] > thr[h - 1] + h * tol:
+            win = membership_window(thr, h, tol, precision)
+            if S[i, h - 1] > thr[h - 1] + win:
                 assert key in gd, key
                 found += 1
-            elif S[i, h - 1] < thr[h - 1] - h * tol:
+            elif S[i, h - 1] < thr[h - 1] - win:
                 assert key not in gd, key
     assert found >= 2          # both injected fundamentals
     print(precision, "sampled worst/max", worst / pmax, "pmax", pmax, "cands", res.count, "found", found)
@@ -460,7 +475,8 @@ def test_tensor_core_path_odd_banks(fdas, torch_, oracle, precision, zmax):
     res = plan.read_cands(d_c, d_n)
     oc = oracle.candidates(Pg, H, thr.astype(np.float64), 16)
     s_at, margin = oracle_margin_fn(oracle, Pg, H, 16)
-    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * Pg.max(), None, s_at, margin)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * Pg.max(), None, s_at, margin,
+                               strict_rel=1e-5)
     assert stats["only_gpu"] + stats["only_orc"] <= 2 and stats["common"] > 10, stats
 
 
@@ -524,7 +540,7 @@ def test_ska_zero_padded_2p24_sampled_parity(fdas, torch_, oracle):
     tol = TOL["bf16_tc"] * pmax
     for i, (r, j, h) in enumerate(keys):
         so = S[i, h - 1]
-        assert h <= hmax[i] and so > thr[h - 1] - h * tol
+        assert h <= hmax[i] and so > thr[h - 1] - membership_window(thr, h, tol, "bf16_tc")
         assert abs(gd[(r, j, h)][0] - so) <= min(h * tol, REL_POW["bf16_tc"] * so)
 
 
@@ -619,5 +635,216 @@ def test_batch_ska_members_full_size(fdas, torch_, oracle, half_res, precision):
                                            np.array([k[1] for k in keys], dtype=np.int32))
     for i, (r, j, h) in enumerate(keys):
         so = S[i, h - 1]
-        assert h <= hmax[i] and so > thr[h - 1] - h * TOL["bf16"] * pmax
+        assert h <= hmax[i] and so > thr[h - 1] - membership_window(thr, h, TOL["bf16"] * pmax, "bf16")
         assert abs(got[(r, j, h)][0] - so) <= min(h * TOL["bf16"] * pmax, REL_POW["bf16"] * so)
+
+
+# ------------------------------------------ configs[2] at full size: EVERY plane point and candidate
+@pytest.fixture(scope="module")
+def ska_oracle_full(oracle):
+    """The oracle's whole SKA-like plane (193 x 2^22 doubles, 6.5 GB) and its candidate list."""
+    wl = inputs.ska()
+    x = inputs.series_for(wl)
+    w = oracle.whiten(oracle.spectrum(x, wl.nfft))
+    bank = oracle.template_bank(wl.zmax, wl.zstep)
+    P = oracle.plane(w, bank)
+    return wl, x, w, P, local_amplitude(w)
+
+
+@pytest.mark.parametrize("precision", ["bf16_tc", "bf16", "fp32"])
+def test_ska_full_plane_parity(fdas, torch_, oracle, ska_oracle_full, precision):
+    """The benched configuration, compared in full (not sampled): all 8.1e8 plane points against the
+    oracle (max-norm and the noise-floor statistic), and the complete candidate list under the literal
+    north_star window plus the strict 3 % window."""
+    torch = torch_
+    wl, x, w, P, W = ska_oracle_full
+    plan, d_spec, d_plane, res, thr = run_gpu(fdas, torch, wl, x, precision)
+    nz, nb = plan.info.nz, plan.info.nbins
+    assert P.shape == (nz, nb)
+    pmax = float(P.max())
+    ps = PlaneStats(precision)
+    for j0 in range(0, nz, 8):
+        Pg = d_plane[j0:j0 + 8].float().cpu().numpy().astype(np.float64)
+        assert not np.isnan(Pg).any()
+        ps.add(Pg, P[j0:j0 + 8], W)
+    ps.check(pmax)
+    oc = oracle.candidates(P, wl.nharm, thr.astype(np.float64), wl.r_lo)
+    s_at, margin = oracle_margin_fn(oracle, P, wl.nharm, wl.r_lo)
+    gd = gpu_cand_dict(res.cands)
+    assert res.count == len(gd)
+    stats = compare_candidates(gd, oc.as_dict(), thr, TOL[precision] * pmax, REL_POW[precision], s_at, margin,
+                               strict_rel=STRICT_REL[precision])
+    if precision == "fp32":
+        assert stats["only_gpu"] + stats["only_orc"] == 0, stats
+    for s in wl.signals:                       # both injected pulsars: fundamental and second harmonic sum
+        r0, j0 = int(round(s.r_c)), int(round(s.z + wl.zmax))
+        assert (r0, j0, 1) in gd and (r0, j0, 2) in gd, s
+    record_stats("ska_full_" + precision, {**ps.summary(pmax), **stats, "pmax": pmax})
+    print(precision, ps.summary(pmax), stats)
+
+
+# ---------------------------------------------------------------- K3: paths no other test reaches
+def test_harmonic_maybe_list_overflow_falls_back_to_full_scan(fdas, torch_, oracle):
+    """Thresholds so low that the prefilter flags more fundamentals than its list holds (2^22): pass B
+    must fall back to scanning every fundamental.  The true count and a capped list are compared with
+    the oracle."""
+    torch = torch_
+    plan = fdas.Plan(1 << 19, 64e-6, 16.0, 1.0, 2048, "fp32")       # 33 x 2^18 points
+    nb, nz = plan.info.nbins, plan.info.nz
+    rng = np.random.default_rng(41)
+    P32 = rng.exponential(1.0, size=(nz, nb)).astype(np.float32)
+    d_plane = torch.from_numpy(P32).cuda()
+    H = 2
+    thr = np.array([0.1, 0.25], dtype=np.float32)
+    d_c, d_n = plan.alloc_cands(1 << 16)
+    plan.harmonic_sum_peaks(d_plane, H, thr, 3, d_c, d_n)
+    torch.cuda.synchronize()
+    res = plan.read_cands(d_c, d_n)
+    oc = oracle.candidates(P32.astype(np.float64), H, thr.astype(np.float64), 3, capacity=1 << 24)
+    assert oc.count > (1 << 22) + (1 << 20)                        # far more than the list holds
+    assert abs(res.count - oc.count) <= 8, (res.count, oc.count)   # fp32 vs double sums at the threshold
+    # membership of the 65536 stored records in the oracle's ~1e7 triples, by sorted integer keys
+    okey = (oc.r.astype(np.int64) * 64 + oc.j) * 64 + oc.h
+    order = np.argsort(okey)
+    okey, opow = okey[order], oc.power[order]
+    c = res.cands
+    assert len(c) == 1 << 16
+    gkey = (c["r"].astype(np.int64) * 64 + c["zidx"]) * 64 + c["h"]
+    assert np.unique(gkey).size == gkey.size
+    pos = np.minimum(np.searchsorted(okey, gkey), okey.size - 1)
+    hit = okey[pos] == gkey
+    assert np.all(np.abs(c["power"][hit] - opow[pos[hit]]) <= 1e-5 * opow[pos[hit]])
+    assert (~hit).sum() <= 8
+    s_at, _ = oracle_margin_fn(oracle, P32.astype(np.float64), H, 3)
+    for rec in c[~hit]:
+        key = (int(rec["r"]), int(rec["zidx"]), int(rec["h"]))
+        assert abs(s_at(*key) - thr[key[2] - 1]) <= 1e-5 * thr[key[2] - 1], key
+
+
+def test_harmonic_even_nz_half_integer_rows(fdas, torch_, oracle):
+    """Reading A20 on the GPU: with an even number of templates (z = -7.5 .. 7.5) the odd harmonics
+    of a row fall between two rows and round half away from zero, on both sides."""
+    torch = torch_
+    plan = fdas.Plan(1 << 14, 64e-6, 7.5, 1.0, 2048, "fp32")
+    nb, nz = plan.info.nbins, plan.info.nz
+    assert nz == 16
+    rng = np.random.default_rng(43)
+    P32 = rng.exponential(1.0, size=(nz, nb)).astype(np.float32)
+    for j in range(nz):                       # a spike per row at harmonics of r = 500 + 7 j
+        for k in (1, 2, 3):
+            P32[j, k * (500 + 7 * j)] += 15.0
+    d_plane = torch.from_numpy(P32).cuda()
+    H = 8
+    thr = fdas.thresholds_from_sigma(H, 3.0)
+    d_c, d_n = plan.alloc_cands(1 << 18)
+    plan.harmonic_sum_peaks(d_plane, H, thr, 10, d_c, d_n)
+    torch.cuda.synchronize()
+    res = plan.read_cands(d_c, d_n)
+    P = P32.astype(np.float64)
+    oc = oracle.candidates(P, H, thr.astype(np.float64), 10)
+    s_at, margin = oracle_margin_fn(oracle, P, H, 10)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * P.max(), None, s_at, margin,
+                               strict_rel=1e-5)
+    assert stats["only_gpu"] + stats["only_orc"] <= 2 and stats["common"] > 100, stats
+    assert any(k[2] >= 3 for k in gpu_cand_dict(res.cands))        # sums that use a half-integer row
+
+
+def test_plane_refilled_in_place_and_invalidate(fdas, torch_, oracle):
+    """The block-max side plane is never trusted for a plane this plan did not write (it is rebuilt on
+    every call), and fdas_plan_invalidate_plane covers a convolve-written plane modified in place."""
+    torch = torch_
+    plan = fdas.Plan(1 << 14, 64e-6, 16.0, 1.0, 2048, "fp32")
+    nb, nz = plan.info.nbins, plan.info.nz
+    H = 4
+    thr = fdas.thresholds_from_sigma(H, 3.5)
+    d_c, d_n = plan.alloc_cands(1 << 16)
+    rng = np.random.default_rng(47)
+    d_plane = torch.empty((nz, nb), dtype=torch.float32, device="cuda")
+    for it in range(3):                                  # same tensor, new contents every time
+        P32 = rng.exponential(1.0 + it, size=(nz, nb)).astype(np.float32)
+        d_plane.copy_(torch.from_numpy(P32))
+        plan.harmonic_sum_peaks(d_plane, H, thr, 8, d_c, d_n)
+        torch.cuda.synchronize()
+        got = set(gpu_cand_dict(plan.read_cands(d_c, d_n).cands))
+        want = oracle.candidates(P32.astype(np.float64), H, thr.astype(np.float64), 8).triples()
+        assert len(got ^ want) <= 2 and len(want) > 20 * (it + 1), (it, len(got), len(want))
+    # a plane written by fdas_convolve_plane, then changed by the caller
+    w = (rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)
+    d_spec = spec_from_complex(torch, w, "fp32")
+    plan.convolve_plane(d_spec, d_plane)
+    plan.harmonic_sum_peaks(d_plane, H, thr, 8, d_c, d_n)
+    before = set(gpu_cand_dict(plan.read_cands(d_c, d_n).cands))
+    d_plane[5, 4000] = 99.0
+    d_plane[20, 7001] = 77.0
+    plan.invalidate_plane()
+    plan.harmonic_sum_peaks(d_plane, H, thr, 8, d_c, d_n)
+    after = set(gpu_cand_dict(plan.read_cands(d_c, d_n).cands))
+    assert (4000, 5, 1) in after and (7001, 20, 1) in after and before <= after
+    want = oracle.candidates(d_plane.cpu().numpy().astype(np.float64), H, thr.astype(np.float64), 8).triples()
+    assert len(after ^ want) <= 2
+
+
+def test_two_streams_share_one_plan(fdas, torch_):
+    """Calls of one plan issued on two streams without host synchronisation are ordered on the device
+    (plan scratch is shared): both trials give what they give alone."""
+    torch = torch_
+    wl = inputs.tiny()
+    plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, "fp32")
+    thr = fdas.thresholds_from_sigma(wl.nharm, 4.5)
+    xs = [inputs.make_series(wl.n, 700 + i, wl.signals if i == 0 else ()) for i in range(2)]
+    want = [gpu_cand_dict(_sequential(fdas, torch, plan, x, wl, thr)[0].cands) for x in xs]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    bufs = []
+    for x in xs:
+        d_c, d_n = plan.alloc_cands(1 << 14)
+        bufs.append((torch.from_numpy(x).cuda(), plan.alloc_spec(), plan.alloc_plane(), d_c, d_n))
+    torch.cuda.synchronize()
+    for rep in range(4):
+        for (d_x, d_spec, d_plane, d_c, d_n), st in zip(bufs, streams):
+            plan.prepare_spectrum(d_x, d_spec, stream=st)
+            plan.convolve_plane(d_spec, d_plane, stream=st)
+            plan.harmonic_sum_peaks(d_plane, wl.nharm, thr, wl.r_lo, d_c, d_n, stream=st)
+    torch.cuda.synchronize()
+    for (d_x, d_spec, d_plane, d_c, d_n), w_ in zip(bufs, want):
+        assert gpu_cand_dict(plan.read_cands(d_c, d_n).cands) == w_
+
+
+# ----------------------------------------------------- other template banks (SURVEY.md 8(f) #3)
+@pytest.mark.parametrize("precision", ALL_PREC)
+@pytest.mark.parametrize("zstep", [0.5, 2.0])
+def test_other_z_spacings_full_parity(fdas, torch_, oracle, precision, zstep):
+    """Half-bin and coarse banks (zmax 16, zstep 0.5 -> 65 templates, zstep 2 -> 17): the plane
+    element by element against the oracle's bank of the same spacing, and the harmonic sums (whose
+    rows are idx(k z_j) = (k z_j + zmax)/zstep) against the oracle's candidates on the GPU's plane."""
+    torch = torch_
+    n = 1 << 16
+    plan = fdas.Plan(n, 64e-6, 16.0, zstep, 2048, precision)
+    nb, nz = plan.info.nbins, plan.info.nz
+    assert nz == int(round(32 / zstep)) + 1
+    rng = np.random.default_rng(int(10 * zstep))
+    w = (rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)
+    for k, a in ((3000, 9.0), (6000, 9.0), (9000, 6.0), (12000, 6.0), (nb - 1, 8.0), (0, 8.0)):
+        w[k] += a
+    d_spec = spec_from_complex(torch, w, precision)
+    d_plane = plan.alloc_plane(); d_plane.fill_(float("nan"))
+    plan.convolve_plane(d_spec, d_plane)
+    H = 8
+    thr = fdas.thresholds_from_sigma(H, 3.5)
+    d_c, d_n = plan.alloc_cands(1 << 17)
+    plan.harmonic_sum_peaks(d_plane, H, thr, 16, d_c, d_n)
+    torch.cuda.synchronize()
+    Pg = d_plane.float().cpu().numpy().astype(np.float64)
+    assert not np.isnan(Pg).any()
+    bank = oracle.template_bank(16.0, zstep)
+    assert bank.shape[0] == nz and np.abs(plan.templates_host() - bank).max() < 1e-12
+    P = oracle.plane(w, bank)
+    ps = PlaneStats(precision)
+    ps.add(Pg, P, local_amplitude(w))
+    ps.check(P.max())
+    res = plan.read_cands(d_c, d_n)
+    oc = oracle.candidates(Pg, H, thr.astype(np.float64), 16)
+    s_at, margin = oracle_margin_fn(oracle, Pg, H, 16)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * Pg.max(), None, s_at, margin,
+                               strict_rel=1e-5)
+    assert stats["only_gpu"] + stats["only_orc"] <= 2 and stats["common"] > 50, stats
+    record_stats(f"zstep{zstep}_{precision}", {**ps.summary(P.max()), **stats})
