@@ -2,7 +2,6 @@
 
   libfdas.so      the product: C ABI of include/fdas.h (K1 whitening, K2 fused convolution,
                   K3 harmonic sum, plan-time host mathematics, cuFFT R2C)
-  libfdas_emu.so  TEST-ONLY host emulator of the K2 CTA (tests/test_host_logic.py)
 
 nvcc cross-compiles without a GPU.  Run ``python -m paper_2211_13517_b200.build``.
 """
@@ -15,7 +14,6 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfdas.so")
-EMU = os.path.join(HERE, "libfdas_emu.so")
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 NVCC = os.path.join(CUDA_HOME, "bin", "nvcc")
 
@@ -23,7 +21,6 @@ ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 LIB_SOURCES = ["fdas_api.cu", "fdas_batch.cu", "fdas_convolve.cu", "fdas_convolve_tc.cu", "fdas_whiten.cu", "fdas_harmonic.cu", "fdas_host.cpp"]
-EMU_SOURCES = ["fdas_emu.cu", "fdas_host.cpp"]
 HEADERS = ["fdas_fft_core.cuh", "fdas_tc_common.h", "fdas_host.h", "fdas_kernels.h", "fdas_plan_priv.h", os.path.join("..", "..", "include", "fdas.h")]
 
 
@@ -43,8 +40,7 @@ def _run(cmd, verbose):
 
 def build_lib(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> str:
     if force or _stale(LIB, LIB_SOURCES):
-        extra = os.environ.get("FDAS_NVCC_FLAGS", "").split()   # experiments: -DFDAS_K2_...=n
-        cmd = [NVCC] + ARCH + COMMON + extra + (["-Xptxas", "-v"] if ptxas_v else []) + [
+        cmd = [NVCC] + ARCH + COMMON + (["-Xptxas", "-v"] if ptxas_v else []) + [
             "-shared", "-o", LIB] + LIB_SOURCES + [
             "-L" + os.path.join(CUDA_HOME, "lib64"), "-lcufft",
             "-Xlinker", "-rpath," + os.path.join(CUDA_HOME, "lib64")]
@@ -52,16 +48,8 @@ def build_lib(force: bool = False, verbose: bool = False, ptxas_v: bool = False)
     return LIB
 
 
-def build_emu(force: bool = False, verbose: bool = False) -> str:
-    if force or _stale(EMU, EMU_SOURCES):
-        cmd = [NVCC, "-O2", "-std=c++17", "-Xcompiler", "-fPIC", "-Wno-deprecated-gpu-targets",
-               "-shared", "-o", EMU] + EMU_SOURCES
-        _run(cmd, verbose)
-    return EMU
-
-
 def build_all(force: bool = False, verbose: bool = False):
-    return build_lib(force, verbose), build_emu(force, verbose)
+    return build_lib(force, verbose)
 
 
 if __name__ == "__main__":

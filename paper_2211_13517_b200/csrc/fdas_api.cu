@@ -75,27 +75,25 @@ static int build_plan(fdas_plan_s* p) {
     p->bank_time = bank.time;
     if (fdas_is_tc(in.precision)) {
         bool fits = tc_geometry(in.nz, in.halfwidth, &p->tc) && in.nbins % 128 == 0;
-        if (fits) {   // bank image + window stages + epilogue tiles within the CTA's shared memory
-            ConvTcParams t{};
-            t.bimg_bytes = p->tc.bytes; t.kp = p->tc.kp;
+        if (fits) {   // window stages + epilogue tiles within the CTA's shared memory
             int dev0 = 0, optin = 0;
             CU(cudaGetDevice(&dev0));
             CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev0));
-            fits = convolve_tc_smem_bytes(t) <= optin;
+            fits = convolve_tc_smem_bytes(p->tc.kp, p->tc.npair, fdas_plane16(in.precision)) <= optin;
         }
         if (!fits) {
-            g_detail = "FDAS_BF16_TC: template bank does not fit the tensor-core kernel";
+            g_detail = "FDAS_BF16_TC: template bank does not fit the tensor-core kernel (1..128 conjugate pairs, <= 255 taps, nbins % 128 == 0)";
             return FDAS_EUNSUPPORTED;
         }
-        std::vector<uint16_t> img;
+        std::vector<uint32_t> img;
         double asym = 0.0;
         pack_bank_tc(bank, p->tc, &img, &asym);
         if (asym > 1e-12) {
             g_detail = "FDAS_BF16_TC: bank is not conjugate-symmetric in z";
             return FDAS_EUNSUPPORTED;
         }
-        CU(cudaMalloc(&p->d_bank, img.size() * sizeof(uint16_t)));
-        CU(cudaMemcpy(p->d_bank, img.data(), img.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        CU(cudaMalloc(&p->d_bank, img.size() * sizeof(uint32_t)));
+        CU(cudaMemcpy(p->d_bank, img.data(), img.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
     } else if (in.precision == FDAS_FP32) {
         std::vector<float> packed;
         pack_bank_fp32(bank, &packed);
@@ -163,12 +161,12 @@ int fdas_enqueue_convolve(fdas_plan_s* plan, const void* d_spec, void* d_plane,
                           unsigned short* d_maxplane, cudaStream_t st) {
     if (fdas_is_tc(plan->info.precision)) {
         ConvTcParams t;
-        t.spec = reinterpret_cast<const unsigned*>(d_spec); t.plane = d_plane; t.bimg = plan->d_bank;
-        t.bimg_bytes = plan->tc.bytes; t.nbins = plan->info.nbins; t.pitch = plan->info.plane_pitch;
-        t.nz = plan->info.nz; t.h = plan->info.halfwidth; t.kp = plan->tc.kp;
-        t.ngroups = plan->tc.ngroups; t.gch = plan->tc.gch;
+        t.spec = reinterpret_cast<const unsigned*>(d_spec); t.plane = d_plane;
+        t.bimg = reinterpret_cast<const uint32_t*>(plan->d_bank);
+        t.nbins = plan->info.nbins; t.pitch = plan->info.plane_pitch;
+        t.nz = plan->info.nz; t.h = plan->info.halfwidth; t.kp = plan->tc.kp; t.npair = plan->tc.npair;
         t.maxplane = d_maxplane; t.mpitch = plan->info.nbins / 8;
-        CU(launch_convolve_tc(fdas_plane16(plan->info.precision), t, plan->nsm, st));
+        CU(launch_convolve_tc(fdas_plane16(plan->info.precision), t, &plan->tc_maps, plan->nsm, st));
         plan->launches += 1;
         return FDAS_OK;
     }

@@ -167,34 +167,25 @@ void pack_bank_bf16(const Bank& bank, std::vector<uint32_t>* out) {
 }
 
 bool tc_geometry(int nz, int h, TcGeom* g) {
-    if (nz < 3 || (nz & 1) == 0 || h < 1) return false;
-    g->npair = (nz - 1) / 2;
+    if (nz < 2 || h < 1) return false;
+    g->npair = nz / 2;
     g->kp = ((2 * h + 1) + 15) / 16 * 16;
-    g->nch = (g->npair + 7) / 8;
-    g->ngroups = (g->nch + 5) / 6;
-    g->gch = (g->nch + g->ngroups - 1) / g->ngroups;
-    g->ng = 16 * g->gch;
-    g->ntot = g->ngroups * g->ng;
-    g->lbo = (g->ntot / 8) * 128;
-    g->bytes = g->ntot * g->kp * 2;
-    // descriptor fields are 14 bits of 16-byte units; the image must leave room for the H stages
-    return g->lbo < (1 << 18) && g->bytes <= 160 * 1024;
+    // 256 tensor-memory columns hold the two accumulator stages, the rest the two bank images
+    return g->npair <= 128 && 256 + g->kp <= 512;
 }
 
-void pack_bank_tc(const Bank& bank, const TcGeom& g, std::vector<uint16_t>* out, double* asym) {
-    const int taps = 2 * bank.h + 1, mid = (bank.nz - 1) / 2;
-    out->assign((size_t)g.ntot * g.kp, (uint16_t)0);
+void pack_bank_tc(const Bank& bank, const TcGeom& g, std::vector<uint32_t>* out, double* asym) {
+    const int taps = 2 * bank.h + 1, kw = g.kp / 2;
+    out->assign((size_t)2 * 128 * kw, 0u);
     double worst = 0.0;
     for (int p = 0; p < g.npair; ++p) {
-        const cd* tp = &bank.time[(size_t)(mid + 1 + p) * taps];
-        const cd* tm = &bank.time[(size_t)(mid - 1 - p) * taps];
-        const int grp = p / (8 * g.gch), pl = p % (8 * g.gch);
+        const cd* tp = &bank.time[(size_t)(bank.nz - g.npair + p) * taps];
+        const cd* tm = &bank.time[(size_t)(g.npair - 1 - p) * taps];
         for (int k = 0; k < taps; ++k) {
             worst = std::max(worst, std::abs(tm[k] - std::conj(tp[k])));
             for (int part = 0; part < 2; ++part) {
-                const int n = grp * g.ng + 2 * pl + part;
-                const size_t idx = (((size_t)(k / 8) * (g.ntot / 8) + n / 8) * 8 + n % 8) * 8 + k % 8;
-                (*out)[idx] = (uint16_t)bf16_rne((float)(part ? tp[k].imag() : tp[k].real()));
+                const uint32_t b = bf16_rne((float)(part ? tp[k].imag() : tp[k].real()));
+                (*out)[((size_t)part * 128 + p) * kw + k / 2] |= b << (16 * (k & 1));
             }
         }
     }

@@ -36,22 +36,20 @@ void host_fft(cd* a, int n, int sign);
 void pack_bank_fp32(const Bank& bank, std::vector<float>* out);
 void pack_bank_bf16(const Bank& bank, std::vector<uint32_t>* out);
 
-// K2-TC operand geometry (fdas_convolve_tc.cu).  The nz templates are the z = 0 row plus
-// npair = (nz-1)/2 conjugate pairs (T_{-z} = conj(T_z)); pair p uses row j = mid+1+p.  Pairs are cut
-// into chunks of 8 (16 operand columns: Re T, Im T interleaved) and groups of gch <= 6 chunks.
+// K2-TC operand geometry (fdas_convolve_tc.cu).  The nz templates are npair = nz/2 conjugate pairs
+// (T_{-z} = conj(T_z)) plus, for odd nz, the z = 0 row; pair p is rows j+ = nz - npair + p and
+// j- = npair - 1 - p.
 struct TcGeom {
-    int npair = 0, kp = 0, nch = 0, ngroups = 0, gch = 0;
-    int ng = 0;      // operand columns per group = 16 gch
-    int ntot = 0;    // ngroups * ng
-    int lbo = 0;     // bytes between the two 8-tap halves of one K = 16 step = (ntot/8) * 128
-    int bytes = 0;   // ntot * kp * 2
+    int npair = 0;   // 1..128: one TMEM lane per pair
+    int kp = 0;      // taps 2h+1 padded to a multiple of 16
 };
-// false when the bank does not fit the kernel (shared memory) or nz is even.
+// false when the bank does not fit the kernel (more than 128 pairs, none, or too many taps for the
+// tensor-memory columns left beside the accumulators).
 bool tc_geometry(int nz, int h, TcGeom* g);
-// B image: bf16 (RNE) of B[n][k] = Re/Im T_j[k - h], zero for k > 2h and for padding columns, at
-// 16-bit index ((k/8 * ntot/8 + n/8) * 8 + n%8) * 8 + k%8 (8x16-byte core matrices, K-major).
-// *asym receives max |T_{-z}[m] - conj(T_z[m])| over the bank (must be ~1e-16 for the pairing).
-void pack_bank_tc(const Bank& bank, const TcGeom& g, std::vector<uint16_t>* out, double* asym);
+// Bank image for tensor memory: word [(part*128 + p)*(kp/2) + c] = bf16(X[2c]) | bf16(X[2c+1]) << 16
+// (RNE), X[k] = Re (part 0) or Im (part 1) of T_{j+(p)}[k - h], zero for k > 2h and for rows p >= npair.
+// *asym receives max |T_{j-}[m] - conj(T_{j+}[m])| over the bank (must be ~1e-16 for the pairing).
+void pack_bank_tc(const Bank& bank, const TcGeom& g, std::vector<uint32_t>* out, double* asym);
 
 // tw1[k0][n1-1] = exp(+2 pi i n1 k0 / 2048), n1 = 1..15 (128 x 15 complex fp32)
 // tw2[q][k-1]   = exp(+2 pi i q k / 128), q = 0..15, k = 1..7 (16 x 7 complex fp32)

@@ -27,24 +27,34 @@ cudaError_t launch_convolve(int precision, const ConvParams& p, int64_t nseg, in
 int convolve_ctas_per_sm();  // resident CTAs per SM K2 is launched for (sizes the template split)
 
 // K2-TC: the convolution stage as a dense contraction on the tensor cores (fdas_convolve_tc.cu).
-// Direct correlation y_j(r) = sum_m w[r+m] conj(T_j[m]) written as D[r][n] = sum_k A[r][k] B[n][k]
-// with A the sliding-window (Hankel) matrix of the bf16 spectrum and B the bf16 tap-domain bank.
+// Direct correlation y_j(r) = sum_m w[r+m] conj(T_j[m]) written as D[p][n] = sum_k A[p][k] B[n][k]
+// with A the bf16 tap-domain bank (one row per conjugate pair of templates, kept in tensor memory) and
+// B the sliding-window (Hankel) matrix of the bf16 spectrum.
 struct ConvTcParams {
     const unsigned* spec;      // nbins packed bf16x2 (re low, im high)
     void* plane;               // nz x pitch: float or bf16
-    const void* bimg;          // B operand image in UMMA K-major no-swizzle order (fdas_host.h)
-    int bimg_bytes;
+    const uint32_t* bimg;      // bank image [2 parts][128 rows][kp/2 words] (fdas_host.h pack_bank_tc)
     int64_t nbins, pitch;
     int nz, h;
     int kp;                    // taps 2h+1 padded to a multiple of 16
-    int ngroups, gch;          // template-pair groups per tile, chunks of 8 pairs per group (<= 6)
+    int npair;                 // conjugate template pairs (nz / 2), 1..128
     unsigned short* maxplane;  // as ConvParams
     int64_t mpitch;
-    __host__ __device__ int ng_cols() const { return 16 * gch; }
+};
+// Tensor maps of the plane buffers seen so far (encoded on the host once per buffer).
+struct TcMapCache {
+    static constexpr int kEntries = 4;
+    struct Entry {
+        alignas(64) unsigned char pmap[128];        // CUtensorMap of the plane (boxes of 32 rows x 64 bins)
+        alignas(64) unsigned char pmap_tail[128];   // the same with boxes of npair % 32 rows (ragged banks)
+        const void* plane = nullptr;
+        bool valid = false;
+    } e[kEntries];
+    int next = 0;
 };
 // One persistent CTA per SM; `nsm` CTAs are launched.  plane16 != 0 stores the plane as bf16.
-cudaError_t launch_convolve_tc(int plane16, const ConvTcParams& p, int nsm, cudaStream_t st);
-int convolve_tc_smem_bytes(const ConvTcParams& p);
+cudaError_t launch_convolve_tc(int plane16, const ConvTcParams& p, TcMapCache* cache, int nsm, cudaStream_t st);
+int convolve_tc_smem_bytes(int kp, int npair, int plane16);
 
 struct WhitenParams {
     const float2* X;         // nfft/2 + 1 complex from cuFFT R2C

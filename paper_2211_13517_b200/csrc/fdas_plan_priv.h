@@ -38,6 +38,7 @@ struct fdas_plan_s {
     int nblk = 0;
     int nsplit = 1;
     fdas::TcGeom tc;                          // K2-TC operand geometry (FDAS_BF16_TC*)
+    fdas::TcMapCache tc_maps;                 // K2-TC tensor maps of the output buffers seen so far
     int nsm = 148;
     int64_t launches = 0;
     unsigned short* d_maxplane = nullptr;    // block-max plane M (nz x nbins/8, bf16 bits), written by K2

@@ -1,5 +1,5 @@
-// fdas_emu.cu -- TEST-ONLY host emulator of the K2 CTA (libfdas_emu.so).  NOT part of the product:
-// libfdas.so does not contain it and the Python binding never loads it.  It steps the exact
+// fdas_emu.cu -- TEST-ONLY host emulator of the K2 CTA (tests/emu/libfdas_emu.so).  NOT part of the
+// product: it lives under tests/, libfdas.so does not contain it and the Python binding never loads it.  It steps the exact
 // __host__ __device__ building blocks of fdas_fft_core.cuh thread by thread, phase by phase (one
 // loop over the 128 "threads" per barrier interval), with the same packed template bank, twiddle
 // tables and index arithmetic as fdas_convolve.cu, so that layout or indexing mistakes show up in
@@ -11,9 +11,9 @@
 #include <vector>
 
 #include "../../include/fdas.h"
-#include "fdas_fft_core.cuh"
-#include "fdas_host.h"
-#include "fdas_tc_common.h"
+#include "../../paper_2211_13517_b200/csrc/fdas_fft_core.cuh"
+#include "../../paper_2211_13517_b200/csrc/fdas_host.h"
+#include "../../paper_2211_13517_b200/csrc/fdas_tc_common.h"
 
 using namespace fdas;
 
@@ -171,33 +171,34 @@ int fdas_emu_convolve(const float* spec, int64_t nb, double zmax, double zstep, 
 }  // extern "C"
 
 // ------------------------------------------------------------------------------------------------
-// K2-TC stepped on the host: the same shared-memory image, descriptor encodings, producer row
-// builder, MMA issue order, TMEM column map and epilogue as fdas_convolve_tc.cu; only tcgen05.mma is
-// replaced by `emu_umma`, which decodes the two shared-memory descriptors and the instruction
-// descriptor as the hardware is documented to (K-major, no swizzle, M = 128, K = 16).
+// K2-TC stepped on the host: the same bank image (as the kernel writes it to tensor memory), window
+// image in shared memory, descriptor encodings, MMA issue order, TMEM column map and epilogue as
+// fdas_convolve_tc.cu; only tcgen05.mma is replaced by `emu_umma_ts`, which reads the A operand from
+// the emulated tensor memory (lane = row, two bf16 per 32-bit column) and decodes the shared-memory
+// descriptor of the B operand as the hardware is documented to (K-major, no swizzle, K = 16).
 namespace {
 
 inline float bf16_to_f(uint16_t b) { return bf16_bits_to_f32(b); }
 
-void emu_umma(const std::vector<unsigned char>& smem, float (*D)[256], int dcol, uint64_t adesc,
-              uint64_t bdesc, uint32_t idesc, bool accumulate) {
-    const uint32_t a0 = (uint32_t)(adesc & 0x3fff) << 4, alb = (uint32_t)((adesc >> 16) & 0x3fff) << 4,
-                   asb = (uint32_t)((adesc >> 32) & 0x3fff) << 4;
+// D[lane][dcol + n] (+)= sum_k A[lane][acol*2 + k] B[n][k]; A words are TMEM columns of packed pairs.
+void emu_umma_ts(const std::vector<unsigned char>& smem, std::vector<uint32_t>& tmem /*128 x 512*/, int dcol,
+                 int acol, uint64_t bdesc, uint32_t idesc, bool accumulate) {
     const uint32_t b0 = (uint32_t)(bdesc & 0x3fff) << 4, blb = (uint32_t)((bdesc >> 16) & 0x3fff) << 4,
                    bsb = (uint32_t)((bdesc >> 32) & 0x3fff) << 4;
     const int N = (int)((idesc >> 17) & 0x3f) << 3, M = (int)((idesc >> 24) & 0x1f) << 4;
     for (int i = 0; i < M; ++i)
         for (int n = 0; n < N; ++n) {
-            float acc = accumulate ? D[i][dcol + n] : 0.0f;
+            float acc = 0.0f;
+            if (accumulate) std::memcpy(&acc, &tmem[(size_t)i * 512 + dcol + n], 4);
             for (int k = 0; k < 16; ++k) {
-                const uint32_t ao = a0 + (i % 8) * 16 + (i / 8) * asb + (k / 8) * alb + (k % 8) * 2;
+                const uint32_t aw = tmem[(size_t)i * 512 + acol + k / 2];
+                const uint16_t av = (uint16_t)(aw >> (16 * (k & 1)));
                 const uint32_t bo = b0 + (n % 8) * 16 + (n / 8) * bsb + (k / 8) * blb + (k % 8) * 2;
-                uint16_t av, bv;
-                std::memcpy(&av, &smem[ao], 2);
+                uint16_t bv;
                 std::memcpy(&bv, &smem[bo], 2);
                 acc += bf16_to_f(av) * bf16_to_f(bv);
             }
-            D[i][dcol + n] = acc;
+            std::memcpy(&tmem[(size_t)i * 512 + dcol + n], &acc, 4);
         }
 }
 
@@ -216,18 +217,26 @@ int fdas_emu_convolve_tc(const float* spec, int64_t nb, double zmax, double zste
     build_bank(zmax, zstep, nz, h, kL, &bank);
     TcGeom g;
     if (!tc_geometry(nz, h, &g)) return FDAS_EUNSUPPORTED;
-    std::vector<uint16_t> img;
+    std::vector<uint32_t> img;
     double asym = 0.0;
     pack_bank_tc(bank, g, &img, &asym);
     if (asym > 1e-12) return FDAS_EUNSUPPORTED;
-    const Layout L = make_layout(g.bytes, g.kp);
+    const int kw = g.kp / 2, npair = g.npair, jplus0 = nz - npair, ksteps = g.kp / 16;
+    const Layout L = make_layout(g.kp, 2 * ((npair + 31) / 32), 2, plane16);
     std::vector<unsigned char> smem((size_t)L.total, 0xff);   // 0xff: unwritten bf16 reads as NaN
-    std::memcpy(&smem[L.b_off], img.data(), (size_t)g.bytes);
+    std::vector<uint32_t> tmem((size_t)128 * 512, 0x7fc00000u);
+    for (int part = 0; part < 2; ++part)                      // the kernel's tcgen05.st of the bank
+        for (int lane = 0; lane < 128; ++lane)
+            for (int c = 0; c < kw; ++c)
+                tmem[(size_t)lane * 512 + kBankCol0 + part * kw + c] = img[((size_t)part * 128 + lane) * kw + c];
     std::vector<uint32_t> specq((size_t)nb);
     for (int64_t k = 0; k < nb; ++k) specq[k] = pack_bf16x2(spec[2 * k], spec[2 * k + 1]);
-    const int npair = (nz - 1) / 2, mid = npair, ksteps = g.kp / 16;
     const int64_t mpitch = nb / 8, ntiles = nb / kTileR;
-    auto D = new float[2][128][256];
+    auto store = [&](int j, int64_t r, float P) {
+        if (j < 0 || j >= nz) return;                         // clipped by the TMA store
+        if (plane16) P = bf16_bits_to_f32(f32_to_bf16_rne(P));
+        plane[(size_t)j * nb + r] = P;
+    };
     uint32_t item = 0;
     int it = 0;
     for (int64_t tile = 0; tile < ntiles; ++tile, ++it) {
@@ -235,7 +244,7 @@ int fdas_emu_convolve_tc(const float* spec, int64_t nb, double zmax, double zste
         const int hs = it % kHStages;
         uint16_t* sre = reinterpret_cast<uint16_t*>(&smem[L.st_off]);
         uint16_t* sim = reinterpret_cast<uint16_t*>(&smem[L.st_off + L.st_part]);
-        const int nrows = g.kp + 120, nsrc = g.kp + 130;
+        const int nrows = window_rows(g.kp), nsrc = nrows + 24;
         const int64_t base = tile * kTileR - h;
         for (int i = 0; i < nsrc; ++i) {
             const int64_t idx = base + i;
@@ -248,47 +257,39 @@ int fdas_emu_convolve_tc(const float* spec, int64_t nb, double zmax, double zste
             for (int part = 0; part < 2; ++part) {
                 const uint32_t* w32 = reinterpret_cast<const uint32_t*>(part ? sim : sre) + (rho >> 1);
                 const uint4 o = window_row(w32, rho);
-                std::memcpy(hst + part * L.h_part + rho * 16, &o, 16);
+                std::memcpy(hst + window_row_offset(rho, part), &o, 16);
+            }
+        if (nz & 1)
+            for (int b = 0; b < kTileR; ++b) {
+                const float2 w = unpack_bf16x2(specq[tile * kTileR + b]);
+                store(npair, tile * kTileR + b, fmaf(w.x, w.x, w.y * w.y));
             }
         // MMA issuer + epilogue, one accumulator stage at a time
-        const uint32_t idesc = instr_desc(16 * g.gch);
-        const uint32_t lbo = (uint32_t)(g.ngroups * g.gch * 2) * 128u;
-        const uint32_t a_re = (uint32_t)(L.h_off + hs * L.h_stage), a_im = a_re + L.h_part;
-        for (int grp = 0; grp < g.ngroups; ++grp, ++item) {
-            const uint32_t st = item & 1u;
-            const uint32_t bbase = (uint32_t)L.b_off + (uint32_t)(grp * g.gch * 2) * 128u;
+        const uint32_t idesc = instr_desc(2 * kSubR);
+        const uint32_t hbase = (uint32_t)(L.h_off + hs * L.h_stage);
+        for (int s = 0; s < kSubTiles; ++s, ++item) {
+            const int st = (int)(item & 1u);
+            const int d_r = st * kAccCols, d_i = d_r + 2 * kSubR;
             for (int ks = 0; ks < ksteps; ++ks) {
-                const uint64_t bd = smem_desc(bbase + (uint32_t)ks * 2u * lbo, lbo, 128u);
-                emu_umma(smem, D[st], 0, smem_desc(a_re + ks * 256u, 128u, 128u), bd, idesc, ks > 0);
-                emu_umma(smem, D[st], 128, smem_desc(a_im + ks * 256u, 128u, 128u), bd, idesc, ks > 0);
+                const uint64_t bd = smem_desc(hbase + window_desc_offset(s, ks), kWinLbo, kWinSbo);
+                emu_umma_ts(smem, tmem, d_r, kBankCol0 + 8 * ks, bd, idesc, ks > 0);
+                emu_umma_ts(smem, tmem, d_i, kBankCol0 + kw + 8 * ks, bd, idesc, ks > 0);
             }
-            for (int lane_r = 0; lane_r < 128; ++lane_r) {
-                const int64_t r = tile * kTileR + lane_r;
-                if (grp == 0) {
-                    const float2 w = unpack_bf16x2(specq[r]);
-                    float P = fmaf(w.x, w.x, w.y * w.y);
-                    if (plane16) P = bf16_bits_to_f32(f32_to_bf16_rne(P));
-                    plane[(size_t)mid * nb + r] = P;
-                }
-                for (int c = 0; c < g.gch; ++c)
-                    for (int pp = 0; pp < 8; ++pp) {
-                        const int pr = (grp * g.gch + c) * 8 + pp;
-                        if (pr >= npair) continue;
-                        float Pp, Pm;
-                        pair_powers(D[st][lane_r][16 * c + 2 * pp], D[st][lane_r][16 * c + 2 * pp + 1],
-                                    D[st][lane_r][128 + 16 * c + 2 * pp], D[st][lane_r][128 + 16 * c + 2 * pp + 1],
-                                    &Pp, &Pm);
-                        if (plane16) {
-                            Pp = bf16_bits_to_f32(f32_to_bf16_rne(Pp));
-                            Pm = bf16_bits_to_f32(f32_to_bf16_rne(Pm));
-                        }
-                        plane[(size_t)(mid + 1 + pr) * nb + r] = Pp;
-                        plane[(size_t)(mid - 1 - pr) * nb + r] = Pm;
+            for (int p = 0; p < 32 * ((npair + 31) / 32); ++p)
+                for (int bg = 0; bg < kSubR / 8; ++bg)
+                    for (int e = 0; e < 8; ++e) {
+                        float Ar, Ai, Br, Bi, Pp, Pm;
+                        std::memcpy(&Ar, &tmem[(size_t)p * 512 + d_r + 16 * bg + e], 4);
+                        std::memcpy(&Ai, &tmem[(size_t)p * 512 + d_r + 16 * bg + 8 + e], 4);
+                        std::memcpy(&Br, &tmem[(size_t)p * 512 + d_i + 16 * bg + e], 4);
+                        std::memcpy(&Bi, &tmem[(size_t)p * 512 + d_i + 16 * bg + 8 + e], 4);
+                        pair_powers(Ar, Br, Ai, Bi, &Pp, &Pm);
+                        const int64_t r = tile * kTileR + kSubR * s + 8 * bg + e;
+                        store(jplus0 + p, r, Pp);
+                        store(npair - 1 - p, r, Pm);
                     }
-            }
         }
     }
-    delete[] D;
     // block maxima of the values as stored, rounded toward +inf to bf16
     for (int j = 0; j < nz; ++j)
         for (int64_t b = 0; b < mpitch; ++b) {

@@ -20,7 +20,9 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 @pytest.fixture(scope="module")
 def emu():
-    L = C.CDLL(build.build_emu())
+    sys.path.insert(0, os.path.join(ROOT, "tests", "emu"))
+    import build_emu
+    L = C.CDLL(build_emu.build_emu())
     L.fdas_emu_convolve.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_int, C.c_void_p]
     L.fdas_emu_templates.argtypes = [C.c_double, C.c_double, C.c_int, C.c_int, C.c_void_p]
     L.fdas_emu_ifft2048.argtypes = [C.c_void_p, C.c_void_p]
