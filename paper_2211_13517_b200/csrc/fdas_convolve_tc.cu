@@ -191,12 +191,17 @@ __device__ __forceinline__ unsigned group_to_smem(const uint32_t* __restrict__ a
         mp = max(xp & 0xffffu, xp >> 16);
         mm = max(xm & 0xffffu, xm >> 16);
     } else {
+        // The swizzle phase of a row's chunk, (2 row + half) & 7, takes only 4 values over the 8 rows of a
+        // shared-memory store phase, so the lanes with bit 2 set write their two 16-byte units in the
+        // opposite order: every store instruction then touches 8 different 16-byte bank groups.
+        const bool flip = (threadIdx.x & 4) != 0;
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
-            *reinterpret_cast<float4*>(tile_p + stage_unit_offset(rowp, half, 2 * bg + c, 0)) =
-                make_float4(Pp[4 * c], Pp[4 * c + 1], Pp[4 * c + 2], Pp[4 * c + 3]);
-            *reinterpret_cast<float4*>(tile_m + stage_unit_offset(rowm, half, 2 * bg + c, 0)) =
-                make_float4(Pm[4 * c], Pm[4 * c + 1], Pm[4 * c + 2], Pm[4 * c + 3]);
+            const int u = 2 * bg + (flip ? 1 - c : c);
+            const float4 vp = (c == 0) == !flip ? make_float4(Pp[0], Pp[1], Pp[2], Pp[3]) : make_float4(Pp[4], Pp[5], Pp[6], Pp[7]);
+            const float4 vm = (c == 0) == !flip ? make_float4(Pm[0], Pm[1], Pm[2], Pm[3]) : make_float4(Pm[4], Pm[5], Pm[6], Pm[7]);
+            *reinterpret_cast<float4*>(tile_p + stage_unit_offset(rowp, half, u, 0)) = vp;
+            *reinterpret_cast<float4*>(tile_m + stage_unit_offset(rowm, half, u, 0)) = vm;
         }
         const float fp = fmaxf(fmaxf(fmaxf(Pp[0], Pp[1]), fmaxf(Pp[2], Pp[3])), fmaxf(fmaxf(Pp[4], Pp[5]), fmaxf(Pp[6], Pp[7])));
         const float fm = fmaxf(fmaxf(fmaxf(Pm[0], Pm[1]), fmaxf(Pm[2], Pm[3])), fmaxf(fmaxf(Pm[4], Pm[5]), fmaxf(Pm[6], Pm[7])));
