@@ -222,8 +222,8 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
     const uint32_t bar0 = smem_u32(smem + L.bar_off);
     // barriers: hfull[3] | hempty[3] | tfull[4] | tempty[4]; then the TMEM base address slot.
     // tfull / tempty are indexed by the SUB-TILE (one phase per tile: a waiter must see every phase of
-    // its barrier, and sub-tiles s and s ^ 2 are drained by different warps); the accumulator stage of
-    // sub-tile s is s & 1, so the MMA of sub-tile s waits for the drain of sub-tile s ^ 2.
+    // its barrier); the accumulator stage of sub-tile s is s >> 1 (one stage per epilogue set), so the
+    // MMA of sub-tile s waits for the drain of sub-tile s ^ 1.
     auto hfull = [&](int s) { return bar0 + 8u * s; };
     auto hempty = [&](int s) { return bar0 + 8u * (kHStages + s); };
     auto tfull = [&](int s) { return bar0 + 8u * (2 * kHStages + s); };
@@ -365,11 +365,15 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
             tc_fence_after();
             const uint32_t hbase = smem_u32(smem + L.h_off + hs * L.h_stage);
 #pragma unroll
-            for (int s = 0; s < kSubTiles; ++s) {
-                const uint32_t st = s & 1u;
-                // the stage was last filled for sub-tile s ^ 2: of this tile (s >= 2) or the previous
-                if (s >= 2 || it > 0) {
-                    mbar_wait(tempty(s ^ 2), (uint32_t)(s >= 2 ? it : it - 1) & 1u);
+            for (int pos = 0; pos < kSubTiles; ++pos) {
+                // issue order s = 0, 2, 1, 3: the two epilogue sets (sub-tiles {0, 1} and {2, 3}) take turns,
+                // each with its own accumulator stage, so one set computes while the other one loads
+                const int s = 2 * (pos & 1) + (pos >> 1);
+                const uint32_t st = pos & 1u;
+                // the stage was last filled for this set's previous sub-tile: s - 1 of this tile or s + 1 of
+                // the previous one
+                if ((s & 1) || it > 0) {
+                    mbar_wait(tempty(s ^ 1), (uint32_t)((s & 1) ? it : it - 1) & 1u);
                     tc_fence_after();
                 }
                 const uint32_t d_r = tmem_base + st * kAccCols, d_i = d_r + 2 * kSubR;
@@ -390,7 +394,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
         }
     } else {
         // ===== epilogue warps: lane quarter q = 32 template pairs; set 0 drains sub-tiles 0, 1 and
-        // set 1 sub-tiles 2, 3 of every tile (the accumulator stage of sub-tile s is s & 1)
+        // set 1 sub-tiles 2, 3 of every tile, each set through its own accumulator stage
         const int q = warp & 3, set = warp >> 2;
         const bool active = q < nq;
         const int slot = set * nq + q;                    // staging buffers of the active warps
@@ -416,7 +420,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
 #pragma unroll
             for (int ss = 0; ss < 2; ++ss) {
                 const int s = 2 * set + ss;
-                const uint32_t st = s & 1u;
+                const uint32_t st = (uint32_t)set;
                 mbar_wait(tfull(s), (uint32_t)tile_iter & 1u);
                 if (!active) {
                     __syncwarp();
