@@ -38,11 +38,54 @@ HBM_BYTES_PER_POINT = {"fp32": 4.05, "bf16": 4.02, "bf16_plane16": 2.02, "bf16_t
 # ALU peak: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x 1.965 GHz (B200_PROFILING.md unit counts/clocks)
 N_SM, LANES, SM_MAX_GHZ = 148, 128, 1.965
 ALU_PEAK_TFLOPS = N_SM * LANES * 2 * SM_MAX_GHZ / 1e3
-# dram__bytes_read.sum + dram__bytes_write.sum of one K2 launch from `ncu --set full`
-# (profiles/); None until captured for that (workload, precision).
-NCU_K2_TRAFFIC_BYTES = {("ska", "bf16"): 18.5e6 + 3.381e9,       # profiles/r01c_packed_fp32x2.md
-                        ("ska", "bf16_tc"): 17.4e6 + 3.383e9}   # profiles/r01d_tensor_core_k2.md
 TC_PRECISIONS = ("bf16_tc", "bf16_tc_plane16")
+PROFILES = os.path.join(ROOT, "profiles")
+
+
+def ncu_traffic(workload: str, precision: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE K2 launch, from the committed
+    profiles/*_traffic.json files (written by `bench.py --traffic-from-ncu` out of an `ncu --set full`
+    capture; each names its kernel, command and commit).  The newest matching record wins; None if no
+    capture exists for this (workload, precision)."""
+    best = None
+    try:
+        names = sorted(f for f in os.listdir(PROFILES) if f.endswith("_traffic.json"))
+    except OSError:
+        return None
+    for f in names:
+        try:
+            for rec in json.load(open(os.path.join(PROFILES, f)))["records"]:
+                if rec["workload"] == workload and rec["precision"] == precision:
+                    best = dict(rec, file="profiles/" + f)
+        except Exception:
+            continue
+    return best
+
+
+def write_traffic_json(rep: str, out: str, workload: str, precision: str, command: str):
+    """`ncu -i rep --page raw --csv` -> profiles/<run>_traffic.json (appends one record per launch)."""
+    import csv
+    import subprocess
+    raw = subprocess.run(["ncu", "-i", rep, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
+    rows = list(csv.reader(raw.splitlines()))
+    hdr, units = rows[0], rows[1]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    commit = subprocess.run(["git", "rev-parse", "--short", "HEAD"], capture_output=True, text=True).stdout.strip()
+    recs = []
+    for r in rows[2:]:
+        def val(k):
+            return float(r[hdr.index(k)]) * scale.get(units[hdr.index(k)], 1.0)
+        rd, wr = val("dram__bytes_read.sum"), val("dram__bytes_write.sum")
+        recs.append({"kernel": r[hdr.index("Kernel Name")], "workload": workload, "precision": precision,
+                     "dram_bytes_read": rd, "dram_bytes_write": wr, "traffic": rd + wr,
+                     "duration_us_under_ncu": float(r[hdr.index("gpu__time_duration.sum")]), "command": command,
+                     "commit": commit})
+    doc = {"records": []}
+    if os.path.exists(out):
+        doc = json.load(open(out))
+    doc["records"] += recs
+    json.dump(doc, open(out, "w"), indent=1)
+    print(f"wrote {len(recs)} record(s) to {out}")
 
 
 def measured_peaks():
@@ -69,15 +112,17 @@ def measured_tensor_peak():
 
 def tc_mma_flops(info):
     """Tensor-core flops one K2-TC launch issues (padded operand shapes, K2-TC): per tile of
-    128 bins, per group of gch chunks: ceil((2h+1)/16) K-steps x 2 parts (Re w, Im w) of a
-    128 x (16 gch) x 16 MMA."""
-    npair = (int(info.nz) - 1) // 2
+    128 bins 4 sub-tiles x ceil((2h+1)/16) K-steps x 2 bank images (Re T, Im T) of a 128 x 64 x 16 MMA
+    (M = 128 template-pair lanes, N = 32 bins x {re, im})."""
     kp = (2 * int(info.halfwidth) + 1 + 15) // 16 * 16
-    nch = (npair + 7) // 8
-    ngroups = (nch + 5) // 6
-    gch = (nch + ngroups - 1) // ngroups
     ntiles = int(info.nbins) // 128
-    return ntiles * ngroups * (kp // 16) * 2 * (2 * 128 * 16 * gch * 16)
+    return ntiles * 4 * (kp // 16) * 2 * (2 * 128 * 64 * 16)
+
+
+def workload_string(wl):
+    """The same text in both arms' config.workload (the arms differ in config.precision / impl)."""
+    return (f"{wl.name}: N={wl.n} samples at {wl.tsamp * 1e6:.0f} us, nfft={wl.nfft}, nz={wl.nz} (zmax={wl.zmax:g}, "
+            f"zstep={wl.zstep:g}), seg_len={wl.seg_len}, H={wl.nharm}, {wl.nsigma:g} sigma, r_lo={wl.r_lo}")
 
 
 def workload_for(name: str, inputs):
@@ -217,7 +262,7 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * wl.nz * nb / value, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{wl.name}: N={wl.n}, nfft={wl.nfft}, nz={wl.nz}, seg_len={wl.seg_len}, H={wl.nharm}",
+        "config": {"workload": workload_string(wl), "precision": "f64 (CPU oracle)",
                    "note": "ms_per_step is the oracle's time for a whole trial extrapolated from the sample"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -228,6 +273,167 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------------- CUDA arm
+def time_path(plan, fdas, torch, wl, dev_pool, thr, steps, warmup, energy_seconds, local_rank, barrier):
+    """`steps` DM trials (prepare_spectrum -> convolve_plane -> harmonic_sum_peaks) of one plan on resident
+    series: CUDA events on the launching stream around every call, NVML clocks during the timed region,
+    and a second, seconds-long loop of the same steps for the energy per trial (the NVML counter needs
+    seconds; that loop also shows the sustained step time)."""
+    dev = dev_pool[0].device
+    d_spec, d_plane = plan.alloc_spec(dev), plan.alloc_plane(dev)
+    d_c, d_n = plan.alloc_cands(1 << 16, dev)
+    stream = torch.cuda.current_stream()
+    pool_n = len(dev_pool)
+
+    def step(i, evs=None):
+        x = dev_pool[i % pool_n]
+        if evs is not None:
+            evs[0].record(stream)
+        plan.prepare_spectrum(x, d_spec, stream)
+        if evs is not None:
+            evs[1].record(stream)
+        plan.convolve_plane(d_spec, d_plane, stream)
+        if evs is not None:
+            evs[2].record(stream)
+        plan.harmonic_sum_peaks(d_plane, wl.nharm, thr, wl.r_lo, d_c, d_n, stream)
+        if evs is not None:
+            evs[3].record(stream)
+
+    for i in range(warmup):
+        step(i)
+    torch.cuda.synchronize()
+    n_cands = int(d_n.item())
+    sampler = ClockSampler(local_rank)
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
+    launches0 = plan.launch_count()
+    barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    for i in range(steps):
+        step(i, evs[i])
+    torch.cuda.synchronize()
+    sampler.stop_flag.set()
+    barrier()
+    t_total_ms = evs[0][0].elapsed_time(evs[-1][3])
+    launches = plan.launch_count() - launches0
+    sampler.join(timeout=2.0)
+    res = {
+        "total_ms": t_total_ms, "ms_per_step": t_total_ms / steps, "launches": launches, "candidates_last_step": n_cands,
+        "kernel_ms": {"prepare_spectrum": statistics.mean(e[0].elapsed_time(e[1]) for e in evs),
+                      "convolve_plane": statistics.mean(e[1].elapsed_time(e[2]) for e in evs),
+                      "harmonic_sum_peaks": statistics.mean(e[2].elapsed_time(e[3]) for e in evs)},
+        "clocks": sampler.summary(), "energy": None,
+    }
+    if sampler.ok and energy_seconds > 0:
+        n_e = max(steps, int(energy_seconds * 1e3 / max(res["ms_per_step"], 1e-3)) + 1)
+        es = ClockSampler(local_rank, period=0.05)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        es.start()
+        j0 = es.energy_mj()
+        ev0.record(stream)
+        for i in range(n_e):
+            step(i)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        j1 = es.energy_mj()
+        es.stop_flag.set()
+        es.join(timeout=2.0)
+        sec = ev0.elapsed_time(ev1) * 1e-3
+        if j0 is not None and j1 is not None and j1 > j0:
+            res["energy"] = {"joules_per_step": (j1 - j0) / 1e3 / n_e, "mean_power_w": (j1 - j0) / 1e3 / sec,
+                             "steps": n_e, "seconds": sec, "ms_per_step": 1e3 * sec / n_e,
+                             "source": "NVML total energy counter over a separate, sustained loop of identical steps",
+                             "clocks": es.summary()}
+    res["buffers"] = (d_spec, d_plane)
+    return res
+
+
+def k2_rooflines(info, precision, workload, t_conv_ms):
+    """The convolve kernel of one path against its binding roof and against HBM (north_star's yardstick)."""
+    points = int(info.nz) * int(info.nbins)
+    hbm_peak, peak_kind = measured_peaks()
+    gbs = HBM_BYTES_PER_POINT[precision] * points / (t_conv_ms * 1e-3) / 1e9
+    traffic = ncu_traffic(workload, precision)
+    hbm = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+           "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json)",
+           "bytes_per_point": HBM_BYTES_PER_POINT[precision], "bytes_per_launch": HBM_BYTES_PER_POINT[precision] * points,
+           "frac_of_8TBs_nominal": gbs / 8000.0,
+           "traffic": None if traffic is None else traffic["traffic"],
+           "traffic_source": None if traffic is None else {k: traffic[k] for k in ("file", "kernel", "commit", "command")}}
+    if precision in TC_PRECISIONS:
+        tpeak, tkind = measured_tensor_peak()
+        tflops = tc_mma_flops(info) / (t_conv_ms * 1e-3) / 1e12
+        main = dict(hbm, kernel="K2-TC convolve_tc_kernel",
+                    tensor={"achieved": tflops, "peak": tpeak, "unit": "TFLOP/s", "frac": tflops / tpeak,
+                            "peak_kind": f"{tkind} cuBLAS bf16 burst", "flops_per_launch": tc_mma_flops(info)})
+    else:
+        flops = int(info.nseg) * (int(info.nz) * (FLOP_IFFT + FLOP_MUL + 3 * int(info.valid)) + FLOP_IFFT)
+        tflops = flops / (t_conv_ms * 1e-3) / 1e12
+        main = {"kernel": "K2 convolve_kernel", "bound": "alu", "achieved": tflops, "peak": ALU_PEAK_TFLOPS,
+                "unit": "TFLOP/s", "frac": tflops / ALU_PEAK_TFLOPS,
+                "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz", "flops_per_launch": flops,
+                "traffic": hbm["traffic"], "traffic_source": hbm["traffic_source"]}
+    return main, dict(hbm, kernel=main["kernel"])
+
+
+def survey_block(fdas, torch, inputs, precision, trials_each, pool, thr, local_rank):
+    """configs[4] in small: `trials_each` DM trials of each resolution (64 us: N = 9,375,000; 128 us:
+    N = 4,687,500) through fdas_search_batch from PINNED HOST memory (the H2D copy of every series and the
+    D2H of every candidate list inside the timed region); series cycle a resident host pool."""
+    stream = torch.cuda.current_stream()
+    cap = 1 << 13
+    out = {"api": "fdas_search_batch, pinned host series in, candidates on the host out", "precision": precision,
+           "trials_each": trials_each, "shapes": [],
+           "note": f"the paper's survey is {inputs.SURVEY_TRIALS_FULL} + {inputs.SURVEY_TRIALS_HALF} trials "
+                   f"(PAPER.md:35, BASELINE.json configs[4]); this block runs {trials_each} of each shape, the "
+                   f"{pool} distinct seeded series of each shape cycled (throughput is data-independent apart "
+                   "from candidate counts); `survey_total_s_extrapolated` scales the per-trial times to the full counts"}
+    sampler = ClockSampler(local_rank, period=0.05)
+    plans = []
+    for half in (False, True):
+        wl = inputs.ska(half_res=half)
+        plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, precision)
+        host = []
+        for i in range(pool):
+            ht = torch.empty(wl.n, dtype=torch.float32).pin_memory()
+            ht.numpy()[:] = inputs.series_for(inputs.batched_member(i, half_res=half))
+            host.append(ht)
+        buf = np.empty((trials_each, cap), dtype=fdas.CAND_DTYPE)
+        series = [host[i % pool] for i in range(trials_each)]
+        plan.search_batch(series[:4], wl.nharm, thr, wl.r_lo, capacity=cap, out=buf, stream=stream)   # workspace + warm-up
+        plans.append((wl, plan, series, buf))
+    torch.cuda.synchronize()
+    sampler.start()
+    j0 = sampler.energy_mj() if sampler.ok else None
+    t_all0 = time.perf_counter()
+    for wl, plan, series, buf in plans:
+        t0 = time.perf_counter()
+        counts, _, st = plan.search_batch(series, wl.nharm, thr, wl.r_lo, capacity=cap, out=buf, stream=stream)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        assert st in (fdas.FDAS_OK, fdas.FDAS_EOVERFLOW), st
+        out["shapes"].append({"workload": workload_string(wl), "trials": trials_each, "seconds": dt,
+                              "ms_per_trial": 1e3 * dt / trials_each,
+                              "points_per_s": trials_each * int(plan.info.nz) * int(plan.info.nbins) / dt,
+                              "h2d_bytes_per_trial": int(plan.info.nfft) * 4,
+                              "candidates_per_trial": float(counts.mean())})
+    total = time.perf_counter() - t_all0
+    j1 = sampler.energy_mj() if sampler.ok else None
+    sampler.stop_flag.set()
+    sampler.join(timeout=2.0)
+    out["total_seconds"] = total
+    out["ms_per_trial"] = 1e3 * total / (2 * trials_each)
+    if j0 is not None and j1 is not None and j1 > j0:
+        out["joules_per_trial"] = (j1 - j0) / 1e3 / (2 * trials_each)
+        out["mean_power_w"] = (j1 - j0) / 1e3 / total
+    out["survey_total_s_extrapolated"] = (inputs.SURVEY_TRIALS_FULL * out["shapes"][0]["ms_per_trial"]
+                                          + inputs.SURVEY_TRIALS_HALF * out["shapes"][1]["ms_per_trial"]) * 1e-3
+    out["clocks"] = sampler.summary()
+    for _, plan, _, _ in plans:
+        plan.close()
+    return out
+
+
 def run_cuda(args):
     import torch
     from paper_2211_13517_b200 import dist as fd, fdas, inputs
@@ -251,80 +457,17 @@ def run_cuda(args):
         host_pool.append(ht)
     dev_pool = [h.to(dev, non_blocking=False) for h in host_pool]
     pool_bytes = pool_n * wl.n * 4
-
-    d_spec, d_plane = plan.alloc_spec(dev), plan.alloc_plane(dev)
     cap = 1 << 16
-    d_c, d_n = plan.alloc_cands(cap, dev)
     thr = fdas.thresholds_from_sigma(wl.nharm, wl.nsigma)
     stream = torch.cuda.current_stream()
 
-    def step(i, evs=None):
-        x = dev_pool[i % pool_n]
-        if evs is not None:
-            evs[0].record(stream)
-        plan.prepare_spectrum(x, d_spec, stream)
-        if evs is not None:
-            evs[1].record(stream)
-        plan.convolve_plane(d_spec, d_plane, stream)
-        if evs is not None:
-            evs[2].record(stream)
-        plan.harmonic_sum_peaks(d_plane, wl.nharm, thr, wl.r_lo, d_c, d_n, stream)
-        if evs is not None:
-            evs[3].record(stream)
-
-    for i in range(args.warmup):
-        step(i)
-    torch.cuda.synchronize()
-    n_cands = int(d_n.item())
-
-    sampler = ClockSampler(ctx.local_rank)
-    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
-    launches0 = plan.launch_count()
-    fd.barrier(ctx)
-    torch.cuda.synchronize()
-    sampler.start()
-    e0 = sampler.energy_mj() if sampler.ok else None
-    for i in range(args.steps):
-        step(i, evs[i])
-    torch.cuda.synchronize()
-    e1 = sampler.energy_mj() if sampler.ok else None
-    sampler.stop_flag.set()
-    fd.barrier(ctx)
-    t_total_ms = evs[0][0].elapsed_time(evs[-1][3])
-    launches = plan.launch_count() - launches0
-    sampler.join(timeout=2.0)
-    e_short = (e0, e1)
-    # energy per DM trial (PAPER.md:39-43 reports energy): the NVML counter needs seconds, not
-    # milliseconds -- a separate loop of the same steps, >= args.energy_seconds long, not part of `value`
-    energy = None
-    if sampler.ok and args.energy_seconds > 0:
-        n_e = max(args.steps, int(args.energy_seconds * 1e3 / max(t_total_ms / args.steps, 1e-3)) + 1)
-        es = ClockSampler(ctx.local_rank, period=0.05)
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        es.start()
-        j0 = es.energy_mj()
-        ev0.record(stream)
-        for i in range(n_e):
-            step(i)
-        ev1.record(stream)
-        torch.cuda.synchronize()
-        j1 = es.energy_mj()
-        es.stop_flag.set()
-        es.join(timeout=2.0)
-        sec = ev0.elapsed_time(ev1) * 1e-3
-        if j0 is not None and j1 is not None and j1 > j0:
-            energy = {"joules_per_step": (j1 - j0) / 1e3 / n_e, "mean_power_w": (j1 - j0) / 1e3 / sec,
-                      "steps": n_e, "seconds": sec, "ms_per_step": 1e3 * sec / n_e,
-                      "source": "NVML total energy counter over a separate loop of identical steps",
-                      "clocks": es.summary()}
-    t_prep = statistics.mean(e[0].elapsed_time(e[1]) for e in evs)
-    t_conv = statistics.mean(e[1].elapsed_time(e[2]) for e in evs)
-    t_harm = statistics.mean(e[2].elapsed_time(e[3]) for e in evs)
-
-    t_max_ms = fd.max_over_ranks(ctx, t_total_ms)
+    m = time_path(plan, fdas, torch, wl, dev_pool, thr, args.steps, args.warmup, args.energy_seconds,
+                  ctx.local_rank, lambda: fd.barrier(ctx))
+    d_spec, d_plane = m.pop("buffers")
+    t_max_ms = fd.max_over_ranks(ctx, m["total_ms"])
     total_points = fd.sum_over_ranks(ctx, float(points * args.steps))
     value = total_points / (t_max_ms * 1e-3)
+    launches_total = int(fd.sum_over_ranks(ctx, int(m["launches"])))
 
     # ---- end to end through the public API: pinned host series in, candidates on the host out, every
     # step.  fdas_search_batch is the call a user with many DM trials makes (the H2D copy of trial t+1
@@ -334,15 +477,14 @@ def run_cuda(args):
     out = np.empty(cap, dtype=fdas.CAND_DTYPE)
     thr_c = thr.ctypes.data_as(C.POINTER(C.c_float))
     sp = int(stream.cuda_stream)
-    cnt = 0
     for i in range(min(3, args.warmup)):
         plan.search_host_raw(host_pool[i % pool_n].data_ptr(), wl.nharm, thr_c, wl.r_lo, out.ctypes.data, cap, sp)
     fd.barrier(ctx)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     for i in range(e2e_steps):
-        st, cnt = plan.search_host_raw(host_pool[i % pool_n].data_ptr(), wl.nharm, thr_c, wl.r_lo,
-                                       out.ctypes.data, cap, sp)
+        st, _cnt = plan.search_host_raw(host_pool[i % pool_n].data_ptr(), wl.nharm, thr_c, wl.r_lo,
+                                        out.ctypes.data, cap, sp)
         assert st in (fdas.FDAS_OK, fdas.FDAS_EOVERFLOW), st
     torch.cuda.synchronize()
     t_sync = fd.max_over_ranks(ctx, time.perf_counter() - t0)
@@ -360,62 +502,43 @@ def run_cuda(args):
     t_e2e = fd.max_over_ranks(ctx, time.perf_counter() - t0)
     e2e_value = fd.sum_over_ranks(ctx, float(points * e2e_steps)) / t_e2e
     d2h = int(np.minimum(counts, bcap).sum()) * 16 + 8 * e2e_steps
+    del d_spec, d_plane
+    plan.close()
+    torch.cuda.empty_cache()
 
-    # ---- beside the tensor-core K2: north_star's literal FFT kernel on the same spectrum, K2 alone
+    is_tc = precision in TC_PRECISIONS
+    roofline, roofline_hbm = k2_rooflines(info, precision, args.workload, m["kernel_ms"]["convolve_plane"])
+
+    # ---- beside the tensor-core path: north_star's literal kernel (overlap-save FFT, bf16 storage, fp32
+    # arithmetic, no tensor cores) as a FULL record in the same run: step, kernel split, energy, rooflines
     fft_path = None
-    if precision in TC_PRECISIONS and not args.no_fft_path:
+    if is_tc and not args.no_fft_path and ctx.world == 1:
         fprec = "bf16_plane16" if precision.endswith("plane16") else "bf16"
         plan_f = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, fprec)
-        for _ in range(3):
-            plan_f.convolve_plane(d_spec, d_plane, stream)
-        ev_a, ev_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        nrep = 10
-        ev_a.record(stream)
-        for _ in range(nrep):
-            plan_f.convolve_plane(d_spec, d_plane, stream)
-        ev_b.record(stream)
-        torch.cuda.synchronize()
-        t_f = ev_a.elapsed_time(ev_b) / nrep
-        fi = plan_f.info
-        f_flops = int(fi.nseg) * (int(fi.nz) * (FLOP_IFFT + FLOP_MUL + 3 * int(fi.valid)) + FLOP_IFFT)
-        fft_path = {"precision": fprec, "kernel": "K2 convolve_kernel (overlap-save FFT, fp32 arithmetic, no tensor cores)",
-                    "convolve_plane_ms": t_f, "alu_frac": f_flops / (t_f * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
-                    "hbm_frac": HBM_BYTES_PER_POINT[fprec] * points / (t_f * 1e-3) / 1e9 / measured_peaks()[0],
-                    "launches": nrep}
+        mf = time_path(plan_f, fdas, torch, wl, dev_pool, thr, args.steps, args.warmup, args.energy_seconds,
+                       ctx.local_rank, lambda: None)
+        mf.pop("buffers")
+        rf, rf_hbm = k2_rooflines(plan_f.info, fprec, args.workload, mf["kernel_ms"]["convolve_plane"])
+        fft_path = {"precision": fprec,
+                    "kernel": "K2 convolve_kernel (overlap-save FFT, bf16 storage, fp32 arithmetic, no tensor cores): "
+                              "north_star's literal convolve+power kernel",
+                    "value": points * args.steps / (mf["total_ms"] * 1e-3), "unit": UNIT,
+                    "ms_per_step": mf["ms_per_step"], "kernel_ms": mf["kernel_ms"], "energy": mf["energy"],
+                    "gpu_launches": int(mf["launches"]), "candidates_last_step": mf["candidates_last_step"],
+                    "roofline": rf, "roofline_hbm": rf_hbm, "clocks": mf["clocks"],
+                    "ncu_counters": "profiles/r01c_packed_fp32x2.md (FMA pipe 64.5 %, LSU data pipe 75 %, issue 74 %)"}
         plan_f.close()
-        plan.convolve_plane(d_spec, d_plane, stream)      # leave the plane as the timed path wrote it
-        torch.cuda.synchronize()
+        torch.cuda.empty_cache()
 
-    hbm_peak, peak_kind = measured_peaks()
-    seg_flops = FLOP_IFFT + FLOP_MUL + 3 * int(info.valid)
-    k2_flops = int(info.nseg) * (int(info.nz) * seg_flops + FLOP_IFFT)
-    k2_tflops = k2_flops / (t_conv * 1e-3) / 1e12
-    k2_gbs = HBM_BYTES_PER_POINT[precision] * points / (t_conv * 1e-3) / 1e9
+    survey = None
+    if args.survey_trials > 0 and args.workload == "ska" and ctx.world == 1:
+        del dev_pool
+        torch.cuda.empty_cache()
+        survey = survey_block(fdas, torch, inputs, precision, args.survey_trials, min(4, args.pool), thr, ctx.local_rank)
+
     plane_bytes = points * int(info.plane_elem_bytes)
-    k3_gbs = int(info.nz) * (int(info.nbins) // 8) * 2 / (t_harm * 1e-3) / 1e9
-    is_tc = precision in TC_PRECISIONS
-    k2_name = "K2-TC convolve_tc_kernel" if is_tc else "K2 convolve_kernel"
-    if is_tc:
-        # dense contraction on the tensor cores: the plane write is the binding roof (K2-TC)
-        tpeak, tkind = measured_tensor_peak()
-        tflops = tc_mma_flops(info) / (t_conv * 1e-3) / 1e12
-        roofline = {
-            "kernel": k2_name, "bound": "hbm", "achieved": k2_gbs, "peak": hbm_peak, "unit": "GB/s",
-            "frac": k2_gbs / hbm_peak, "traffic": NCU_K2_TRAFFIC_BYTES.get((args.workload, precision)),
-            "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json)",
-            "bytes_per_launch": HBM_BYTES_PER_POINT[precision] * points,
-            "tensor": {"achieved": tflops, "peak": tpeak, "unit": "TFLOP/s", "frac": tflops / tpeak,
-                       "peak_kind": f"{tkind} cuBLAS bf16 burst", "flops_per_launch": tc_mma_flops(info)},
-        }
-    else:
-        roofline = {
-            "kernel": k2_name, "bound": "alu", "achieved": k2_tflops, "peak": ALU_PEAK_TFLOPS,
-            "unit": "TFLOP/s", "frac": k2_tflops / ALU_PEAK_TFLOPS,
-            "traffic": NCU_K2_TRAFFIC_BYTES.get((args.workload, precision)),
-            "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz",
-            "flops_per_launch": k2_flops,
-        }
-
+    k3_gbs = int(info.nz) * (int(info.nbins) // 8) * 2 / (m["kernel_ms"]["harmonic_sum_peaks"] * 1e-3) / 1e9
+    hbm_peak, peak_kind = measured_peaks()
     arith = "bf16 operands, fp32 accumulation on the tensor cores" if is_tc else "fp32 arithmetic"
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ctx.world, "steps": args.steps,
@@ -423,45 +546,41 @@ def run_cuda(args):
         "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16 x bf16 -> f32 (tensor cores)" if is_tc else "f32", "data": "synthetic",
         "config": {
-            "workload": f"{wl.name}: N={wl.n} samples at {wl.tsamp * 1e6:.0f} us, nfft={info.nfft}, nz={info.nz} "
-                        f"(zmax={wl.zmax:g}), seg_len={info.seg_len}, h={info.halfwidth}, S={info.nseg}, H={wl.nharm}, "
-                        f"{wl.nsigma:g} sigma, storage={precision} ({arith})",
-            "precision": precision, "plane_points_per_step": points,
+            "workload": workload_string(wl),
+            "precision": f"{precision} ({arith})", "plane_points_per_step": points,
+            "geometry": f"h={info.halfwidth}, V={info.valid}, S={info.nseg}, Nb={info.nbins}",
             "parallelism": f"dm-trial replicas x{ctx.world} (no data-path collective)",
             "l2": f"plane of {plane_bytes / 1e9:.2f} GB per step exceeds the 126 MB L2; input pool of "
                   f"{pool_n} series ({pool_bytes / 1e6:.0f} MB) cycled",
-            "timed": "cuFFT R2C + K1a/K1b whitening + K2 convolve + K3 harmonic sum per step; CUDA events on the launching stream",
+            "timed": "cuFFT R2C + K1a/K1b whitening + K2 convolve + K3 harmonic sum per step; CUDA events on the "
+                     f"launching stream over {args.steps} steps; the `energy` loop ({args.energy_seconds:g} s of the "
+                     "same steps) is the sustained figure",
         },
-        "kernel_ms": {"prepare_spectrum": t_prep, "convolve_plane": t_conv, "harmonic_sum_peaks": t_harm},
-        "candidates_last_step": n_cands,
-        "gpu_launches": int(fd.sum_over_ranks(ctx, int(launches))),
+        "kernel_ms": m["kernel_ms"],
+        "candidates_last_step": m["candidates_last_step"],
+        "gpu_launches": launches_total,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(info.nfft) * 4,
                 "d2h_bytes_per_step": d2h // e2e_steps, "steps": e2e_steps,
                 "api": "fdas_search_batch (pinned host series -> candidates on host, copies pipelined with "
                        "compute), wall clock",
                 "one_trial_per_call": {"value": e2e_sync_value, "api": "fdas_search_host, synchronous"}},
         "roofline": roofline,
-        "roofline_hbm": {
-            "kernel": k2_name, "bound": "hbm", "achieved": k2_gbs, "peak": hbm_peak, "unit": "GB/s",
-            "frac": k2_gbs / hbm_peak, "peak_kind": f"{peak_kind} copy bandwidth",
-            "bytes_per_point": HBM_BYTES_PER_POINT[precision], "frac_of_8TBs_nominal": k2_gbs / 8000.0,
-        },
+        "roofline_hbm": roofline_hbm,
         "roofline_k3": {
-            "kernel": "K3 prefilter_kernel + exact_kernel + flag_kernel", "bound": "hbm", "achieved": k3_gbs,
+            "kernel": "K3 prefilter kernels + exact_kernel + flag_kernel", "bound": "hbm", "achieved": k3_gbs,
             "peak": hbm_peak, "unit": "GB/s", "frac": k3_gbs / hbm_peak,
             "note": "algorithmic bytes = one read of the bf16 block-max side plane (nz x Nb/8) that the "
                     "branch-and-bound prefilter scans; K3 is bound by its own select arithmetic, not by DRAM "
-                    "(profiles/r01c: ALU pipe 45 %, 0.22 GB read per launch)",
+                    "(profiles/r01e: issue 59 %, 0.18 GB read per launch)",
         },
-        "clocks": sampler.summary(),
+        "clocks": m["clocks"],
     }
     if fft_path is not None:
         line["fft_path"] = fft_path
-    if energy is not None:
-        line["energy"] = energy
-    elif e_short[0] is not None and e_short[1] is not None and e_short[1] > e_short[0]:
-        line["energy"] = {"joules_per_step": (e_short[1] - e_short[0]) / 1e3 / args.steps,
-                          "source": "NVML total energy counter over the timed region (short: coarse)"}
+    if m["energy"] is not None:
+        line["energy"] = m["energy"]
+    if survey is not None:
+        line["survey"] = survey
     if ctx.rank == 0 and ctx.world == 1 and not args.no_cpu_baseline:
         v, cores, desc, _ = oracle_sample(host_pool[0].numpy(), wl, args.cpu_budget)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
@@ -633,10 +752,26 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=20)
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle plane work")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-fft-path", action="store_true", help="skip the side measurement of the FFT K2")
+    ap.add_argument("--no-fft-path", action="store_true", help="skip the full record of the FFT K2 path")
+    ap.add_argument("--survey-trials", type=int, default=768,
+                    help="ska workload, 1 GPU: DM trials of EACH resolution in the `survey` block (0 = off)")
+    ap.add_argument("--traffic-from-ncu", default=None, metavar="REP",
+                    help="write the DRAM traffic of the launches in an ncu report to --traffic-out and exit")
+    ap.add_argument("--traffic-out", default=os.path.join(PROFILES, "r02_traffic.json"))
+    ap.add_argument("--traffic-command", default="", help="the command the ncu report was captured with")
     args = ap.parse_args()
+    if args.traffic_from_ncu:
+        write_traffic_json(args.traffic_from_ncu, args.traffic_out, args.workload, args.precision, args.traffic_command)
+        return 0
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
+    if args.impl == "cuda" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # launched plainly with --gpus N: start the N ranks ourselves, one per GPU (DM-trial replicas)
+        import subprocess
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(29500 + os.getpid() % 2000),
+               os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd, env=dict(os.environ, NCCL_DEBUG=os.environ.get("NCCL_DEBUG", "INFO")))
     if args.impl == "reference":
         if args.workload in ("batched", "survey"):
             args.workload = "ska"      # the oracle's per-trial rate is the same for every member
