@@ -78,7 +78,9 @@ def write_traffic_json(rep: str, out: str, workload: str, precision: str, comman
         rd, wr = val("dram__bytes_read.sum"), val("dram__bytes_write.sum")
         recs.append({"kernel": r[hdr.index("Kernel Name")], "workload": workload, "precision": precision,
                      "dram_bytes_read": rd, "dram_bytes_write": wr, "traffic": rd + wr,
-                     "duration_us_under_ncu": float(r[hdr.index("gpu__time_duration.sum")]), "command": command,
+                     "duration_us_under_ncu": float(r[hdr.index("gpu__time_duration.sum")]) *
+                     {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}[units[hdr.index("gpu__time_duration.sum")]],
+                     "command": command,
                      "commit": commit})
     doc = {"records": []}
     if os.path.exists(out):

@@ -18,6 +18,8 @@
  *   O5 orc_harmonic_sums_at / O6 orc_candidates  north_star "harmonic summing and thresholding"
  *                                                 (A12,A13,A14)                  pinned: P9,P10
  *   orc_thresholds       north_star "threshold 6 sigma" (A13)                    pinned: P10
+ *   O5n orc_harmonic_sums_nbr_at / orc_candidates_nbr  harmonic sums that do not lose power when the
+ *                        fundamental lies between two bins (reading A24)  pinned: P13
  * No function here is "parity unpinned"; the pins live in tests/test_oracle_pins.py.
  *
  * Complex arrays are interleaved (re, im) doubles.  OpenMP is used only to spread independent
@@ -411,6 +413,77 @@ int orc_harmonic_sums_sampled(const double* w_, int64_t nb, const double* bank_,
         hmax[i] = hm;
     }
     return 0;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O5n -- neighbour-maximised harmonic sums (reading A24; serves PAPER.md:9
+ * "sacrificing less than 3 % in numerical sensitivity").  A signal whose fundamental lies at
+ * r_c = r + delta, |delta| <= 1/2, has its k-th harmonic at k r_c = k r + k delta, up to k/2 bins from
+ * k r, so harmonic k is taken where it is largest within that reach:
+ *   S'_h(r,j) = sum_{k=1..h} max_{|d| <= floor(k/2), 0 <= k r + d <= nb-1} P[row_k(j)][k r + d]
+ * defined exactly when S_h is (h r <= nb-1 and |h z_j| <= zmax).  S'_1 = S_1; S'_h >= S_h.
+ * ------------------------------------------------------------------------------------------- */
+int orc_harmonic_sums_nbr_at(const double* P, int64_t nb, int nz, int H, int64_t r, int j, double* S) {
+    double acc = 0.0;
+    int hmax = 0;
+    for (int k = 1; k <= H; ++k) {
+        int row;
+        if ((int64_t)k * r > nb - 1) break;
+        if (!harmonic_row(j, k, nz, &row)) break;
+        double best = -1.0;
+        for (int64_t d = -(k / 2); d <= k / 2; ++d) {
+            int64_t c = (int64_t)k * r + d;
+            if (c < 0 || c > nb - 1) continue;
+            double v = P[(size_t)row * (size_t)nb + (size_t)c];
+            if (v > best) best = v;
+        }
+        acc += best;
+        S[k - 1] = acc;
+        hmax = k;
+    }
+    return hmax;
+}
+
+static int sum_defined_nbr(const double* P, int64_t nb, int nz, int64_t r_lo, int64_t r, int j, int h,
+                           double* val) {
+    if (j < 0 || j >= nz || r < r_lo || r >= nb) return 0;
+    double S[64];
+    int hmax = orc_harmonic_sums_nbr_at(P, nb, nz, h, r, j, S);
+    if (hmax < h) return 0;
+    *val = S[h - 1];
+    return 1;
+}
+
+/* Candidates of the neighbour-maximised sums: the rule of orc_candidates (O6) applied to S'. */
+int64_t orc_candidates_nbr(const double* P, int64_t nb, int nz, int H, const double* thr, int64_t r_lo,
+                           int64_t* c_r, int32_t* c_j, int32_t* c_h, double* c_pow, int32_t* c_flag,
+                           int64_t capacity) {
+    int64_t count = 0;
+    if (H < 1 || H > 64) return -1;
+    for (int j = 0; j < nz; ++j) {
+        for (int64_t r = r_lo; r < nb; ++r) {
+            double S[64];
+            int hmax = orc_harmonic_sums_nbr_at(P, nb, nz, H, r, j, S);
+            for (int h = 1; h <= hmax; ++h) {
+                if (!(S[h - 1] > thr[h - 1])) continue;
+                int flag = 1;
+                for (int dj = -1; dj <= 1 && flag; ++dj)
+                    for (int dr = -1; dr <= 1 && flag; ++dr) {
+                        if (dj == 0 && dr == 0) continue;
+                        double nv;
+                        if (!sum_defined_nbr(P, nb, nz, r_lo, r + dr, j + dj, h, &nv)) continue;
+                        int precedes = (dj < 0) || (dj == 0 && dr < 0);
+                        if (precedes ? !(S[h - 1] > nv) : !(S[h - 1] >= nv)) flag = 0;
+                    }
+                if (count < capacity) {
+                    c_r[count] = r; c_j[count] = j; c_h[count] = h;
+                    c_pow[count] = S[h - 1]; c_flag[count] = flag;
+                }
+                ++count;
+            }
+        }
+    }
+    return count;
 }
 
 static int sum_defined(const double* P, int64_t nb, int nz, int64_t r_lo, int64_t r, int j, int h,

@@ -61,6 +61,10 @@ def lib():
         L.orc_candidates.argtypes = [_d, C.c_int64, C.c_int, C.c_int, _d, C.c_int64,
                                      _i64, _i32, _i32, _d, _i32, C.c_int64]
         L.orc_candidates.restype = C.c_int64
+        L.orc_harmonic_sums_nbr_at.argtypes = [_d, C.c_int64, C.c_int, C.c_int, C.c_int64, C.c_int, _d]
+        L.orc_candidates_nbr.argtypes = [_d, C.c_int64, C.c_int, C.c_int, _d, C.c_int64,
+                                         _i64, _i32, _i32, _d, _i32, C.c_int64]
+        L.orc_candidates_nbr.restype = C.c_int64
         L.orc_thresholds.argtypes = [C.c_int, C.c_double, _d]
         _lib = L
     return _lib
@@ -186,6 +190,15 @@ def harmonic_sums_at(P, H, r, j):
     return S[:hmax]
 
 
+def harmonic_sums_nbr_at(P, H, r, j):
+    """Neighbour-maximised sums S'_1..S'_hmax at (r, j) (reading A24)."""
+    P = np.ascontiguousarray(P, dtype=np.float64)
+    nz, nb = P.shape
+    S = np.zeros(H)
+    hmax = lib().orc_harmonic_sums_nbr_at(_p(P, _d), nb, nz, H, int(r), int(j), _p(S, _d))
+    return S[:hmax]
+
+
 def harmonic_sums_sampled(w, bank, H, rr, jj):
     """S (npts x H, NaN where undefined) and hmax (npts) at sampled fundamentals, from w directly."""
     w, wv = _c128(w)
@@ -224,7 +237,9 @@ class Candidates:
                 for r, j, h, p, f in zip(self.r, self.j, self.h, self.power, self.flag)}
 
 
-def candidates(P, H, thr, r_lo, capacity=1 << 20):
+def candidates(P, H, thr, r_lo, capacity=1 << 20, nbr=False):
+    """Thresholded (r, j, h) triples of the plain sums (O6) or, nbr=True, of the neighbour-maximised
+    sums (O5n)."""
     P = np.ascontiguousarray(P, dtype=np.float64)
     nz, nb = P.shape
     thr = np.ascontiguousarray(thr, dtype=np.float64)
@@ -233,8 +248,9 @@ def candidates(P, H, thr, r_lo, capacity=1 << 20):
     c_h = np.empty(capacity, dtype=np.int32)
     c_p = np.empty(capacity, dtype=np.float64)
     c_f = np.empty(capacity, dtype=np.int32)
-    n = int(lib().orc_candidates(_p(P, _d), nb, nz, H, _p(thr, _d), int(r_lo), _p(c_r, _i64),
-                                 _p(c_j, _i32), _p(c_h, _i32), _p(c_p, _d), _p(c_f, _i32), capacity))
+    fn = lib().orc_candidates_nbr if nbr else lib().orc_candidates
+    n = int(fn(_p(P, _d), nb, nz, H, _p(thr, _d), int(r_lo), _p(c_r, _i64),
+               _p(c_j, _i32), _p(c_h, _i32), _p(c_p, _d), _p(c_f, _i32), capacity))
     m = min(n, capacity)
     return Candidates(c_r[:m].copy(), c_j[:m].copy(), c_h[:m].copy(), c_p[:m].copy(),
                       c_f[:m].copy(), n)

@@ -406,3 +406,78 @@ def test_p9_sampled_harmonic_sums_equal_the_full_plane_route(oracle):
         assert hmax[i] == len(ref)
         assert np.allclose(S[i, :hmax[i]], ref, rtol=1e-13)
         assert np.all(np.isnan(S[i, hmax[i]:]))
+
+
+# ----------------------------------------------------------------------------------------- P13
+def test_p13_neighbour_maximised_sums_on_hand_made_planes(oracle):
+    """O5n (reading A24): harmonic k is taken at its largest value within floor(k/2) bins of k r.
+    Pinned by closed forms on constructed planes: a constant plane, the first sum, monotonicity,
+    the harmonics of a fundamental at r0 + 0.37 (all recovered, the plain sum loses 7 of 8), the exact
+    reach of the window and its clipping at the ends of the plane."""
+    nz, nb, H = 33, 4000, 8
+    mid = 16
+    # constant plane: S'_h = h, defined exactly where S_h is
+    P = np.ones((nz, nb))
+    for r, j in ((5, 16), (37, 18), (499, 0), (3999, 16), (2000, 16)):
+        S, Sn = oracle.harmonic_sums_at(P, H, r, j), oracle.harmonic_sums_nbr_at(P, H, r, j)
+        assert len(S) == len(Sn) and np.allclose(Sn, np.arange(1, len(Sn) + 1))
+    # S'_1 = S_1 and S'_h >= S_h on a random plane
+    rng = np.random.default_rng(131)
+    P = rng.exponential(1.0, size=(nz, nb))
+    for r, j in ((7, 16), (123, 14), (400, 17), (1999, 16), (64, 20)):
+        S, Sn = oracle.harmonic_sums_at(P, H, r, j), oracle.harmonic_sums_nbr_at(P, H, r, j)
+        assert len(S) == len(Sn) and Sn[0] == S[0] and np.all(Sn >= S - 1e-15)
+        assert np.all(np.diff(Sn) <= P.max() + 1e-12) and np.all(np.diff(Sn) > 0)
+    # a pulsar whose fundamental sits at r_c = r0 + 0.37 (z = 2): harmonic k peaks at round(k r_c)
+    r0, z, A = 300, 2, 10.0
+    P = np.zeros((nz, nb))
+    shifts = [int(np.floor(0.37 * k + 0.5)) for k in range(1, H + 1)]         # 0 1 1 1 2 2 3 3
+    assert shifts == [0, 1, 1, 1, 2, 2, 3, 3] and all(s <= (k + 1) // 2 for k, s in enumerate(shifts))
+    for k, s in zip(range(1, H + 1), shifts):
+        P[mid + k * z, k * r0 + s] = A
+    assert np.allclose(oracle.harmonic_sums_nbr_at(P, H, r0, mid + z), A * np.arange(1, H + 1))
+    assert np.allclose(oracle.harmonic_sums_at(P, H, r0, mid + z), A)          # only k = 1 lies on k r0
+    # the reach is exactly floor(k/2): a spike one bin further is not picked up
+    for k in (2, 3, 4, 7, 8):
+        w = k // 2
+        for d, seen in ((w, True), (-w, True), (w + 1, False), (-w - 1, False)):
+            P = np.zeros((nz, nb))
+            P[mid, k * 100 + d] = 3.0
+            Sn = oracle.harmonic_sums_nbr_at(P, H, 100, mid)
+            assert (Sn[k - 1] == 3.0) == seen and (k == 1 or Sn[k - 2] == 0.0)
+    # clipping: the window of the last defined harmonic stops at bin nb - 1, that of r = 0 at bin 0
+    P = np.zeros((nz, nb))
+    P[mid, nb - 1] = 2.0
+    Sn = oracle.harmonic_sums_nbr_at(P, H, (nb - 1) // 4, mid)       # 4 r = 3996: window 3994..3998 -> no
+    assert len(Sn) == 4 and Sn[3] == 0.0
+    Sn = oracle.harmonic_sums_nbr_at(P, H, 1333, mid)                # 3 r = 3999 = nb - 1, window 3998..3999
+    assert len(Sn) == 3 and Sn[2] == 2.0
+    P = np.zeros((nz, nb)); P[mid, 0] = 4.0; P[mid, 1] = 1.0
+    assert np.allclose(oracle.harmonic_sums_nbr_at(P, 4, 0, mid), [4, 8, 12, 16])   # every window contains bin 0
+
+
+def test_p13_neighbour_maximised_candidates(oracle):
+    """orc_candidates_nbr = the O6 rule on S': the triples of a constructed plane, the count of defined
+    triples under a negative threshold (identical to the plain sums'), powers and the tie rule."""
+    nz, nb, H, r_lo = 33, 600, 16, 5
+    mid = 16
+    P = np.ones((nz, nb))
+    c = oracle.candidates(P, H, -np.ones(H), r_lo, nbr=True)
+    expect = sum(((nb - 1) // h - r_lo + 1) * (2 * (16 // h) + 1) for h in range(1, H + 1))
+    assert c.count == expect == oracle.candidates(P, H, -np.ones(H), r_lo).count
+    # one off-bin second harmonic: (r0, z = 3) fundamental 5.0 at r0, second harmonic 5.0 at 2 r0 + 1
+    P = np.zeros((nz, nb))
+    r0 = 100
+    P[mid + 3, r0] = 5.0
+    P[mid + 6, 2 * r0 + 1] = 5.0
+    plain = oracle.candidates(P, 2, np.array([4.0, 9.0]), r_lo).as_dict()
+    nbr = oracle.candidates(P, 2, np.array([4.0, 9.0]), r_lo, nbr=True).as_dict()
+    assert (r0, mid + 3, 2) not in plain and nbr[(r0, mid + 3, 2)][0] == 10.0
+    # the spike at 2 r0 + 1 is also the k = 2 neighbour of fundamentals r0 + 1 (2 r0 + 2 - 1): S'_2 = 5 < 9
+    assert (r0 + 1, mid + 3, 2) not in nbr
+    assert set(k for k in nbr if k[2] == 1) == set(k for k in plain if k[2] == 1)    # h = 1 is unchanged
+    assert nbr[(r0, mid + 3, 2)][1] == 1                                            # isolated: local maximum
+    # tie rule on S': two equal neighbouring fundamentals, the first in (j, r) order keeps the flag
+    P = np.zeros((nz, nb)); P[mid, 50] = 3.0; P[mid, 51] = 3.0
+    d = oracle.candidates(P, 1, np.array([1.0]), 1, nbr=True).as_dict()
+    assert d[(50, mid, 1)][1] == 1 and d[(51, mid, 1)][1] == 0
