@@ -346,8 +346,37 @@ def time_path(plan, fdas, torch, wl, dev_pool, thr, steps, warmup, energy_second
                              "steps": n_e, "seconds": sec, "ms_per_step": 1e3 * sec / n_e,
                              "source": "NVML total energy counter over a separate, sustained loop of identical steps",
                              "clocks": es.summary()}
+    # both harmonic-sum modes on the plane of the last step: K3 alone, 10 launches each
+    modes = {}
+    for mode in ("plain", "neighbour_max"):
+        plan.set_harmonic_mode(mode)
+        t = thr if mode == "plain" else nbr_thresholds(thr)
+        for _ in range(2):
+            plan.harmonic_sum_peaks(d_plane, wl.nharm, t, wl.r_lo, d_c, d_n, stream)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(10):
+            plan.harmonic_sum_peaks(d_plane, wl.nharm, t, wl.r_lo, d_c, d_n, stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        modes[mode] = {"harmonic_sum_peaks_ms": a.elapsed_time(b) / 10, "candidates": int(d_n.item())}
+    plan.set_harmonic_mode("plain")
+    modes["note"] = ("neighbour_max: S'_h = sum_k max_{|d| <= k/2} P[k z][k r + d] (DESIGN.md reading A24), thresholds "
+                     "= the plain ones raised by the growth of the noise mean")
+    res["harmonic_modes"] = modes
     res["buffers"] = (d_spec, d_plane)
     return res
+
+
+def nbr_thresholds(thr):
+    """Thresholds for the neighbour-maximised sums in this benchmark: T_h + sum_{k<=h} (H_m - 1), m = 2 (k/2) + 1,
+    H_m = mean of the maximum of m unit exponentials (the caller's choice; the library takes any)."""
+    out, shift = [], 0.0
+    for k, t in enumerate(thr, start=1):
+        m = 2 * (k // 2) + 1
+        shift += sum(1.0 / i for i in range(1, m + 1)) - 1.0
+        out.append(t + shift)
+    return np.array(out, dtype=np.float32)
 
 
 def k2_rooflines(info, precision, workload, t_conv_ms):
@@ -559,6 +588,7 @@ def run_cuda(args):
                      "same steps) is the sustained figure",
         },
         "kernel_ms": m["kernel_ms"],
+        "harmonic_modes": m["harmonic_modes"],
         "candidates_last_step": m["candidates_last_step"],
         "gpu_launches": launches_total,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(info.nfft) * 4,

@@ -146,6 +146,21 @@ int fdas_harmonic_sum_peaks(fdas_plan_t plan, const void* d_plane, int H, const 
                             int64_t r_lo, fdas_cand_t* d_cands, int64_t capacity,
                             unsigned long long* d_count, void* cuda_stream);
 
+/*
+ * fdas_plan_set_harmonic_mode -- which harmonic sum fdas_harmonic_sum_peaks (and the search calls)
+ * evaluate from now on (reading A24; serves PAPER.md:9 "less than 3 % in
+ * numerical sensitivity"):
+ *   FDAS_HSUM_PLAIN          S_h(r,j)  = sum_{k<=h} P[row(k z_j)][k r]                       (default)
+ *   FDAS_HSUM_NEIGHBOUR_MAX  S'_h(r,j) = sum_{k<=h} max_{|d| <= floor(k/2)} P[row(k z_j)][k r + d]
+ * (bins clipped to [0, Nb); defined where S_h is).  A fundamental at r + delta, |delta| <= 1/2, has
+ * harmonic k at k r + k delta: the plain sum misses it as soon as |k delta| > 1/2, the second form does
+ * not.  S'_1 = S_1 and S'_h >= S_h, so thresholds for a given false-alarm rate are higher for S'; they
+ * are the caller's.  The first switch to FDAS_HSUM_NEIGHBOUR_MAX allocates a second side plane
+ * (nz x nbins/8 x 2 bytes).  FDAS_EARG: NULL plan, unknown mode.
+ */
+enum { FDAS_HSUM_PLAIN = 0, FDAS_HSUM_NEIGHBOUR_MAX = 1 };
+int fdas_plan_set_harmonic_mode(fdas_plan_t plan, int mode);
+
 /* Tells the plan that the plane fdas_convolve_plane wrote last has been modified (or its buffer reused)
  * by the caller: the next fdas_harmonic_sum_peaks rebuilds the block maxima from the plane it is given. */
 int fdas_plan_invalidate_plane(fdas_plan_t plan);

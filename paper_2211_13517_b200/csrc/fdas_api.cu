@@ -26,7 +26,7 @@ static const int64_t kMaybeCapacity = 1 << 22;  // K3 prefilter survivors (funda
 static void free_plan(fdas_plan_s* p) {
     if (!p) return;
     free_batch_state(p->batch);
-    cudaFree(p->d_maxplane); cudaFree(p->d_maybe); cudaFree(p->d_maybe_count);
+    cudaFree(p->d_maxplane); cudaFree(p->d_maxplane_nbr); cudaFree(p->d_maybe); cudaFree(p->d_maybe_count);
     cudaFree(p->d_bank); cudaFree(p->d_tw1); cudaFree(p->d_tw2); cudaFree(p->d_fft_work);
     cudaFree(p->d_X); cudaFree(p->d_blk_start); cudaFree(p->d_blk_len); cudaFree(p->d_blk_med);
     cudaFree(p->ws_series); cudaFree(p->ws_spec); cudaFree(p->ws_plane); cudaFree(p->ws_cands);
@@ -192,6 +192,8 @@ int fdas_enqueue_harmonic(fdas_plan_s* plan, const void* d_plane, unsigned short
     hp.maxplane = d_maxplane; hp.mpitch = plan->info.nbins / 8;
     hp.maybe = plan->d_maybe; hp.maybe_capacity = kMaybeCapacity; hp.maybe_count = plan->d_maybe_count;
     hp.overflow = reinterpret_cast<unsigned*>(plan->d_maybe_count + 1);
+    hp.nbr = plan->hsum_mode == FDAS_HSUM_NEIGHBOUR_MAX ? 1 : 0;
+    hp.maxplane_nbr = plan->d_maxplane_nbr;
     int nl = 0;
     CU(launch_harmonic(fdas_plane16(plan->info.precision), build_max, hp, st, &nl));
     plan->launches += nl;
@@ -265,6 +267,15 @@ int fdas_convolve_plane(fdas_plan_t plan, const void* d_spec, void* d_plane, voi
     if (rc == FDAS_OK) rc = order_after(plan, st);
     if (rc == FDAS_OK) plan->max_valid_for = d_plane;
     return rc;
+}
+
+int fdas_plan_set_harmonic_mode(fdas_plan_t plan, int mode) {
+    if (!plan || (mode != FDAS_HSUM_PLAIN && mode != FDAS_HSUM_NEIGHBOUR_MAX)) return FDAS_EARG;
+    if (mode == FDAS_HSUM_NEIGHBOUR_MAX && !plan->d_maxplane_nbr)
+        CU(cudaMalloc(&plan->d_maxplane_nbr,
+                      (size_t)plan->info.nz * (size_t)(plan->info.nbins / 8) * sizeof(unsigned short)));
+    plan->hsum_mode = mode;
+    return FDAS_OK;
 }
 
 int fdas_plan_invalidate_plane(fdas_plan_t plan) {

@@ -16,6 +16,13 @@
 //   pass C (flags)      one thread per (stored candidate, neighbour): local-maximum attribute.
 // Results are identical to evaluating every fundamental exactly.  When the plane was not produced by
 // fdas_convolve_plane of this plan (hand-made planes), M is first rebuilt from it (build_max_kernel).
+//
+// Neighbour-maximised sums (FDAS_HSUM_NEIGHBOUR_MAX, reading A24):
+//   S'_h(r,j) = sum_{k<=h} max_{|d| <= floor(k/2)} P[row_k(j)][k r + d]   (bins clipped to [0, Nb))
+// so that a fundamental between two bins does not lose its harmonics.  The same branch-and-bound
+// runs on a DILATED side plane M'[j][b] = max_{|e| <= D} M[j][b+e], D = ceil(floor(H/2) / 8) blocks: the
+// window of harmonic k lies inside blocks (k r >> 3) - D .. + D, so M'[row_k][(k r) >> 3] bounds its
+// maximum and pass A is unchanged; passes B and C evaluate the windowed maxima on the real plane.
 #include <cuda_bf16.h>
 
 #include <algorithm>
@@ -166,6 +173,46 @@ __device__ __noinline__ void exact_fundamental(const T* P, const HarmGeom g, con
     }
 }
 
+// Neighbour-maximised variant of the plain definition (reading A24): harmonic h is the largest plane
+// value within floor(h/2) bins of h r (clipped to the plane); sums stay in k order.
+template <typename T>
+__device__ __forceinline__ float window_max(const T* prow, int64_t c, int w, int64_t nbins) {
+    const int64_t lo = max((int64_t)0, c - w), hi = min(nbins - 1, c + w);
+    float best = ldp(prow + lo);
+    for (int64_t x = lo + 1; x <= hi; ++x) best = fmaxf(best, ldp(prow + x));
+    return best;
+}
+template <typename T>
+__device__ bool harmonic_sum_nbr_at(const T* P, const HarmGeom& g, int64_t r, int j, int h, float* out) {
+    if (j < 0 || j >= g.nz || r < g.r_lo || r >= g.nbins) return false;
+    const int c2 = g.nz - 1;
+    {
+        const int v2 = 2 * h * j - (h - 1) * c2;
+        if (v2 < 0 || v2 > 2 * c2 || (int64_t)h * r > g.nbins - 1) return false;
+    }
+    float S = 0.f;
+    for (int k = 1; k <= h; ++k) {
+        const int row = min((2 * k * j - (k - 1) * c2 + 1) >> 1, c2);
+        S += window_max(P + (size_t)row * g.pitch, (int64_t)k * r, k >> 1, g.nbins);
+    }
+    *out = S;
+    return true;
+}
+template <typename T>
+__device__ __noinline__ void exact_fundamental_nbr(const T* P, const HarmGeom g, const float* thr, int64_t r,
+                                                   int j) {
+    if (r < g.r_lo || r >= g.nbins) return;
+    const int c2 = g.nz - 1;
+    float S = 0.f;
+    for (int h = 1; h <= g.H; ++h) {
+        const int v2 = 2 * h * j - (h - 1) * c2;
+        if (v2 < 0 || v2 > 2 * c2 || (int64_t)h * r > g.nbins - 1) break;
+        const int row = min((v2 + 1) >> 1, c2);
+        S += window_max(P + (size_t)row * g.pitch, (int64_t)h * r, h >> 1, g.nbins);
+        if (S > thr[h - 1]) emit_candidate(g, r, j, h, S);
+    }
+}
+
 // bf16 bit pattern of a non-negative power rounded toward +inf, and back.
 __device__ __forceinline__ unsigned short bf16_up(float v) {
     return (unsigned short)((__float_as_uint(v) + 0xffffu) >> 16);
@@ -184,6 +231,17 @@ __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
 #pragma unroll
     for (int i = 1; i < 8; ++i) m = fmaxf(m, ldp(src + i));
     p.maxplane[(size_t)j * p.mpitch + b] = bf16_up(m);
+}
+
+// ---- M' = M dilated by D blocks on either side (neighbour-maximised sums): one thread per block.
+__global__ void __launch_bounds__(256) dilate_max_kernel(const unsigned short* __restrict__ src,
+                                                         unsigned short* __restrict__ dst, int64_t mpitch, int D) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= mpitch) return;
+    const unsigned short* row = src + (size_t)blockIdx.y * mpitch;
+    unsigned m = 0;     // bf16 patterns of non-negative values order like the values
+    for (int64_t e = max((int64_t)0, b - D); e <= min(mpitch - 1, b + D); ++e) m = max(m, (unsigned)__ldg(row + e));
+    dst[(size_t)blockIdx.y * mpitch + b] = (unsigned short)m;
 }
 
 // ---- pass A: upper bounds from the block-max plane.
@@ -550,7 +608,7 @@ __global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmPara
 
 // ---- pass B: one thread per maybe record (r, j): the plain definition on the real plane.
 // If the maybe list overflowed (pathological thresholds), every fundamental is evaluated instead.
-template <typename T>
+template <typename T, int NBR>
 __global__ void __launch_bounds__(128) exact_kernel(const HarmParams p) {
     __shared__ float sthr[32];
     if (threadIdx.x < 32) sthr[threadIdx.x] = p.thr[threadIdx.x];
@@ -563,20 +621,24 @@ __global__ void __launch_bounds__(128) exact_kernel(const HarmParams p) {
         const unsigned long long n = *p.maybe_count;
         for (unsigned long long q = tid; q < n; q += nthr) {
             const uint2 rec = p.maybe[q];
-            exact_fundamental(P, g, sthr, (int64_t)rec.x, (int)rec.y);
+            if (NBR) exact_fundamental_nbr(P, g, sthr, (int64_t)rec.x, (int)rec.y);
+            else exact_fundamental(P, g, sthr, (int64_t)rec.x, (int)rec.y);
         }
     } else {
         const unsigned long long n = (unsigned long long)p.nbins * (unsigned long long)p.nz;
-        for (unsigned long long q = tid; q < n; q += nthr)
-            exact_fundamental(P, g, sthr, (int64_t)(q % (unsigned long long)p.nbins),
-                              (int)(q / (unsigned long long)p.nbins));
+        for (unsigned long long q = tid; q < n; q += nthr) {
+            const int64_t r = (int64_t)(q % (unsigned long long)p.nbins);
+            const int j = (int)(q / (unsigned long long)p.nbins);
+            if (NBR) exact_fundamental_nbr(P, g, sthr, r, j);
+            else exact_fundamental(P, g, sthr, r, j);
+        }
     }
 }
 
 // ---- pass C: local-maximum attribute, one thread per (stored candidate, neighbour): the flag is
 // cleared unless S_h(r,j) >= S_h at the neighbour (r+dr, j+dj) where that is defined, strictly >
 // for the neighbours that precede (j, r) lexicographically (reading A14).
-template <typename T>
+template <typename T, int NBR>
 __global__ void __launch_bounds__(128) flag_kernel(const HarmParams p) {
     const T* P = reinterpret_cast<const T*>(p.plane);
     const HarmGeom g = geom_of(p);
@@ -589,15 +651,18 @@ __global__ void __launch_bounds__(128) flag_kernel(const HarmParams p) {
         const int idx = nb < 4 ? nb : nb + 1;          // skip the centre of the 3 x 3 stencil
         const int dj = idx / 3 - 1, dr = idx % 3 - 1;
         float nv;
-        if (!harmonic_sum_at(P, g, (int64_t)c.r + dr, (int)c.zidx + dj, (int)c.h, &nv)) continue;
+        if (!(NBR ? harmonic_sum_nbr_at(P, g, (int64_t)c.r + dr, (int)c.zidx + dj, (int)c.h, &nv)
+                  : harmonic_sum_at(P, g, (int64_t)c.r + dr, (int)c.zidx + dj, (int)c.h, &nv)))
+            continue;
         const bool precedes = (dj < 0) || (dj == 0 && dr < 0);
         if (precedes ? !(c.power > nv) : !(c.power >= nv)) atomicAnd(&p.cands[q >> 3].flags, ~1u);
     }
 }
 
-cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams& p, cudaStream_t st,
+cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams& p_in, cudaStream_t st,
                             int* launches) {
     *launches = 0;
+    HarmParams p = p_in;
     cudaError_t e = cudaMemsetAsync(p.count, 0, sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(p.maybe_count, 0, 2 * sizeof(unsigned long long), st);   // + overflow flag
@@ -609,6 +674,16 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         else build_max_kernel<float><<<grid, 256, 0, st>>>(p);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
+    }
+    if (p.nbr) {
+        // the prefilter (and nothing else) scans the dilated side plane from here on
+        if (!p.maxplane_nbr) return cudaErrorInvalidValue;
+        const int D = ((p.H >> 1) + 7) >> 3;
+        dim3 grid((unsigned)((p.mpitch + 255) / 256), (unsigned)p.nz);
+        dilate_max_kernel<<<grid, 256, 0, st>>>(p.maxplane, p.maxplane_nbr, p.mpitch, D);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        ++*launches;
+        p.maxplane = p.maxplane_nbr;
     }
     // rows j < nlow and j >= nz - nlow have at most kShallowDepth harmonics inside the plane (reading
     // A12), rows j < nlow2 and j >= nz - nlow2 at most two
@@ -637,13 +712,23 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
     }
-    if (plane_is_bf16) exact_kernel<__nv_bfloat16><<<kExactBlocks, 128, 0, st>>>(p);
-    else exact_kernel<float><<<kExactBlocks, 128, 0, st>>>(p);
+    if (p.nbr) {
+        if (plane_is_bf16) exact_kernel<__nv_bfloat16, 1><<<kExactBlocks, 128, 0, st>>>(p);
+        else exact_kernel<float, 1><<<kExactBlocks, 128, 0, st>>>(p);
+    } else {
+        if (plane_is_bf16) exact_kernel<__nv_bfloat16, 0><<<kExactBlocks, 128, 0, st>>>(p);
+        else exact_kernel<float, 0><<<kExactBlocks, 128, 0, st>>>(p);
+    }
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     ++*launches;
     if (p.capacity > 0) {
-        if (plane_is_bf16) flag_kernel<__nv_bfloat16><<<kFlagBlocks, 128, 0, st>>>(p);
-        else flag_kernel<float><<<kFlagBlocks, 128, 0, st>>>(p);
+        if (p.nbr) {
+            if (plane_is_bf16) flag_kernel<__nv_bfloat16, 1><<<kFlagBlocks, 128, 0, st>>>(p);
+            else flag_kernel<float, 1><<<kFlagBlocks, 128, 0, st>>>(p);
+        } else {
+            if (plane_is_bf16) flag_kernel<__nv_bfloat16, 0><<<kFlagBlocks, 128, 0, st>>>(p);
+            else flag_kernel<float, 0><<<kFlagBlocks, 128, 0, st>>>(p);
+        }
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
     }

@@ -83,6 +83,8 @@ struct HarmParams {
     int64_t maybe_capacity;
     unsigned long long* maybe_count;  // plan-owned; followed by the overflow flag
     unsigned* overflow;               // plan-owned: set if the maybe list was too small
+    int nbr;                          // 1: neighbour-maximised sums (reading A24)
+    unsigned short* maxplane_nbr;     // plan-owned dilated side plane the prefilter scans when nbr = 1
 };
 // K3: [build_max] + prefilter (pass A) + exact (pass B) + flags (pass C); `launches` receives the
 // number of kernels launched.

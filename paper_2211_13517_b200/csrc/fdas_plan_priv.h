@@ -43,6 +43,8 @@ struct fdas_plan_s {
     int64_t launches = 0;
     unsigned short* d_maxplane = nullptr;    // block-max plane M (nz x nbins/8, bf16 bits), written by K2
     const void* max_valid_for = nullptr;     // the plane M currently describes (nullptr: none)
+    int hsum_mode = 0;                       // FDAS_HSUM_PLAIN | FDAS_HSUM_NEIGHBOUR_MAX
+    unsigned short* d_maxplane_nbr = nullptr;   // dilated side plane (allocated when the mode is first set)
     cudaEvent_t ev_last = nullptr;           // end of the last public per-trial call (cross-stream ordering)
     cudaStream_t last_stream = nullptr;
     bool have_last = false;

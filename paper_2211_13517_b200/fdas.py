@@ -19,11 +19,12 @@ LIB_PATH = os.path.join(_HERE, "libfdas.so")
 FDAS_FP32, FDAS_BF16, FDAS_BF16_PLANE16, FDAS_BF16_TC, FDAS_BF16_TC_PLANE16 = 0, 1, 2, 3, 4
 PRECISIONS = {"fp32": FDAS_FP32, "bf16": FDAS_BF16, "bf16_plane16": FDAS_BF16_PLANE16,
               "bf16_tc": FDAS_BF16_TC, "bf16_tc_plane16": FDAS_BF16_TC_PLANE16}
+FDAS_HSUM_PLAIN, FDAS_HSUM_NEIGHBOUR_MAX = 0, 1
 FDAS_OK, FDAS_EARG, FDAS_EALLOC, FDAS_ECUDA, FDAS_ECUFFT, FDAS_EOVERFLOW, FDAS_EUNSUPPORTED = range(7)
 
 EXPORTS = (
     "fdas_plan", "fdas_plan_info", "fdas_prepare_spectrum", "fdas_convolve_plane",
-    "fdas_harmonic_sum_peaks", "fdas_plan_invalidate_plane", "fdas_search_host", "fdas_search_batch", "fdas_thresholds_from_sigma",
+    "fdas_harmonic_sum_peaks", "fdas_plan_invalidate_plane", "fdas_plan_set_harmonic_mode", "fdas_search_host", "fdas_search_batch", "fdas_thresholds_from_sigma",
     "fdas_plan_templates_host", "fdas_plan_debug_maxplane", "fdas_plan_launch_count", "fdas_destroy", "fdas_strerror",
     "fdas_last_error_detail",
 )
@@ -62,6 +63,7 @@ def _load():
     L.fdas_convolve_plane.argtypes = [vp, vp, vp, vp]
     L.fdas_harmonic_sum_peaks.argtypes = [vp, vp, ci, C.POINTER(C.c_float), i64, vp, i64, vp, vp]
     L.fdas_plan_invalidate_plane.argtypes = [vp]
+    L.fdas_plan_set_harmonic_mode.argtypes = [vp, ci]
     L.fdas_search_host.argtypes = [vp, vp, ci, C.POINTER(C.c_float), i64, vp, i64, C.POINTER(i64), vp]
     L.fdas_search_batch.argtypes = [vp, C.POINTER(vp), ci, ci, ci, C.POINTER(C.c_float), i64, vp, i64,
                                     C.POINTER(i64), vp]
@@ -164,6 +166,11 @@ class Plan:
             self._h, d_plane.data_ptr(), int(H), thr.ctypes.data_as(C.POINTER(C.c_float)), int(r_lo),
             d_cands.data_ptr() if d_cands is not None else None, cap, d_count.data_ptr(),
             _stream_ptr(stream)), "fdas_harmonic_sum_peaks")
+
+    def set_harmonic_mode(self, mode):
+        """"plain" (S_h) or "neighbour_max" (S'_h: harmonic k at its maximum within floor(k/2) bins of k r)."""
+        m = {"plain": FDAS_HSUM_PLAIN, "neighbour_max": FDAS_HSUM_NEIGHBOUR_MAX}.get(mode, mode)
+        _check(_lib.fdas_plan_set_harmonic_mode(self._h, int(m)), "fdas_plan_set_harmonic_mode")
 
     def invalidate_plane(self):
         """The plane convolve_plane wrote last was modified by the caller: rebuild the block maxima."""

@@ -130,6 +130,14 @@ def medium() -> Workload:
                     ("fp32", "bf16"), 2, _medium_signals(2))
 
 
+def offbin() -> Workload:
+    """A pulsar whose fundamental lies BETWEEN two Fourier bins (r_c = integer + 0.37, 8 harmonics of equal
+    amplitude, z = 2): harmonic k sits at k r_c, up to k/2 bins from k round(r_c), so the plain harmonic
+    sum loses it and the neighbour-maximised sum (reading A24) does not.  Medium-sized."""
+    return Workload("offbin", 1 << 21, TSAMP_FULL, 96.0, 1.0, 2048, 8, 6.0, 64, ("fp32", "bf16"), 7,
+                    (Signal(r_c=40000.37, z=2.0, amp=0.006, phase=0.7, nharm=8, harm_decay=1.0),))
+
+
 def ska(seed: int = 3, half_res: bool = False, signals=None) -> Workload:
     """BASELINE.json configs[2] (and the 128 us series of configs[4] with half_res=True)."""
     n = N_SKA_HALF if half_res else N_SKA_FULL

@@ -848,3 +848,109 @@ def test_other_z_spacings_full_parity(fdas, torch_, oracle, precision, zstep):
                                strict_rel=1e-5)
     assert stats["only_gpu"] + stats["only_orc"] <= 2 and stats["common"] > 50, stats
     record_stats(f"zstep{zstep}_{precision}", {**ps.summary(P.max()), **stats})
+
+
+# ------------------------------------- neighbour-maximised harmonic sums
+def nbr_thresholds(thr):
+    """A caller's choice of thresholds for S': the plain T_h raised by the growth of the noise mean,
+    sum_k (H_{2 floor(k/2) + 1} - 1), H_m = mean of the maximum of m unit exponentials."""
+    out, shift = [], 0.0
+    for k, t in enumerate(thr, start=1):
+        m = 2 * (k // 2) + 1
+        shift += sum(1.0 / i for i in range(1, m + 1)) - 1.0
+        out.append(t + shift)
+    return np.array(out, dtype=np.float32)
+
+
+@pytest.mark.parametrize("precision,H", [("fp32", 16), ("bf16_plane16", 16), ("fp32", 32), ("fp32", 3)])
+def test_neighbour_max_mode_alone_on_hand_made_planes(fdas, torch_, oracle, precision, H):
+    """K3 in FDAS_HSUM_NEIGHBOUR_MAX mode on a hand-made plane against the oracle's O5n candidates:
+    the dilated side plane (1 block either side for H <= 17, 2 for H = 32) must not lose a candidate,
+    the windowed maxima, the clipping at the ends of the plane and the flags must agree."""
+    torch = torch_
+    plan = fdas.Plan(1 << 14, 64e-6, 16.0, 1.0, 2048, precision)
+    nb, nz = plan.info.nbins, plan.info.nz
+    rng = np.random.default_rng(61 + H)
+    P32 = rng.exponential(1.0, size=(nz, nb)).astype(np.float32)
+    for k in (1, 2, 3, 5):                       # spikes next to the harmonic cut-offs and the plane's ends
+        P32[:, min(nb - 1, (nb - 1) // k + 1)] += 8.0
+    P32[:, 0] += 20.0; P32[:, nb - 1] += 20.0
+    d_plane = torch.from_numpy(P32).cuda()
+    if precision == "bf16_plane16":
+        d_plane = d_plane.to(torch.bfloat16)
+    P = d_plane.float().cpu().numpy().astype(np.float64)
+    thr = nbr_thresholds(fdas.thresholds_from_sigma(H, 2.5))
+    r_lo = 3
+    d_c, d_n = plan.alloc_cands(1 << 19)
+    plan.set_harmonic_mode("neighbour_max")
+    plan.harmonic_sum_peaks(d_plane, H, thr, r_lo, d_c, d_n)
+    torch.cuda.synchronize()
+    res = plan.read_cands(d_c, d_n)
+    oc = oracle.candidates(P, H, thr.astype(np.float64), r_lo, nbr=True)
+    assert oc.count > 300 and res.count == len(res.cands)
+
+    def s_at(r, j, h):
+        if j < 0 or j >= nz or r < r_lo or r >= nb:
+            return None
+        S = oracle.harmonic_sums_nbr_at(P, h, r, j)
+        return float(S[h - 1]) if len(S) >= h else None
+
+    def margin(r, j, h):
+        vals = [s_at(r + dr, j + dj, h) for dj in (-1, 0, 1) for dr in (-1, 0, 1) if (dj, dr) != (0, 0)]
+        vals = [abs(s_at(r, j, h) - v) for v in vals if v is not None]
+        return min(vals) if vals else None
+
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * P.max(), None, s_at, margin,
+                               strict_rel=1e-5)
+    assert stats["only_gpu"] + stats["only_orc"] <= 3 and stats["flags_checked"] > 50, stats
+    assert any(k[2] == H for k in gpu_cand_dict(res.cands)) or H == 32
+    # back to the plain sums on the same plan: the plain candidate set again
+    plan.set_harmonic_mode("plain")
+    thr_p = fdas.thresholds_from_sigma(H, 3.0)
+    plan.harmonic_sum_peaks(d_plane, H, thr_p, r_lo, d_c, d_n)
+    got = set(gpu_cand_dict(plan.read_cands(d_c, d_n).cands))
+    want = oracle.candidates(P, H, thr_p.astype(np.float64), r_lo).triples()
+    assert len(got ^ want) <= 3
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16_tc"])
+def test_neighbour_max_mode_recovers_an_off_bin_pulsar(fdas, torch_, oracle, precision):
+    """End to end on a pulsar at r_c = 40000.37 with 8 equal harmonics: candidate-set parity of the
+    neighbour-maximised mode against the oracle (O1..O4, O5n), and the recovered S_8 of both modes."""
+    torch = torch_
+    wl = inputs.offbin()
+    x = inputs.series_for(wl)
+    orc = oracle.run(x, wl.nfft, wl.zmax, wl.zstep, wl.nharm, wl.nsigma, wl.r_lo, want_candidates=False)
+    plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, precision)
+    d_spec, d_plane = plan.alloc_spec(), plan.alloc_plane()
+    d_c, d_n = plan.alloc_cands(1 << 16)
+    thr_p = fdas.thresholds_from_sigma(wl.nharm, wl.nsigma)
+    thr_n = nbr_thresholds(thr_p)
+    plan.prepare_spectrum(torch.from_numpy(x).cuda(), d_spec)
+    plan.convolve_plane(d_spec, d_plane)
+    plan.harmonic_sum_peaks(d_plane, wl.nharm, thr_p, wl.r_lo, d_c, d_n)
+    plain = gpu_cand_dict(plan.read_cands(d_c, d_n).cands)
+    plan.set_harmonic_mode("neighbour_max")
+    plan.harmonic_sum_peaks(d_plane, wl.nharm, thr_n, wl.r_lo, d_c, d_n)
+    nbr = gpu_cand_dict(plan.read_cands(d_c, d_n).cands)
+    s = wl.signals[0]
+    r0, j0 = int(round(s.r_c)), int(round(s.z + wl.zmax))
+    S_plain = oracle.harmonic_sums_at(orc.P, wl.nharm, r0, j0)
+    S_nbr = oracle.harmonic_sums_nbr_at(orc.P, wl.nharm, r0, j0)
+    assert len(S_nbr) == 8 and S_nbr[7] > 1.5 * S_plain[7] and S_nbr[7] > thr_n[7] + 20
+    assert (r0, j0, 8) in nbr and (r0, j0, 8) not in plain            # the deep sum is found by S' only
+    tol = TOL[precision] * orc.P.max()
+    oc = oracle.candidates(orc.P, wl.nharm, thr_n.astype(np.float64), wl.r_lo, nbr=True)
+
+    def s_at(r, j, h):
+        S = oracle.harmonic_sums_nbr_at(orc.P, h, r, j)
+        return float(S[h - 1]) if len(S) >= h else None
+
+    stats = compare_candidates(nbr, oc.as_dict(), thr_n, tol, REL_POW[precision], s_at, None,
+                               strict_rel=STRICT_REL[precision])
+    assert stats["common"] >= 8
+    if precision == "fp32":
+        assert stats["only_gpu"] + stats["only_orc"] == 0, stats
+    record_stats("offbin_nbr_" + precision, {**stats, "S8_plain": float(S_plain[7]), "S8_nbr": float(S_nbr[7]),
+                                             "gpu_S8_nbr": nbr[(r0, j0, 8)][0], "T8_plain": float(thr_p[7]),
+                                             "T8_nbr": float(thr_n[7])})
