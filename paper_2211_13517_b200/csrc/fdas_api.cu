@@ -79,10 +79,10 @@ static int build_plan(fdas_plan_s* p) {
             int dev0 = 0, optin = 0;
             CU(cudaGetDevice(&dev0));
             CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev0));
-            fits = convolve_tc_smem_bytes(p->tc.kp, p->tc.npair, fdas_plane16(in.precision)) <= optin;
+            fits = convolve_tc_smem_bytes(p->tc.kp, p->tc.chunk, fdas_plane16(in.precision)) <= optin;
         }
         if (!fits) {
-            g_detail = "FDAS_BF16_TC: template bank does not fit the tensor-core kernel (1..128 conjugate pairs, <= 255 taps, nbins % 128 == 0)";
+            g_detail = "FDAS_BF16_TC: template bank does not fit the tensor-core kernel (at least one conjugate pair, <= 255 taps, nbins % 128 == 0)";
             return FDAS_EUNSUPPORTED;
         }
         std::vector<uint32_t> img;
@@ -162,12 +162,18 @@ int fdas_enqueue_convolve(fdas_plan_s* plan, const void* d_spec, void* d_plane,
     if (fdas_is_tc(plan->info.precision)) {
         ConvTcParams t;
         t.spec = reinterpret_cast<const unsigned*>(d_spec); t.plane = d_plane;
-        t.bimg = reinterpret_cast<const uint32_t*>(plan->d_bank);
         t.nbins = plan->info.nbins; t.pitch = plan->info.plane_pitch;
-        t.nz = plan->info.nz; t.h = plan->info.halfwidth; t.kp = plan->tc.kp; t.npair = plan->tc.npair;
+        t.nz = plan->info.nz; t.h = plan->info.halfwidth; t.kp = plan->tc.kp; t.npair_total = plan->tc.npair;
         t.maxplane = d_maxplane; t.mpitch = plan->info.nbins / 8;
-        CU(launch_convolve_tc(fdas_plane16(plan->info.precision), t, &plan->tc_maps, plan->nsm, st));
-        plan->launches += 1;
+        // a bank of more than 128 conjugate pairs takes one launch per chunk of pairs (each reads the
+        // spectrum again, 17 MB, and writes its own rows of the plane)
+        for (int c = 0; c < plan->tc.nchunk; ++c) {
+            t.pair0 = c * plan->tc.chunk;
+            t.npair = std::min(plan->tc.chunk, plan->tc.npair - t.pair0);
+            t.bimg = reinterpret_cast<const uint32_t*>(plan->d_bank) + (size_t)c * 2 * 128 * (plan->tc.kp / 2);
+            CU(launch_convolve_tc(fdas_plane16(plan->info.precision), t, &plan->tc_maps, plan->nsm, st));
+            plan->launches += 1;
+        }
         return FDAS_OK;
     }
     ConvParams c;

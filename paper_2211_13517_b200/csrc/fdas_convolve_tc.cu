@@ -275,15 +275,17 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
 
     const int64_t ntiles = p.nbins / kTileR;
     const int ksteps = p.kp >> 4;
-    const int npair = p.npair;
-    const int jplus0 = p.nz - npair;                      // row of pair 0's +z member
+    const int npair = p.npair;                            // pairs of this launch: lanes 0 .. npair - 1
+    const int jplus0 = p.nz - p.npair_total + p.pair0;    // row of lane 0's +z member
+    const int jminus0 = p.npair_total - 1 - p.pair0;      // row of lane 0's -z member
 
     if (warp == kProducerWarp) {
         // ===== producer: the tile's spectrum slice -> interleaved sliding-window rows; z = 0 row
         unsigned short* sre = reinterpret_cast<unsigned short*>(smem + L.st_off);
         unsigned short* sim = reinterpret_cast<unsigned short*>(smem + L.st_off + L.st_part);
         const int nrows = window_rows(p.kp), nsrc = nrows + 24;
-        const bool zero_row = (p.nz & 1) != 0;
+        const bool zero_row = (p.nz & 1) != 0 && p.pair0 == 0;
+        const int mid = p.npair_total;                    // the z = 0 row of an odd bank
         // the slice s[i] = w[128 tile - h + i], i < nsrc (<= 384), as 16-byte loads of 4 bins per lane; the
         // next tile's loads are issued before this tile's window is built, so their latency is hidden
         uint4 v[3];
@@ -340,16 +342,16 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
                     unsigned short b[4];
 #pragma unroll
                     for (int e = 0; e < 4; ++e) b[e] = __bfloat16_as_ushort(__float2bfloat16_rn(P[e]));
-                    __stcs(reinterpret_cast<uint2*>(reinterpret_cast<unsigned short*>(p.plane) + (int64_t)npair * p.pitch + r),
+                    __stcs(reinterpret_cast<uint2*>(reinterpret_cast<unsigned short*>(p.plane) + (int64_t)mid * p.pitch + r),
                            make_uint2((unsigned)b[0] | ((unsigned)b[1] << 16), (unsigned)b[2] | ((unsigned)b[3] << 16)));
                     m = max(max((unsigned)b[0], (unsigned)b[1]), max((unsigned)b[2], (unsigned)b[3]));
                 } else {
-                    __stcs(reinterpret_cast<float4*>(reinterpret_cast<float*>(p.plane) + (int64_t)npair * p.pitch + r),
+                    __stcs(reinterpret_cast<float4*>(reinterpret_cast<float*>(p.plane) + (int64_t)mid * p.pitch + r),
                            make_float4(P[0], P[1], P[2], P[3]));
                     m = (__float_as_uint(fmaxf(fmaxf(P[0], P[1]), fmaxf(P[2], P[3]))) + 0xffffu) >> 16;
                 }
                 m = max(m, __shfl_xor_sync(0xffffffffu, m, 1));
-                if ((lane & 1) == 0) p.maxplane[(int64_t)npair * p.mpitch + (r >> 3)] = (unsigned short)m;
+                if ((lane & 1) == 0) p.maxplane[(int64_t)mid * p.mpitch + (r >> 3)] = (unsigned short)m;
             }
             __syncwarp();      // the slice staging is rewritten by the next iteration
         }
@@ -407,7 +409,7 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
         // >= nreal, which no box reads.
         const int nreal = min(32, npair - 32 * q);
         const int row_p = jplus0 + 32 * q;
-        const int row_m = npair - 32 * q - nreal;
+        const int row_m = jminus0 - 32 * q - nreal + 1;
         const int rowm = lane < nreal ? nreal - 1 - lane : lane;
         const CUtensorMap* const pm = nreal == 32 ? &pmap : &pmap_tail;
         constexpr int kTileBytes = 32 * 2 * kSubR * (PLANE16 ? 2 : 4);   // 32 rows x this warp's 64 bins
@@ -492,11 +494,16 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
 
 }  // namespace tc
 
-static int tc_nbuf(int npair) { return ((npair + 31) >> 5) <= 3 ? 2 : 1; }
+// Staging buffers per epilogue warp: two (a tile's stores drain while the next tile is computed) when
+// the CTA's shared memory holds them -- up to 96 pairs with templates of up to 145 taps -- else one.
+static int tc_nbuf(int kp, int npair, int plane16) {
+    const int nq = (npair + 31) >> 5;
+    return tc::make_layout(kp, 2 * nq, 2, plane16).total <= 227 * 1024 ? 2 : 1;
+}
 
 int convolve_tc_smem_bytes(int kp, int npair, int plane16) {
     const int nq = (npair + 31) >> 5;
-    return tc::make_layout(kp, 2 * nq, tc_nbuf(npair), plane16).total;
+    return tc::make_layout(kp, 2 * nq, tc_nbuf(kp, npair, plane16), plane16).total;
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (libfdas.so does not link libcuda).
@@ -556,7 +563,9 @@ static cudaError_t get_maps(TcMapCache* cache, int plane16, const ConvTcParams& 
     TcMapCache::Entry& e = cache->e[cache->next];
     cache->next = (cache->next + 1) % TcMapCache::kEntries;
     e.valid = false;
-    const int tail = (p.npair & 31) ? (p.npair & 31) : 32;     // rows of the ragged last quarter's boxes
+    // rows of the boxes of a ragged last lane quarter (launches of a split bank are multiples of 32 pairs
+    // except the last, so one tail size serves them all)
+    const int tail = (p.npair_total & 31) ? (p.npair_total & 31) : 32;
     cudaError_t err = make_plane_map(p.plane, plane16, p.nbins, p.nz, p.pitch, 32, reinterpret_cast<CUtensorMap*>(e.pmap));
     if (err == cudaSuccess)
         err = make_plane_map(p.plane, plane16, p.nbins, p.nz, p.pitch, tail, reinterpret_cast<CUtensorMap*>(e.pmap_tail));
@@ -586,7 +595,8 @@ static cudaError_t launch_tc(const ConvTcParams& p, const TcMapCache::Entry& m, 
 }
 
 cudaError_t launch_convolve_tc(int plane16, const ConvTcParams& p, TcMapCache* cache, int nsm, cudaStream_t st) {
-    if (p.nbins % tc::kTileR != 0 || p.kp % 16 != 0 || p.npair < 1 || p.npair > 128 ||
+    if (p.nbins % tc::kTileR != 0 || p.kp % 16 != 0 || p.npair < 1 || p.npair > 128 || p.pair0 < 0 ||
+        p.pair0 + p.npair > p.npair_total || 2 * p.npair_total > p.nz ||
         tc::kBankCol0 + p.kp > 512 || (reinterpret_cast<uintptr_t>(p.plane) & 15u) ||
         (reinterpret_cast<uintptr_t>(p.spec) & 15u) ||
         ((p.pitch * (plane16 ? 2 : 4)) & 15) || ((p.mpitch * 2) & 15) ||
@@ -595,7 +605,7 @@ cudaError_t launch_convolve_tc(int plane16, const ConvTcParams& p, TcMapCache* c
     const TcMapCache::Entry* m = nullptr;
     const cudaError_t e = get_maps(cache, plane16, p, &m);
     if (e != cudaSuccess) return e;
-    if (tc_nbuf(p.npair) == 2) return plane16 ? launch_tc<1, 2>(p, *m, nsm, st) : launch_tc<0, 2>(p, *m, nsm, st);
+    if (tc_nbuf(p.kp, p.npair, plane16) == 2) return plane16 ? launch_tc<1, 2>(p, *m, nsm, st) : launch_tc<0, 2>(p, *m, nsm, st);
     return plane16 ? launch_tc<1, 1>(p, *m, nsm, st) : launch_tc<0, 1>(p, *m, nsm, st);
 }
 

@@ -170,22 +170,25 @@ bool tc_geometry(int nz, int h, TcGeom* g) {
     if (nz < 2 || h < 1) return false;
     g->npair = nz / 2;
     g->kp = ((2 * h + 1) + 15) / 16 * 16;
+    g->nchunk = (g->npair + 127) / 128;
+    g->chunk = (((g->npair + g->nchunk - 1) / g->nchunk) + 31) / 32 * 32;     // balanced, whole lane quarters
     // 256 tensor-memory columns hold the two accumulator stages, the rest the two bank images
-    return g->npair <= 128 && 256 + g->kp <= 512;
+    return 256 + g->kp <= 512;
 }
 
 void pack_bank_tc(const Bank& bank, const TcGeom& g, std::vector<uint32_t>* out, double* asym) {
     const int taps = 2 * bank.h + 1, kw = g.kp / 2;
-    out->assign((size_t)2 * 128 * kw, 0u);
+    out->assign((size_t)g.nchunk * 2 * 128 * kw, 0u);
     double worst = 0.0;
     for (int p = 0; p < g.npair; ++p) {
         const cd* tp = &bank.time[(size_t)(bank.nz - g.npair + p) * taps];
         const cd* tm = &bank.time[(size_t)(g.npair - 1 - p) * taps];
+        const int c = p / g.chunk, l = p % g.chunk;
         for (int k = 0; k < taps; ++k) {
             worst = std::max(worst, std::abs(tm[k] - std::conj(tp[k])));
             for (int part = 0; part < 2; ++part) {
                 const uint32_t b = bf16_rne((float)(part ? tp[k].imag() : tp[k].real()));
-                (*out)[((size_t)part * 128 + p) * kw + k / 2] |= b << (16 * (k & 1));
+                (*out)[(((size_t)c * 2 + part) * 128 + l) * kw + k / 2] |= b << (16 * (k & 1));
             }
         }
     }

@@ -40,14 +40,17 @@ void pack_bank_bf16(const Bank& bank, std::vector<uint32_t>* out);
 // (T_{-z} = conj(T_z)) plus, for odd nz, the z = 0 row; pair p is rows j+ = nz - npair + p and
 // j- = npair - 1 - p.
 struct TcGeom {
-    int npair = 0;   // 1..128: one TMEM lane per pair
-    int kp = 0;      // taps 2h+1 padded to a multiple of 16
+    int npair = 0;    // nz / 2 conjugate pairs
+    int kp = 0;       // taps 2h+1 padded to a multiple of 16
+    int nchunk = 0;   // kernel launches: the kernel holds up to 128 pairs (one TMEM lane each)
+    int chunk = 0;    // pairs per launch (a multiple of 32; the last launch takes the remainder)
 };
-// false when the bank does not fit the kernel (more than 128 pairs, none, or too many taps for the
-// tensor-memory columns left beside the accumulators).
+// false when the bank does not fit the kernel (no pair at all, or too many taps for the tensor-memory
+// columns left beside the accumulators).
 bool tc_geometry(int nz, int h, TcGeom* g);
-// Bank image for tensor memory: word [(part*128 + p)*(kp/2) + c] = bf16(X[2c]) | bf16(X[2c+1]) << 16
-// (RNE), X[k] = Re (part 0) or Im (part 1) of T_{j+(p)}[k - h], zero for k > 2h and for rows p >= npair.
+// Bank images for tensor memory, one per launch c: word [((c*2 + part)*128 + l)*(kp/2) + w] =
+// bf16(X[2w]) | bf16(X[2w+1]) << 16 (RNE), X[k] = Re (part 0) or Im (part 1) of T_{j+(p)}[k - h] for pair
+// p = c*chunk + l, zero for k > 2h and for lanes beyond the launch's pairs.
 // *asym receives max |T_{j-}[m] - conj(T_{j+}[m])| over the bank (must be ~1e-16 for the pairing).
 void pack_bank_tc(const Bank& bank, const TcGeom& g, std::vector<uint32_t>* out, double* asym);
 

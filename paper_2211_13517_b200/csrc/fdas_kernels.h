@@ -37,7 +37,9 @@ struct ConvTcParams {
     int64_t nbins, pitch;
     int nz, h;
     int kp;                    // taps 2h+1 padded to a multiple of 16
-    int npair;                 // conjugate template pairs (nz / 2), 1..128
+    int npair;                 // conjugate template pairs handled by THIS launch, 1..128 (one TMEM lane each)
+    int npair_total;           // nz / 2: pair p is rows j+ = nz - npair_total + p, j- = npair_total - 1 - p
+    int pair0;                 // first pair of this launch (a bank of more than 128 pairs takes several)
     unsigned short* maxplane;  // as ConvParams
     int64_t mpitch;
 };

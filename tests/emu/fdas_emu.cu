@@ -221,22 +221,25 @@ int fdas_emu_convolve_tc(const float* spec, int64_t nb, double zmax, double zste
     double asym = 0.0;
     pack_bank_tc(bank, g, &img, &asym);
     if (asym > 1e-12) return FDAS_EUNSUPPORTED;
-    const int kw = g.kp / 2, npair = g.npair, jplus0 = nz - npair, ksteps = g.kp / 16;
-    const Layout L = make_layout(g.kp, 2 * ((npair + 31) / 32), 2, plane16);
-    std::vector<unsigned char> smem((size_t)L.total, 0xff);   // 0xff: unwritten bf16 reads as NaN
-    std::vector<uint32_t> tmem((size_t)128 * 512, 0x7fc00000u);
-    for (int part = 0; part < 2; ++part)                      // the kernel's tcgen05.st of the bank
-        for (int lane = 0; lane < 128; ++lane)
-            for (int c = 0; c < kw; ++c)
-                tmem[(size_t)lane * 512 + kBankCol0 + part * kw + c] = img[((size_t)part * 128 + lane) * kw + c];
+    const int kw = g.kp / 2, ksteps = g.kp / 16;
     std::vector<uint32_t> specq((size_t)nb);
     for (int64_t k = 0; k < nb; ++k) specq[k] = pack_bf16x2(spec[2 * k], spec[2 * k + 1]);
     const int64_t mpitch = nb / 8, ntiles = nb / kTileR;
     auto store = [&](int j, int64_t r, float P) {
-        if (j < 0 || j >= nz) return;                         // clipped by the TMA store
+        if (j < 0 || j >= nz) return;                         // lanes beyond the launch's pairs: no row
         if (plane16) P = bf16_bits_to_f32(f32_to_bf16_rne(P));
         plane[(size_t)j * nb + r] = P;
     };
+    for (int c = 0; c < g.nchunk; ++c) {                       // one kernel launch per chunk of pairs
+    const int pair0 = c * g.chunk, npair = std::min(g.chunk, g.npair - pair0);
+    const int jplus0 = nz - g.npair + pair0, jminus0 = g.npair - 1 - pair0;
+    const Layout L = make_layout(g.kp, 2 * ((npair + 31) / 32), 1, plane16);
+    std::vector<unsigned char> smem((size_t)L.total, 0xff);   // 0xff: unwritten bf16 reads as NaN
+    std::vector<uint32_t> tmem((size_t)128 * 512, 0x7fc00000u);
+    for (int part = 0; part < 2; ++part)                      // the kernel's tcgen05.st of the bank
+        for (int lane = 0; lane < 128; ++lane)
+            for (int w = 0; w < kw; ++w)
+                tmem[(size_t)lane * 512 + kBankCol0 + part * kw + w] = img[(((size_t)c * 2 + part) * 128 + lane) * kw + w];
     uint32_t item = 0;
     int it = 0;
     for (int64_t tile = 0; tile < ntiles; ++tile, ++it) {
@@ -259,23 +262,24 @@ int fdas_emu_convolve_tc(const float* spec, int64_t nb, double zmax, double zste
                 const uint4 o = window_row(w32, rho);
                 std::memcpy(hst + window_row_offset(rho, part), &o, 16);
             }
-        if (nz & 1)
+        if ((nz & 1) && pair0 == 0)
             for (int b = 0; b < kTileR; ++b) {
                 const float2 w = unpack_bf16x2(specq[tile * kTileR + b]);
-                store(npair, tile * kTileR + b, fmaf(w.x, w.x, w.y * w.y));
+                store(g.npair, tile * kTileR + b, fmaf(w.x, w.x, w.y * w.y));
             }
-        // MMA issuer + epilogue, one accumulator stage at a time
+        // MMA issuer (sub-tiles in the order 0, 2, 1, 3; accumulator stage = s >> 1) + epilogue
         const uint32_t idesc = instr_desc(2 * kSubR);
         const uint32_t hbase = (uint32_t)(L.h_off + hs * L.h_stage);
-        for (int s = 0; s < kSubTiles; ++s, ++item) {
-            const int st = (int)(item & 1u);
+        for (int pos = 0; pos < kSubTiles; ++pos, ++item) {
+            const int s = 2 * (pos & 1) + (pos >> 1);
+            const int st = pos & 1;
             const int d_r = st * kAccCols, d_i = d_r + 2 * kSubR;
             for (int ks = 0; ks < ksteps; ++ks) {
                 const uint64_t bd = smem_desc(hbase + window_desc_offset(s, ks), kWinLbo, kWinSbo);
                 emu_umma_ts(smem, tmem, d_r, kBankCol0 + 8 * ks, bd, idesc, ks > 0);
                 emu_umma_ts(smem, tmem, d_i, kBankCol0 + kw + 8 * ks, bd, idesc, ks > 0);
             }
-            for (int p = 0; p < 32 * ((npair + 31) / 32); ++p)
+            for (int p = 0; p < npair; ++p)
                 for (int bg = 0; bg < kSubR / 8; ++bg)
                     for (int e = 0; e < 8; ++e) {
                         float Ar, Ai, Br, Bi, Pp, Pm;
@@ -286,9 +290,10 @@ int fdas_emu_convolve_tc(const float* spec, int64_t nb, double zmax, double zste
                         pair_powers(Ar, Br, Ai, Bi, &Pp, &Pm);
                         const int64_t r = tile * kTileR + kSubR * s + 8 * bg + e;
                         store(jplus0 + p, r, Pp);
-                        store(npair - 1 - p, r, Pm);
+                        store(jminus0 - p, r, Pm);
                     }
         }
+    }
     }
     // block maxima of the values as stored, rounded toward +inf to bf16
     for (int j = 0; j < nz; ++j)

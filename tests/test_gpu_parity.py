@@ -433,16 +433,18 @@ def test_blockmax_plane_and_prefilter_equivalence(fdas, torch_, precision):
 
 
 @pytest.mark.parametrize("precision", ["bf16_tc", "bf16_tc_plane16"])
-@pytest.mark.parametrize("zmax", [4.0, 10.0, 20.0, 52.0])
+@pytest.mark.parametrize("zmax", [4.0, 10.0, 20.0, 52.0, 7.5, 110.0, 140.0])
 def test_tensor_core_path_odd_banks(fdas, torch_, oracle, precision, zmax):
-    """K2-TC with banks whose pair count is not a multiple of 8 (4, 10, 20, 52 pairs: a chunk with
-    padded pairs, fewer chunks than epilogue warpgroups, two groups with a ragged last chunk): the rows
-    of the padded pairs lie outside the plane and must be clipped by the TMA stores (plane and
-    block-max side plane), every real row must be written, and the candidates must match."""
+    """K2-TC with banks whose pair count is not a multiple of 32 (4, 10, 20, 52 pairs: a ragged last
+    lane quarter, stored through the tail tensor map), an even bank without a z = 0 row (zmax 7.5: 8
+    pairs), 110 pairs (all four lane quarters, single-buffered staging) and 140 pairs (two launches of 96
+    and 44): no row outside the plane may be touched (canaries), every real row must be written, the
+    block-max side plane must be exact and the candidates must match."""
     torch = torch_
     n = 1 << 14                                   # nbins = 8192: 64 tiles over <= 148 CTAs
     plan = fdas.Plan(n, 64e-6, zmax, 1.0, 2048, precision)
     nb, nz = plan.info.nbins, plan.info.nz
+    assert nz == int(2 * zmax) + 1
     rng = np.random.default_rng(int(zmax))
     w = (rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)
     for k in (0, 127, 128, 129, 5000, nb - 1):
@@ -482,9 +484,9 @@ def test_tensor_core_path_odd_banks(fdas, torch_, oracle, precision, zmax):
 
 def test_tensor_core_path_unsupported_banks(fdas, torch_):
     """Banks the tensor-core kernel cannot hold are refused at plan time (no silent fallback):
-    nz = 1 (no conjugate pairs) and a half-bin bank whose image does not fit the CTA's shared memory;
-    the FFT path takes the same plans."""
-    for zmax, zstep in ((0.0, 1.0), (96.0, 0.5)):
+    nz = 1 (no conjugate pairs) and templates of more than 255 taps (zmax 260: h = 160; the bank images
+    would not fit the tensor-memory columns beside the accumulators); the FFT path takes the same plans."""
+    for zmax, zstep in ((0.0, 1.0), (260.0, 1.0)):
         with pytest.raises(fdas.FdasError) as ei:
             fdas.Plan(1 << 14, 64e-6, zmax, zstep, 2048, "bf16_tc")
         assert ei.value.status == fdas.FDAS_EUNSUPPORTED
@@ -811,16 +813,17 @@ def test_two_streams_share_one_plan(fdas, torch_):
 
 # ----------------------------------------------------- other template banks
 @pytest.mark.parametrize("precision", ALL_PREC)
-@pytest.mark.parametrize("zstep", [0.5, 2.0])
-def test_other_z_spacings_full_parity(fdas, torch_, oracle, precision, zstep):
-    """Half-bin and coarse banks (zmax 16, zstep 0.5 -> 65 templates, zstep 2 -> 17): the plane
-    element by element against the oracle's bank of the same spacing, and the harmonic sums (whose
-    rows are idx(k z_j) = (k z_j + zmax)/zstep) against the oracle's candidates on the GPU's plane."""
+@pytest.mark.parametrize("zmax,zstep", [(16.0, 0.5), (16.0, 2.0), (96.0, 0.5)])
+def test_other_z_spacings_full_parity(fdas, torch_, oracle, precision, zmax, zstep):
+    """Half-bin and coarse banks (zmax 16, zstep 0.5 -> 65 templates, zstep 2 -> 17; the paper's zmax 96
+    at half-bin spacing -> 385 templates = 192 conjugate pairs, two K2-TC launches): the plane element by
+    element against the oracle's bank of the same spacing, and the harmonic sums (whose rows are
+    idx(k z_j) = (k z_j + zmax)/zstep) against the oracle's candidates on the GPU's plane."""
     torch = torch_
     n = 1 << 16
-    plan = fdas.Plan(n, 64e-6, 16.0, zstep, 2048, precision)
+    plan = fdas.Plan(n, 64e-6, zmax, zstep, 2048, precision)
     nb, nz = plan.info.nbins, plan.info.nz
-    assert nz == int(round(32 / zstep)) + 1
+    assert nz == int(round(2 * zmax / zstep)) + 1
     rng = np.random.default_rng(int(10 * zstep))
     w = (rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)
     for k, a in ((3000, 9.0), (6000, 9.0), (9000, 6.0), (12000, 6.0), (nb - 1, 8.0), (0, 8.0)):
@@ -835,7 +838,7 @@ def test_other_z_spacings_full_parity(fdas, torch_, oracle, precision, zstep):
     torch.cuda.synchronize()
     Pg = d_plane.float().cpu().numpy().astype(np.float64)
     assert not np.isnan(Pg).any()
-    bank = oracle.template_bank(16.0, zstep)
+    bank = oracle.template_bank(zmax, zstep)
     assert bank.shape[0] == nz and np.abs(plan.templates_host() - bank).max() < 1e-12
     P = oracle.plane(w, bank)
     ps = PlaneStats(precision)
@@ -847,7 +850,7 @@ def test_other_z_spacings_full_parity(fdas, torch_, oracle, precision, zstep):
     stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * Pg.max(), None, s_at, margin,
                                strict_rel=1e-5)
     assert stats["only_gpu"] + stats["only_orc"] <= 2 and stats["common"] > 50, stats
-    record_stats(f"zstep{zstep}_{precision}", {**ps.summary(P.max()), **stats})
+    record_stats(f"zmax{zmax:g}_zstep{zstep}_{precision}", {**ps.summary(P.max()), **stats})
 
 
 # ------------------------------------- neighbour-maximised harmonic sums

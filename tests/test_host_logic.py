@@ -144,12 +144,13 @@ def test_emulated_k2_matches_the_oracle_plane(emu, oracle, zmax, nb):
         assert np.abs(out - P).max() <= tol * P.max(), (prec, np.abs(out - P).max() / P.max())
 
 
-@pytest.mark.parametrize("zmax,nb", [(16.0, 1152), (96.0, 640), (10.0, 384), (52.0, 256)])
+@pytest.mark.parametrize("zmax,nb", [(16.0, 1152), (96.0, 640), (10.0, 384), (52.0, 256), (140.0, 256)])
 def test_emulated_k2_tc_matches_the_oracle_plane(emu, oracle, zmax, nb):
-    """K2-TC (tensor-core contraction) stepped on the CPU: same shared-memory image, UMMA descriptor
-    encodings (sliding-window A operand with LBO = SBO = 128 B, packed bank B), issue order, TMEM
-    column map and pair epilogue as fdas_convolve_tc.cu; tcgen05.mma replaced by a descriptor walker.
-    Several tiles, both edges (zero fill below bin 0 and above nb), strong lines at the edges."""
+    """K2-TC (tensor-core contraction) stepped on the CPU: same bank image in (emulated) tensor memory,
+    interleaved re/im sliding-window image in shared memory with its UMMA descriptor (SBO = 128 B,
+    LBO = 256 B), issue order, TMEM column map and pair epilogue as fdas_convolve_tc.cu; tcgen05.mma
+    replaced by an operand walker.  Several tiles, both edges (zero fill below bin 0 and above nb), strong
+    lines at the edges; zmax = 140 (140 pairs) takes two launches of 96 and 44 pairs."""
     rng = np.random.default_rng(5)
     w = ((rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)).astype(np.complex64)
     w[nb // 3] += 15.0
