@@ -767,6 +767,14 @@ def run_batch(args):
     return 0
 
 
+def spawn_command(ngpus, argv):
+    """`python bench.py --gpus N ...` without a launcher: one rank per GPU on this node through
+    torch.distributed.run (the ranks then find WORLD_SIZE / RANK / LOCAL_RANK in their environment)."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={ngpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(29500 + os.getpid() % 2000),
+            os.path.abspath(__file__)] + list(argv)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -800,10 +808,8 @@ def main():
     if args.impl == "cuda" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # launched plainly with --gpus N: start the N ranks ourselves, one per GPU (DM-trial replicas)
         import subprocess
-        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
-               "--master-addr", "127.0.0.1", "--master-port", str(29500 + os.getpid() % 2000),
-               os.path.abspath(__file__)] + sys.argv[1:]
-        return subprocess.call(cmd, env=dict(os.environ, NCCL_DEBUG=os.environ.get("NCCL_DEBUG", "INFO")))
+        return subprocess.call(spawn_command(args.gpus, sys.argv[1:]),
+                               env=dict(os.environ, NCCL_DEBUG=os.environ.get("NCCL_DEBUG", "INFO")))
     if args.impl == "reference":
         if args.workload in ("batched", "survey"):
             args.workload = "ska"      # the oracle's per-trial rate is the same for every member

@@ -12,20 +12,12 @@
 // variants only change the storage format of w, Khat (and optionally P) -- reading A10.
 #include <cuda_bf16.h>
 
-#include <cstdlib>
-
 #include "fdas_fft_core.cuh"
 #include "fdas_kernels.h"
 
 namespace fdas {
 
-constexpr int kDefaultOcc = 3;
-// Where the next template is prefetched: 0 = between the exchange-2 stores and their barrier (the x
-// registers are dead there), 1 = after pass 3 (keeps the 16/32 K registers out of pass 3).
-#ifndef FDAS_K2_PREFETCH_AT
-#define FDAS_K2_PREFETCH_AT 1
-#endif
-constexpr int kPrefetchAt = FDAS_K2_PREFETCH_AT;  // resident CTAs per SM the kernel is compiled for (FDAS_K2_OCC=3|4 overrides)
+constexpr int kCtasPerSm = 3;   // resident CTAs per SM the kernel is compiled for (3 beat 4: profiles/r01c)
 
 // First half of the inverse FFT: up to the write of exchange 2 (x is dead afterwards).
 __device__ __forceinline__ void ifft2048_head(float2 (&x)[16], float2* X1, float2* X2, const int tid,
@@ -50,10 +42,10 @@ __device__ __forceinline__ void ifft2048(float2 (&x)[16], float2* X1, float2* X2
     ifft2048_tail(x, X2, tid, tw2);
 }
 
-// 128-bit read-only loads of the next template, issued as volatile asm between the exchange-2
-// stores and the barrier (where the 32 x registers are dead): the compiler can neither sink them to
-// the point of use nor hoist them into the register-heavy passes, so the L2 latency is hidden by
-// pass 3 and the epilogue at the cost of 16 (bf16) / 32 (fp32) registers over that span only.
+// 128-bit read-only loads of the next template, issued as volatile asm after pass 3: the compiler can
+// neither sink them to the point of use nor hoist them into the register-heavy passes, so the L2 latency
+// is hidden by the epilogue (powers, stores, block maxima) at the cost of 16 (bf16) / 32 (fp32) registers
+// over that span only.
 __device__ __forceinline__ uint4 ldg_v4(const void* ptr) {
     uint4 v;
     // plain ld.global (not .nc): a non-coherent load may legally be moved across bar.sync
@@ -188,12 +180,8 @@ __global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvPara
         }
         ifft2048_head(x, X1, X2, tid, tw1);
         bank += NK * 128;
-        if (kPrefetchAt == 0 && j + 1 < jend) {
-#pragma unroll
-            for (int c = 0; c < NK; ++c) K[c] = ldg_v4(bank + c * 128);
-        }
         ifft2048_tail(x, X2, tid, tw2);
-        if (kPrefetchAt == 1 && j + 1 < jend) {
+        if (j + 1 < jend) {   // the next template, fetched after pass 3 (keeps its registers out of the passes)
 #pragma unroll
             for (int c = 0; c < NK; ++c) K[c] = ldg_v4(bank + c * 128);
         }
@@ -203,32 +191,18 @@ __global__ void __launch_bounds__(kThreads, MINB) convolve_kernel(const ConvPara
     }
 }
 
-int convolve_ctas_per_sm() {
-    static int occ = [] {
-        const char* e = std::getenv("FDAS_K2_OCC");
-        const int v = e ? std::atoi(e) : 0;
-        return (v == 3 || v == 4) ? v : kDefaultOcc;
-    }();
-    return occ;
-}
-
-template <int MINB>
-static cudaError_t launch_occ(int precision, const ConvParams& p, dim3 grid, cudaStream_t st) {
-    const dim3 block(kThreads);
-    switch (precision) {
-        case FDAS_FP32: convolve_kernel<FDAS_FP32, MINB><<<grid, block, 0, st>>>(p); break;
-        case FDAS_BF16: convolve_kernel<FDAS_BF16, MINB><<<grid, block, 0, st>>>(p); break;
-        case FDAS_BF16_PLANE16: convolve_kernel<FDAS_BF16_PLANE16, MINB><<<grid, block, 0, st>>>(p); break;
-        default: return cudaErrorInvalidValue;
-    }
-    return cudaGetLastError();
-}
+int convolve_ctas_per_sm() { return kCtasPerSm; }
 
 cudaError_t launch_convolve(int precision, const ConvParams& p, int64_t nseg, int nsplit,
                             cudaStream_t st) {
-    const dim3 grid((unsigned)nseg, (unsigned)nsplit);
-    return convolve_ctas_per_sm() == 4 ? launch_occ<4>(precision, p, grid, st)
-                                       : launch_occ<3>(precision, p, grid, st);
+    const dim3 grid((unsigned)nseg, (unsigned)nsplit), block(kThreads);
+    switch (precision) {
+        case FDAS_FP32: convolve_kernel<FDAS_FP32, kCtasPerSm><<<grid, block, 0, st>>>(p); break;
+        case FDAS_BF16: convolve_kernel<FDAS_BF16, kCtasPerSm><<<grid, block, 0, st>>>(p); break;
+        case FDAS_BF16_PLANE16: convolve_kernel<FDAS_BF16_PLANE16, kCtasPerSm><<<grid, block, 0, st>>>(p); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
 }
 
 }  // namespace fdas

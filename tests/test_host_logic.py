@@ -224,3 +224,19 @@ def test_gloo_world2_sharding(tmp_path):
     assert res["t_max"] == 2.0
     assert res["allc"] == [[str(t), (t * 3) % 5] for t in sorted(range(7), key=str)] or \
         dict((int(k), v) for k, v in res["allc"]) == {t: (t * 3) % 5 for t in range(7)}
+
+
+def test_bench_starts_its_own_ranks_and_shares_one_workload_string():
+    """`bench.py --gpus N` launched plainly re-executes itself under torch.distributed.run with N ranks;
+    both arms describe the workload with the same string; the DRAM traffic comes from profiles/."""
+    sys.path.insert(0, ROOT)
+    import bench
+    cmd = bench.spawn_command(4, ["--gpus", "4", "--steps", "7"])
+    assert cmd[1:3] == ["-m", "torch.distributed.run"] and "--nproc-per-node=4" in cmd and "127.0.0.1" in cmd
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "7"] and cmd[-5].endswith("bench.py")
+    wl = inputs.ska()
+    assert "N=9375000" in bench.workload_string(wl) and "nz=193" in bench.workload_string(wl)
+    t = bench.ncu_traffic("ska", "bf16_tc")
+    assert t is not None and t["file"].startswith("profiles/") and 3.2e9 < t["traffic"] < 3.6e9
+    assert "convolve_tc_kernel" in t["kernel"] and t["commit"]
+    assert bench.ncu_traffic("tiny", "bf16_tc") is None
