@@ -53,7 +53,7 @@ enum {
     FDAS_ECUDA = 3,        /* a CUDA runtime call or kernel launch failed */
     FDAS_ECUFFT = 4,       /* a cuFFT call failed */
     FDAS_EOVERFLOW = 5,    /* more candidates than capacity (host-side helper only) */
-    FDAS_EUNSUPPORTED = 6  /* valid request this build does not implement (e.g. seg_len != 2048, nfft > 2^30) */
+    FDAS_EUNSUPPORTED = 6  /* valid request this build does not implement (e.g. seg_len not in {1024, 2048, 4096}, nfft > 2^30) */
 };
 
 typedef struct {
@@ -93,8 +93,10 @@ typedef struct {
  *   N        samples per time series (>= 2*seg_len); tsamp  sampling time in seconds (> 0; units only)
  *   zmax     largest |z| searched, in Fourier bins of drift over the observation (>= 0)
  *   zstep    template spacing in z (> 0); 2*zmax/zstep must be an integer (nz = that + 1 <= 32767)
- *   seg_len  L; this build supports 2048 only (FDAS_EUNSUPPORTED otherwise; FDAS_EARG if not a
- *            power of two or if V = L - 2h <= 0)
+ *   seg_len  L, the overlap-save segment length in complex bins: 1024, 2048 or 4096 (another power of two:
+ *            FDAS_EUNSUPPORTED; FDAS_EARG if not a power of two or if V = L - 2h <= 0).  SURVEY.md 8(f) #3:
+ *            the flop count per plane point, 5 L log2(L) / (L - 2h), has its minimum near 1024-2048 for the
+ *            129 taps of the zmax = 96 bank.
  *   precision  FDAS_FP32 | FDAS_BF16 | FDAS_BF16_PLANE16 | FDAS_BF16_TC | FDAS_BF16_TC_PLANE16
  * On success *out receives the handle (release with fdas_destroy).
  */

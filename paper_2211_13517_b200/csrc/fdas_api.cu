@@ -64,7 +64,7 @@ static int derive_info(int64_t N, double tsamp, double zmax, double zstep, int s
     o->plane_elem_bytes = fdas_plane16(precision) ? 2 : 4;
     o->precision = precision;
     o->zmax = zmax; o->zstep = zstep; o->tsamp = tsamp; o->tobs = (double)nfft * tsamp;
-    if (seg_len != kL) return FDAS_EUNSUPPORTED;
+    if (!seg_len_supported(seg_len)) return FDAS_EUNSUPPORTED;
     return FDAS_OK;
 }
 
@@ -106,7 +106,7 @@ static int build_plan(fdas_plan_s* p) {
         CU(cudaMemcpy(p->d_bank, packed.data(), packed.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
     }
     std::vector<float> t1, t2;
-    build_twiddles(&t1, &t2);
+    build_twiddles(in.seg_len, &t1, &t2);
     CU(cudaMalloc(&p->d_tw1, t1.size() * sizeof(float)));
     CU(cudaMalloc(&p->d_tw2, t2.size() * sizeof(float)));
     CU(cudaMemcpy(p->d_tw1, t1.data(), t1.size() * sizeof(float), cudaMemcpyHostToDevice));
@@ -137,7 +137,7 @@ static int build_plan(fdas_plan_s* p) {
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
     p->nsm = nsm;
-    const int64_t slots = (int64_t)convolve_ctas_per_sm() * nsm;
+    const int64_t slots = (int64_t)convolve_ctas_per_sm(in.seg_len) * nsm;
     int nsplit = 1;
     if (in.nseg < 4 * slots) nsplit = (int)std::min<int64_t>(in.nz, (4 * slots + in.nseg - 1) / in.nseg);
     p->nsplit = nsplit;
@@ -181,7 +181,7 @@ int fdas_enqueue_convolve(fdas_plan_s* plan, const void* d_spec, void* d_plane,
     c.nbins = plan->info.nbins; c.pitch = plan->info.plane_pitch;
     c.nz = plan->info.nz; c.h = plan->info.halfwidth; c.V = plan->info.valid;
     c.maxplane = d_maxplane; c.mpitch = plan->info.nbins / 8;
-    CU(launch_convolve(plan->info.precision, c, plan->info.nseg, plan->nsplit, st));
+    CU(launch_convolve(plan->info.precision, plan->info.seg_len, c, plan->info.nseg, plan->nsplit, st));
     plan->launches += 1;
     return FDAS_OK;
 }
@@ -386,7 +386,7 @@ const char* fdas_strerror(int status) {
         case FDAS_ECUDA: return "CUDA error";
         case FDAS_ECUFFT: return "cuFFT error";
         case FDAS_EOVERFLOW: return "more candidates than capacity";
-        case FDAS_EUNSUPPORTED: return "unsupported configuration (this build: seg_len = 2048 only)";
+        case FDAS_EUNSUPPORTED: return "unsupported configuration (this build: seg_len = 1024, 2048 or 4096; nfft <= 2^30)";
         default: return "unknown status";
     }
 }

@@ -1,17 +1,18 @@
-// fdas_fft_core.cuh -- per-thread building blocks of the 2048-point segment FFT used by the fused
-// convolution kernel (fdas_convolve.cu).  Every function is __host__ __device__ so that the exact
+// fdas_fft_core.cuh -- per-thread building blocks of the L-point segment FFT (L = 1024, 2048, 4096) used by
+// the fused convolution kernel (fdas_convolve.cu).  Every function is __host__ __device__ so that the exact
 // index arithmetic and exchange-buffer layouts can also be stepped on the CPU, thread by thread, by
-// the test-only emulator (fdas_emu.cu) -- there is no GPU on the development box.
+// the test-only emulator (tests/emu/fdas_emu.cu) -- there is no GPU on the development box.
 //
-// Inverse transform y[n] = sum_p Y[p] exp(+2 pi i n p / 2048) (unnormalised), 128 threads x 16 points,
-// three register passes (16 x 16 x 8) with two shared-memory exchanges:
-//   p = k0 + 128 k1            k0 = 8 k0a + k0b in [0,128), k1 in [0,16)
-//   n = n1 + 16 n2a + 256 n2b  n1, n2a in [0,16), n2b in [0,8)
-//   pass 1 (thread k0)        A[n1]  = w2048^(n1 k0) * sum_k1 Y[k0+128 k1] w16^(n1 k1)
-//   pass 2 (thread n1*8+k0b)  C[n2a] = sum_k0a A[n1][8 k0a+k0b] w16^(n2a k0a)
-//   pass 3 (thread t, m = 2t+e, n1 = m%16, n2a = m/16 = t/8)
-//                             y[m + 256 n2b] = sum_k0b w128^(n2a k0b) C[m][k0b] w8^(n2b k0b)
-// with wN^(x) = exp(+2 pi i x / N).  Convolution stage of PAPER.md:23 (section 2.2).
+// Inverse transform y[n] = sum_p Y[p] exp(+2 pi i n p / L) (unnormalised), T = L/16 threads x 16 points,
+// three register passes (16 x Rb x Ra, L = 16 Ra Rb) with two shared-memory exchanges:
+//   p = k0 + T k1               k0 = kA + Ra kB in [0,T), kA in [0,Ra), kB in [0,Rb), k1 in [0,16)
+//   n = n1 + 16 (nB + Rb nA)    n1 in [0,16), nB in [0,Rb), nA in [0,Ra)
+//   pass 1 (thread tid = kB + Rb kA)   A[n1]  = wL^(n1 k0) * sum_k1 Y[k0 + T k1] w16^(n1 k1)
+//   pass 2 (row (n1, kA))              C[nB]  = sum_kB A[n1][kA + Ra kB] wRb^(nB kB)
+//   pass 3 (row (n1, nB))              y[n1 + 16 nB + 16 Rb nA] = sum_kA wT^(nB kA) C[kA][nB] wRa^(nA kA)
+// with wN^(x) = exp(+2 pi i x / N).  A pass of radix 16 is one 16-point DFT per thread, a pass of radix 8
+// two 8-point DFTs per thread (rows of 16 = two groups of 8).  L = 1024: Rb = Ra = 8; 2048: Rb = 16,
+// Ra = 8; 4096: Rb = Ra = 16.  Convolution stage of PAPER.md:23 (section 2.2).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -19,11 +20,26 @@
 
 namespace fdas {
 
-constexpr int kL = 2048;        // segment length (complex bins)
-constexpr int kThreads = 128;   // threads per segment
 constexpr int kPts = 16;        // points per thread
 constexpr int kRowStride = 18;  // float2 per exchange-buffer row: 16 data + 2 pad (144 B: LDS.128 conflict-free)
-constexpr int kXbufElems = kThreads * kRowStride;  // float2 elements per exchange buffer (18,432 B)
+
+// Geometry of the L-point segment transform.
+template <int L>
+struct SegGeom {
+    static_assert(L == 1024 || L == 2048 || L == 4096, "segment lengths built: 1024, 2048, 4096");
+    static constexpr int kL = L;
+    static constexpr int T = L / 16;                   // threads per segment
+    static constexpr int Rb = (L == 1024) ? 8 : 16;    // radix of pass 2 (over kB)
+    static constexpr int Ra = T / Rb;                  // radix of pass 3 (over kA): 8, 8, 16
+    static constexpr int RowsPerN1 = T / 16;           // exchange-1 rows that share one n1
+    static constexpr int NTw2 = Ra - 1;                // pass-3 twiddles per thread
+    static constexpr int OutStride = 16 * Rb;          // thread v holds y[m + OutStride nA]
+    static constexpr int XbufElems = T * kRowStride;   // float2 elements per exchange buffer
+    // The input bin k0 of thread tid (tid = kB + Rb kA holds Y[k0 + T k1], k0 = kA + Ra kB): with this
+    // assignment the 16 (8) threads that feed one pass-2 row are consecutive, so a half-warp writes one
+    // contiguous 128-byte row segment in both exchanges.
+    static __host__ __device__ constexpr int k0_of(int tid) { return tid / Rb + Ra * (tid % Rb); }
+};
 
 // ---- complex arithmetic on (re, im) register pairs.
 // On sm_100a every operation below is ONE packed instruction (FADD2 / FMUL2 / FFMA2, PTX *.f32x2):
@@ -207,19 +223,21 @@ FDAS_HD void dft8_inv(float2 (&x)[16], const int o) {
     for (int i = 0; i < 8; ++i) x[o + i] = y[i];
 }
 
-// ---- pass 1: thread k0 = tid holds x[k1] = Y[tid + 128 k1];  tw1[n1-1] = w2048^(n1 * tid)
+// ---- pass 1: thread tid holds x[k1] = Y[k0_of(tid) + T k1];  tw1[n1-1] = wL^(n1 * k0_of(tid))
 FDAS_HD void pass1(float2 (&x)[16], const float2 (&tw1)[15]) {
     dft16_inv(x);
 #pragma unroll
     for (int n1 = 1; n1 < 16; ++n1) x[n1] = cmul(x[n1], tw1[n1 - 1]);
 }
 
-// Exchange 1 write: element (n1, k0) goes to row n1*8 + k0b, column k0a (16 x 64-bit stores;
-// a half-warp covers all 32 banks exactly once).
+// Exchange 1 write: element (n1, kA, kB) of thread tid = kB + Rb kA goes to row n1 (T/16) + tid/16,
+// column tid % 16 -- for Rb = 16 that is row (n1, kA), column kB; for Rb = 8 row (n1, kA/2), column
+// 8 (kA % 2) + kB.  16 x 64-bit stores; a half-warp writes one contiguous 128-byte row segment.
+template <int L>
 FDAS_HD void x1_store(float2* X1, const int tid, const float2 (&x)[16]) {
-    const int base = (tid & 7) * kRowStride + (tid >> 3);
+    const int base = (tid >> 4) * kRowStride + (tid & 15);
 #pragma unroll
-    for (int n1 = 0; n1 < 16; ++n1) X1[base + n1 * 8 * kRowStride] = x[n1];
+    for (int n1 = 0; n1 < 16; ++n1) X1[base + n1 * SegGeom<L>::RowsPerN1 * kRowStride] = x[n1];
 }
 
 // Row read used after both exchanges: thread tid reads its own 16-element row with 8 x 128-bit
@@ -234,28 +252,66 @@ FDAS_HD void xrow_load(const float2* X, const int tid, float2 (&x)[16]) {
     }
 }
 
-// ---- pass 2: thread tid = n1*8 + k0b holds x[k0a]; result x[n2a]
-FDAS_HD void pass2(float2 (&x)[16]) { dft16_inv(x); }
-
-// Exchange 2 write: element (m = n1 + 16 n2a, k0b) goes to row m/2, column (m%2)*8 + k0b
-// (a half-warp writes one contiguous 128-byte row segment).
-FDAS_HD void x2_store(float2* X2, const int tid, const float2 (&x)[16]) {
-    const int n1 = tid >> 3, k0b = tid & 7;
-    const int base = (n1 >> 1) * kRowStride + (n1 & 1) * 8 + k0b;
-#pragma unroll
-    for (int n2a = 0; n2a < 16; ++n2a) X2[base + n2a * 8 * kRowStride] = x[n2a];
+// ---- pass 2: thread u = n1 (T/16) + w holds row (n1, w).  Rb = 16: x[kB] of kA = w -> x[nB];
+// Rb = 8: x[8 e + kB] of kA = 2 w + e -> x[8 e + nB].
+template <int L>
+FDAS_HD void pass2(float2 (&x)[16]) {
+    if constexpr (SegGeom<L>::Rb == 16) {
+        dft16_inv(x);
+    } else {
+        dft8_inv(x, 0);
+        dft8_inv(x, 8);
+    }
 }
 
-// ---- pass 3: thread tid holds x[e*8 + k0b] for m = 2 tid + e;  tw2[k0b-1] = w128^((tid/8) * k0b)
-// result x[e*8 + n2b] = y[2 tid + e + 256 n2b]
-FDAS_HD void pass3(float2 (&x)[16], const float2 (&tw2)[7]) {
+// Exchange 2 write by thread u = n1 (T/16) + w: element (n1, kA, nB) goes to the pass-3 row of (n1, nB),
+// column kA (Ra = 16: row n1 + 16 nB) or column 8 (n1 % 2) + kA (Ra = 8: row n1/2 + 8 nB, shared by
+// n1 = 2a, 2a+1).  A half-warp (a quarter-warp of the 128-bit stores of L = 1024) writes one contiguous
+// 128-byte row segment.
+template <int L>
+FDAS_HD void x2_store(float2* X2, const int u, const float2 (&x)[16]) {
+    typedef SegGeom<L> G;
+    const int n1 = u / G::RowsPerN1, w = u % G::RowsPerN1;
+    if constexpr (G::Ra == 16) {
+        const int base = n1 * kRowStride + w;
 #pragma unroll
-    for (int k = 1; k < 8; ++k) {
-        x[k] = cmul(x[k], tw2[k - 1]);
-        x[8 + k] = cmul(x[8 + k], tw2[k - 1]);
+        for (int nB = 0; nB < 16; ++nB) X2[base + nB * 16 * kRowStride] = x[nB];
+    } else if constexpr (G::Rb == 16) {
+        const int base = (n1 >> 1) * kRowStride + (n1 & 1) * 8 + w;
+#pragma unroll
+        for (int nB = 0; nB < 16; ++nB) X2[base + nB * 8 * kRowStride] = x[nB];
+    } else {
+        const int base = (n1 >> 1) * kRowStride + (n1 & 1) * 8 + 2 * w;     // kA = 2 w, 2 w + 1: one 16-byte store
+#pragma unroll
+        for (int nB = 0; nB < 8; ++nB)
+            *reinterpret_cast<float4*>(X2 + base + nB * 8 * kRowStride) = make_float4(x[nB].x, x[nB].y, x[8 + nB].x, x[8 + nB].y);
     }
-    dft8_inv(x, 0);
-    dft8_inv(x, 8);
+}
+
+// ---- pass 3: thread v holds its row of kA values; tw2[kA-1] = wT^(nB kA), nB = v / 16 (Ra = 16) or v / 8.
+// Ra = 16: x[kA] of (n1, nB) = (v % 16, v / 16) -> x[nA] = y[v + 256 nA].
+// Ra = 8:  x[8 e + kA] of n1 = 2 (v % 8) + e, nB = v / 8 -> x[8 e + nA] = y[2 v + e + 16 Rb nA].
+template <int L>
+FDAS_HD void pass3(float2 (&x)[16], const float2 (&tw2)[SegGeom<L>::NTw2]) {
+    if constexpr (SegGeom<L>::Ra == 16) {
+#pragma unroll
+        for (int k = 1; k < 16; ++k) x[k] = cmul(x[k], tw2[k - 1]);
+        dft16_inv(x);
+    } else {
+#pragma unroll
+        for (int k = 1; k < 8; ++k) {
+            x[k] = cmul(x[k], tw2[k - 1]);
+            x[8 + k] = cmul(x[8 + k], tw2[k - 1]);
+        }
+        dft8_inv(x, 0);
+        dft8_inv(x, 8);
+    }
+}
+// Output index of x[i] after pass 3 in thread v.
+template <int L>
+FDAS_HD int out_index(const int v, const int i) {
+    typedef SegGeom<L> G;
+    return G::Ra == 16 ? v + G::OutStride * i : 2 * v + (i >> 3) + G::OutStride * (i & 7);
 }
 
 // Round-to-nearest-even float -> bfloat16 bits and back (storage format of the bf16 path,

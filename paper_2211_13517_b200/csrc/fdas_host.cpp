@@ -132,15 +132,30 @@ void build_bank(double zmax, double zstep, int nz, int h, int L, Bank* bank) {
     }
 }
 
+bool seg_len_supported(int L) { return L == 1024 || L == 2048 || L == 4096; }
+
+// (Rb, Ra) of fdas_fft_core.cuh SegGeom<L>: L = 16 Ra Rb.
+static void seg_radices(int L, int* Rb, int* Ra) {
+    *Rb = (L == 1024) ? 8 : 16;
+    *Ra = (L / 16) / *Rb;
+}
+
+int seg_k0_of(int L, int tid) {
+    int Rb, Ra;
+    seg_radices(L, &Rb, &Ra);
+    return tid / Rb + Ra * (tid % Rb);
+}
+
 void pack_bank_fp32(const Bank& bank, std::vector<float>* out) {
-    const int L = bank.L;  // 2048: thread k0 in [0,128), k1 in [0,16)
+    const int L = bank.L, T = L / 16;
     out->assign((size_t)bank.nz * L * 2, 0.0f);
     for (int j = 0; j < bank.nz; ++j)
         for (int c = 0; c < 8; ++c)
-            for (int k0 = 0; k0 < 128; ++k0) {
-                float* w = &(*out)[(((size_t)j * 8 + c) * 128 + k0) * 4];
-                const cd a = bank.freq[(size_t)j * L + k0 + 128 * (2 * c)];
-                const cd b = bank.freq[(size_t)j * L + k0 + 128 * (2 * c + 1)];
+            for (int tid = 0; tid < T; ++tid) {
+                const int k0 = seg_k0_of(L, tid);
+                float* w = &(*out)[(((size_t)j * 8 + c) * T + tid) * 4];
+                const cd a = bank.freq[(size_t)j * L + k0 + T * (2 * c)];
+                const cd b = bank.freq[(size_t)j * L + k0 + T * (2 * c + 1)];
                 w[0] = (float)a.real(); w[1] = (float)a.imag();
                 w[2] = (float)b.real(); w[3] = (float)b.imag();
             }
@@ -154,16 +169,18 @@ static uint32_t bf16_rne(float f) {
 }
 
 void pack_bank_bf16(const Bank& bank, std::vector<uint32_t>* out) {
-    const int L = bank.L;
+    const int L = bank.L, T = L / 16;
     out->assign((size_t)bank.nz * L, 0u);
     for (int j = 0; j < bank.nz; ++j)
         for (int c = 0; c < 4; ++c)
-            for (int k0 = 0; k0 < 128; ++k0)
+            for (int tid = 0; tid < T; ++tid) {
+                const int k0 = seg_k0_of(L, tid);
                 for (int q = 0; q < 4; ++q) {
-                    const cd a = bank.freq[(size_t)j * L + k0 + 128 * (4 * c + q)];
-                    (*out)[(((size_t)j * 4 + c) * 128 + k0) * 4 + q] =
+                    const cd a = bank.freq[(size_t)j * L + k0 + T * (4 * c + q)];
+                    (*out)[(((size_t)j * 4 + c) * T + tid) * 4 + q] =
                         bf16_rne((float)a.real()) | (bf16_rne((float)a.imag()) << 16);
                 }
+            }
 }
 
 bool tc_geometry(int nz, int h, TcGeom* g) {
@@ -195,20 +212,23 @@ void pack_bank_tc(const Bank& bank, const TcGeom& g, std::vector<uint32_t>* out,
     if (asym) *asym = worst;
 }
 
-void build_twiddles(std::vector<float>* tw1, std::vector<float>* tw2) {
-    tw1->assign(128 * 15 * 2, 0.0f);
-    for (int k0 = 0; k0 < 128; ++k0)
+void build_twiddles(int L, std::vector<float>* tw1, std::vector<float>* tw2) {
+    const int T = L / 16;
+    int Rb, Ra;
+    seg_radices(L, &Rb, &Ra);
+    tw1->assign((size_t)T * 15 * 2, 0.0f);
+    for (int tid = 0; tid < T; ++tid)
         for (int n1 = 1; n1 < 16; ++n1) {
-            const double ang = 2.0 * kPi * (double)((n1 * k0) % 2048) / 2048.0;
-            (*tw1)[(k0 * 15 + n1 - 1) * 2 + 0] = (float)std::cos(ang);
-            (*tw1)[(k0 * 15 + n1 - 1) * 2 + 1] = (float)std::sin(ang);
+            const double ang = 2.0 * kPi * (double)((n1 * seg_k0_of(L, tid)) % L) / (double)L;
+            (*tw1)[(tid * 15 + n1 - 1) * 2 + 0] = (float)std::cos(ang);
+            (*tw1)[(tid * 15 + n1 - 1) * 2 + 1] = (float)std::sin(ang);
         }
-    tw2->assign(16 * 7 * 2, 0.0f);
-    for (int q = 0; q < 16; ++q)
-        for (int k = 1; k < 8; ++k) {
-            const double ang = 2.0 * kPi * (double)((q * k) % 128) / 128.0;
-            (*tw2)[(q * 7 + k - 1) * 2 + 0] = (float)std::cos(ang);
-            (*tw2)[(q * 7 + k - 1) * 2 + 1] = (float)std::sin(ang);
+    tw2->assign((size_t)Rb * (Ra - 1) * 2, 0.0f);
+    for (int q = 0; q < Rb; ++q)
+        for (int k = 1; k < Ra; ++k) {
+            const double ang = 2.0 * kPi * (double)((q * k) % T) / (double)T;
+            (*tw2)[(q * (Ra - 1) + k - 1) * 2 + 0] = (float)std::cos(ang);
+            (*tw2)[(q * (Ra - 1) + k - 1) * 2 + 1] = (float)std::sin(ang);
         }
 }
 

@@ -30,9 +30,14 @@ void build_bank(double zmax, double zstep, int nz, int h, int L, Bank* bank);
 // In-place iterative radix-2 FFT (sign = -1 forward, +1 inverse, unnormalised).
 void host_fft(cd* a, int n, int sign);
 
-// Kernel register order (see fdas_fft_core.cuh): thread k0 holds Khat[k0 + 128 k1], k1 = 0..15.
-// fp32: float4 words [nz][8][128] = {K[k0+128(2c)], K[k0+128(2c+1)]}  (re, im, re, im)
-// bf16: uint4  words [nz][4][128] = 4 complex k1 = 4c..4c+3, each (bf16 im << 16) | bf16 re
+// Segment lengths the FFT kernel is built for, and the input bin k0 of thread tid of its CTA
+// (fdas_fft_core.cuh SegGeom: T = L/16 threads, tid = kB + Rb kA holds bins k0 + T k1, k0 = kA + Ra kB).
+bool seg_len_supported(int L);
+int seg_k0_of(int L, int tid);
+
+// Kernel register order: thread tid holds Khat[k0_of(tid) + T k1], k1 = 0..15.
+// fp32: float4 words [nz][8][T] = {K[k0+T(2c)], K[k0+T(2c+1)]}  (re, im, re, im)
+// bf16: uint4  words [nz][4][T] = 4 complex k1 = 4c..4c+3, each (bf16 im << 16) | bf16 re
 void pack_bank_fp32(const Bank& bank, std::vector<float>* out);
 void pack_bank_bf16(const Bank& bank, std::vector<uint32_t>* out);
 
@@ -54,9 +59,9 @@ bool tc_geometry(int nz, int h, TcGeom* g);
 // *asym receives max |T_{j-}[m] - conj(T_{j+}[m])| over the bank (must be ~1e-16 for the pairing).
 void pack_bank_tc(const Bank& bank, const TcGeom& g, std::vector<uint32_t>* out, double* asym);
 
-// tw1[k0][n1-1] = exp(+2 pi i n1 k0 / 2048), n1 = 1..15 (128 x 15 complex fp32)
-// tw2[q][k-1]   = exp(+2 pi i q k / 128), q = 0..15, k = 1..7 (16 x 7 complex fp32)
-void build_twiddles(std::vector<float>* tw1, std::vector<float>* tw2);
+// tw1[tid][n1-1] = exp(+2 pi i n1 k0_of(tid) / L), n1 = 1..15 (T x 15 complex fp32)
+// tw2[nB][kA-1]  = exp(+2 pi i nB kA / T), nB = 0..Rb-1, kA = 1..Ra-1 (Rb x (Ra-1) complex fp32)
+void build_twiddles(int L, std::vector<float>* tw1, std::vector<float>* tw2);
 
 // Whitening block schedule (reading A3): s_0 = 1, len = clamp(2^(floor(log2 s) - 2), 32, 4096),
 // truncated at nb.

@@ -11,8 +11,8 @@ struct ConvParams {
     const void* spec;    // nbins complex: float2 (FDAS_FP32) or packed bf16x2 (re low, im high)
     void* plane;         // nz x pitch: float or bf16
     const void* bank;    // packed Khat, register order (fdas_host.h)
-    const float2* tw1;   // [128][15]
-    const float2* tw2;   // [16][7]
+    const float2* tw1;   // [T][15], T = seg_len / 16 (fdas_host.h build_twiddles)
+    const float2* tw2;   // [Rb][Ra - 1]
     int64_t nbins;
     int64_t pitch;
     int nz, h, V;
@@ -21,10 +21,11 @@ struct ConvParams {
     int64_t mpitch;      // nbins / 8
 };
 
-// K2: one CTA of 128 threads per (segment, template chunk); grid = (nseg, nsplit).
-cudaError_t launch_convolve(int precision, const ConvParams& p, int64_t nseg, int nsplit,
+// K2: one CTA of seg_len / 16 threads per (segment, template chunk); grid = (nseg, nsplit);
+// seg_len = 1024, 2048 or 4096.
+cudaError_t launch_convolve(int precision, int seg_len, const ConvParams& p, int64_t nseg, int nsplit,
                             cudaStream_t st);
-int convolve_ctas_per_sm();  // resident CTAs per SM K2 is launched for (sizes the template split)
+int convolve_ctas_per_sm(int seg_len);  // resident CTAs per SM K2 is launched for (sizes the template split)
 
 // K2-TC: the convolution stage as a dense contraction on the tensor cores (fdas_convolve_tc.cu).
 // Direct correlation y_j(r) = sum_m w[r+m] conj(T_j[m]) written as D[p][n] = sum_k A[p][k] B[n][k]

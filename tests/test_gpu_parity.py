@@ -853,6 +853,85 @@ def test_other_z_spacings_full_parity(fdas, torch_, oracle, precision, zmax, zst
     record_stats(f"zmax{zmax:g}_zstep{zstep}_{precision}", {**ps.summary(P.max()), **stats})
 
 
+# ------------------------------------------- other segment lengths (seg_len 1024 / 4096)
+FFT_PREC = ["fp32", "bf16", "bf16_plane16"]
+
+
+@pytest.mark.parametrize("precision", FFT_PREC)
+@pytest.mark.parametrize("zmax,seg_len", [(16.0, 1024), (96.0, 1024), (16.0, 4096), (96.0, 4096), (96.0, 2048)])
+def test_other_segment_lengths_full_parity(fdas, torch_, oracle, precision, zmax, seg_len):
+    """The FFT kernel at L = 1024 (16 x 8 x 8, 64 threads) and L = 4096 (16 x 16 x 16, 256 threads): plane
+    element by element against the oracle with lines on and around the seams of THIS segmentation
+    (V = L - 2h), a ragged last segment, the side plane through the harmonic sums on the GPU's own plane."""
+    torch = torch_
+    n = 1 << 16
+    plan = fdas.Plan(n, 64e-6, zmax, 1.0, seg_len, precision)
+    nb, nz, V = plan.info.nbins, plan.info.nz, plan.info.valid
+    assert plan.info.seg_len == seg_len and V == seg_len - 2 * plan.info.halfwidth
+    assert plan.info.nseg == -(-nb // V) and nb % V != 0
+    rng = np.random.default_rng(seg_len + int(zmax))
+    w = (rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)
+    for k in (0, 1, V - 1, V, V + 1, 2 * V, 5 * V - 3, nb - 1):
+        w[k] += 12.0
+    d_spec = spec_from_complex(torch, w, precision)
+    d_plane = plan.alloc_plane(); d_plane.fill_(float("nan"))
+    plan.convolve_plane(d_spec, d_plane)
+    H = 8
+    thr = fdas.thresholds_from_sigma(H, 3.5)
+    d_c, d_n = plan.alloc_cands(1 << 17)
+    plan.harmonic_sum_peaks(d_plane, H, thr, 16, d_c, d_n)
+    torch.cuda.synchronize()
+    Pg = d_plane.float().cpu().numpy().astype(np.float64)
+    assert not np.isnan(Pg).any()
+    bank = oracle.template_bank(zmax, 1.0)
+    P = oracle.plane(w, bank)
+    ps = PlaneStats(precision)
+    ps.add(Pg, P, local_amplitude(w))
+    ps.check(P.max())
+    # block-max side plane of this segmentation: bit-exact upper bounds of the stored plane
+    ptr, pitch = plan.debug_maxplane()
+    M = _device_view(torch, ptr, nz * pitch).view(nz, pitch).clone()
+    ref = d_plane.float().view(nz, pitch, 8).amax(dim=2)
+    assert torch.equal(M, ((ref.view(torch.int32) + 0xFFFF) >> 16).to(torch.int16))
+    res = plan.read_cands(d_c, d_n)
+    oc = oracle.candidates(Pg, H, thr.astype(np.float64), 16)
+    s_at, margin = oracle_margin_fn(oracle, Pg, H, 16)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, 2e-6 * Pg.max(), None, s_at, margin,
+                               strict_rel=1e-5)
+    assert stats["only_gpu"] + stats["only_orc"] <= 2 and stats["common"] > 50, stats
+    record_stats(f"seg{seg_len}_zmax{zmax:g}_{precision}", {**ps.summary(P.max()), **stats})
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+@pytest.mark.parametrize("seg_len", [1024, 4096])
+def test_medium_other_segment_lengths(fdas, torch_, oracle, medium_oracle, precision, seg_len):
+    """configs[1] end to end (547 -> 1171 / 265 segments) at the other two segment lengths: every plane
+    point and the candidate list against the oracle."""
+    import dataclasses
+    torch = torch_
+    wl0, x, orc = medium_oracle
+    wl = dataclasses.replace(wl0, seg_len=seg_len)
+    plan, d_spec, d_plane, res, thr = run_gpu(fdas, torch, wl, x, precision)
+    assert plan.info.seg_len == seg_len and plan.info.nseg == -(-plan.info.nbins // (seg_len - 128))
+    pmax = orc.P.max()
+    ps = PlaneStats(precision)
+    W = local_amplitude(orc.w)
+    for j0 in range(0, plan.info.nz, 16):
+        Pg = d_plane[j0:j0 + 16].float().cpu().numpy().astype(np.float64)
+        assert not np.isnan(Pg).any()
+        ps.add(Pg, orc.P[j0:j0 + 16], W)
+    ps.check(pmax)
+    oc = oracle.candidates(orc.P, wl.nharm, thr.astype(np.float64), wl.r_lo)
+    s_at, margin = oracle_margin_fn(oracle, orc.P, wl.nharm, wl.r_lo)
+    stats = compare_candidates(gpu_cand_dict(res.cands), oc.as_dict(), thr, TOL[precision] * pmax, REL_POW[precision],
+                               s_at, margin, strict_rel=STRICT_REL[precision])
+    if precision == "fp32":
+        assert stats["only_gpu"] + stats["only_orc"] == 0, stats
+    else:
+        assert stats["only_gpu"] + stats["only_orc"] <= 0.01 * stats["common"], stats
+    record_stats(f"medium_seg{seg_len}_{precision}", {**ps.summary(pmax), **stats})
+
+
 # ------------------------------------- neighbour-maximised harmonic sums (SURVEY.md 8(f) #2, A24)
 def nbr_thresholds(thr):
     """A caller's choice of thresholds for S': the plain T_h raised by the growth of the noise mean,

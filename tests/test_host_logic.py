@@ -23,9 +23,9 @@ def emu():
     sys.path.insert(0, os.path.join(ROOT, "tests", "emu"))
     import build_emu
     L = C.CDLL(build_emu.build_emu())
-    L.fdas_emu_convolve.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_int, C.c_void_p]
+    L.fdas_emu_convolve.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_int, C.c_int, C.c_void_p]
     L.fdas_emu_templates.argtypes = [C.c_double, C.c_double, C.c_int, C.c_int, C.c_void_p]
-    L.fdas_emu_ifft2048.argtypes = [C.c_void_p, C.c_void_p]
+    L.fdas_emu_ifft.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
     L.fdas_emu_fresnel.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.fdas_emu_thresholds.argtypes = [C.c_int, C.c_double, C.c_void_p]
     L.fdas_emu_whitening_blocks.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_int64]
@@ -72,7 +72,8 @@ def test_argument_validation_needs_no_device(fdaslib):
     for args in bad:
         assert lib.fdas_plan(C.byref(h), *args) == E.FDAS_EARG, args
         assert not h.value
-    assert lib.fdas_plan(C.byref(h), 1 << 17, 64e-6, 16.0, 1.0, 1024, 0) == E.FDAS_EUNSUPPORTED
+    for seg in (256, 512, 8192):                 # powers of two the FFT kernel is not built for
+        assert lib.fdas_plan(C.byref(h), 1 << 17, 64e-6, 16.0, 1.0, seg, 0) == E.FDAS_EUNSUPPORTED
     assert lib.fdas_plan(None, 1 << 17, 64e-6, 16.0, 1.0, 2048, 0) == E.FDAS_EARG
     assert lib.fdas_plan_info(None, None) == E.FDAS_EARG
     assert lib.fdas_destroy(None) == E.FDAS_EARG
@@ -116,19 +117,31 @@ def test_library_thresholds_and_blocks_match_the_oracle(emu, oracle, fdaslib):
         assert s[0] == 1 and s[n - 1] + l[n - 1] == nb
 
 
-def test_emulated_segment_fft(emu):
+@pytest.mark.parametrize("L", [1024, 2048, 4096])
+def test_emulated_segment_fft(emu, L):
+    """The three register passes and two exchanges of the segment transform (fdas_fft_core.cuh), stepped
+    thread by thread, against numpy for every segment length the kernel is built for."""
     rng = np.random.default_rng(0)
-    x = (rng.standard_normal(2048) + 1j * rng.standard_normal(2048)).astype(np.complex64)
-    out = np.empty(2048, dtype=np.complex64)
-    emu.fdas_emu_ifft2048(x.ctypes.data, out.ctypes.data)
-    ref = np.fft.ifft(x.astype(np.complex128)) * 2048
+    x = (rng.standard_normal(L) + 1j * rng.standard_normal(L)).astype(np.complex64)
+    out = np.full(L, np.nan, dtype=np.complex64)
+    assert emu.fdas_emu_ifft(L, x.ctypes.data, out.ctypes.data) == 0
+    ref = np.fft.ifft(x.astype(np.complex128)) * L
     assert np.abs(out - ref).max() < 1e-6 * np.abs(ref).max()
+    # a single tone lands in exactly one output sample (index maps of both exchanges)
+    for p0 in (1, 17, L // 16 + 3, L - 1):
+        x = np.zeros(L, dtype=np.complex64)
+        x[p0] = 1.0
+        assert emu.fdas_emu_ifft(L, x.ctypes.data, out.ctypes.data) == 0
+        assert np.abs(out - np.exp(2j * np.pi * p0 * np.arange(L) / L)).max() < 2e-6
+    assert emu.fdas_emu_ifft(512, x.ctypes.data, out.ctypes.data) != 0
 
 
-@pytest.mark.parametrize("zmax,nb", [(16.0, 7000), (96.0, 4500), (0.0, 4096)])
-def test_emulated_k2_matches_the_oracle_plane(emu, oracle, zmax, nb):
+@pytest.mark.parametrize("zmax,nb,seg_len", [(16.0, 7000, 2048), (96.0, 4500, 2048), (0.0, 4096, 2048),
+                                             (16.0, 7000, 1024), (96.0, 4500, 1024), (16.0, 9000, 4096),
+                                             (96.0, 8200, 4096)])
+def test_emulated_k2_matches_the_oracle_plane(emu, oracle, zmax, nb, seg_len):
     """Same index arithmetic, packed bank and exchange layouts as the CUDA kernel, stepped on the
-    CPU: several segments, a ragged tail, a strong line, all three storage precisions."""
+    CPU: several segments, a ragged tail, a strong line, all three storage precisions, every seg_len."""
     rng = np.random.default_rng(4)
     w = ((rng.standard_normal(nb) + 1j * rng.standard_normal(nb)) / np.sqrt(2)).astype(np.complex64)
     w[nb // 3] += 15.0
@@ -139,7 +152,7 @@ def test_emulated_k2_matches_the_oracle_plane(emu, oracle, zmax, nb):
     P = oracle.plane(w.astype(np.complex128), bank)
     for prec, tol in ((0, 1e-6), (1, 2e-2), (2, 2e-2)):
         out = np.full((nz, nb), np.nan, dtype=np.float32)
-        assert emu.fdas_emu_convolve(w.ctypes.data, nb, zmax, 1.0, prec, out.ctypes.data) == 0
+        assert emu.fdas_emu_convolve(w.ctypes.data, nb, zmax, 1.0, seg_len, prec, out.ctypes.data) == 0
         assert not np.isnan(out).any()                      # every r < nb written, nothing else
         assert np.abs(out - P).max() <= tol * P.max(), (prec, np.abs(out - P).max() / P.max())
 
