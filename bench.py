@@ -15,6 +15,7 @@ from __future__ import annotations
 import argparse
 import ctypes as C
 import json
+import math
 import os
 import statistics
 import sys
@@ -407,6 +408,34 @@ def k2_rooflines(info, precision, workload, t_conv_ms):
     return main, dict(hbm, kernel=main["kernel"])
 
 
+def seg_len_sweep(fdas, torch, wl, precision, d_x, launches=10):
+    """K2 (FFT formulation) alone at every segment length the kernel is built for: ms per launch by CUDA
+    events, the segmentation, and the nominal flop count per plane point of that L."""
+    out = []
+    for L in (1024, 2048, 4096):
+        plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, L, precision)
+        info = plan.info
+        d_spec, d_plane = plan.alloc_spec(), plan.alloc_plane()
+        plan.prepare_spectrum(d_x, d_spec)
+        for _ in range(3):
+            plan.convolve_plane(d_spec, d_plane)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(launches):
+            plan.convolve_plane(d_spec, d_plane)
+        b.record()
+        torch.cuda.synchronize()
+        V = int(info.valid)
+        flop_pt = (5.0 * L * math.log2(L) + 6.0 * L + 3.0 * V) / V
+        out.append({"seg_len": L, "valid": V, "nseg": int(info.nseg), "threads_per_cta": L // 16,
+                    "convolve_plane_ms": a.elapsed_time(b) / launches, "flop_per_point": round(flop_pt, 1)})
+        del d_spec, d_plane
+        plan.close()
+        torch.cuda.empty_cache()
+    return out
+
+
 def survey_block(fdas, torch, inputs, precision, trials_each, pool, thr, local_rank):
     """configs[4] in small: `trials_each` DM trials of each resolution (64 us: N = 9,375,000; 128 us:
     N = 4,687,500) through fdas_search_batch from PINNED HOST memory (the H2D copy of every series and the
@@ -560,6 +589,9 @@ def run_cuda(args):
                     "ncu_counters": "profiles/r01c_packed_fp32x2.md (FMA pipe 64.5 %, LSU data pipe 75 %, issue 74 %)"}
         plan_f.close()
         torch.cuda.empty_cache()
+        # the same kernel at the other segment lengths (K2 alone, 10 launches each, same
+        # spectrum; flop per plane point 5 L log2 L / (L - 2h) has its minimum near L = 1024-2048 for 129 taps)
+        fft_path["seg_len_sweep"] = seg_len_sweep(fdas, torch, wl, fprec, dev_pool[0])
 
     survey = None
     if args.survey_trials > 0 and args.workload == "ska" and ctx.world == 1:

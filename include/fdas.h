@@ -17,7 +17,7 @@
  *   - pointers named d_* are DEVICE pointers owned by the caller (allocate them with the sizes
  *     fdas_plan_info reports); pointers named h_* are HOST pointers; the plan owns its templates,
  *     twiddle tables, cuFFT plan + workspace, whitening scratch and the harmonic-sum scratch
- *     (block-maximum plane of nz x nbins/8 floats, prefilter list);
+ *     (block-maximum plane of nz x nbins/8 16-bit codes, prefilter list);
  *   - the three per-trial calls only ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
  *     void*, NULL = legacy default stream) and return; they never synchronise, allocate or free;
  *   - the plan's scratch is not duplicated, so the per-trial calls of one plan are ordered on the
@@ -225,8 +225,8 @@ int fdas_plan_templates_host(fdas_plan_t plan, double* h_out);
 /*
  * fdas_plan_debug_maxplane -- diagnostic: device pointer and row pitch (elements) of the plan-owned
  * block-maximum plane that fdas_convolve_plane writes for the harmonic-sum prefilter:
- * M[j][b] = bfloat16 bit pattern of max(P[j][8b..8b+7]) rounded toward +infinity (an upper bound;
- * the prefilter only needs M >= P).  The buffer stays owned by the plan.
+ * M[j][b] = min(1023, ceil(8 * max(P[j][8b..8b+7]))) as a 16-bit code: code/8 is an upper bound of the 8
+ * stored values (the prefilter only needs M >= P), 1023 means "no bound".  The buffer stays owned by the plan.
  */
 int fdas_plan_debug_maxplane(fdas_plan_t plan, const uint16_t** d_out, int64_t* pitch_out);
 

@@ -21,7 +21,7 @@ ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC"]
 
 LIB_SOURCES = ["fdas_api.cu", "fdas_batch.cu", "fdas_convolve.cu", "fdas_convolve_tc.cu", "fdas_whiten.cu", "fdas_harmonic.cu", "fdas_host.cpp"]
-HEADERS = ["fdas_fft_core.cuh", "fdas_tc_common.h", "fdas_host.h", "fdas_kernels.h", "fdas_plan_priv.h", os.path.join("..", "..", "include", "fdas.h")]
+HEADERS = ["fdas_fft_core.cuh", "fdas_tc_common.h", "fdas_host.h", "fdas_kernels.h", "fdas_maxcode.h", "fdas_plan_priv.h", os.path.join("..", "..", "include", "fdas.h")]
 
 
 def _stale(target: str, sources) -> bool:

@@ -14,6 +14,7 @@
 
 #include "fdas_fft_core.cuh"
 #include "fdas_kernels.h"
+#include "fdas_maxcode.h"
 
 namespace fdas {
 
@@ -66,10 +67,9 @@ __device__ __forceinline__ float2 cmul_k16(float2 s, unsigned v) {
 // Epilogue of one (segment, template).  Ra = 8 (L = 1024, 2048): thread t holds y[2t + e + OutStride q] in
 // x[e*8 + q]; Ra = 16 (L = 4096): y[t + 256 q] in x[q].  Writes the powers of the valid samples with
 // streaming stores and, for K3's prefilter, an upper bound of the maximum of every aligned block of 8
-// plane columns (= 4 or 8 consecutive lanes) of the values AS STORED: bf16 rounded toward +inf (powers are
-// >= 0, so adding 0xffff to the bit pattern and truncating rounds up; for non-negative values the bf16
-// order is the order of the bit patterns).  Two blocks (q, q+1) share one 32-bit word through the
-// shuffles.  `prow` / `mrow` already point at this thread's first column of row j, so every store has an
+// plane columns (= 4 or 8 consecutive lanes) of the values AS STORED, as the 16-bit code of
+// fdas_maxcode.h (units of 1/8, rounded up; codes order like the values).  Two blocks (q, q+1) share one
+// 32-bit word through the shuffles.  `prow` / `mrow` already point at this thread's first column of row j, so every store has an
 // immediate offset; q < qmax <=> the sample is valid (r < Nb and t < V), q < qmax_m <=> this lane also
 // writes the block maximum.
 template <int PREC, int L>
@@ -112,8 +112,8 @@ __device__ __forceinline__ void store_powers(const float2 (&x)[16], void* prow, 
                 mx[u] = fmaxf(p0, p1);
             }
         }
-        // bytes 2,3 of each rounded-up pattern: low half = block q2, high half = block q2 + 1
-        unsigned w = __byte_perm(__float_as_uint(mx[0]) + 0xffffu, __float_as_uint(mx[1]) + 0xffffu, 0x7632);
+        // block-max codes (fdas_maxcode.h): low half = block q2, high half = block q2 + 1
+        unsigned w = max_code(mx[0]) | (max_code(mx[1]) << 16);
         w = __vmaxu2(w, __shfl_xor_sync(0xffffffffu, w, 1));
         w = __vmaxu2(w, __shfl_xor_sync(0xffffffffu, w, 2));
         if constexpr (G::Ra == 16) w = __vmaxu2(w, __shfl_xor_sync(0xffffffffu, w, 4));

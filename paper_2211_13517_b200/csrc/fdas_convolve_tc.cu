@@ -39,6 +39,7 @@
 #include <cstdint>
 
 #include "fdas_kernels.h"
+#include "fdas_maxcode.h"
 #include "fdas_tc_common.h"
 
 namespace fdas {
@@ -164,8 +165,8 @@ __device__ __forceinline__ void tma_wait_all() { asm volatile("cp.async.bulk.wai
 // Powers of 8 consecutive bins of the rows +z and -z of this thread's pair from one group of
 // accumulator columns (a = 16 columns of D_R: Ar[0..7] | Ai[0..7]; b = 16 columns of D_I: Br | Bi),
 // into this thread's rows (rowp, rowm) of the two staging tiles, 16-byte unit `2 * bg` (fp32) / `bg`
-// (bf16) of half `half` of the row; returns the block maxima as bf16 bit patterns (upper bounds of the
-// values AS STORED: rounded toward +inf for an fp32 plane, exact for bf16).
+// (bf16) of half `half` of the row; returns the block maxima as the codes of fdas_maxcode.h (upper bounds of
+// the values AS STORED).
 template <int PLANE16>
 __device__ __forceinline__ unsigned group_to_smem(const uint32_t* __restrict__ a, const uint32_t* __restrict__ b,
                                                   unsigned char* tile_p, unsigned char* tile_m, const int rowp,
@@ -188,8 +189,8 @@ __device__ __forceinline__ unsigned group_to_smem(const uint32_t* __restrict__ a
         // powers are >= 0: the order of the bf16 bit patterns is the order of the values
         const unsigned xp = __vmaxu2(__vmaxu2(up.x, up.y), __vmaxu2(up.z, up.w));
         const unsigned xm = __vmaxu2(__vmaxu2(um.x, um.y), __vmaxu2(um.z, um.w));
-        mp = max(xp & 0xffffu, xp >> 16);
-        mm = max(xm & 0xffffu, xm >> 16);
+        mp = max_code(__uint_as_float(max(xp & 0xffffu, xp >> 16) << 16));
+        mm = max_code(__uint_as_float(max(xm & 0xffffu, xm >> 16) << 16));
     } else {
         // The swizzle phase of a row's chunk, (2 row + half) & 7, takes only 4 values over the 8 rows of a
         // shared-memory store phase, so the lanes with bit 2 set write their two 16-byte units in the
@@ -205,8 +206,8 @@ __device__ __forceinline__ unsigned group_to_smem(const uint32_t* __restrict__ a
         }
         const float fp = fmaxf(fmaxf(fmaxf(Pp[0], Pp[1]), fmaxf(Pp[2], Pp[3])), fmaxf(fmaxf(Pp[4], Pp[5]), fmaxf(Pp[6], Pp[7])));
         const float fm = fmaxf(fmaxf(fmaxf(Pm[0], Pm[1]), fmaxf(Pm[2], Pm[3])), fmaxf(fmaxf(Pm[4], Pm[5]), fmaxf(Pm[6], Pm[7])));
-        mp = (__float_as_uint(fp) + 0xffffu) >> 16;
-        mm = (__float_as_uint(fm) + 0xffffu) >> 16;
+        mp = max_code(fp);
+        mm = max_code(fm);
     }
     return mp | (mm << 16);
 }
@@ -344,11 +345,11 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
                     for (int e = 0; e < 4; ++e) b[e] = __bfloat16_as_ushort(__float2bfloat16_rn(P[e]));
                     __stcs(reinterpret_cast<uint2*>(reinterpret_cast<unsigned short*>(p.plane) + (int64_t)mid * p.pitch + r),
                            make_uint2((unsigned)b[0] | ((unsigned)b[1] << 16), (unsigned)b[2] | ((unsigned)b[3] << 16)));
-                    m = max(max((unsigned)b[0], (unsigned)b[1]), max((unsigned)b[2], (unsigned)b[3]));
+                    m = max_code(__uint_as_float(max(max((unsigned)b[0], (unsigned)b[1]), max((unsigned)b[2], (unsigned)b[3])) << 16));
                 } else {
                     __stcs(reinterpret_cast<float4*>(reinterpret_cast<float*>(p.plane) + (int64_t)mid * p.pitch + r),
                            make_float4(P[0], P[1], P[2], P[3]));
-                    m = (__float_as_uint(fmaxf(fmaxf(P[0], P[1]), fmaxf(P[2], P[3]))) + 0xffffu) >> 16;
+                    m = max_code(fmaxf(fmaxf(P[0], P[1]), fmaxf(P[2], P[3])));
                 }
                 m = max(m, __shfl_xor_sync(0xffffffffu, m, 1));
                 if ((lane & 1) == 0) p.maxplane[(int64_t)mid * p.mpitch + (r >> 3)] = (unsigned short)m;

@@ -5,10 +5,10 @@
 //   (half-integers round away from zero).  A candidate (r, j, h) is emitted for every S_h > T_h.
 //
 // The direct evaluation is HBM-bound: the stride-k gathers touch 3.2x the plane in 32-byte sectors.
-// K3 therefore works branch-and-bound on the block-max plane M[j][b] >= max P[j][8b..8b+7] (bf16, rounded
-// toward +inf) that K2 writes beside the plane (1/16 of its bytes):
-//   pass A (prefilter)  U_h(r,j) = sum_{k<=h} M[row_k][(k r) >> 3] >= S_h(r,j) term by term, in the
-//                       same summation order, and fp32 addition is monotone -- so U_h <= T_h for all
+// K3 therefore works branch-and-bound on the block-max plane M[j][b] >= max P[j][8b..8b+7] (16-bit codes in
+// units of 1/8, rounded up, fdas_maxcode.h) that K2 writes beside the plane (1/16 of its bytes):
+//   pass A (prefilter)  U_h(r,j) = sum_{k<=h} M[row_k][(k r) >> 3] >= S_h(r,j) term by term (exact integer
+//                       sums of the codes, two fundamentals per 32-bit add) -- so U_h <= T_h for all
 //                       h proves that (r, j) has no candidate without touching the plane.  The few
 //                       fundamentals for which some bound fails go to a "maybe" list.
 //   pass B (exact)      one thread per listed fundamental: the plain definition above on the real
@@ -26,8 +26,10 @@
 #include <cuda_bf16.h>
 
 #include <algorithm>
+#include <cmath>
 
 #include "fdas_kernels.h"
+#include "fdas_maxcode.h"
 
 namespace fdas {
 
@@ -46,7 +48,7 @@ struct HarmGeom {
     int64_t nbins, pitch, r_lo, capacity;
     fdas_cand_t* cands;
     unsigned long long* count;
-    const unsigned short* maxplane;   // block-max side plane (bf16 bits, upper bounds), nz x mpitch
+    const unsigned short* maxplane;   // block-max side plane (codes of fdas_maxcode.h), nz x mpitch
     int64_t mpitch;
     int nz, H;
 };
@@ -150,8 +152,8 @@ __device__ __noinline__ void exact_fundamental(const T* P, const HarmGeom g, con
             for (int q = 0; q < 8; ++q) {
                 const int h = h0 + q;
                 if (h > hmax) break;
-                U += __uint_as_float((unsigned)m[q] << 16);
-                if (U > thr[h - 1]) deeper = true;
+                U += (float)m[q] * (1.0f / kMaxCodeScale);
+                if (U > thr[h - 1] || m[q] >= kMaxCodeSat) deeper = true;   // a saturated code bounds nothing
             }
         }
         if (!deeper) return;
@@ -213,13 +215,6 @@ __device__ __noinline__ void exact_fundamental_nbr(const T* P, const HarmGeom g,
     }
 }
 
-// bf16 bit pattern of a non-negative power rounded toward +inf, and back.
-__device__ __forceinline__ unsigned short bf16_up(float v) {
-    return (unsigned short)((__float_as_uint(v) + 0xffffu) >> 16);
-}
-__device__ __forceinline__ float bf16_lo(unsigned w) { return __uint_as_float(w << 16); }
-__device__ __forceinline__ float bf16_hi(unsigned w) { return __uint_as_float(w & 0xffff0000u); }
-
 // ---- M from an arbitrary plane (only when K2 did not just write it): one thread per block of 8.
 template <typename T>
 __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
@@ -230,7 +225,7 @@ __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
     float m = ldp(src);
 #pragma unroll
     for (int i = 1; i < 8; ++i) m = fmaxf(m, ldp(src + i));
-    p.maxplane[(size_t)j * p.mpitch + b] = bf16_up(m);
+    p.maxplane[(size_t)j * p.mpitch + b] = (unsigned short)max_code(m);
 }
 
 // ---- M' = M dilated by D blocks on either side (neighbour-maximised sums): one thread per block.
@@ -239,119 +234,161 @@ __global__ void __launch_bounds__(256) dilate_max_kernel(const unsigned short* _
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= mpitch) return;
     const unsigned short* row = src + (size_t)blockIdx.y * mpitch;
-    unsigned m = 0;     // bf16 patterns of non-negative values order like the values
+    unsigned m = 0;     // codes order like the values
     for (int64_t e = max((int64_t)0, b - D); e <= min(mpitch - 1, b + D); ++e) m = max(m, (unsigned)__ldg(row + e));
     dst[(size_t)blockIdx.y * mpitch + b] = (unsigned short)m;
 }
 
-// ---- pass A: upper bounds from the block-max plane.
+// ---- pass A: upper bounds from the block-max plane, in integer arithmetic on the codes of fdas_maxcode.h.
+// U_h(r,j) = sum_{k<=h} M[row_k][(k r) >> 3] (codes) >= 8 S_h(r,j), and with the integer thresholds
+// tq_h <= 8 T_h (1 - 2^-18) of launch_harmonic, U_h <= tq_h for all h proves that (r, j) has no candidate.
+// Two fundamentals share one 32-bit register: X = U_h + (0x7fff - tq_h) per half-word, so that bit 15 of
+// a half-word is set exactly when U_h > tq_h.  All quantities stay within 16 bits (32 x 1023 + 0x7fff <
+// 2^16; tq_h in [-1, 1022], so a saturated code trips its flag alone): no carry ever crosses the
+// half-words, and one IADD3 (sum + next code pair + threshold step) and one LOP3 (flag accumulation) serve
+// two (fundamental, harmonic) pairs.
+//
 // Thread <-> 4 consecutive blocks of M = 32 consecutive fundamentals r = 32 Q + i of row j, so that
-// harmonic k <= 8 is k contiguous 128-bit loads (M[row_k][4kQ .. 4kQ+4k-1]) and every fundamental
-// picks element (k i) >> 3 of them -- a compile-time register choice once k and i are unrolled.  The
-// loads of harmonics 1..4 (then 5-6, 7-8, then one harmonic at a time) are all issued before the
-// first add: the kernel moves < 1 GB and would otherwise be bound by DRAM latency, not bandwidth.
-// One FADD, one FSETP and one predicated OR per (fundamental, harmonic) for h >= 3 (h = 1, 2 are
-// evaluated once per block / half block); fundamentals with any U_h > T_h go to the maybe list as (r, j).
+// harmonic k is the 4k codes M[row_k][4kQ .. 4kQ+4k-1] (k contiguous 64-bit loads) and fundamental i picks
+// code (k i) >> 3 of them -- a compile-time choice once k and i are unrolled (one PRMT per pair of
+// fundamentals, none where the pair is an aligned word).
 constexpr int kPfThreads = 128;
 
-// Harmonic K for the 32 fundamentals of quad-block Q, all of them valid (K (32Q+31) <= Nb-1).
-template <int K, int NV>
-__device__ __forceinline__ void pf_load(const unsigned short* __restrict__ mrow, const unsigned Q,
-                                        const bool on, float (&m)[NV]) {
-    if constexpr (K <= 8) {
-        static_assert(NV == 4 * K, "k <= 8 loads 4k contiguous elements");
-        const uint2* src = reinterpret_cast<const uint2*>(mrow + (size_t)4 * K * Q);   // 8K bytes, 8-byte aligned
-#pragma unroll
-        for (int q = 0; q < K; ++q) {
-            uint2 v = make_uint2(0u, 0u);
-            if (on) v = __ldg(src + q);
-            m[4 * q] = bf16_lo(v.x); m[4 * q + 1] = bf16_hi(v.x);
-            m[4 * q + 2] = bf16_lo(v.y); m[4 * q + 3] = bf16_hi(v.y);
-        }
-    } else {
-        static_assert(NV == 32, "k > 8 gathers one element per fundamental");
-        const unsigned short* src = mrow + (size_t)4 * K * Q;
-#pragma unroll
-        for (int i = 0; i < 32; ++i) m[i] = on ? bf16_lo(__ldg(src + ((K * i) >> 3))) : 0.f;
-    }
-}
-
-template <int K, int NV>
-__device__ __forceinline__ void pf_add(const float (&m)[NV], const float thr, const bool on,
-                                       float (&U)[32], unsigned& flagged) {
-    if (on) {
-#pragma unroll
-        for (int i = 0; i < 32; ++i) {
-            U[i] += m[K <= 8 ? ((K * i) >> 3) : i];
-            if (U[i] > thr) flagged |= 1u << i;
-        }
-    }
-}
-
-struct PfRow { const unsigned short* mrow; float thr; };
+struct PfRow { const unsigned short* mrow; int tq; };
 
 __device__ __forceinline__ PfRow pf_row(const HarmParams& p, const int j, const int k) {
     const int c2 = p.nz - 1;
     const int v2 = 2 * k * j - (k - 1) * c2;   // only called for k <= hz: v2 is in range
     PfRow r;
     r.mrow = p.maxplane + (size_t)min((v2 + 1) >> 1, c2) * p.mpitch;
-    r.thr = p.thr[k - 1];
+    r.tq = p.tq[k - 1];
     return r;
 }
 
-// Harmonic K > 8 of the 32 fundamentals of quad-block Q: the thread's slice M[row_K][4KQ .. 4KQ+4K-1]
-// (8K bytes) is read with 64-bit loads in two halves -- fundamentals 0..15 pick elements
-// (K i) >> 3 < 2K (words 0..K-1), fundamentals 16..31 elements >= 2K (words K..2K-1) -- instead of one
-// 16-bit gather per fundamental: half the load instructions, K + 2 live registers instead of 32.
+// Harmonic K <= 4 for the 32 fundamentals of quad-block Q: the 4K codes M[row_K][4KQ .. 4KQ+4K-1].
 template <int K>
-__device__ __forceinline__ void pf_deep(const unsigned short* __restrict__ mrow, const unsigned Q,
-                                        const float thr, float (&U)[32], unsigned& flagged) {
-    const unsigned* words = reinterpret_cast<const unsigned*>(mrow + (size_t)4 * K * Q);   // 8-byte aligned
+__device__ __forceinline__ void pf_load(const unsigned short* __restrict__ mrow, const unsigned Q, const bool on,
+                                        int (&m)[4 * K]) {
+    const uint2* src = reinterpret_cast<const uint2*>(mrow + (size_t)4 * K * Q);   // 8K bytes, 8-byte aligned
 #pragma unroll
-    for (int half = 0; half < 2; ++half) {
-        constexpr int kPairs = K / 2 + 1;                 // 64-bit loads covering the half's K words
-        const int w0 = half ? (K & ~1) : 0;               // first word loaded (even: aligned)
-        unsigned wv[2 * kPairs];
-#pragma unroll
-        for (int c = 0; c < kPairs; ++c) {
-            // the last pair of the second half may reach one word past the slice when K is even
-            if (w0 + 2 * c + 1 < 2 * K) {
-                const uint2 v = __ldg(reinterpret_cast<const uint2*>(words + w0) + c);
-                wv[2 * c] = v.x;
-                wv[2 * c + 1] = v.y;
-            } else if (w0 + 2 * c < 2 * K) {
-                wv[2 * c] = __ldg(words + w0 + 2 * c);
-                wv[2 * c + 1] = 0u;
-            } else {
-                wv[2 * c] = wv[2 * c + 1] = 0u;
-            }
-        }
-#pragma unroll
-        for (int ii = 0; ii < 16; ++ii) {
-            const int i = 16 * half + ii;
-            const int e = (K * i) >> 3;                   // element of the slice (compile time)
-            const unsigned w = wv[(e >> 1) - w0];
-            U[i] += (e & 1) ? bf16_hi(w) : bf16_lo(w);
-            if (U[i] > thr) flagged |= 1u << i;
-        }
+    for (int q = 0; q < K; ++q) {
+        uint2 v = make_uint2(0u, 0u);
+        if (on) v = __ldg(src + q);
+        m[4 * q] = (int)(v.x & 0xffffu); m[4 * q + 1] = (int)(v.x >> 16);
+        m[4 * q + 2] = (int)(v.y & 0xffffu); m[4 * q + 3] = (int)(v.y >> 16);
     }
 }
 
+// The pair (code e0, code e1) of a slice held as 32-bit words (two codes per word), e0 and e1 static.
+template <int E0, int E1, int W0, int NW>
+__device__ __forceinline__ unsigned pf_pair(const unsigned (&w)[NW]) {
+    constexpr int a = (E0 >> 1) - W0, b = (E1 >> 1) - W0;
+    static_assert(a >= 0 && a < NW && b >= 0 && b < NW, "code outside the loaded words");
+    if constexpr (a == b && (E0 & 1) == 0 && (E1 & 1) == 1) {
+        return w[a];
+    } else {
+        constexpr unsigned sel = ((E0 & 1) ? 0x32u : 0x10u) | ((E1 & 1) ? 0x7600u : 0x5400u);
+        return __byte_perm(w[a], w[b], sel);
+    }
+}
+
+// One harmonic K for the pairs P0 .. P0 + NP - 1 of fundamentals (2p, 2p+1) from the words w (first word W0
+// of the slice): X += codes + step, F |= X.
+template <int K, int P0, int NP, int W0, int NW, int PI = 0>
+__device__ __forceinline__ void pf_pairs(const unsigned (&w)[NW], const unsigned step, unsigned (&X)[16],
+                                         unsigned (&F)[16]) {
+    if constexpr (PI < NP) {
+        constexpr int p = P0 + PI;
+        const unsigned m2 = pf_pair<((K * (2 * p)) >> 3), ((K * (2 * p + 1)) >> 3), W0, NW>(w);
+        X[p] = X[p] + m2 + step;
+        F[p] |= X[p];
+        pf_pairs<K, P0, NP, W0, NW, PI + 1>(w, step, X, F);
+    }
+}
+
+// The words of harmonic K that one HALF of the thread's fundamentals pick: fundamentals 0..15 pick codes
+// (K i) >> 3 < 2K (words 0 .. K-1), fundamentals 16..31 codes 2K .. 4K-1 (words from K rounded down to even,
+// so that the 64-bit loads stay aligned).
+template <int K, int HALF> struct PfHalf {
+    static constexpr int W0 = HALF ? (K & ~1) : 0;
+    static constexpr int kLoads = HALF ? (2 * K - W0) / 2 : (K + 1) / 2;     // 64-bit loads
+    static constexpr int NW = 2 * kLoads;
+};
+template <int K, int HALF>
+__device__ __forceinline__ void pf_half_load(const unsigned short* __restrict__ mrow, const unsigned Q,
+                                             unsigned (&w)[PfHalf<K, HALF>::NW]) {
+    const uint2* src = reinterpret_cast<const uint2*>(mrow + (size_t)4 * K * Q + 2 * PfHalf<K, HALF>::W0);
+#pragma unroll
+    for (int c = 0; c < PfHalf<K, HALF>::kLoads; ++c) {
+        const uint2 v = __ldg(src + c);
+        w[2 * c] = v.x;
+        w[2 * c + 1] = v.y;
+    }
+}
+
+// Harmonic K alone (all 32 fundamentals inside the plane), half by half: at most K + 2 words live.
 template <int K>
-__device__ __forceinline__ void pf_single_from(const HarmParams& p, const int j, const unsigned Q,
-                                               const int he_max, const int he, float (&U)[32],
-                                               unsigned& flagged) {
+__device__ __forceinline__ void pf_harmonic(const unsigned short* __restrict__ mrow, const unsigned Q,
+                                            const unsigned step, unsigned (&X)[16], unsigned (&F)[16]) {
+    {
+        unsigned w[PfHalf<K, 0>::NW];
+        pf_half_load<K, 0>(mrow, Q, w);
+        pf_pairs<K, 0, 8, PfHalf<K, 0>::W0, PfHalf<K, 0>::NW>(w, step, X, F);
+    }
+    {
+        unsigned w[PfHalf<K, 1>::NW];
+        pf_half_load<K, 1>(mrow, Q, w);
+        pf_pairs<K, 8, 8, PfHalf<K, 1>::W0, PfHalf<K, 1>::NW>(w, step, X, F);
+    }
+}
+
+// Harmonics K and K + 1 together: the loads of both are in flight before the first add of either -- the
+// kernel is bound by the latency of its dependent loads (L2 / DRAM), so every step that carries two harmonics
+// shortens the chain of a thread that has sixteen.
+template <int K>
+__device__ __forceinline__ void pf_harmonic2(const unsigned short* __restrict__ mrowa,
+                                             const unsigned short* __restrict__ mrowb, const unsigned Q,
+                                             const unsigned stepa, const unsigned stepb, unsigned (&X)[16],
+                                             unsigned (&F)[16]) {
+    {
+        unsigned wa[PfHalf<K, 0>::NW], wb[PfHalf<K + 1, 0>::NW];
+        pf_half_load<K, 0>(mrowa, Q, wa);
+        pf_half_load<K + 1, 0>(mrowb, Q, wb);
+        pf_pairs<K, 0, 8, PfHalf<K, 0>::W0, PfHalf<K, 0>::NW>(wa, stepa, X, F);
+        pf_pairs<K + 1, 0, 8, PfHalf<K + 1, 0>::W0, PfHalf<K + 1, 0>::NW>(wb, stepb, X, F);
+    }
+    {
+        unsigned wa[PfHalf<K, 1>::NW], wb[PfHalf<K + 1, 1>::NW];
+        pf_half_load<K, 1>(mrowa, Q, wa);
+        pf_half_load<K + 1, 1>(mrowb, Q, wb);
+        pf_pairs<K, 8, 8, PfHalf<K, 1>::W0, PfHalf<K, 1>::NW>(wa, stepa, X, F);
+        pf_pairs<K + 1, 8, 8, PfHalf<K + 1, 1>::W0, PfHalf<K + 1, 1>::NW>(wb, stepb, X, F);
+    }
+}
+
+// Harmonics K, K+1, .. while every fundamental of the thread has them (k <= he; he_max is the CTA's deepest),
+// two per step.
+template <int K>
+__device__ __forceinline__ void pf_from(const HarmParams& p, const int j, const unsigned Q, const int he_max,
+                                        const int he, unsigned (&X)[16], unsigned (&F)[16]) {
     if constexpr (K <= 32) {
         if (K > he_max) return;                 // CTA-uniform: no thread of this CTA goes deeper
-        const PfRow r = pf_row(p, j, K);
-        if constexpr (K <= 8) {
-            float m[4 * K];
-            pf_load<K>(r.mrow, Q, he >= K, m);
-            pf_add<K>(m, r.thr, he >= K, U, flagged);
-        } else {
-            if (he >= K) pf_deep<K>(r.mrow, Q, r.thr, U, flagged);
+        if (he >= K) {
+            const PfRow ra = pf_row(p, j, K);
+            // threshold step of a harmonic on both half-words: -(tq_K - tq_{K-1}) as one 32-bit integer
+            const unsigned stepa = (unsigned)(p.tq[K - 2] - ra.tq) * 0x10001u;
+            if constexpr (K + 1 <= 32) {
+                if (he >= K + 1) {
+                    const PfRow rb = pf_row(p, j, K + 1);
+                    pf_harmonic2<K>(ra.mrow, rb.mrow, Q, stepa, (unsigned)(ra.tq - rb.tq) * 0x10001u, X, F);
+                } else {
+                    pf_harmonic<K>(ra.mrow, Q, stepa, X, F);
+                }
+            } else {
+                pf_harmonic<K>(ra.mrow, Q, stepa, X, F);
+            }
         }
-        pf_single_from<K + 1>(p, j, Q, he_max, he, U, flagged);
+        pf_from<K + 2>(p, j, Q, he_max, he, X, F);
     }
 }
 
@@ -378,43 +415,69 @@ __device__ __forceinline__ void pf_emit(const HarmParams& p, const unsigned Q, c
     }
 }
 
+// The same for a whole (converged) warp: one atomic slot claim per warp instead of one per thread -- with
+// 16-harmonic rows most threads of the general kernel have a flagged fundamental, and their claims would all
+// queue at the one L2 slice that holds the counter.
+__device__ __forceinline__ void pf_emit_warp(const HarmParams& p, const unsigned Q, const int j, unsigned flagged) {
+    if (32 * (int64_t)Q < p.r_lo) {
+        const int64_t cut = p.r_lo - 32 * (int64_t)Q;
+        flagged = (cut >= 32) ? 0u : (flagged & ~((1u << (int)cut) - 1u));
+    }
+    const unsigned lane = threadIdx.x & 31u;
+    const int n = __popc(flagged);
+    int incl = n;                                   // inclusive prefix sum over the lanes
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, incl, d);
+        if ((int)lane >= d) incl += v;
+    }
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    if (total == 0) return;
+    unsigned long long base = 0;
+    if (lane == 0) base = atomicAdd(p.maybe_count, (unsigned long long)total);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (base + (unsigned long long)total <= (unsigned long long)p.maybe_capacity) {
+        unsigned long long slot = base + (unsigned long long)(incl - n);
+        while (flagged) {
+            const int i = __ffs(flagged) - 1;
+            flagged &= flagged - 1;
+            p.maybe[slot++] = make_uint2(32u * Q + (unsigned)i, (unsigned)j);
+        }
+    } else if (lane == 0) {
+        atomicExch(p.overflow, 1u);   // pass B then falls back to the full scan
+    }
+}
+
 // Rows with at most kShallowDepth = 4 harmonics inside the plane (|z| > zmax/5: the nlow first and the
 // nlow last rows, four fifths of the plane).  Harmonic k picks block (k i) >> 3 for fundamental i of a
 // block of 8, so U_1 is the same for all 8 fundamentals, U_2 for halves, U_3 takes 4 and U_4 5 distinct
 // values per block: 12 sums and compares stand for 32.  A thread streams 8 blocks (64 fundamentals) of
 // M[j] and the 8k blocks of M[row_k] they map to; few registers, every load issued up front.
 constexpr int kPfShallowThreads = 256;
-constexpr int kShallowDepth = 4;
 
-__device__ __forceinline__ float bf16_at(const uint4 (&w)[4], const int e) {   // element e of up to 32 (static e)
+__device__ __forceinline__ int code_at(const uint4 (&w)[4], const int e) {   // code e of up to 32 (static e)
     const uint4 v = w[e >> 3];
     const unsigned x = ((e >> 1) & 3) == 0 ? v.x : ((e >> 1) & 3) == 1 ? v.y : ((e >> 1) & 3) == 2 ? v.z : v.w;
-    return (e & 1) ? bf16_hi(x) : bf16_lo(x);
+    return (int)((e & 1) ? (x >> 16) : (x & 0xffffu));
 }
 
 // DMAX = 2 | 4: deepest harmonic of the rows this instance scans, rows [ja, jb) and their mirror images
 // [nz - jb, nz - ja) (the two-harmonic instance needs a third of the registers of the four-harmonic one).
+// The 64 fundamentals of octet O (8 blocks of M) of row j, for at most DMAX harmonics: the caller guarantees
+// that no fundamental of the octet has a harmonic DMAX + 1 inside the plane (in z or in r).
 template <int DMAX>
-__global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(const HarmParams p, const int ja,
-                                                                              const int jb) {
-    const int y = blockIdx.y;
-    const int j = y < jb - ja ? ja + y : p.nz - jb + (y - (jb - ja));
+__device__ __forceinline__ void pf_shallow_octet(const HarmParams& p, const unsigned O, const int j) {
     const int c2 = p.nz - 1;
-    const unsigned O = blockIdx.x * (unsigned)kPfShallowThreads + threadIdx.x;   // octet of blocks
-    if (O >= (unsigned)(p.mpitch >> 3)) return;
     const unsigned last = (unsigned)(p.nbins - 1);
     const int d = abs(2 * j - c2);
-    const int hz = min(DMAX, d == 0 ? p.H : min(p.H, c2 / d));   // 1 .. DMAX here (CTA-uniform)
+    const int hz = min(DMAX, d == 0 ? p.H : min(p.H, c2 / d));   // 1 .. DMAX here
     const PfRow r1 = pf_row(p, j, 1);
     uint4 m1[4], m2[4], m3[4], m4[4];   // (only the first DMAX arrays are live)
     m1[0] = __ldg(reinterpret_cast<const uint4*>(r1.mrow) + O);
-    if (hz <= 1 && r1.thr >= 0.f) {
-        // one harmonic only (half of the plane's rows): M > T_1 on the bf16 bit patterns.  For
-        // non-negative values the order of the patterns is the order of the values, and with
-        // tb = pattern of T_1 truncated to bf16, M > T_1 <=> pattern(M) > tb (M is a bf16 value).
-        // (A negative T_1 passes every point, M = 0 included: no early exit then.)
-        const unsigned tb = __float_as_uint(r1.thr) >> 16;
-        const unsigned tb2 = tb | (tb << 16);
+    if (hz <= 1 && r1.tq >= 0) {
+        // one harmonic only (half of the plane's rows): code > tq_1 on the packed half-words.
+        // (tq_1 = -1 passes every point, code 0 included: no early exit then.)
+        const unsigned tb2 = (unsigned)r1.tq * 0x10001u;
         if ((__vcmpgtu2(m1[0].x, tb2) | __vcmpgtu2(m1[0].y, tb2) | __vcmpgtu2(m1[0].z, tb2) |
              __vcmpgtu2(m1[0].w, tb2)) == 0u)
             return;                                   // nothing above threshold: almost every thread
@@ -442,62 +505,148 @@ __global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(co
     for (int q = 0; q < 8; ++q) {          // block q: fundamentals 8q..8q+7
         const int sh = 8 * (q & 3);
         unsigned fl = 0u;
-        const float u1 = bf16_at(m1, q);
-        if (u1 > r1.thr) fl |= 0xffu;
+        const int u1 = code_at(m1, q);
+        if (u1 > r1.tq) fl |= 0xffu;
         if (dep >= 2) {
             // U_2: fundamentals 0..3 -> block 2q, 4..7 -> block 2q+1 of row_2
-            const float u2[2] = {u1 + bf16_at(m2, 2 * q), u1 + bf16_at(m2, 2 * q + 1)};
-            if (u2[0] > r2.thr) fl |= 0x0fu;
-            if (u2[1] > r2.thr) fl |= 0xf0u;
+            const int u2[2] = {u1 + code_at(m2, 2 * q), u1 + code_at(m2, 2 * q + 1)};
+            if (u2[0] > r2.tq) fl |= 0x0fu;
+            if (u2[1] > r2.tq) fl |= 0xf0u;
             if (DMAX >= 3 && dep >= 3) {
                 // U_3: (i >> 2, (3 i) >> 3) = (0,0) for i = 0,1,2; (0,1) for 3; (1,1) for 4,5; (1,2) for 6,7
-                const float u3[4] = {u2[0] + bf16_at(m3, 3 * q), u2[0] + bf16_at(m3, 3 * q + 1),
-                                     u2[1] + bf16_at(m3, 3 * q + 1), u2[1] + bf16_at(m3, 3 * q + 2)};
-                if (u3[0] > r3.thr) fl |= 0x07u;
-                if (u3[1] > r3.thr) fl |= 0x08u;
-                if (u3[2] > r3.thr) fl |= 0x30u;
-                if (u3[3] > r3.thr) fl |= 0xc0u;
+                const int u3[4] = {u2[0] + code_at(m3, 3 * q), u2[0] + code_at(m3, 3 * q + 1),
+                                   u2[1] + code_at(m3, 3 * q + 1), u2[1] + code_at(m3, 3 * q + 2)};
+                if (u3[0] > r3.tq) fl |= 0x07u;
+                if (u3[1] > r3.tq) fl |= 0x08u;
+                if (u3[2] > r3.tq) fl |= 0x30u;
+                if (u3[3] > r3.tq) fl |= 0xc0u;
                 if (DMAX >= 4 && dep >= 4) {
                     // U_4 adds block i >> 1 of row_4: i = 0,1 | 2 | 3 | 4,5 | 6,7
-                    if (u3[0] + bf16_at(m4, 4 * q) > r4.thr) fl |= 0x03u;
-                    if (u3[0] + bf16_at(m4, 4 * q + 1) > r4.thr) fl |= 0x04u;
-                    if (u3[1] + bf16_at(m4, 4 * q + 1) > r4.thr) fl |= 0x08u;
-                    if (u3[2] + bf16_at(m4, 4 * q + 2) > r4.thr) fl |= 0x30u;
-                    if (u3[3] + bf16_at(m4, 4 * q + 3) > r4.thr) fl |= 0xc0u;
+                    if (u3[0] + code_at(m4, 4 * q) > r4.tq) fl |= 0x03u;
+                    if (u3[0] + code_at(m4, 4 * q + 1) > r4.tq) fl |= 0x04u;
+                    if (u3[1] + code_at(m4, 4 * q + 1) > r4.tq) fl |= 0x08u;
+                    if (u3[2] + code_at(m4, 4 * q + 2) > r4.tq) fl |= 0x30u;
+                    if (u3[3] + code_at(m4, 4 * q + 3) > r4.tq) fl |= 0xc0u;
                 }
             }
         }
         f[q >> 2] |= fl << sh;
     }
-    if (dep < hz) {
-        // the thread that straddles r = (Nb-1)/(dep+1): harmonic dep+1 exists for its first
-        // fundamentals only (no deeper one can: see DESIGN.md K3); U_dep is rebuilt in k order
-        const int k = dep + 1;
-        const unsigned rmax = last / (unsigned)k;
-        if (64u * O <= rmax) {
-            const int nv = (int)min(64u, rmax - 64u * O + 1u);
-            const float thr_k = p.thr[k - 1];
-            for (int i = 0; i < nv; ++i) {
-                float u = 0.f;
-                for (int kk = 1; kk <= k; ++kk) {
-                    const PfRow rk = pf_row(p, j, kk);
-                    u += bf16_lo(__ldg(rk.mrow + (size_t)8 * kk * O + ((kk * i) >> 3)));
-                }
-                if (u > thr_k) f[i >> 5] |= 1u << (i & 31);
-            }
-        }
+    if (dep < hz && 64u * O <= last / (unsigned)(dep + 1)) {
+        // the thread that straddles the end of harmonic dep+1's range (one per harmonic and row): harmonic
+        // dep+1 exists for its first fundamentals only -- all 64 go to the exact pass, which knows
+        f[0] = f[1] = 0xffffffffu;
     }
     pf_emit(p, 2u * O, j, f[0]);
     pf_emit(p, 2u * O + 1u, j, f[1]);
 }
 
-__global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmParams p, const int nlow) {
+// ---- level 0 of pass A: the same bound on COARSE blocks of 64 plane columns.
+// M2[j][B] = max of the 8 codes M[j][8B .. 8B+7] (row-major, 1/8 of M: 25 MB at the SKA size, L2-resident).
+// For a fundamental r of coarse block B harmonic k lies in the coarse blocks kB .. kB + k - 1 of row_k, so
+//     U0_h(B,j) = sum_{k<=h} max_{i<k} M2[row_k][kB + i]  >=  U_h(r,j)  >=  8 S_h(r,j)   for all r in B:
+// U0_h <= tq_h for all h settles 64 fundamentals at once.  It serves the parts of the plane with at most
+// kShallowDepth harmonics -- the shallow rows, and of the deep rows the fundamentals r >= 64 b_deep -- where
+// the sum of a few maxima of Exp(1) noise stays far below the thresholds; the (B, j) that fail go to a list
+// for pf_shallow_octet.  (With 16 harmonics the coarse bound is useless: the deep part of the deep rows is
+// prefilter_kernel's.)
+__global__ void __launch_bounds__(256) coarsen_max_kernel(const unsigned short* __restrict__ M, const int64_t mpitch,
+                                                          unsigned short* __restrict__ M2) {
+    const int64_t nB = mpitch >> 3;
+    const int64_t B = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (B >= nB) return;
+    const uint4 v = __ldg(reinterpret_cast<const uint4*>(M + (size_t)blockIdx.y * mpitch) + B);
+    unsigned m = __vmaxu2(__vmaxu2(v.x, v.y), __vmaxu2(v.z, v.w));
+    m = max(m & 0xffffu, m >> 16);
+    M2[(size_t)blockIdx.y * nB + B] = (unsigned short)m;
+}
+
+constexpr int kShallowDepth = 4;
+
+// Thread <-> 8 consecutive coarse blocks B = 8 G + q of row j (one 128-bit word of M2[j]); harmonic k needs
+// the 8k coarse blocks 8kG .. 8kG + 8k - 1 of row_k (k words); all loads are issued up front.
+__global__ void __launch_bounds__(256) prefilter_coarse_kernel(const HarmParams p, const unsigned b_deep) {
+    const unsigned nB = (unsigned)(p.mpitch >> 3), nG = nB >> 3;      // nB is a multiple of 8 here
+    const unsigned G = blockIdx.x * 256u + threadIdx.x;
+    const int j = blockIdx.y;
+    if (G >= nG) return;
+    const unsigned last = (unsigned)(p.nbins - 1);
+    const int c2 = p.nz - 1;
+    const int d = abs(2 * j - c2);
+    const int hzr = d == 0 ? p.H : min(p.H, c2 / d);
+    const bool deep = hzr > kShallowDepth;
+    if (deep && 8u * G + 7u < b_deep) return;                          // the deep part of a deep row
+    const int hz = min(hzr, kShallowDepth);                            // CTA-uniform
+    const unsigned short* const M2 = p.max2;
+    const uint4 m1 = __ldg(reinterpret_cast<const uint4*>(M2 + (size_t)j * nB) + G);
+    if (hz <= 1 && p.tq[0] >= 0 && !deep) {
+        const unsigned tb2 = (unsigned)p.tq[0] * 0x10001u;
+        if ((__vcmpgtu2(m1.x, tb2) | __vcmpgtu2(m1.y, tb2) | __vcmpgtu2(m1.z, tb2) | __vcmpgtu2(m1.w, tb2)) == 0u)
+            return;                                                    // almost every thread of a one-harmonic row
+    }
+    // harmonic k of coarse block B exists iff some fundamental of the block has it: 64 k B <= Nb - 1
+    uint4 mk[3][4];
+#pragma unroll
+    for (int k = 2; k <= kShallowDepth; ++k) {
+        const int row = min((2 * k * j - (k - 1) * c2 + 1) >> 1, c2);     // (unused when k > hz)
+        const uint4* src = reinterpret_cast<const uint4*>(M2 + (size_t)row * nB);
+#pragma unroll
+        for (int c = 0; c < k; ++c) {
+            const unsigned g = (unsigned)k * G + (unsigned)c;
+            mk[k - 2][c] = (k <= hz && g < nG) ? __ldg(src + g) : make_uint4(0u, 0u, 0u, 0u);
+        }
+    }
+    auto code = [](const uint4& v, const int e) {                          // code e of 8 (static e)
+        const unsigned x = (e >> 1) == 0 ? v.x : (e >> 1) == 1 ? v.y : (e >> 1) == 2 ? v.z : v.w;
+        return (int)((e & 1) ? (x >> 16) : (x & 0xffffu));
+    };
+    unsigned fl = 0u;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const unsigned B = 8u * G + (unsigned)q;
+        int U = code(m1, q);
+        bool f = U > p.tq[0];
+#pragma unroll
+        for (int k = 2; k <= kShallowDepth; ++k) {
+            int m = 0;
+#pragma unroll
+            for (int i = 0; i < k; ++i) m = max(m, code(mk[k - 2][(k * q + i) >> 3], (k * q + i) & 7));
+            // (a harmonic beyond hz, or beyond the plane in r for the whole block, was loaded as zeros or is skipped)
+            if (k <= hz && (unsigned long long)k * 64ull * B <= last) {
+                U += m;
+                f = f || U > p.tq[k - 1];
+            }
+        }
+        if (f && !(deep && B < b_deep)) fl |= 1u << q;
+    }
+    while (fl) {
+        const int q = __ffs(fl) - 1;
+        fl &= fl - 1;
+        const unsigned long long slot = atomicAdd(p.coarse_count, 1ULL);
+        if (slot < (unsigned long long)p.coarse_capacity) p.coarse[slot] = make_uint2(8u * G + (unsigned)q, (unsigned)j);
+        else atomicExch(p.overflow, 1u);                                   // pass B then falls back to the full scan
+    }
+}
+
+// Level 1 for the listed (coarse block = octet of blocks, row) pairs: one thread each.
+__global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(const HarmParams p) {
+    const unsigned long long n = min(*p.coarse_count, (unsigned long long)p.coarse_capacity);
+    for (unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; q < n;
+         q += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint2 rec = p.coarse[q];
+        pf_shallow_octet<kShallowDepth>(p, rec.x, (int)rec.y);
+    }
+}
+
+__global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmParams p, const int nlow,
+                                                                  const unsigned q_end) {
     const int j = nlow + blockIdx.y;   // the rows with more than kShallowDepth harmonics (|z| <= zmax/5)
     const int c2 = p.nz - 1;
     const unsigned Q0 = blockIdx.x * (unsigned)kPfThreads;
-    const unsigned Q = Q0 + threadIdx.x;
-    const unsigned nquad = (unsigned)(p.mpitch >> 2);   // nbins / 32
-    if (Q >= nquad) return;
+    // q_end <= nbins / 32: the quad-blocks beyond it belong to the coarse level.  The threads beyond stay (with
+    // nothing to do) for the warp-wide slot claim at the end; they redo the last quad-block's loads.
+    const bool mine = Q0 + threadIdx.x < q_end;
+    const unsigned Q = mine ? Q0 + threadIdx.x : q_end - 1u;
     const unsigned last = (unsigned)(p.nbins - 1);
     // hz: harmonics inside the plane in z for this row (CTA-uniform): twice the row of harmonic k is
     // v2 = k d + c2 with d = 2 j - c2, and 0 <= v2 <= 2 c2  <=>  k |d| <= c2
@@ -506,104 +655,98 @@ __global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmPara
     // he: harmonics for which all 32 fundamentals of this thread are inside the plane in r
     const int he = (int)min((unsigned)hz, last / (32u * Q + 31u));
     const int he_max = (int)min((unsigned)hz, last / (32u * Q0 + 31u));   // deepest in this CTA
-    float U[32];
-    unsigned flagged = 0u;   // bit i: some U_h of fundamental 32 Q + i exceeds T_h
-
-    {   // harmonics 1..4: ten 128-bit loads in flight
+    unsigned flagged = 0u;   // bit i: some U_h of fundamental 32 Q + i exceeds tq_h
+    int U4[20];              // U_4 of block b: [5b] i = 0,1  [5b+1] i = 2  [5b+2] i = 3  [5b+3] i = 4,5  [5b+4] i = 6,7
+    {   // harmonics 1..4: ten 64-bit loads in flight; harmonic k picks block (k i) >> 3 for fundamental i of a
+        // block of 8: U_1 is the same for all 8, U_2 for the 4 of a half block, U_3 takes 4 and U_4 5 distinct
+        // values per block -- 12 sums and compares per block stand for 32 (h <= 4 are 90 % of all (r, j, h)
+        // triples of the plane)
         const PfRow r1 = pf_row(p, j, 1);
-        float m1[4], m2[8], m3[12], m4[16];
+        int m1[4], m2[8], m3[12], m4[16];
         pf_load<1>(r1.mrow, Q, true, m1);
         PfRow r2 = r1, r3 = r1, r4 = r1;
         if (he_max >= 2) { r2 = pf_row(p, j, 2); pf_load<2>(r2.mrow, Q, he >= 2, m2); }
         if (he_max >= 3) { r3 = pf_row(p, j, 3); pf_load<3>(r3.mrow, Q, he >= 3, m3); }
         if (he_max >= 4) { r4 = pf_row(p, j, 4); pf_load<4>(r4.mrow, Q, he >= 4, m4); }
-        // harmonic k picks block (k i) >> 3 for fundamental i of a block of 8: U_1 is the same for all
-        // 8, U_2 for the 4 of a half block, U_3 takes 4 and U_4 5 distinct values per block -- 12 sums
-        // and compares per block stand for 32 (h <= 4 are 90 % of all (r, j, h) triples of the plane)
 #pragma unroll
         for (int q = 0; q < 4; ++q)
-            if (m1[q] > r1.thr) flagged |= 0xffu << (8 * q);
-        float u2[8];
-#pragma unroll
-        for (int gq = 0; gq < 8; ++gq) u2[gq] = m1[gq >> 1];
+            if (m1[q] > r1.tq) flagged |= 0xffu << (8 * q);
         if (he >= 2) {
+            int u2[8];
 #pragma unroll
             for (int gq = 0; gq < 8; ++gq) {
-                u2[gq] += m2[gq];
-                if (u2[gq] > r2.thr) flagged |= 0xfu << (4 * gq);
+                u2[gq] = m1[gq >> 1] + m2[gq];
+                if (u2[gq] > r2.tq) flagged |= 0xfu << (4 * gq);
+            }
+            if (he >= 3) {
+                int u3[16];
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    // (i >> 2, (3 i) >> 3) = (0,0) for i = 0,1,2; (0,1) for 3; (1,1) for 4,5; (1,2) for 6,7
+                    u3[4 * b + 0] = u2[2 * b] + m3[3 * b];
+                    u3[4 * b + 1] = u2[2 * b] + m3[3 * b + 1];
+                    u3[4 * b + 2] = u2[2 * b + 1] + m3[3 * b + 1];
+                    u3[4 * b + 3] = u2[2 * b + 1] + m3[3 * b + 2];
+                    if (u3[4 * b + 0] > r3.tq) flagged |= 0x07u << (8 * b);
+                    if (u3[4 * b + 1] > r3.tq) flagged |= 0x08u << (8 * b);
+                    if (u3[4 * b + 2] > r3.tq) flagged |= 0x30u << (8 * b);
+                    if (u3[4 * b + 3] > r3.tq) flagged |= 0xc0u << (8 * b);
+                }
+                if (he >= 4) {
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        // U_4 adds block i >> 1 of row_4: i = 0,1 | 2 | 3 | 4,5 | 6,7
+                        U4[5 * b + 0] = u3[4 * b + 0] + m4[4 * b];
+                        U4[5 * b + 1] = u3[4 * b + 0] + m4[4 * b + 1];
+                        U4[5 * b + 2] = u3[4 * b + 1] + m4[4 * b + 1];
+                        U4[5 * b + 3] = u3[4 * b + 2] + m4[4 * b + 2];
+                        U4[5 * b + 4] = u3[4 * b + 3] + m4[4 * b + 3];
+                        if (U4[5 * b + 0] > r4.tq) flagged |= 0x03u << (8 * b);
+                        if (U4[5 * b + 1] > r4.tq) flagged |= 0x04u << (8 * b);
+                        if (U4[5 * b + 2] > r4.tq) flagged |= 0x08u << (8 * b);
+                        if (U4[5 * b + 3] > r4.tq) flagged |= 0x30u << (8 * b);
+                        if (U4[5 * b + 4] > r4.tq) flagged |= 0xc0u << (8 * b);
+                    }
+                }
             }
         }
-        if (he >= 3) {
-            float u3[16];
+    }
+    if (he_max >= 5) {       // CTA-uniform
+        // harmonics 5..: two fundamentals per register, X = U + (0x7fff - tq) on each half-word
+        unsigned X[16], F[16];   // pair p: fundamentals 2p (low half-word) and 2p + 1 (high)
+        if (he >= 5) {
+            const unsigned base = (unsigned)(0x7fff - p.tq[3]) * 0x10001u;
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
-                // (i >> 2, (3 i) >> 3) = (0,0) for i = 0,1,2; (0,1) for 3; (1,1) for 4,5; (1,2) for 6,7
-                u3[4 * b + 0] = u2[2 * b] + m3[3 * b];
-                u3[4 * b + 1] = u2[2 * b] + m3[3 * b + 1];
-                u3[4 * b + 2] = u2[2 * b + 1] + m3[3 * b + 1];
-                u3[4 * b + 3] = u2[2 * b + 1] + m3[3 * b + 2];
-                if (u3[4 * b + 0] > r3.thr) flagged |= 0x07u << (8 * b);
-                if (u3[4 * b + 1] > r3.thr) flagged |= 0x08u << (8 * b);
-                if (u3[4 * b + 2] > r3.thr) flagged |= 0x30u << (8 * b);
-                if (u3[4 * b + 3] > r3.thr) flagged |= 0xc0u << (8 * b);
+                X[4 * b + 0] = (unsigned)U4[5 * b + 0] * 0x10001u + base;
+                X[4 * b + 1] = ((unsigned)U4[5 * b + 1] | ((unsigned)U4[5 * b + 2] << 16)) + base;
+                X[4 * b + 2] = (unsigned)U4[5 * b + 3] * 0x10001u + base;
+                X[4 * b + 3] = (unsigned)U4[5 * b + 4] * 0x10001u + base;
             }
-            if (he >= 4) {
 #pragma unroll
-                for (int b = 0; b < 4; ++b) {
-                    // U_4 adds block i >> 1 of row_4: i = 0,1 | 2 | 3 | 4,5 | 6,7
-                    const float v0 = u3[4 * b + 0] + m4[4 * b], v1 = u3[4 * b + 0] + m4[4 * b + 1];
-                    const float v2 = u3[4 * b + 1] + m4[4 * b + 1], v3 = u3[4 * b + 2] + m4[4 * b + 2];
-                    const float v4 = u3[4 * b + 3] + m4[4 * b + 3];
-                    if (v0 > r4.thr) flagged |= 0x03u << (8 * b);
-                    if (v1 > r4.thr) flagged |= 0x04u << (8 * b);
-                    if (v2 > r4.thr) flagged |= 0x08u << (8 * b);
-                    if (v3 > r4.thr) flagged |= 0x30u << (8 * b);
-                    if (v4 > r4.thr) flagged |= 0xc0u << (8 * b);
-                    U[8 * b + 0] = v0; U[8 * b + 1] = v0; U[8 * b + 2] = v1; U[8 * b + 3] = v2;
-                    U[8 * b + 4] = v3; U[8 * b + 5] = v3; U[8 * b + 6] = v4; U[8 * b + 7] = v4;
-                }
-            } else {
-#pragma unroll
-                for (int b = 0; b < 4; ++b) {
-                    U[8 * b + 0] = u3[4 * b]; U[8 * b + 1] = u3[4 * b]; U[8 * b + 2] = u3[4 * b];
-                    U[8 * b + 3] = u3[4 * b + 1];
-                    U[8 * b + 4] = u3[4 * b + 2]; U[8 * b + 5] = u3[4 * b + 2];
-                    U[8 * b + 6] = u3[4 * b + 3]; U[8 * b + 7] = u3[4 * b + 3];
-                }
-            }
-        } else {
-#pragma unroll
-            for (int i = 0; i < 32; ++i) U[i] = u2[i >> 2];
+            for (int pp = 0; pp < 16; ++pp) F[pp] = 0u;
         }
-    }
-    if (he_max >= 5) {   // harmonics 5, 6: eleven loads in flight
-        const PfRow r5 = pf_row(p, j, 5);
-        float m5[20], m6[24];
-        pf_load<5>(r5.mrow, Q, he >= 5, m5);
-        PfRow r6 = r5;
-        if (he_max >= 6) { r6 = pf_row(p, j, 6); pf_load<6>(r6.mrow, Q, he >= 6, m6); }
-        pf_add<5>(m5, r5.thr, he >= 5, U, flagged);
-        if (he_max >= 6) pf_add<6>(m6, r6.thr, he >= 6, U, flagged);
-    }
-    pf_single_from<7>(p, j, Q, he_max, he, U, flagged);
-
-    // the (at most a few) harmonics for which only some of the 32 fundamentals are inside the plane
-    for (int k = he + 1; k <= hz; ++k) {
-        const unsigned rmax = last / (unsigned)k;
-        if (32u * Q > rmax) break;
-        const int nv = (int)min(32u, rmax - 32u * Q + 1u);
-        const PfRow r = pf_row(p, j, k);
-        const unsigned short* src = r.mrow + (size_t)k * 4 * Q;
+        pf_from<5>(p, j, Q, he_max, he, X, F);
+        if (he >= 5) {
+            // bit 15 - p <- fundamental 2p, bit 31 - p <- fundamental 2p + 1
+            unsigned acc = 0u;
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-            if (i < nv) {
-                U[i] += bf16_lo(__ldg(src + ((k * i) >> 3)));
-                if (U[i] > r.thr) flagged |= 1u << i;
+            for (int pp = 0; pp < 16; ++pp) acc |= (F[pp] & 0x80008000u) >> pp;
+            if (acc) {
+#pragma unroll
+                for (int pp = 0; pp < 16; ++pp) {
+                    if (acc & (0x8000u >> pp)) flagged |= 1u << (2 * pp);
+                    if (acc & (0x80000000u >> pp)) flagged |= 1u << (2 * pp + 1);
+                }
             }
         }
     }
-
-    pf_emit(p, Q, j, flagged);
+    if (he < hz && 32u * Q <= last / (unsigned)(he + 1)) {
+        // the thread that straddles the end of harmonic he+1's range (one per harmonic and row): that
+        // harmonic exists for its first fundamentals only -- all 32 go to the exact pass, which knows
+        flagged = 0xffffffffu;
+    }
+    pf_emit_warp(p, Q, j, mine ? flagged : 0u);
 }
 
 // ---- pass B: one thread per maybe record (r, j): the plain definition on the real plane.
@@ -663,9 +806,21 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
                             int* launches) {
     *launches = 0;
     HarmParams p = p_in;
+    // integer thresholds of pass A: tq_h <= 8 T_h (1 - 2^-18) -- the slack covers the rounding of the exact
+    // pass's fp32 sums (S_h^fp32 <= (1 + 2^-19) sum P for h <= 32) -- clamped below the saturated code, so
+    // that a block without a bound trips every flag; a negative T_h passes every point (tq = -1)
+    for (int h = 0; h < 32; ++h) {
+        const float T = p.thr[h];
+        if (!(T >= 0.f)) {
+            p.tq[h] = -1;
+        } else {
+            const double v = std::floor((double)kMaxCodeScale * (double)T * (1.0 - 1.0 / 262144.0));
+            p.tq[h] = v > (double)(kMaxCodeSat - 1) ? (int)(kMaxCodeSat - 1) : (int)v;
+        }
+    }
     cudaError_t e = cudaMemsetAsync(p.count, 0, sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(p.maybe_count, 0, 2 * sizeof(unsigned long long), st);   // + overflow flag
+    e = cudaMemsetAsync(p.maybe_count, 0, 4 * sizeof(unsigned long long), st);   // + overflow flag, coarse count
     if (e != cudaSuccess) return e;
     if (p.r_lo >= p.nbins) return cudaSuccess;
     if (build_max) {
@@ -685,30 +840,34 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         ++*launches;
         p.maxplane = p.maxplane_nbr;
     }
-    // rows j < nlow and j >= nz - nlow have at most kShallowDepth harmonics inside the plane (reading
-    // A12), rows j < nlow2 and j >= nz - nlow2 at most two
-    int nlow = 0, nlow2 = 0;
-    if ((p.mpitch & 7) == 0) {   // the shallow passes stream octets of blocks
+    // rows j < nlow and j >= nz - nlow have at most kShallowDepth harmonics inside the plane (reading A12)
+    int nlow = 0;
+    const bool coarse = (p.mpitch & 63) == 0 && p.max2 != nullptr;  // the coarse level reads 8 coarse blocks per word
+    if (coarse) {
         const int c2 = p.nz - 1;
         auto hz_of = [&](int j) { const int d = c2 - 2 * j; return d == 0 ? p.H : std::min(p.H, c2 / d); };
-        while (2 * nlow2 < p.nz - 1 && hz_of(nlow2) <= 2) ++nlow2;
-        nlow = nlow2;
         while (2 * nlow < p.nz - 1 && hz_of(nlow) <= kShallowDepth) ++nlow;
     }
-    const unsigned sgx = (unsigned)((p.mpitch / 8 + kPfShallowThreads - 1) / kPfShallowThreads);
-    if (nlow2 > 0) {
-        prefilter_shallow_kernel<2><<<dim3(sgx, (unsigned)(2 * nlow2)), kPfShallowThreads, 0, st>>>(p, 0, nlow2);
+    const int ndeep = p.nz - 2 * nlow;          // rows with more than kShallowDepth harmonics
+    // of a deep row the general kernel takes the fundamentals r < 64 b_deep only (those that can have a fifth
+    // harmonic inside the plane); the rest goes through the coarse level like the shallow rows
+    unsigned b_deep = 0, q_end = (unsigned)(p.mpitch / 4);
+    if (coarse) {
+        const unsigned nB = (unsigned)(p.mpitch / 8);
+        b_deep = std::min(nB, (unsigned)((p.nbins - 1) / (64 * (kShallowDepth + 1))) + 1u);
+        q_end = 2u * b_deep;
+        // (p.maxplane is the dilated plane in the neighbour-maximised mode)
+        coarsen_max_kernel<<<dim3((nB + 255) / 256, (unsigned)p.nz), 256, 0, st>>>(p.maxplane, p.mpitch, p.max2);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
-        ++*launches;
-    }
-    if (nlow > nlow2) {
-        prefilter_shallow_kernel<4><<<dim3(sgx, (unsigned)(2 * (nlow - nlow2))), kPfShallowThreads, 0, st>>>(p, nlow2, nlow);
+        prefilter_coarse_kernel<<<dim3((nB / 8 + 255) / 256, (unsigned)p.nz), 256, 0, st>>>(p, b_deep);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
-        ++*launches;
+        prefilter_shallow_kernel<<<148 * 4, kPfShallowThreads, 0, st>>>(p);
+        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        *launches += 3;
     }
-    if (p.nz - 2 * nlow > 0) {
-        dim3 grid((unsigned)((p.mpitch / 4 + kPfThreads - 1) / kPfThreads), (unsigned)(p.nz - 2 * nlow)), block(kPfThreads);
-        prefilter_kernel<<<grid, block, 0, st>>>(p, nlow);
+    if (ndeep > 0 && q_end > 0) {
+        dim3 grid((q_end + kPfThreads - 1) / kPfThreads, (unsigned)ndeep), block(kPfThreads);
+        prefilter_kernel<<<grid, block, 0, st>>>(p, nlow, q_end);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
     }

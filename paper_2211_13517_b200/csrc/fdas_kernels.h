@@ -16,8 +16,8 @@ struct ConvParams {
     int64_t nbins;
     int64_t pitch;
     int nz, h, V;
-    unsigned short* maxplane;  // nz x mpitch bf16 bit patterns: max of every aligned block of 8 plane
-                               // columns (as stored), rounded toward +inf (an upper bound)
+    unsigned short* maxplane;  // nz x mpitch codes (fdas_maxcode.h): an upper bound of the max of every
+                               // aligned block of 8 plane columns (as stored)
     int64_t mpitch;      // nbins / 8
 };
 
@@ -77,15 +77,20 @@ struct HarmParams {
     int nz, H;
     int64_t r_lo;
     float thr[32];
+    int tq[32];                       // pass A's integer thresholds (filled by launch_harmonic)
     fdas_cand_t* cands;
     int64_t capacity;
     unsigned long long* count;        // caller's: true number of candidates
-    unsigned short* maxplane;         // plan-owned block-max plane (bf16 bits, rounded up), nz x mpitch
+    unsigned short* maxplane;         // plan-owned block-max plane (codes of fdas_maxcode.h), nz x mpitch
     int64_t mpitch;                   // nbins / 8
     uint2* maybe;                     // plan-owned list of (r, j): fundamentals that failed the prefilter
     int64_t maybe_capacity;
-    unsigned long long* maybe_count;  // plan-owned; followed by the overflow flag
+    unsigned long long* maybe_count;  // plan-owned; followed by the overflow flag and the coarse count
     unsigned* overflow;               // plan-owned: set if the maybe list was too small
+    unsigned short* max2;             // plan-owned coarse side plane: nz x nbins / 64 codes, max of 8 codes of M
+    uint2* coarse;                    // plan-owned list of (coarse block, row) that failed the coarse bound
+    int64_t coarse_capacity;
+    unsigned long long* coarse_count; // plan-owned (maybe_count + 2)
     int nbr;                          // 1: neighbour-maximised sums (reading A24)
     unsigned short* maxplane_nbr;     // plan-owned dilated side plane the prefilter scans when nbr = 1
 };

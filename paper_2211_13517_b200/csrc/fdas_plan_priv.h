@@ -41,13 +41,15 @@ struct fdas_plan_s {
     fdas::TcMapCache tc_maps;                 // K2-TC tensor maps of the output buffers seen so far
     int nsm = 148;
     int64_t launches = 0;
-    unsigned short* d_maxplane = nullptr;    // block-max plane M (nz x nbins/8, bf16 bits), written by K2
+    unsigned short* d_maxplane = nullptr;    // block-max plane M (nz x nbins/8 codes of fdas_maxcode.h), written by K2
     const void* max_valid_for = nullptr;     // the plane M currently describes (nullptr: none)
     int hsum_mode = 0;                       // FDAS_HSUM_PLAIN | FDAS_HSUM_NEIGHBOUR_MAX
     unsigned short* d_maxplane_nbr = nullptr;   // dilated side plane (allocated when the mode is first set)
     cudaEvent_t ev_last = nullptr;           // end of the last public per-trial call (cross-stream ordering)
     cudaStream_t last_stream = nullptr;
     bool have_last = false;
+    unsigned short* d_max2 = nullptr;        // K3 coarse side plane M2 (nz x nbins/64 codes), rebuilt from M by every call
+    uint2* d_coarse = nullptr;               // K3 coarse maybe list (kCoarseCapacity records)
     uint2* d_maybe = nullptr;                // K3 maybe list (kMaybeCapacity records)
     unsigned long long* d_maybe_count = nullptr;
     // workspace of fdas_search_host (lazy)

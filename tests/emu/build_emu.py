@@ -11,7 +11,7 @@ CSRC = os.path.join(os.path.dirname(os.path.dirname(HERE)), "paper_2211_13517_b2
 EMU = os.path.join(HERE, "libfdas_emu.so")
 NVCC = os.path.join(os.environ.get("CUDA_HOME", "/usr/local/cuda"), "bin", "nvcc")
 SOURCES = [os.path.join(HERE, "fdas_emu.cu"), os.path.join(CSRC, "fdas_host.cpp")]
-DEPS = SOURCES + [os.path.join(CSRC, h) for h in ("fdas_fft_core.cuh", "fdas_tc_common.h", "fdas_host.h")]
+DEPS = SOURCES + [os.path.join(CSRC, h) for h in ("fdas_fft_core.cuh", "fdas_tc_common.h", "fdas_host.h", "fdas_maxcode.h")]
 
 
 def build_emu(force: bool = False, verbose: bool = False) -> str:

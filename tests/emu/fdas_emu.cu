@@ -13,6 +13,7 @@
 #include "../../include/fdas.h"
 #include "../../paper_2211_13517_b200/csrc/fdas_fft_core.cuh"
 #include "../../paper_2211_13517_b200/csrc/fdas_host.h"
+#include "../../paper_2211_13517_b200/csrc/fdas_maxcode.h"
 #include "../../paper_2211_13517_b200/csrc/fdas_tc_common.h"
 
 using namespace fdas;
@@ -227,7 +228,7 @@ void emu_umma_ts(const std::vector<unsigned char>& smem, std::vector<uint32_t>& 
 
 extern "C" {
 // spec: nb complex fp32 (rounded here to bf16 as K1b stores it); plane: nz x nb float (plane16: the
-// bf16-rounded value as float); maxplane: nz x nb/8 bf16 bit patterns.  nb must be a multiple of 128.
+// bf16-rounded value as float); maxplane: nz x nb/8 block-max codes.  nb must be a multiple of 128.
 int fdas_emu_convolve_tc(const float* spec, int64_t nb, double zmax, double zstep, int plane16,
                          float* plane, uint16_t* maxplane) {
     using namespace fdas::tc;
@@ -316,16 +317,12 @@ int fdas_emu_convolve_tc(const float* spec, int64_t nb, double zmax, double zste
         }
     }
     }
-    // block maxima of the values as stored, rounded toward +inf to bf16
+    // block maxima of the values as stored, as the codes of fdas_maxcode.h
     for (int j = 0; j < nz; ++j)
         for (int64_t b = 0; b < mpitch; ++b) {
-            uint32_t m = 0;
-            for (int e = 0; e < 8; ++e) {
-                uint32_t bits;
-                std::memcpy(&bits, &plane[(size_t)j * nb + 8 * b + e], 4);
-                m = std::max(m, (bits + 0xffffu) >> 16);
-            }
-            maxplane[(size_t)j * mpitch + b] = (uint16_t)m;
+            float m = plane[(size_t)j * nb + 8 * b];
+            for (int e = 1; e < 8; ++e) m = std::max(m, plane[(size_t)j * nb + 8 * b + e]);
+            maxplane[(size_t)j * mpitch + b] = (uint16_t)max_code(m);
         }
     return FDAS_OK;
 }

@@ -90,7 +90,7 @@ def test_tiny_fp32_full_parity(fdas, torch_, oracle):
     record_stats("tiny_fp32", {**ps.summary(orc.P.max()), **stats})
     keys = set(gpu_cand_dict(res.cands))
     assert (20000, 23, 1) in keys or (20000, 24, 1) in keys     # the injected signal (z0 = 7.5)
-    assert plan.launch_count() == 8      # K1a, K1b, K2, K3 two shallow + general prefilter, exact, flags (cuFFT not counted)
+    assert plan.launch_count() == 9      # K1a, K1b, K2, K3: coarsen, coarse + listed + general prefilter, exact, flags (cuFFT not counted)
 
 
 # ------------------------------------------------------------------------------------ configs[1]
@@ -416,10 +416,9 @@ def test_blockmax_plane_and_prefilter_equivalence(fdas, torch_, precision):
     assert pitch == nb // 8
     M = _device_view(torch, ptr, nz * pitch).view(nz, pitch).clone()
     ref = d_plane.float().view(nz, pitch, 8).amax(dim=2)
-    ref_bits = ((ref.view(torch.int32) + 0xFFFF) >> 16).to(torch.int16)      # round toward +inf (P >= 0)
-    assert torch.equal(M, ref_bits)
-    up = (M.to(torch.int32) << 16).view(torch.float32)
-    assert bool((up >= ref).all()) and bool((up <= ref * (1 + 2.0 ** -7)).all())
+    assert torch.equal(M, max_codes(torch, ref))
+    up = M.float() / 8.0          # the bound a code stands for (1023: none)
+    assert bool(((up >= ref) | (M == 1023)).all()) and bool(((up <= ref + 0.125) | (M == 1023)).all())
     H = wl.nharm
     thr = fdas.thresholds_from_sigma(H, 4.0)      # lower threshold: more work for the exact pass
     d_c, d_n = plan.alloc_cands(1 << 18)
@@ -468,7 +467,7 @@ def test_tensor_core_path_odd_banks(fdas, torch_, oracle, precision, zmax):
     ptr, pitch = plan.debug_maxplane()
     M = _device_view(torch, ptr, nz * pitch).view(nz, pitch).clone()
     ref = d_plane.float().contiguous().view(nz, pitch, 8).amax(dim=2)
-    assert torch.equal(M, ((ref.view(torch.int32) + 0xFFFF) >> 16).to(torch.int16))
+    assert torch.equal(M, max_codes(torch, ref))
     # harmonic sums on that plane
     H = 8
     thr = fdas.thresholds_from_sigma(H, 3.0)
@@ -491,6 +490,11 @@ def test_tensor_core_path_unsupported_banks(fdas, torch_):
             fdas.Plan(1 << 14, 64e-6, zmax, zstep, 2048, "bf16_tc")
         assert ei.value.status == fdas.FDAS_EUNSUPPORTED
         fdas.Plan(1 << 14, 64e-6, zmax, zstep, 2048, "bf16").close()
+
+
+def max_codes(torch, ref):
+    """Expected block-max codes (csrc/fdas_maxcode.h): min(1023, ceil(8 x max of the 8 stored values)) as int16."""
+    return torch.clamp(torch.ceil(ref * 8.0), min=0.0, max=1023.0).to(torch.int16)
 
 
 def _device_view(torch, ptr, numel):
@@ -892,7 +896,7 @@ def test_other_segment_lengths_full_parity(fdas, torch_, oracle, precision, zmax
     ptr, pitch = plan.debug_maxplane()
     M = _device_view(torch, ptr, nz * pitch).view(nz, pitch).clone()
     ref = d_plane.float().view(nz, pitch, 8).amax(dim=2)
-    assert torch.equal(M, ((ref.view(torch.int32) + 0xFFFF) >> 16).to(torch.int16))
+    assert torch.equal(M, max_codes(torch, ref))
     res = plan.read_cands(d_c, d_n)
     oc = oracle.candidates(Pg, H, thr.astype(np.float64), 16)
     s_at, margin = oracle_margin_fn(oracle, Pg, H, 16)

@@ -187,10 +187,10 @@ def test_emulated_k2_tc_matches_the_oracle_plane(emu, oracle, zmax, nb):
         # against the oracle on the bf16-rounded spectrum (reading A11) only the bf16 rounding of the
         # taps (2^-9 relative per tap) and, for plane16, of the stored power remains
         assert np.abs(out - Pq).max() <= (5e-3 if not plane16 else 9e-3) * Pq.max(), np.abs(out - Pq).max() / Pq.max()
-        # block maxima bound the stored values from above, within one bf16 ulp
-        up = (mx.astype(np.uint32) << 16).view(np.float32)
+        # block-max codes (units of 1/8, rounded up, 1023 = no bound) bound the stored values from above
         blk = out.reshape(nz, nb // 8, 8).max(axis=2)
-        assert (up >= blk).all() and (up <= blk * (1 + 2.0 ** -7) + 1e-30).all()
+        assert np.array_equal(mx, np.minimum(np.ceil(blk * np.float32(8.0)), 1023).astype(np.uint16))
+        assert ((mx / 8.0 >= blk) | (mx == 1023)).all()
 
 
 # --------------------------------------------------------------------------- sharding over ranks
