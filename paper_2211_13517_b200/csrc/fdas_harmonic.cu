@@ -252,7 +252,7 @@ __global__ void __launch_bounds__(256) dilate_max_kernel(const unsigned short* _
 // harmonic k is the 4k codes M[row_k][4kQ .. 4kQ+4k-1] (k contiguous 64-bit loads) and fundamental i picks
 // code (k i) >> 3 of them -- a compile-time choice once k and i are unrolled (one PRMT per pair of
 // fundamentals, none where the pair is an aligned word).
-constexpr int kPfThreads = 128;
+constexpr int kPfThreads = 128;   // (coarsen_items assumes 128)
 
 struct PfRow { const unsigned short* mrow; int tq; };
 
@@ -550,15 +550,23 @@ __device__ __forceinline__ void pf_shallow_octet(const HarmParams& p, const unsi
 // the sum of a few maxima of Exp(1) noise stays far below the thresholds; the (B, j) that fail go to a list
 // for pf_shallow_octet.  (With 16 harmonics the coarse bound is useless: the deep part of the deep rows is
 // prefilter_kernel's.)
-__global__ void __launch_bounds__(256) coarsen_max_kernel(const unsigned short* __restrict__ M, const int64_t mpitch,
-                                                          unsigned short* __restrict__ M2) {
-    const int64_t nB = mpitch >> 3;
-    const int64_t B = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (B >= nB) return;
-    const uint4 v = __ldg(reinterpret_cast<const uint4*>(M + (size_t)blockIdx.y * mpitch) + B);
-    unsigned m = __vmaxu2(__vmaxu2(v.x, v.y), __vmaxu2(v.z, v.w));
-    m = max(m & 0xffffu, m >> 16);
-    M2[(size_t)blockIdx.y * nB + B] = (unsigned short)m;
+// M2[i] = max of the 8 codes M[8 i .. 8 i + 7] over the items [begin, end) (M's rows are contiguous, so both
+// planes are linear arrays); a CTA of kPfThreads threads, four 128-bit loads in flight per thread.
+__device__ __forceinline__ void coarsen_items(const unsigned short* __restrict__ M, unsigned short* __restrict__ M2,
+                                              const int64_t begin, const int64_t end) {
+    const uint4* src = reinterpret_cast<const uint4*>(M);
+    for (int64_t i0 = begin + threadIdx.x; i0 < end; i0 += 4 * 128) {
+        uint4 v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            v[u] = (i0 + 128 * u < end) ? __ldg(src + i0 + 128 * u) : make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            unsigned m = __vmaxu2(__vmaxu2(v[u].x, v[u].y), __vmaxu2(v[u].z, v[u].w));
+            m = max(m & 0xffffu, m >> 16);
+            if (i0 + 128 * u < end) M2[i0 + 128 * u] = (unsigned short)m;
+        }
+    }
 }
 
 constexpr int kShallowDepth = 4;
@@ -638,11 +646,26 @@ __global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(co
     }
 }
 
+// The launch also carries the CTAs that build the coarse plane M2 from M (coarsen_items), interleaved with the
+// prefilter's own (odd / even block index): that stream is bound by DRAM bandwidth, the prefilter by the
+// latency of its dependent loads, and neither needs the other's result -- side by side they take the time
+// of the longer one.  gx x gy = the prefilter's grid; per > 0: coarsen items per CTA.
 __global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmParams p, const int nlow,
-                                                                  const unsigned q_end) {
-    const int j = nlow + blockIdx.y;   // the rows with more than kShallowDepth harmonics (|z| <= zmax/5)
+                                                                  const unsigned q_end, const unsigned gx,
+                                                                  const unsigned gy, const int64_t per) {
+    unsigned bid = blockIdx.x;
+    if (per > 0) {
+        if (bid & 1u) {
+            const int64_t total = (int64_t)p.nz * (p.mpitch >> 3), begin = (int64_t)(bid >> 1) * per;
+            coarsen_items(p.maxplane, p.max2, begin, min(total, begin + per));
+            return;
+        }
+        bid >>= 1;
+    }
+    if (bid >= gx * gy) return;
+    const int j = nlow + (int)(bid / gx);   // the rows with more than kShallowDepth harmonics (|z| <= zmax/5)
     const int c2 = p.nz - 1;
-    const unsigned Q0 = blockIdx.x * (unsigned)kPfThreads;
+    const unsigned Q0 = (bid % gx) * (unsigned)kPfThreads;
     // q_end <= nbins / 32: the quad-blocks beyond it belong to the coarse level.  The threads beyond stay (with
     // nothing to do) for the warp-wide slot claim at the end; they redo the last quad-block's loads.
     const bool mine = Q0 + threadIdx.x < q_end;
@@ -856,20 +879,31 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         const unsigned nB = (unsigned)(p.mpitch / 8);
         b_deep = std::min(nB, (unsigned)((p.nbins - 1) / (64 * (kShallowDepth + 1))) + 1u);
         q_end = 2u * b_deep;
+    }
+    {   // the general prefilter (deep rows, r < 64 b_deep) and, interleaved with it, the CTAs that build M2
         // (p.maxplane is the dilated plane in the neighbour-maximised mode)
-        coarsen_max_kernel<<<dim3((nB + 255) / 256, (unsigned)p.nz), 256, 0, st>>>(p.maxplane, p.mpitch, p.max2);
-        if ((e = cudaGetLastError()) != cudaSuccess) return e;
+        const unsigned gx = ndeep > 0 ? (q_end + kPfThreads - 1) / kPfThreads : 0u, gy = (unsigned)std::max(ndeep, 0);
+        unsigned nblk = gx * gy;
+        int64_t per = 0;
+        if (coarse) {
+            const int64_t total = (int64_t)p.nz * (p.mpitch >> 3);
+            nblk = std::max(nblk, 148u * 8u);
+            per = ((total + nblk - 1) / nblk + 511) / 512 * 512;
+            nblk *= 2;
+        }
+        if (nblk > 0) {
+            prefilter_kernel<<<nblk, kPfThreads, 0, st>>>(p, nlow, q_end, gx, gy, per);
+            if ((e = cudaGetLastError()) != cudaSuccess) return e;
+            ++*launches;
+        }
+    }
+    if (coarse) {
+        const unsigned nB = (unsigned)(p.mpitch / 8);
         prefilter_coarse_kernel<<<dim3((nB / 8 + 255) / 256, (unsigned)p.nz), 256, 0, st>>>(p, b_deep);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         prefilter_shallow_kernel<<<148 * 4, kPfShallowThreads, 0, st>>>(p);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
-        *launches += 3;
-    }
-    if (ndeep > 0 && q_end > 0) {
-        dim3 grid((q_end + kPfThreads - 1) / kPfThreads, (unsigned)ndeep), block(kPfThreads);
-        prefilter_kernel<<<grid, block, 0, st>>>(p, nlow, q_end);
-        if ((e = cudaGetLastError()) != cudaSuccess) return e;
-        ++*launches;
+        *launches += 2;
     }
     if (p.nbr) {
         if (plane_is_bf16) exact_kernel<__nv_bfloat16, 1><<<kExactBlocks, 128, 0, st>>>(p);

@@ -90,7 +90,7 @@ def test_tiny_fp32_full_parity(fdas, torch_, oracle):
     record_stats("tiny_fp32", {**ps.summary(orc.P.max()), **stats})
     keys = set(gpu_cand_dict(res.cands))
     assert (20000, 23, 1) in keys or (20000, 24, 1) in keys     # the injected signal (z0 = 7.5)
-    assert plan.launch_count() == 9      # K1a, K1b, K2, K3: coarsen, coarse + listed + general prefilter, exact, flags (cuFFT not counted)
+    assert plan.launch_count() == 8      # K1a, K1b, K2, K3: general prefilter (+ coarsen), coarse, listed, exact, flags (cuFFT not counted)
 
 
 # ------------------------------------------------------------------------------------ configs[1]
