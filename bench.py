@@ -633,9 +633,9 @@ def run_cuda(args):
         "roofline_k3": {
             "kernel": "K3 prefilter kernels + exact_kernel + flag_kernel", "bound": "hbm", "achieved": k3_gbs,
             "peak": hbm_peak, "unit": "GB/s", "frac": k3_gbs / hbm_peak,
-            "note": "algorithmic bytes = one read of the bf16 block-max side plane (nz x Nb/8) that the "
-                    "branch-and-bound prefilter scans; K3 is bound by its own select arithmetic, not by DRAM "
-                    "(profiles/r01e: issue 59 %, 0.18 GB read per launch)",
+            "note": "algorithmic bytes = one read of the block-max side plane (nz x Nb/8 16-bit codes) that the "
+                    "branch-and-bound prefilter scans; K3 is bound by the latency of dependent loads and by its "
+                    "exact pass's random sector reads, not by DRAM bandwidth (profiles/r02b_k3.md)",
         },
         "clocks": m["clocks"],
     }

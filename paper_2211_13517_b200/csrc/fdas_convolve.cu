@@ -113,7 +113,7 @@ __device__ __forceinline__ void store_powers(const float2 (&x)[16], void* prow, 
             }
         }
         // block-max codes (fdas_maxcode.h): low half = block q2, high half = block q2 + 1
-        unsigned w = max_code(mx[0]) | (max_code(mx[1]) << 16);
+        unsigned w = max_code2(mx[0], mx[1]);
         w = __vmaxu2(w, __shfl_xor_sync(0xffffffffu, w, 1));
         w = __vmaxu2(w, __shfl_xor_sync(0xffffffffu, w, 2));
         if constexpr (G::Ra == 16) w = __vmaxu2(w, __shfl_xor_sync(0xffffffffu, w, 4));

@@ -206,8 +206,7 @@ __device__ __forceinline__ unsigned group_to_smem(const uint32_t* __restrict__ a
         }
         const float fp = fmaxf(fmaxf(fmaxf(Pp[0], Pp[1]), fmaxf(Pp[2], Pp[3])), fmaxf(fmaxf(Pp[4], Pp[5]), fmaxf(Pp[6], Pp[7])));
         const float fm = fmaxf(fmaxf(fmaxf(Pm[0], Pm[1]), fmaxf(Pm[2], Pm[3])), fmaxf(fmaxf(Pm[4], Pm[5]), fmaxf(Pm[6], Pm[7])));
-        mp = max_code(fp);
-        mm = max_code(fm);
+        return max_code2(fp, fm);
     }
     return mp | (mm << 16);
 }

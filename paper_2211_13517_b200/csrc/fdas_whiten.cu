@@ -99,7 +99,7 @@ __device__ __forceinline__ int64_t centre2(const WhitenParams& p, int b) {
 }
 
 constexpr int kScaleThreads = 256;
-constexpr int kScalePer = 4;   // bins per thread, strided by the CTA width (coalesced)
+constexpr int kScalePer = 8;   // bins per thread, strided by the CTA width (coalesced)
 
 // One CTA scales kScaleThreads * kScalePer consecutive bins.  The bracketing pair of block centres is
 // found once per CTA by binary search for its first bin; every bin then walks forward from there (the
@@ -120,7 +120,11 @@ __global__ void __launch_bounds__(kScaleThreads) whiten_scale_kernel(const White
     }
     __syncthreads();
     const int64_t c2_first = centre2(p, 0), c2_last = centre2(p, last);
-    int lo = s_lo;
+    const float m_first = p.blk_med[0], m_last = p.blk_med[last];
+    // the bracketing pair of centres and its medians stay in registers while the bins remain between them
+    int lo = min(s_lo, max(last - 1, 0));
+    int64_t c2lo = centre2(p, lo), c2hi = centre2(p, min(lo + 1, last));
+    float mlo = p.blk_med[lo], mhi = p.blk_med[min(lo + 1, last)];
 #pragma unroll
     for (int q = 0; q < kScalePer; ++q) {
         const int64_t k = k0 + threadIdx.x + q * kScaleThreads;
@@ -129,13 +133,15 @@ __global__ void __launch_bounds__(kScaleThreads) whiten_scale_kernel(const White
         if (k > 0) {
             const int64_t k2 = 2 * k;
             float m;
-            if (k2 <= c2_first) m = p.blk_med[0];
-            else if (k2 >= c2_last) m = p.blk_med[last];
+            if (k2 <= c2_first) m = m_first;
+            else if (k2 >= c2_last) m = m_last;
             else {
-                while (lo + 1 < last && centre2(p, lo + 1) <= k2) ++lo;   // c2[lo] <= k2 < c2[lo+1]
-                const int64_t c2lo = centre2(p, lo), c2hi = centre2(p, lo + 1);
+                if (k2 >= c2hi) {                                       // c2[lo] <= k2 < c2[lo+1]
+                    while (lo + 1 < last && centre2(p, lo + 1) <= k2) ++lo;
+                    c2lo = centre2(p, lo); c2hi = centre2(p, lo + 1);
+                    mlo = p.blk_med[lo]; mhi = p.blk_med[lo + 1];
+                }
                 const float t = (float)(k2 - c2lo) / (float)(c2hi - c2lo);
-                const float mlo = p.blk_med[lo], mhi = p.blk_med[lo + 1];
                 m = mlo + t * (mhi - mlo);
             }
             const float sc = sqrtf(0.69314718055994530942f / m);
