@@ -635,7 +635,7 @@ def run_cuda(args):
             "peak": hbm_peak, "unit": "GB/s", "frac": k3_gbs / hbm_peak,
             "note": "algorithmic bytes = one read of the block-max side plane (nz x Nb/8 16-bit codes) that the "
                     "branch-and-bound prefilter scans; K3 is bound by the latency of dependent loads and by its "
-                    "exact pass's random sector reads, not by DRAM bandwidth (profiles/r02b_k3.md)",
+                    "exact pass's random sector reads, not by DRAM bandwidth (profiles/r02b_k3_seglen.md)",
         },
         "clocks": m["clocks"],
     }

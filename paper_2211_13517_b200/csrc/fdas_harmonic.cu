@@ -228,15 +228,35 @@ __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
     p.maxplane[(size_t)j * p.mpitch + b] = (unsigned short)max_code(m);
 }
 
-// ---- M' = M dilated by D blocks on either side (neighbour-maximised sums): one thread per block.
+// ---- M' = M dilated by D <= 8 blocks on either side (neighbour-maximised sums): one thread per octet of
+// blocks (a 128-bit word and its two neighbours; codes order like the values, missing neighbours count 0).
 __global__ void __launch_bounds__(256) dilate_max_kernel(const unsigned short* __restrict__ src,
                                                          unsigned short* __restrict__ dst, int64_t mpitch, int D) {
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= mpitch) return;
-    const unsigned short* row = src + (size_t)blockIdx.y * mpitch;
-    unsigned m = 0;     // codes order like the values
-    for (int64_t e = max((int64_t)0, b - D); e <= min(mpitch - 1, b + D); ++e) m = max(m, (unsigned)__ldg(row + e));
-    dst[(size_t)blockIdx.y * mpitch + b] = (unsigned short)m;
+    const int64_t nO = mpitch >> 3;                       // mpitch is a multiple of 8
+    const int64_t O = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (O >= nO) return;
+    const uint4* row = reinterpret_cast<const uint4*>(src + (size_t)blockIdx.y * mpitch);
+    const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+    const uint4 w[3] = {O > 0 ? __ldg(row + O - 1) : z, __ldg(row + O), O + 1 < nO ? __ldg(row + O + 1) : z};
+    unsigned c[24];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        c[8 * q + 0] = w[q].x & 0xffffu; c[8 * q + 1] = w[q].x >> 16;
+        c[8 * q + 2] = w[q].y & 0xffffu; c[8 * q + 3] = w[q].y >> 16;
+        c[8 * q + 4] = w[q].z & 0xffffu; c[8 * q + 5] = w[q].z >> 16;
+        c[8 * q + 6] = w[q].w & 0xffffu; c[8 * q + 7] = w[q].w >> 16;
+    }
+    unsigned o[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+        unsigned m = c[8 + e];
+#pragma unroll
+        for (int x = 1; x <= 8; ++x)
+            if (x <= D) m = max(m, max(c[8 + e - x], c[8 + e + x]));
+        o[e] = m;
+    }
+    reinterpret_cast<uint4*>(dst + (size_t)blockIdx.y * mpitch)[O] =
+        make_uint4(o[0] | (o[1] << 16), o[2] | (o[3] << 16), o[4] | (o[5] << 16), o[6] | (o[7] << 16));
 }
 
 // ---- pass A: upper bounds from the block-max plane, in integer arithmetic on the codes of fdas_maxcode.h.
@@ -857,7 +877,8 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         // the prefilter (and nothing else) scans the dilated side plane from here on
         if (!p.maxplane_nbr) return cudaErrorInvalidValue;
         const int D = ((p.H >> 1) + 7) >> 3;
-        dim3 grid((unsigned)((p.mpitch + 255) / 256), (unsigned)p.nz);
+        if (D > 8 || (p.mpitch & 7)) return cudaErrorInvalidValue;     // H <= 32 gives D <= 2; mpitch = nbins / 8
+        dim3 grid((unsigned)((p.mpitch / 8 + 255) / 256), (unsigned)p.nz);
         dilate_max_kernel<<<grid, 256, 0, st>>>(p.maxplane, p.maxplane_nbr, p.mpitch, D);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
