@@ -727,6 +727,36 @@ def test_harmonic_maybe_list_overflow_falls_back_to_full_scan(fdas, torch_, orac
         assert abs(s_at(*key) - thr[key[2] - 1]) <= 1e-5 * thr[key[2] - 1], key
 
 
+def test_harmonic_coarse_list_overflow_falls_back_to_full_scan(fdas, torch_):
+    """More coarse blocks (64 fundamentals each) fail the coarse bound than the coarse list holds (2^20): pass B
+    must scan every fundamental.  H = 1, so the expected set is the definition itself: every P > T_1, r >= r_lo."""
+    torch = torch_
+    plan = fdas.Plan(1 << 21, 64e-6, 32.0, 1.0, 2048, "fp32")       # 65 x 2^20 points, 65 x 16384 coarse blocks
+    nb, nz = plan.info.nbins, plan.info.nz
+    assert nz * (nb // 64) > (1 << 20)
+    rng = np.random.default_rng(43)
+    P32 = rng.exponential(1.0, size=(nz, nb)).astype(np.float32)
+    d_plane = torch.from_numpy(P32).cuda()
+    thr = np.array([0.05], dtype=np.float32)
+    r_lo = 5
+    d_c, d_n = plan.alloc_cands(1 << 16)
+    plan.harmonic_sum_peaks(d_plane, 1, thr, r_lo, d_c, d_n)
+    torch.cuda.synchronize()
+    res = plan.read_cands(d_c, d_n)
+    assert res.count == int((P32[:, r_lo:] > thr[0]).sum())          # bit-exact: S_1 is the stored value
+    c = res.cands
+    assert len(c) == 1 << 16 and np.all(c["h"] == 1) and np.all(c["r"] >= r_lo)
+    key = c["zidx"].astype(np.int64) * nb + c["r"]
+    assert np.unique(key).size == key.size
+    assert np.array_equal(c["power"], P32[c["zidx"], c["r"]]) and np.all(c["power"] > thr[0])
+    # and the same call on a quiet plane with one line finds exactly that line through the two lists
+    d_plane.zero_()
+    d_plane[40, 123457] = 3.0
+    plan.harmonic_sum_peaks(d_plane, 1, thr, r_lo, d_c, d_n)
+    res = plan.read_cands(d_c, d_n)
+    assert res.count == 1 and (int(res.cands[0]["r"]), int(res.cands[0]["zidx"]), int(res.cands[0]["h"])) == (123457, 40, 1)
+
+
 def test_harmonic_even_nz_half_integer_rows(fdas, torch_, oracle):
     """Reading A20 on the GPU: with an even number of templates (z = -7.5 .. 7.5) the odd harmonics
     of a row fall between two rows and round half away from zero, on both sides."""
