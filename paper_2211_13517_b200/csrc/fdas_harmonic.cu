@@ -10,7 +10,11 @@
 //   pass A (prefilter)  U_h(r,j) = sum_{k<=h} M[row_k][(k r) >> 3] >= S_h(r,j) term by term (exact integer
 //                       sums of the codes, two fundamentals per 32-bit add) -- so U_h <= T_h for all
 //                       h proves that (r, j) has no candidate without touching the plane.  The few
-//                       fundamentals for which some bound fails go to a "maybe" list.
+//                       fundamentals for which some bound fails go to a "maybe" list.  Where a fundamental
+//                       has at most four harmonics (most of the plane) the same bound is first taken on
+//                       coarse blocks of 64 columns (M2 = max of 8 codes of M, level 0), and only the coarse
+//                       blocks that fail are looked at block by block (level 1); the rest -- the first fifth
+//                       of the 39 rows with |z| <= zmax/5 at the SKA size -- is prefilter_kernel's.
 //   pass B (exact)      one thread per listed fundamental: the plain definition above on the real
 //                       plane, thresholds, atomic slot claim.
 //   pass C (flags)      one thread per (stored candidate, neighbour): local-maximum attribute.
@@ -468,11 +472,11 @@ __device__ __forceinline__ void pf_emit_warp(const HarmParams& p, const unsigned
     }
 }
 
-// Rows with at most kShallowDepth = 4 harmonics inside the plane (|z| > zmax/5: the nlow first and the
-// nlow last rows, four fifths of the plane).  Harmonic k picks block (k i) >> 3 for fundamental i of a
-// block of 8, so U_1 is the same for all 8 fundamentals, U_2 for halves, U_3 takes 4 and U_4 5 distinct
-// values per block: 12 sums and compares stand for 32.  A thread streams 8 blocks (64 fundamentals) of
-// M[j] and the 8k blocks of M[row_k] they map to; few registers, every load issued up front.
+// ---- level 1 of pass A for the parts of the plane with at most kShallowDepth = 4 harmonics: the block-level
+// bound for the 64 fundamentals of an octet of blocks (= one coarse block) that failed the coarse bound below.
+// Harmonic k picks block (k i) >> 3 for fundamental i of a block of 8, so U_1 is the same for all 8
+// fundamentals, U_2 for halves, U_3 takes 4 and U_4 5 distinct values per block: 12 sums and compares stand for
+// 32.  A thread reads 8 blocks of M[j] and the 8k blocks of M[row_k] they map to, every load issued up front.
 constexpr int kPfShallowThreads = 256;
 
 __device__ __forceinline__ int code_at(const uint4 (&w)[4], const int e) {   // code e of up to 32 (static e)
@@ -481,8 +485,6 @@ __device__ __forceinline__ int code_at(const uint4 (&w)[4], const int e) {   // 
     return (int)((e & 1) ? (x >> 16) : (x & 0xffffu));
 }
 
-// DMAX = 2 | 4: deepest harmonic of the rows this instance scans, rows [ja, jb) and their mirror images
-// [nz - jb, nz - ja) (the two-harmonic instance needs a third of the registers of the four-harmonic one).
 // The 64 fundamentals of octet O (8 blocks of M) of row j, for at most DMAX harmonics: the caller guarantees
 // that no fundamental of the octet has a harmonic DMAX + 1 inside the plane (in z or in r).
 template <int DMAX>
@@ -793,7 +795,7 @@ __global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmPara
 }
 
 // ---- pass B: one thread per maybe record (r, j): the plain definition on the real plane.
-// If the maybe list overflowed (pathological thresholds), every fundamental is evaluated instead.
+// If the maybe list or the coarse list overflowed (pathological thresholds), every fundamental is evaluated instead.
 template <typename T, int NBR>
 __global__ void __launch_bounds__(128) exact_kernel(const HarmParams p) {
     __shared__ float sthr[32];
