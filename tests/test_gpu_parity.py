@@ -290,6 +290,63 @@ def test_harmonic_sum_small_h_exact_sets(fdas, torch_, oracle, H):
     assert min(k[0] for k in gpu_cand_dict(res.cands)) >= r_lo
 
 
+@pytest.mark.parametrize("case", range(8))
+def test_harmonic_sum_hand_made_planes_against_the_oracle(fdas, torch_, oracle, case):
+    """K3 alone on seeded hand-made planes that stress the integer bounds of the prefilter: values far above the
+    saturation of the block-max codes (127.875), exact multiples of the code unit (1/8), zeros, thresholds that are
+    not monotone in h, a negative threshold (every point passes), thresholds above the saturation, r_lo inside a
+    block, odd and even template counts, plane widths of 1024 .. 32768 bins -- and in the neighbour-maximised mode
+    as well.  fp32 planes: the candidate set is the oracle's (up to rounding at a threshold)."""
+    torch = torch_
+    rng = np.random.default_rng(900 + case)
+    zmax = [16.0, 7.5, 32.0, 16.0, 96.0, 3.0, 16.0, 7.5][case]
+    n = [1 << 13, 1 << 14, 1 << 15, 1 << 16, 1 << 13, 1 << 14, 1 << 11, 1 << 13][case]
+    H = [16, 8, 5, 32, 16, 12, 4, 16][case]
+    nbr = case in (3, 6)
+    plan = fdas.Plan(n, 64e-6, zmax, 1.0, 1024 if n == (1 << 11) else 2048, "fp32")
+    nb, nz = plan.info.nbins, plan.info.nz
+    P32 = rng.exponential(1.0, size=(nz, nb)).astype(np.float32)
+    P32 = np.ceil(P32 * 8.0).astype(np.float32) / 8.0 if case % 2 else P32          # exact code boundaries
+    P32[rng.random((nz, nb)) < 0.05] = 0.0
+    for _ in range(40):                                                             # lines with harmonics
+        j, r = int(rng.integers(0, nz)), int(rng.integers(1, nb // 4))
+        a = float(rng.choice([6.0, 30.0, 127.875, 128.0, 500.0, 4000.0]))
+        c = (nz - 1) // 2
+        for k in range(1, 9):
+            rk, jk = k * r, k * (j - c) + c                  # row of harmonic k (odd template counts)
+            if nz % 2 and rk < nb and 0 <= jk < nz:
+                P32[jk, rk] += a / k
+    thr = fdas.thresholds_from_sigma(H, [3.0, 2.5, 3.5, 2.0, 3.0, 2.5, 2.5, 3.0][case]).copy()
+    if case == 1:
+        thr[2] = 0.6 * thr[1]; thr[5] = 400.0               # not monotone; one above the saturation
+    if case == 2:
+        thr[0] = -1.0                                       # every point passes h = 1
+    if case == 5:
+        thr[:] = thr * 6.0 + 130.0                          # all above the saturation: only strong lines
+    r_lo = [37, 1, 64, 9, 200, 5, 3, 0][case]
+    if nbr:
+        plan.set_harmonic_mode("neighbour_max")
+    d_plane = torch.from_numpy(P32).cuda()
+    cap = 1 << 22
+    d_c, d_n = plan.alloc_cands(cap)
+    plan.harmonic_sum_peaks(d_plane, H, thr, r_lo, d_c, d_n)
+    torch.cuda.synchronize()
+    res = plan.read_cands(d_c, d_n)
+    P = P32.astype(np.float64)
+    oc = oracle.candidates(P, H, thr.astype(np.float64), r_lo, capacity=cap, nbr=nbr)
+    assert res.count <= cap and oc.count > 50
+    got, want = gpu_cand_dict(res.cands), oc.as_dict()
+    sums = oracle.harmonic_sums_nbr_at if nbr else oracle.harmonic_sums_at
+    for key in set(got) ^ set(want):                        # one-sided: the oracle's sum sits on its threshold
+        so = want[key][0] if key in want else float(sums(P, key[2], key[0], key[1])[key[2] - 1])
+        assert abs(so - thr[key[2] - 1]) <= 2e-6 * max(abs(so), 1.0), (case, key, so, thr[key[2] - 1])
+    assert len(set(got) ^ set(want)) <= 4
+    for key in set(got) & set(want):
+        assert abs(got[key][0] - want[key][0]) <= 2e-6 * max(want[key][0], 1.0), (case, key)
+    assert min(k[0] for k in got) >= r_lo
+    plan.close()
+
+
 def test_abi_errors_on_device(fdas, torch_):
     import ctypes as C
     torch = torch_
