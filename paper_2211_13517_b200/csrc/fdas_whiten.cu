@@ -125,6 +125,7 @@ __global__ void __launch_bounds__(kScaleThreads) whiten_scale_kernel(const White
     int lo = min(s_lo, max(last - 1, 0));
     int64_t c2lo = centre2(p, lo), c2hi = centre2(p, min(lo + 1, last));
     float mlo = p.blk_med[lo], mhi = p.blk_med[min(lo + 1, last)];
+    float slope = (mhi - mlo) / (float)(int)max(c2hi - c2lo, (int64_t)1);       // per half bin (centres are in half bins)
 #pragma unroll
     for (int q = 0; q < kScalePer; ++q) {
         const int64_t k = k0 + threadIdx.x + q * kScaleThreads;
@@ -140,11 +141,11 @@ __global__ void __launch_bounds__(kScaleThreads) whiten_scale_kernel(const White
                     while (lo + 1 < last && centre2(p, lo + 1) <= k2) ++lo;
                     c2lo = centre2(p, lo); c2hi = centre2(p, lo + 1);
                     mlo = p.blk_med[lo]; mhi = p.blk_med[lo + 1];
+                    slope = (mhi - mlo) / (float)(int)(c2hi - c2lo);
                 }
-                const float t = (float)(k2 - c2lo) / (float)(c2hi - c2lo);
-                m = mlo + t * (mhi - mlo);
+                m = fmaf((float)(int)(k2 - c2lo), slope, mlo);         // the distances fit 32 bits (blocks <= 4096 bins)
             }
-            const float sc = sqrtf(0.69314718055994530942f / m);
+            const float sc = 0.83255461115769775635f * rsqrtf(m);       // sqrt(ln 2 / m)
             const float2 x = __ldg(p.X + k);
             w = make_float2(x.x * sc, x.y * sc);
         }
