@@ -162,6 +162,37 @@ __device__ __forceinline__ void tma_wait_read() {
 }
 __device__ __forceinline__ void tma_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
+// Packed fp32x2 arithmetic (two IEEE fp32 results per instruction, sm_100).
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pk2u(uint32_t lo, uint32_t hi) {
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(lo), "r"(hi));
+    return r;
+}
+__device__ __forceinline__ void up2f(u64 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ u64 add2(u64 x, u64 y) {
+    u64 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(x), "l"(y));
+    return r;
+}
+__device__ __forceinline__ u64 sub2(u64 x, u64 y) {
+    u64 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(x), "l"(y));
+    return r;
+}
+__device__ __forceinline__ u64 mul2(u64 x, u64 y) {
+    u64 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(x), "l"(y));
+    return r;
+}
+__device__ __forceinline__ u64 fma2(u64 x, u64 y, u64 z) {
+    u64 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(x), "l"(y), "l"(z));
+    return r;
+}
+
 // Powers of 8 consecutive bins of the rows +z and -z of this thread's pair from one group of
 // accumulator columns (a = 16 columns of D_R: Ar[0..7] | Ai[0..7]; b = 16 columns of D_I: Br | Bi),
 // into this thread's rows (rowp, rowm) of the two staging tiles, 16-byte unit `2 * bg` (fp32) / `bg`
@@ -171,11 +202,27 @@ template <int PLANE16>
 __device__ __forceinline__ unsigned group_to_smem(const uint32_t* __restrict__ a, const uint32_t* __restrict__ b,
                                                   unsigned char* tile_p, unsigned char* tile_m, const int rowp,
                                                   const int rowm, const int half, const int bg) {
+    // pair_powers (fdas_tc_common.h).  With a bf16 plane, two bins per instruction: the packed fp32x2 forms
+    // (FADD2 / FMUL2 / FFMA2) round each half exactly like the scalar ones at half the issue slots of the
+    // drain (K2-TC 0.550 -> 0.532 ms per SKA launch).  With an fp32 plane the kernel is bound by its stores and
+    // the shorter drain makes it SLOWER (0.650 -> 0.716 ms, profiles/r02b): the scalar forms stay.
     float Pp[8], Pm[8];
+    if constexpr (!PLANE16) {
 #pragma unroll
-    for (int e = 0; e < 8; ++e)
-        pair_powers(__uint_as_float(a[e]), __uint_as_float(b[e]), __uint_as_float(a[8 + e]),
-                    __uint_as_float(b[8 + e]), &Pp[e], &Pm[e]);
+        for (int e = 0; e < 8; ++e)
+            pair_powers(__uint_as_float(a[e]), __uint_as_float(b[e]), __uint_as_float(a[8 + e]),
+                        __uint_as_float(b[8 + e]), &Pp[e], &Pm[e]);
+    } else {
+#pragma unroll
+    for (int e = 0; e < 8; e += 2) {
+        const u64 Ar = pk2u(a[e], a[e + 1]), Ai = pk2u(a[8 + e], a[9 + e]);
+        const u64 Br = pk2u(b[e], b[e + 1]), Bi = pk2u(b[8 + e], b[9 + e]);
+        const u64 rp = add2(Ar, Bi), ip = sub2(Ai, Br), rm = sub2(Ar, Bi), im = add2(Ai, Br);
+        const u64 pp = fma2(rp, rp, mul2(ip, ip)), pm = fma2(rm, rm, mul2(im, im));
+        up2f(pp, Pp[e], Pp[e + 1]);
+        up2f(pm, Pm[e], Pm[e + 1]);
+    }
+    }
     unsigned mp, mm;
     if (PLANE16) {
         auto pack = [](float lo, float hi) {
