@@ -586,7 +586,7 @@ def run_cuda(args):
                     "ms_per_step": mf["ms_per_step"], "kernel_ms": mf["kernel_ms"], "energy": mf["energy"],
                     "gpu_launches": int(mf["launches"]), "candidates_last_step": mf["candidates_last_step"],
                     "roofline": rf, "roofline_hbm": rf_hbm, "clocks": mf["clocks"],
-                    "ncu_counters": "profiles/r01c_packed_fp32x2.md (FMA pipe 64.5 %, LSU data pipe 75 %, issue 74 %)"}
+                    "ncu_counters": "profiles/r02b_k3_seglen.md (FMA pipe 63.3 %, LSU wavefronts 73.0 %, issue 52.4 %; SASS: 502 instructions per thread and template)"}
         plan_f.close()
         torch.cuda.empty_cache()
         # the same kernel at the other segment lengths (K2 alone, 10 launches each, same
