@@ -614,37 +614,65 @@ __global__ void __launch_bounds__(256) prefilter_coarse_kernel(const HarmParams 
         if ((__vcmpgtu2(m1.x, tb2) | __vcmpgtu2(m1.y, tb2) | __vcmpgtu2(m1.z, tb2) | __vcmpgtu2(m1.w, tb2)) == 0u)
             return;                                                    // almost every thread of a one-harmonic row
     }
-    // harmonic k of coarse block B exists iff some fundamental of the block has it: 64 k B <= Nb - 1
-    uint4 mk[3][4];
-#pragma unroll
-    for (int k = 2; k <= kShallowDepth; ++k) {
-        const int row = min((2 * k * j - (k - 1) * c2 + 1) >> 1, c2);     // (unused when k > hz)
-        const uint4* src = reinterpret_cast<const uint4*>(M2 + (size_t)row * nB);
-#pragma unroll
-        for (int c = 0; c < k; ++c) {
-            const unsigned g = (unsigned)k * G + (unsigned)c;
-            mk[k - 2][c] = (k <= hz && g < nG) ? __ldg(src + g) : make_uint4(0u, 0u, 0u, 0u);
-        }
+    // harmonic k of coarse block B exists iff some fundamental of the block has it: 64 k B <= Nb - 1, i.e.
+    // B <= bmax_k; the codes of harmonic k as 4k words (two codes each), zeros where not loaded
+    unsigned w2[8], w3[12], w4[16];
+    {
+        auto load = [&](const int k, unsigned* w) {
+            const int row = min((2 * k * j - (k - 1) * c2 + 1) >> 1, c2);     // (unused when k > hz)
+            const uint4* src = reinterpret_cast<const uint4*>(M2 + (size_t)row * nB);
+#pragma unroll 4
+            for (int c = 0; c < 4; ++c) {
+                if (c < k) {
+                    const unsigned g = (unsigned)k * G + (unsigned)c;
+                    const uint4 v = (k <= hz && g < nG) ? __ldg(src + g) : make_uint4(0u, 0u, 0u, 0u);
+                    w[4 * c] = v.x; w[4 * c + 1] = v.y; w[4 * c + 2] = v.z; w[4 * c + 3] = v.w;
+                }
+            }
+        };
+        load(2, w2); load(3, w3); load(4, w4);
     }
-    auto code = [](const uint4& v, const int e) {                          // code e of 8 (static e)
-        const unsigned x = (e >> 1) == 0 ? v.x : (e >> 1) == 1 ? v.y : (e >> 1) == 2 ? v.z : v.w;
-        return (int)((e & 1) ? (x >> 16) : (x & 0xffffu));
-    };
+    const unsigned w1[4] = {m1.x, m1.y, m1.z, m1.w};
+    auto lo = [](unsigned x) { return (int)(x & 0xffffu); };
+    auto hi = [](unsigned x) { return (int)(x >> 16); };
+    auto max2 = [&](unsigned x) { return max(lo(x), hi(x)); };
+    {   // the whole thread at once: V_h = sum_{k<=h} (largest code of harmonic k among all its blocks) >= U0_h(B)
+        // for each of the 8 coarse blocks; V_h <= tq_h for all h settles them together
+        unsigned a1 = __vmaxu2(__vmaxu2(w1[0], w1[1]), __vmaxu2(w1[2], w1[3]));
+        unsigned a2 = 0u, a3 = 0u, a4 = 0u;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) a2 = __vmaxu2(a2, w2[c]);
+#pragma unroll
+        for (int c = 0; c < 12; ++c) a3 = __vmaxu2(a3, w3[c]);
+#pragma unroll
+        for (int c = 0; c < 16; ++c) a4 = __vmaxu2(a4, w4[c]);
+        int V = max2(a1);
+        bool any = V > p.tq[0];
+        V += max2(a2); any = any || (hz >= 2 && V > p.tq[1]);
+        V += max2(a3); any = any || (hz >= 3 && V > p.tq[2]);
+        V += max2(a4); any = any || (hz >= 4 && V > p.tq[3]);
+        if (!any) return;
+    }
+    const unsigned bmax2 = last / 128u, bmax3 = last / 192u, bmax4 = last / 256u;
     unsigned fl = 0u;
 #pragma unroll
     for (int q = 0; q < 8; ++q) {
         const unsigned B = 8u * G + (unsigned)q;
-        int U = code(m1, q);
+        int U = (q & 1) ? hi(w1[q >> 1]) : lo(w1[q >> 1]);
         bool f = U > p.tq[0];
-#pragma unroll
-        for (int k = 2; k <= kShallowDepth; ++k) {
-            int m = 0;
-#pragma unroll
-            for (int i = 0; i < k; ++i) m = max(m, code(mk[k - 2][(k * q + i) >> 3], (k * q + i) & 7));
-            // (a harmonic beyond hz, or beyond the plane in r for the whole block, was loaded as zeros or is skipped)
-            if (k <= hz && (unsigned long long)k * 64ull * B <= last) {
-                U += m;
-                f = f || U > p.tq[k - 1];
+        if (hz >= 2 && B <= bmax2) {                                     // codes 2q, 2q+1: word q
+            U += max2(w2[q]);
+            f = f || U > p.tq[1];
+            if (hz >= 3 && B <= bmax3) {                                 // codes 3q .. 3q+2
+                const int e = 3 * q;
+                const int m3 = (e & 1) ? max(hi(w3[e >> 1]), max2(w3[(e >> 1) + 1]))
+                                       : max(max2(w3[e >> 1]), lo(w3[(e >> 1) + 1]));
+                U += m3;
+                f = f || U > p.tq[2];
+                if (hz >= 4 && B <= bmax4) {                             // codes 4q .. 4q+3: words 2q, 2q+1
+                    U += max2(__vmaxu2(w4[2 * q], w4[2 * q + 1]));
+                    f = f || U > p.tq[3];
+                }
             }
         }
         if (f && !(deep && B < b_deep)) fl |= 1u << q;
