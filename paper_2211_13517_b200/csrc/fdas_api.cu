@@ -22,13 +22,12 @@ using namespace fdas;
 thread_local std::string g_detail;
 
 static const int64_t kMaybeCapacity = 1 << 22;  // K3 prefilter survivors (fundamentals) listed per call
-static const int64_t kCoarseCapacity = 1 << 20; // K3 coarse-level survivors (blocks of 64 fundamentals)
 
 static void free_plan(fdas_plan_s* p) {
     if (!p) return;
     free_batch_state(p->batch);
     cudaFree(p->d_maxplane); cudaFree(p->d_maxplane_nbr); cudaFree(p->d_maybe); cudaFree(p->d_maybe_count);
-    cudaFree(p->d_max2); cudaFree(p->d_coarse);
+    cudaFree(p->d_max2);
     cudaFree(p->d_bank); cudaFree(p->d_tw1); cudaFree(p->d_tw2); cudaFree(p->d_fft_work);
     cudaFree(p->d_X); cudaFree(p->d_blk_start); cudaFree(p->d_blk_len); cudaFree(p->d_blk_med);
     cudaFree(p->ws_series); cudaFree(p->ws_spec); cudaFree(p->ws_plane); cudaFree(p->ws_cands);
@@ -125,10 +124,9 @@ static int build_plan(fdas_plan_s* p) {
 
     CU(cudaMalloc(&p->d_maxplane, (size_t)in.nz * (size_t)(in.nbins / 8) * sizeof(unsigned short)));
     CU(cudaMalloc(&p->d_maybe, (size_t)kMaybeCapacity * sizeof(uint2)));
-    CU(cudaMalloc(&p->d_maybe_count, 4 * sizeof(unsigned long long)));
+    CU(cudaMalloc(&p->d_maybe_count, 2 * sizeof(unsigned long long)));
     if (in.nbins % 64 == 0) {
         CU(cudaMalloc(&p->d_max2, (size_t)(in.nbins / 64) * (size_t)in.nz * sizeof(unsigned short)));
-        CU(cudaMalloc(&p->d_coarse, (size_t)kCoarseCapacity * sizeof(uint2)));
     }
     CU(cudaMalloc(&p->d_X, (size_t)(in.nfft / 2 + 1) * sizeof(float2)));
     size_t ws = 0;
@@ -205,7 +203,6 @@ int fdas_enqueue_harmonic(fdas_plan_s* plan, const void* d_plane, unsigned short
     hp.maybe = plan->d_maybe; hp.maybe_capacity = kMaybeCapacity; hp.maybe_count = plan->d_maybe_count;
     hp.overflow = reinterpret_cast<unsigned*>(plan->d_maybe_count + 1);
     hp.max2 = plan->d_max2;
-    hp.coarse = plan->d_coarse; hp.coarse_capacity = kCoarseCapacity; hp.coarse_count = plan->d_maybe_count + 2;
     hp.nbr = plan->hsum_mode == FDAS_HSUM_NEIGHBOUR_MAX ? 1 : 0;
     hp.maxplane_nbr = plan->d_maxplane_nbr;
     int nl = 0;

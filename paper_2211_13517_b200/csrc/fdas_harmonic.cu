@@ -13,7 +13,7 @@
 //                       fundamentals for which some bound fails go to a "maybe" list.  Where a fundamental
 //                       has at most four harmonics (most of the plane) the same bound is first taken on
 //                       coarse blocks of 64 columns (M2 = max of 8 codes of M, level 0), and only the coarse
-//                       blocks that fail are looked at block by block (level 1); the rest -- the first fifth
+//                       blocks that fail are looked at block by block (level 1, by the same thread); the rest -- the first fifth
 //                       of the 39 rows with |z| <= zmax/5 at the SKA size -- is prefilter_kernel's.
 //   pass B (exact)      one thread per listed fundamental: the plain definition above on the real
 //                       plane, thresholds, atomic slot claim.
@@ -280,7 +280,8 @@ constexpr int kPfThreads = 128;   // (coarsen_items assumes 128)
 
 struct PfRow { const unsigned short* mrow; int tq; };
 
-__device__ __forceinline__ PfRow pf_row(const HarmParams& p, const int j, const int k) {
+template <class P>
+__device__ __forceinline__ PfRow pf_row(const P& p, const int j, const int k) {
     const int c2 = p.nz - 1;
     const int v2 = 2 * k * j - (k - 1) * c2;   // only called for k <= hz: v2 is in range
     PfRow r;
@@ -417,7 +418,8 @@ __device__ __forceinline__ void pf_from(const HarmParams& p, const int j, const 
 }
 
 // Fundamentals of quad-block Q flagged by pass A go to the maybe list as (r, j).
-__device__ __forceinline__ void pf_emit(const HarmParams& p, const unsigned Q, const int j, unsigned flagged) {
+template <class P>
+__device__ __forceinline__ void pf_emit(const P& p, const unsigned Q, const int j, unsigned flagged) {
     // r < r_lo never yields candidates
     if (32 * (int64_t)Q < p.r_lo) {
         const int64_t cut = p.r_lo - 32 * (int64_t)Q;
@@ -473,11 +475,12 @@ __device__ __forceinline__ void pf_emit_warp(const HarmParams& p, const unsigned
 }
 
 // ---- level 1 of pass A for the parts of the plane with at most kShallowDepth = 4 harmonics: the block-level
-// bound for the 64 fundamentals of an octet of blocks (= one coarse block) that failed the coarse bound below.
+// bound for the 64 fundamentals of an octet of blocks (= one coarse block) that failed the coarse bound below
+// (called from prefilter_coarse_kernel for those blocks only).
 // Harmonic k picks block (k i) >> 3 for fundamental i of a block of 8, so U_1 is the same for all 8
 // fundamentals, U_2 for halves, U_3 takes 4 and U_4 5 distinct values per block: 12 sums and compares stand for
 // 32.  A thread reads 8 blocks of M[j] and the 8k blocks of M[row_k] they map to, every load issued up front.
-constexpr int kPfShallowThreads = 256;
+constexpr int kShallowDepth = 4;
 
 __device__ __forceinline__ int code_at(const uint4 (&w)[4], const int e) {   // code e of up to 32 (static e)
     const uint4 v = w[e >> 3];
@@ -487,8 +490,8 @@ __device__ __forceinline__ int code_at(const uint4 (&w)[4], const int e) {   // 
 
 // The 64 fundamentals of octet O (8 blocks of M) of row j, for at most DMAX harmonics: the caller guarantees
 // that no fundamental of the octet has a harmonic DMAX + 1 inside the plane (in z or in r).
-template <int DMAX>
-__device__ __forceinline__ void pf_shallow_octet(const HarmParams& p, const unsigned O, const int j) {
+template <int DMAX, class P>
+__device__ __forceinline__ void pf_shallow_octet(const P& p, const unsigned O, const int j) {
     const int c2 = p.nz - 1;
     const unsigned last = (unsigned)(p.nbins - 1);
     const int d = abs(2 * j - c2);
@@ -563,14 +566,29 @@ __device__ __forceinline__ void pf_shallow_octet(const HarmParams& p, const unsi
     pf_emit(p, 2u * O + 1u, j, f[1]);
 }
 
+// What pf_shallow_octet reads of the kernel parameters, BY VALUE for the out-of-line call from the coarse
+// kernel (a reference to the parameter struct would make every thread copy all of it to local memory).
+struct PfArgs {
+    const unsigned short* maxplane;
+    int64_t mpitch, nbins, r_lo, maybe_capacity;
+    uint2* maybe;
+    unsigned long long* maybe_count;
+    unsigned* overflow;
+    int nz, H;
+    int tq[kShallowDepth];
+};
+__device__ __noinline__ void pf_shallow_octet_call(const PfArgs a, const unsigned O, const int j) {
+    pf_shallow_octet<kShallowDepth>(a, O, j);
+}
+
 // ---- level 0 of pass A: the same bound on COARSE blocks of 64 plane columns.
 // M2[j][B] = max of the 8 codes M[j][8B .. 8B+7] (row-major, 1/8 of M: 25 MB at the SKA size, L2-resident).
 // For a fundamental r of coarse block B harmonic k lies in the coarse blocks kB .. kB + k - 1 of row_k, so
 //     U0_h(B,j) = sum_{k<=h} max_{i<k} M2[row_k][kB + i]  >=  U_h(r,j)  >=  8 S_h(r,j)   for all r in B:
 // U0_h <= tq_h for all h settles 64 fundamentals at once.  It serves the parts of the plane with at most
 // kShallowDepth harmonics -- the shallow rows, and of the deep rows the fundamentals r >= 64 b_deep -- where
-// the sum of a few maxima of Exp(1) noise stays far below the thresholds; the (B, j) that fail go to a list
-// for pf_shallow_octet.  (With 16 harmonics the coarse bound is useless: the deep part of the deep rows is
+// the sum of a few maxima of Exp(1) noise stays far below the thresholds; for the (B, j) that fail the same thread
+// goes on to the block level (pf_shallow_octet).  (With 16 harmonics the coarse bound is useless: the deep part of the deep rows is
 // prefilter_kernel's.)
 // M2[i] = max of the 8 codes M[8 i .. 8 i + 7] over the items [begin, end) (M's rows are contiguous, so both
 // planes are linear arrays); a CTA of kPfThreads threads, four 128-bit loads in flight per thread.
@@ -591,7 +609,6 @@ __device__ __forceinline__ void coarsen_items(const unsigned short* __restrict__
     }
 }
 
-constexpr int kShallowDepth = 4;
 
 // Thread <-> 8 consecutive coarse blocks B = 8 G + q of row j (one 128-bit word of M2[j]); harmonic k needs
 // the 8k coarse blocks 8kG .. 8kG + 8k - 1 of row_k (k words); all loads are issued up front.
@@ -677,22 +694,18 @@ __global__ void __launch_bounds__(256) prefilter_coarse_kernel(const HarmParams 
         }
         if (f && !(deep && B < b_deep)) fl |= 1u << q;
     }
-    while (fl) {
-        const int q = __ffs(fl) - 1;
-        fl &= fl - 1;
-        const unsigned long long slot = atomicAdd(p.coarse_count, 1ULL);
-        if (slot < (unsigned long long)p.coarse_capacity) p.coarse[slot] = make_uint2(8u * G + (unsigned)q, (unsigned)j);
-        else atomicExch(p.overflow, 1u);                                   // pass B then falls back to the full scan
-    }
-}
-
-// Level 1 for the listed (coarse block = octet of blocks, row) pairs: one thread each.
-__global__ void __launch_bounds__(kPfShallowThreads) prefilter_shallow_kernel(const HarmParams p) {
-    const unsigned long long n = min(*p.coarse_count, (unsigned long long)p.coarse_capacity);
-    for (unsigned long long q = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; q < n;
-         q += (unsigned long long)gridDim.x * blockDim.x) {
-        const uint2 rec = p.coarse[q];
-        pf_shallow_octet<kShallowDepth>(p, rec.x, (int)rec.y);
+    if (fl) {   // (rare) level 1 right here: the block-level bound for the 64 fundamentals of each failing coarse block
+        PfArgs a;
+        a.maxplane = p.maxplane; a.mpitch = p.mpitch; a.nbins = p.nbins; a.r_lo = p.r_lo;
+        a.maybe_capacity = p.maybe_capacity; a.maybe = p.maybe; a.maybe_count = p.maybe_count; a.overflow = p.overflow;
+        a.nz = p.nz; a.H = p.H;
+#pragma unroll
+        for (int k = 0; k < kShallowDepth; ++k) a.tq[k] = p.tq[k];
+        while (fl) {
+            const int q = __ffs(fl) - 1;
+            fl &= fl - 1;
+            pf_shallow_octet_call(a, 8u * G + (unsigned)q, j);
+        }
     }
 }
 
@@ -823,7 +836,7 @@ __global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmPara
 }
 
 // ---- pass B: one thread per maybe record (r, j): the plain definition on the real plane.
-// If the maybe list or the coarse list overflowed (pathological thresholds), every fundamental is evaluated instead.
+// If the maybe list overflowed (pathological thresholds), every fundamental is evaluated instead.
 template <typename T, int NBR>
 __global__ void __launch_bounds__(128) exact_kernel(const HarmParams p) {
     __shared__ float sthr[32];
@@ -893,7 +906,7 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
     }
     cudaError_t e = cudaMemsetAsync(p.count, 0, sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(p.maybe_count, 0, 4 * sizeof(unsigned long long), st);   // + overflow flag, coarse count
+    e = cudaMemsetAsync(p.maybe_count, 0, 2 * sizeof(unsigned long long), st);   // + overflow flag
     if (e != cudaSuccess) return e;
     if (p.r_lo >= p.nbins) return cudaSuccess;
     if (build_max) {
@@ -952,9 +965,7 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         const unsigned nB = (unsigned)(p.mpitch / 8);
         prefilter_coarse_kernel<<<dim3((nB / 8 + 255) / 256, (unsigned)p.nz), 256, 0, st>>>(p, b_deep);
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
-        prefilter_shallow_kernel<<<148 * 4, kPfShallowThreads, 0, st>>>(p);
-        if ((e = cudaGetLastError()) != cudaSuccess) return e;
-        *launches += 2;
+        ++*launches;
     }
     if (p.nbr) {
         if (plane_is_bf16) exact_kernel<__nv_bfloat16, 1><<<kExactBlocks, 128, 0, st>>>(p);

@@ -85,12 +85,9 @@ struct HarmParams {
     int64_t mpitch;                   // nbins / 8
     uint2* maybe;                     // plan-owned list of (r, j): fundamentals that failed the prefilter
     int64_t maybe_capacity;
-    unsigned long long* maybe_count;  // plan-owned; followed by the overflow flag and the coarse count
+    unsigned long long* maybe_count;  // plan-owned; followed by the overflow flag
     unsigned* overflow;               // plan-owned: set if the maybe list was too small
     unsigned short* max2;             // plan-owned coarse side plane: nz x nbins / 64 codes, max of 8 codes of M
-    uint2* coarse;                    // plan-owned list of (coarse block, row) that failed the coarse bound
-    int64_t coarse_capacity;
-    unsigned long long* coarse_count; // plan-owned (maybe_count + 2)
     int nbr;                          // 1: neighbour-maximised sums (reading A24)
     unsigned short* maxplane_nbr;     // plan-owned dilated side plane the prefilter scans when nbr = 1
 };

@@ -49,7 +49,6 @@ struct fdas_plan_s {
     cudaStream_t last_stream = nullptr;
     bool have_last = false;
     unsigned short* d_max2 = nullptr;        // K3 coarse side plane M2 (nz x nbins/64 codes), rebuilt from M by every call
-    uint2* d_coarse = nullptr;               // K3 coarse maybe list (kCoarseCapacity records)
     uint2* d_maybe = nullptr;                // K3 maybe list (kMaybeCapacity records)
     unsigned long long* d_maybe_count = nullptr;
     // workspace of fdas_search_host (lazy)

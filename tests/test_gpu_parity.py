@@ -90,7 +90,7 @@ def test_tiny_fp32_full_parity(fdas, torch_, oracle):
     record_stats("tiny_fp32", {**ps.summary(orc.P.max()), **stats})
     keys = set(gpu_cand_dict(res.cands))
     assert (20000, 23, 1) in keys or (20000, 24, 1) in keys     # the injected signal (z0 = 7.5)
-    assert plan.launch_count() == 8      # K1a, K1b, K2, K3: general prefilter (+ coarsen), coarse, listed, exact, flags (cuFFT not counted)
+    assert plan.launch_count() == 7      # K1a, K1b, K2, K3: general prefilter (+ coarsen), coarse + block level, exact, flags (cuFFT not counted)
 
 
 # ------------------------------------------------------------------------------------ configs[1]
@@ -784,9 +784,10 @@ def test_harmonic_maybe_list_overflow_falls_back_to_full_scan(fdas, torch_, orac
         assert abs(s_at(*key) - thr[key[2] - 1]) <= 1e-5 * thr[key[2] - 1], key
 
 
-def test_harmonic_coarse_list_overflow_falls_back_to_full_scan(fdas, torch_):
-    """More coarse blocks (64 fundamentals each) fail the coarse bound than the coarse list holds (2^20): pass B
-    must scan every fundamental.  H = 1, so the expected set is the definition itself: every P > T_1, r >= r_lo."""
+def test_harmonic_every_coarse_block_fails_on_a_large_plane(fdas, torch_):
+    """Every one of the 10^6 coarse blocks (64 fundamentals each) fails the coarse bound, every thread of the coarse
+    level goes on to the block level, the maybe list overflows and pass B scans every fundamental.  H = 1, so the
+    expected set is the definition itself: every P > T_1, r >= r_lo."""
     torch = torch_
     plan = fdas.Plan(1 << 21, 64e-6, 32.0, 1.0, 2048, "fp32")       # 65 x 2^20 points, 65 x 16384 coarse blocks
     nb, nz = plan.info.nbins, plan.info.nz
@@ -806,7 +807,7 @@ def test_harmonic_coarse_list_overflow_falls_back_to_full_scan(fdas, torch_):
     key = c["zidx"].astype(np.int64) * nb + c["r"]
     assert np.unique(key).size == key.size
     assert np.array_equal(c["power"], P32[c["zidx"], c["r"]]) and np.all(c["power"] > thr[0])
-    # and the same call on a quiet plane with one line finds exactly that line through the two lists
+    # and the same call on a quiet plane with one line finds exactly that line through both levels
     d_plane.zero_()
     d_plane[40, 123457] = 3.0
     plan.harmonic_sum_peaks(d_plane, 1, thr, r_lo, d_c, d_n)
