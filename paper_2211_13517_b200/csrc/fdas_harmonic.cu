@@ -115,7 +115,7 @@ __device__ __forceinline__ void emit_candidate(const HarmGeom& g, int64_t r, int
 // fundamentals the prefilter lets through are settled by the first four gathers.
 template <typename T>
 __device__ __noinline__ void exact_fundamental(const T* P, const HarmGeom g, const float* thr,
-                                               int64_t r, int j) {
+                                               int64_t r, int j, unsigned hint) {
     if (r < g.r_lo || r >= g.nbins) return;
     const int c2 = g.nz - 1;
     int hmax = 0;   // number of defined harmonics
@@ -142,7 +142,12 @@ __device__ __noinline__ void exact_fundamental(const T* P, const HarmGeom g, con
         }
     }
     if (hmax <= 4) return;
-    {   // can any deeper sum still exceed its threshold?
+    if (hint != 0xffffu) {
+        // the prefilter's hint (pf_emit_warp): 8 S_h <= 8 S_4 + (U_h - U_4) <= ceil(8 S_4 (1 + 2^-20)) + E + tq_h
+        const float s8 = S * (8.0f * (1.0f + 9.5367431640625e-7f));
+        if (s8 < 60000.f && (int)ceilf(s8) + ((int)hint - 8192) <= 0) return;
+        // (not ruled out: the bound below would say the same -- straight to the gathers)
+    } else {   // no hint (block level, straddling threads, full scan): can any deeper sum still exceed its threshold?
         float U = S;
         bool deeper = false;
         for (int h0 = 5; h0 <= hmax && !deeper; h0 += 8) {
@@ -318,7 +323,7 @@ __device__ __forceinline__ unsigned pf_pair(const unsigned (&w)[NW]) {
 }
 
 // One harmonic K for the pairs P0 .. P0 + NP - 1 of fundamentals (2p, 2p+1) from the words w (first word W0
-// of the slice): X += codes + step, F |= X.
+// of the slice): X += codes + step, F = max(F, X) on each half-word (bit 15 of F: some U_h exceeded tq_h).
 template <int K, int P0, int NP, int W0, int NW, int PI = 0>
 __device__ __forceinline__ void pf_pairs(const unsigned (&w)[NW], const unsigned step, unsigned (&X)[16],
                                          unsigned (&F)[16]) {
@@ -326,7 +331,7 @@ __device__ __forceinline__ void pf_pairs(const unsigned (&w)[NW], const unsigned
         constexpr int p = P0 + PI;
         const unsigned m2 = pf_pair<((K * (2 * p)) >> 3), ((K * (2 * p + 1)) >> 3), W0, NW>(w);
         X[p] = X[p] + m2 + step;
-        F[p] |= X[p];
+        F[p] = __vmaxu2(F[p], X[p]);
         pf_pairs<K, P0, NP, W0, NW, PI + 1>(w, step, X, F);
     }
 }
@@ -433,7 +438,7 @@ __device__ __forceinline__ void pf_emit(const P& p, const unsigned Q, const int 
             while (flagged) {
                 const int i = __ffs(flagged) - 1;
                 flagged &= flagged - 1;
-                p.maybe[slot++] = make_uint2(32u * Q + (unsigned)i, (unsigned)j);
+                p.maybe[slot++] = make_uint2(32u * Q + (unsigned)i, (unsigned)j | (0xffffu << 16));   // no hint
             }
         } else {
             atomicExch(p.overflow, 1u);   // pass B then falls back to the full scan
@@ -444,7 +449,14 @@ __device__ __forceinline__ void pf_emit(const P& p, const unsigned Q, const int 
 // The same for a whole (converged) warp: one atomic slot claim per warp instead of one per thread -- with
 // 16-harmonic rows most threads of the general kernel have a flagged fundamental, and their claims would all
 // queue at the one L2 slice that holds the counter.
-__device__ __forceinline__ void pf_emit_warp(const HarmParams& p, const unsigned Q, const int j, unsigned flagged) {
+// A record is (r, j | hint << 16).  hint = kHintNone, or E + kHintBias with
+//   E = max_{h >= 5} (U_h - tq_h) - U_4   (codes; the thread's `hint` words hold it for its 16 pairs):
+// once the exact pass knows S_4, ceil(8 S_4) + E <= 0 proves that no deeper sum can exceed its threshold
+// (8 S_h <= 8 S_4 + (U_h - U_4)), without gathering the twelve block-max codes again.
+constexpr int kHintBias = 8192;
+constexpr unsigned kHintNone = 0xffffu;
+__device__ __forceinline__ void pf_emit_warp(const HarmParams& p, const unsigned Q, const int j, unsigned flagged,
+                                             const unsigned* hint) {
     if (32 * (int64_t)Q < p.r_lo) {
         const int64_t cut = p.r_lo - 32 * (int64_t)Q;
         flagged = (cut >= 32) ? 0u : (flagged & ~((1u << (int)cut) - 1u));
@@ -467,7 +479,9 @@ __device__ __forceinline__ void pf_emit_warp(const HarmParams& p, const unsigned
         while (flagged) {
             const int i = __ffs(flagged) - 1;
             flagged &= flagged - 1;
-            p.maybe[slot++] = make_uint2(32u * Q + (unsigned)i, (unsigned)j);
+            unsigned hi = kHintNone;
+            if (hint) hi = (i & 1) ? (hint[i >> 1] >> 16) : (hint[i >> 1] & 0xffffu);
+            p.maybe[slot++] = make_uint2(32u * Q + (unsigned)i, (unsigned)j | (hi << 16));
         }
     } else if (lane == 0) {
         atomicExch(p.overflow, 1u);   // pass B then falls back to the full scan
@@ -797,6 +811,10 @@ __global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmPara
             }
         }
     }
+    // Per thread: U_4 of its 16 pairs while the deep harmonics run, then the exact pass's hint (see pf_emit_warp).
+    __shared__ unsigned stash[kPfThreads * 16];
+    unsigned* const my = stash + threadIdx.x * 16;
+    bool hinted = false;
     if (he_max >= 5) {       // CTA-uniform
         // harmonics 5..: two fundamentals per register, X = U + (0x7fff - tq) on each half-word
         unsigned X[16], F[16];   // pair p: fundamentals 2p (low half-word) and 2p + 1 (high)
@@ -804,17 +822,18 @@ __global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmPara
             const unsigned base = (unsigned)(0x7fff - p.tq[3]) * 0x10001u;
 #pragma unroll
             for (int b = 0; b < 4; ++b) {
-                X[4 * b + 0] = (unsigned)U4[5 * b + 0] * 0x10001u + base;
-                X[4 * b + 1] = ((unsigned)U4[5 * b + 1] | ((unsigned)U4[5 * b + 2] << 16)) + base;
-                X[4 * b + 2] = (unsigned)U4[5 * b + 3] * 0x10001u + base;
-                X[4 * b + 3] = (unsigned)U4[5 * b + 4] * 0x10001u + base;
+                const unsigned u0 = (unsigned)U4[5 * b + 0] * 0x10001u;
+                const unsigned u1 = (unsigned)U4[5 * b + 1] | ((unsigned)U4[5 * b + 2] << 16);
+                const unsigned u2 = (unsigned)U4[5 * b + 3] * 0x10001u, u3 = (unsigned)U4[5 * b + 4] * 0x10001u;
+                *reinterpret_cast<uint4*>(my + 4 * b) = make_uint4(u0, u1, u2, u3);
+                X[4 * b + 0] = u0 + base; X[4 * b + 1] = u1 + base; X[4 * b + 2] = u2 + base; X[4 * b + 3] = u3 + base;
             }
 #pragma unroll
             for (int pp = 0; pp < 16; ++pp) F[pp] = 0u;
         }
         pf_from<5>(p, j, Q, he_max, he, X, F);
         if (he >= 5) {
-            // bit 15 - p <- fundamental 2p, bit 31 - p <- fundamental 2p + 1
+            // F = max_{h >= 5} X_h on each half-word.  bit 15 - p <- fundamental 2p, bit 31 - p <- fundamental 2p + 1
             unsigned acc = 0u;
 #pragma unroll
             for (int pp = 0; pp < 16; ++pp) acc |= (F[pp] & 0x80008000u) >> pp;
@@ -825,14 +844,27 @@ __global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmPara
                     if (acc & (0x80000000u >> pp)) flagged |= 1u << (2 * pp + 1);
                 }
             }
+            if (flagged) {
+                // hint for the exact pass: E = max_{h >= 5} (U_h - tq_h) - U_4 = max X - U_4 - 0x7fff, biased by
+                // kHintBias (every half-word of F - U_4 is >= 0x7fff - 1022, so nothing borrows)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const uint4 u = *reinterpret_cast<const uint4*>(my + 4 * b);
+                    constexpr unsigned kSub = (unsigned)(0x7fff - kHintBias) * 0x10001u;
+                    *reinterpret_cast<uint4*>(my + 4 * b) = make_uint4(F[4 * b] - u.x - kSub, F[4 * b + 1] - u.y - kSub,
+                                                                       F[4 * b + 2] - u.z - kSub, F[4 * b + 3] - u.w - kSub);
+                }
+                hinted = true;
+            }
         }
     }
     if (he < hz && 32u * Q <= last / (unsigned)(he + 1)) {
         // the thread that straddles the end of harmonic he+1's range (one per harmonic and row): that
         // harmonic exists for its first fundamentals only -- all 32 go to the exact pass, which knows
         flagged = 0xffffffffu;
+        hinted = false;
     }
-    pf_emit_warp(p, Q, j, mine ? flagged : 0u);
+    pf_emit_warp(p, Q, j, mine ? flagged : 0u, hinted ? my : nullptr);
 }
 
 // ---- pass B: one thread per maybe record (r, j): the plain definition on the real plane.
@@ -850,8 +882,8 @@ __global__ void __launch_bounds__(128) exact_kernel(const HarmParams p) {
         const unsigned long long n = *p.maybe_count;
         for (unsigned long long q = tid; q < n; q += nthr) {
             const uint2 rec = p.maybe[q];
-            if (NBR) exact_fundamental_nbr(P, g, sthr, (int64_t)rec.x, (int)rec.y);
-            else exact_fundamental(P, g, sthr, (int64_t)rec.x, (int)rec.y);
+            if (NBR) exact_fundamental_nbr(P, g, sthr, (int64_t)rec.x, (int)(rec.y & 0xffffu));
+            else exact_fundamental(P, g, sthr, (int64_t)rec.x, (int)(rec.y & 0xffffu), rec.y >> 16);
         }
     } else {
         const unsigned long long n = (unsigned long long)p.nbins * (unsigned long long)p.nz;
@@ -859,7 +891,7 @@ __global__ void __launch_bounds__(128) exact_kernel(const HarmParams p) {
             const int64_t r = (int64_t)(q % (unsigned long long)p.nbins);
             const int j = (int)(q / (unsigned long long)p.nbins);
             if (NBR) exact_fundamental_nbr(P, g, sthr, r, j);
-            else exact_fundamental(P, g, sthr, r, j);
+            else exact_fundamental(P, g, sthr, r, j, 0xffffu);
         }
     }
 }
