@@ -812,8 +812,8 @@ __global__ void __launch_bounds__(kPfThreads, 8) prefilter_kernel(const HarmPara
         }
     }
     // Per thread: U_4 of its 16 pairs while the deep harmonics run, then the exact pass's hint (see pf_emit_warp).
-    __shared__ unsigned stash[kPfThreads * 16];
-    unsigned* const my = stash + threadIdx.x * 16;
+    __shared__ __align__(16) unsigned stash[kPfThreads * 20];   // rows of 16 words, pitch 20: conflict-free 128-bit accesses
+    unsigned* const my = stash + threadIdx.x * 20;
     bool hinted = false;
     if (he_max >= 5) {       // CTA-uniform
         // harmonics 5..: two fundamentals per register, X = U + (0x7fff - tq) on each half-word
