@@ -193,6 +193,12 @@ __device__ __forceinline__ u64 fma2(u64 x, u64 y, u64 z) {
     return r;
 }
 
+__device__ __forceinline__ void st_global_256(void* ptr, const uint4 a, const uint4 b) {
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(ptr), "r"(a.x), "r"(a.y), "r"(a.z),
+                 "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w)
+                 : "memory");
+}
+
 // Powers of 8 consecutive bins of the rows +z and -z of this thread's pair from one group of
 // accumulator columns (a = 16 columns of D_R: Ar[0..7] | Ai[0..7]; b = 16 columns of D_I: Br | Bi),
 // into this thread's rows (rowp, rowm) of the two staging tiles, 16-byte unit `2 * bg` (fp32) / `bg`
@@ -202,17 +208,9 @@ template <int PLANE16>
 __device__ __forceinline__ unsigned group_to_smem(const uint32_t* __restrict__ a, const uint32_t* __restrict__ b,
                                                   unsigned char* tile_p, unsigned char* tile_m, const int rowp,
                                                   const int rowm, const int half, const int bg) {
-    // pair_powers (fdas_tc_common.h).  With a bf16 plane, two bins per instruction: the packed fp32x2 forms
-    // (FADD2 / FMUL2 / FFMA2) round each half exactly like the scalar ones at half the issue slots of the
-    // drain (K2-TC 0.550 -> 0.532 ms per SKA launch).  With an fp32 plane the kernel is bound by its stores and
-    // the shorter drain makes it SLOWER (0.650 -> 0.716 ms, profiles/r02b): the scalar forms stay.
+    // pair_powers (fdas_tc_common.h) for two bins per instruction: the packed fp32x2 forms (FADD2 / FMUL2 /
+    // FFMA2) round each half exactly like the scalar ones, at half the issue slots of the drain
     float Pp[8], Pm[8];
-    if constexpr (!PLANE16) {
-#pragma unroll
-        for (int e = 0; e < 8; ++e)
-            pair_powers(__uint_as_float(a[e]), __uint_as_float(b[e]), __uint_as_float(a[8 + e]),
-                        __uint_as_float(b[8 + e]), &Pp[e], &Pm[e]);
-    } else {
 #pragma unroll
     for (int e = 0; e < 8; e += 2) {
         const u64 Ar = pk2u(a[e], a[e + 1]), Ai = pk2u(a[8 + e], a[9 + e]);
@@ -221,7 +219,6 @@ __device__ __forceinline__ unsigned group_to_smem(const uint32_t* __restrict__ a
         const u64 pp = fma2(rp, rp, mul2(ip, ip)), pm = fma2(rm, rm, mul2(im, im));
         up2f(pp, Pp[e], Pp[e + 1]);
         up2f(pm, Pm[e], Pm[e + 1]);
-    }
     }
     unsigned mp, mm;
     if (PLANE16) {
@@ -267,7 +264,8 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
     const int nq = (p.npair + 31) >> 5;                   // TMEM lane quarters that hold template pairs
     const Layout L = make_layout(p.kp, 2 * nq, NBUF, PLANE16);
     const uint32_t bar0 = smem_u32(smem + L.bar_off);
-    // barriers: hfull[3] | hempty[3] | tfull[4] | tempty[4]; then the TMEM base address slot.
+    // barriers: hfull[3] | hempty[3] | tfull[4] | tempty[4]; then the TMEM base address slot; at +128 the
+    // mailbox barriers mfull[4] | mempty[4] (one pair per lane quarter).
     // tfull / tempty are indexed by the SUB-TILE (one phase per tile: a waiter must see every phase of
     // its barrier); the accumulator stage of sub-tile s is s >> 1 (one stage per epilogue set), so the
     // MMA of sub-tile s waits for the drain of sub-tile s ^ 1.
@@ -275,6 +273,8 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
     auto hempty = [&](int s) { return bar0 + 8u * (kHStages + s); };
     auto tfull = [&](int s) { return bar0 + 8u * (2 * kHStages + s); };
     auto tempty = [&](int s) { return bar0 + 8u * (2 * kHStages + kSubTiles + s); };
+    auto mfull = [&](int q) { return bar0 + 128u + 8u * q; };
+    auto mempty = [&](int q) { return bar0 + 160u + 8u * q; };
     volatile uint32_t* tmem_slot =
         reinterpret_cast<volatile uint32_t*>(smem + L.bar_off + 8 * (2 * kHStages + 2 * kSubTiles));
 
@@ -288,6 +288,10 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
             for (int s = 0; s < kSubTiles; ++s) {
                 mbar_init(tfull(s), 1);
                 mbar_init(tempty(s), 4);          // the four warps of the set that drains the sub-tile
+            }
+            for (int q = 0; q < 4; ++q) {
+                mbar_init(mfull(q), 1);
+                mbar_init(mempty(q), 1);
             }
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
@@ -521,9 +525,34 @@ convolve_tc_kernel(const ConvTcParams p, const __grid_constant__ CUtensorMap pma
                 }
                 tma_commit();
             }
-            if (lane < nreal) {
-                *reinterpret_cast<uint4*>(mrow_p + tile * (kTileR / 8)) = make_uint4(mxp[0], mxp[1], mxp[2], mxp[3]);
-                *reinterpret_cast<uint4*>(mrow_m + tile * (kTileR / 8)) = make_uint4(mxm[0], mxm[1], mxm[2], mxm[3]);
+            if constexpr (PLANE16) {
+                // (with a bf16 plane the two sets store their halves themselves: measured faster, profiles/r02b)
+                if (lane < nreal) {
+                    *reinterpret_cast<uint4*>(mrow_p + tile * (kTileR / 8)) = make_uint4(mxp[0], mxp[1], mxp[2], mxp[3]);
+                    *reinterpret_cast<uint4*>(mrow_m + tile * (kTileR / 8)) = make_uint4(mxm[0], mxm[1], mxm[2], mxm[3]);
+                }
+            } else {
+                // the block maxima of a row and tile leave as ONE 32-byte store (a whole sector): set 0 hands its half
+                // (blocks 0..7) to the warp of set 1 with the same lane quarter through a 1 KB mailbox.  Written as
+                // two 16-byte halves by the two sets, the half-written sectors wait in L2 for their other half, and
+                // the kernel's time depends on how far the sets drift apart (0.650 -> 0.632 ms per SKA launch)
+                uint4* const mbox = reinterpret_cast<uint4*>(smem + L.mb_off) + (q * 32 + lane) * 2;
+                if (set == 0) {
+                    mbar_wait(mempty(q), ((uint32_t)tile_iter & 1u) ^ 1u);
+                    mbox[0] = make_uint4(mxp[0], mxp[1], mxp[2], mxp[3]);
+                    mbox[1] = make_uint4(mxm[0], mxm[1], mxm[2], mxm[3]);
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(mfull(q));
+                } else {
+                    mbar_wait(mfull(q), (uint32_t)tile_iter & 1u);
+                    const uint4 ap = mbox[0], am = mbox[1];
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(mempty(q));
+                    if (lane < nreal) {
+                        st_global_256(mrow_p - 8 + tile * (kTileR / 8), ap, make_uint4(mxp[0], mxp[1], mxp[2], mxp[3]));
+                        st_global_256(mrow_m - 8 + tile * (kTileR / 8), am, make_uint4(mxm[0], mxm[1], mxm[2], mxm[3]));
+                    }
+                }
             }
         }
         if (lane == 0) tma_wait_all();

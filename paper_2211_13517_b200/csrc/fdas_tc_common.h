@@ -71,9 +71,9 @@ __host__ __device__ inline int stage_unit_offset(int row, int half, int unit, in
 __host__ __device__ inline int stage_buf_bytes(int plane16) { return 2 * 32 * 2 * kSubR * (plane16 ? 2 : 4); }
 
 // Shared-memory carve-up (dynamic, 1024-byte aligned): window stages | spectrum-slice staging |
-// per-warp epilogue buffers (nbuf staging buffers) | barriers.
+// per-warp epilogue buffers (nbuf staging buffers) | barriers (256 B) | block-max mailbox (1 KB per lane quarter).
 struct Layout {
-    int h_off, h_stage, st_off, st_part, ep_off, ep_warp, bar_off, total;
+    int h_off, h_stage, st_off, st_part, ep_off, ep_warp, bar_off, mb_off, total;
 };
 __host__ __device__ inline Layout make_layout(int kp, int nactive_warps, int nbuf, int plane16) {
     Layout l;
@@ -84,7 +84,8 @@ __host__ __device__ inline Layout make_layout(int kp, int nactive_warps, int nbu
     l.ep_off = (l.st_off + 2 * l.st_part + 1023) & ~1023;
     l.ep_warp = nbuf * stage_buf_bytes(plane16);
     l.bar_off = l.ep_off + nactive_warps * l.ep_warp;
-    l.total = l.bar_off + 128;
+    l.mb_off = l.bar_off + 256;                                  // mailbox: 1 KB per active lane quarter
+    l.total = l.mb_off + (nactive_warps / 2) * 1024;
     return l;
 }
 
