@@ -27,7 +27,9 @@
 // * Epilogue: the thread that owns lane p reads 16 + 16 consecutive columns (tcgen05.ld 32x32b.x16)
 //   = everything for 8 consecutive bins of rows j+ and j-: powers, the 8-bin block maximum (a register
 //   reduction), two 16-byte shared-memory stores per row into a swizzled [32 rows][32 bins] tile, and
-//   one TMA tensor store per tile.  A warp works alone (no block-level barrier in the epilogue).
+//   one TMA tensor store per tile.  A warp works alone (no block-level barrier in the epilogue); the only
+//   exchange between warps is the 16 bytes of block maxima per row that set 0 hands to set 1 (fp32 plane), so
+//   that they reach memory as whole 32-byte sectors.
 //
 // Warp roles of the persistent CTA (one per SM, 320 threads): warps 0..3 drain sub-tiles 0, 1 of
 // every 128-bin tile and warps 4..7 sub-tiles 2, 3 (warp % 4 = the TMEM lane quarter = 32 template

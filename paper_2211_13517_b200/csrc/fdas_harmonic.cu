@@ -237,10 +237,11 @@ __global__ void __launch_bounds__(256) build_max_kernel(const HarmParams p) {
     p.maxplane[(size_t)j * p.mpitch + b] = (unsigned short)max_code(m);
 }
 
-// ---- M' = M dilated by D <= 8 blocks on either side (neighbour-maximised sums): one thread per octet of
+// ---- M' = M dilated by D <= 8 blocks on either side (D > 2 is served by the D = 8 instance: a larger window is still a bound) (neighbour-maximised sums): one thread per octet of
 // blocks (a 128-bit word and its two neighbours; codes order like the values, missing neighbours count 0).
+template <int D>
 __global__ void __launch_bounds__(256) dilate_max_kernel(const unsigned short* __restrict__ src,
-                                                         unsigned short* __restrict__ dst, int64_t mpitch, int D) {
+                                                         unsigned short* __restrict__ dst, int64_t mpitch) {
     const int64_t nO = mpitch >> 3;                       // mpitch is a multiple of 8
     const int64_t O = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (O >= nO) return;
@@ -260,8 +261,7 @@ __global__ void __launch_bounds__(256) dilate_max_kernel(const unsigned short* _
     for (int e = 0; e < 8; ++e) {
         unsigned m = c[8 + e];
 #pragma unroll
-        for (int x = 1; x <= 8; ++x)
-            if (x <= D) m = max(m, max(c[8 + e - x], c[8 + e + x]));
+        for (int x = 1; x <= D; ++x) m = max(m, max(c[8 + e - x], c[8 + e + x]));
         o[e] = m;
     }
     reinterpret_cast<uint4*>(dst + (size_t)blockIdx.y * mpitch)[O] =
@@ -954,7 +954,12 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
         const int D = ((p.H >> 1) + 7) >> 3;
         if (D > 8 || (p.mpitch & 7)) return cudaErrorInvalidValue;     // H <= 32 gives D <= 2; mpitch = nbins / 8
         dim3 grid((unsigned)((p.mpitch / 8 + 255) / 256), (unsigned)p.nz);
-        dilate_max_kernel<<<grid, 256, 0, st>>>(p.maxplane, p.maxplane_nbr, p.mpitch, D);
+        switch (D) {   // D = 1 for H <= 17, 2 up to H = 32 (compile-time window: the loop unrolls to 2 D maxima per block)
+            case 0: dilate_max_kernel<0><<<grid, 256, 0, st>>>(p.maxplane, p.maxplane_nbr, p.mpitch); break;
+            case 1: dilate_max_kernel<1><<<grid, 256, 0, st>>>(p.maxplane, p.maxplane_nbr, p.mpitch); break;
+            case 2: dilate_max_kernel<2><<<grid, 256, 0, st>>>(p.maxplane, p.maxplane_nbr, p.mpitch); break;
+            default: dilate_max_kernel<8><<<grid, 256, 0, st>>>(p.maxplane, p.maxplane_nbr, p.mpitch); break;
+        }
         if ((e = cudaGetLastError()) != cudaSuccess) return e;
         ++*launches;
         p.maxplane = p.maxplane_nbr;
