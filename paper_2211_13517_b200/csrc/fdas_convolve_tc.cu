@@ -677,8 +677,8 @@ cudaError_t launch_convolve_tc(int plane16, const ConvTcParams& p, TcMapCache* c
         p.pair0 + p.npair > p.npair_total || 2 * p.npair_total > p.nz ||
         tc::kBankCol0 + p.kp > 512 || (reinterpret_cast<uintptr_t>(p.plane) & 15u) ||
         (reinterpret_cast<uintptr_t>(p.spec) & 15u) ||
-        ((p.pitch * (plane16 ? 2 : 4)) & 15) || ((p.mpitch * 2) & 15) ||
-        (reinterpret_cast<uintptr_t>(p.maxplane) & 15u))
+        ((p.pitch * (plane16 ? 2 : 4)) & 15) || ((p.mpitch * 2) & 31) ||          // 32-byte block-max stores
+        (reinterpret_cast<uintptr_t>(p.maxplane) & 31u))
         return cudaErrorInvalidValue;
     const TcMapCache::Entry* m = nullptr;
     const cudaError_t e = get_maps(cache, plane16, p, &m);
