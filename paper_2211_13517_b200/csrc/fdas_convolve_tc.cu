@@ -195,9 +195,13 @@ __device__ __forceinline__ u64 fma2(u64 x, u64 y, u64 z) {
     return r;
 }
 
+// One 32-byte sector of the side plane, marked evict-last in L2: K3 reads the side plane right after this kernel,
+// whose 3.2 GB of plane stores would otherwise push it out (K2-TC -7 us, K3 -3 us per SKA trial).
 __device__ __forceinline__ void st_global_256(void* ptr, const uint4 a, const uint4 b) {
-    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(ptr), "r"(a.x), "r"(a.y), "r"(a.z),
-                 "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w)
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("st.global.L2::cache_hint.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8}, %9;" ::"l"(ptr), "r"(a.x),
+                 "r"(a.y), "r"(a.z), "r"(a.w), "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w), "l"(pol)
                  : "memory");
 }
 
