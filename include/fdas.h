@@ -202,6 +202,39 @@ int fdas_search_batch(fdas_plan_t plan, const float* const* series, int series_o
                       int64_t capacity, int64_t* h_counts, void* cuda_stream);
 
 /*
+ * fdas_whiten_static -- the whitening half of fdas_prepare_spectrum (K1: block medians of |X|^2 over the A3
+ * schedule, interpolation, w[k] = X[k] sqrt(ln2 / m(k)), w[0] = 0; readings A2, A3) as a stand-alone call
+ * that needs no plan and allocates no device memory.
+ *
+ * Who it is for: code that is not allowed to call cudaMalloc.  Two cases we know of: a stage of a real-time
+ * telescope backend that handed all of its HBM to its own pool when it started (a later cudaMalloc may fail
+ * there, and even when it succeeds it synchronises the whole device and stalls the ingest streams), and a
+ * plug-in inside someone else's framework that may only touch the buffers it is handed.  Such a caller
+ * brings its own raw spectrum (its own FFT) and its own output buffer; the medians and the block table, which
+ * fdas_plan would otherwise cudaMalloc, live in a fixed 51 KB array inside libfdas.so.  Every GPU on which the
+ * library is loaded carries those 51 KB until the process exits.
+ *
+ *   d_X        device, at least nbins complex float32 (re, im interleaved), e.g. the output of an R2C FFT
+ *   nbins      number of bins to whiten, 1024 <= nbins <= 2^24 (16 777 216).  LIMIT: the fixed array holds the
+ *              tables of at most 2^24 bins; a longer spectrum is refused with FDAS_EUNSUPPORTED and a text in
+ *              fdas_last_error_detail() -- use a plan for those.
+ *   d_spec     device, nbins complex outputs: float32 pairs (spec_bf16 = 0) or bfloat16 pairs (spec_bf16 = 1)
+ *   The three kernels are only enqueued on cuda_stream; the call does not wait for them.
+ *
+ * The call never calls cudaMalloc, cudaFree, cuFFT or anything else that allocates.  The first call on each
+ * device looks up the device address of the array (cudaGetSymbolAddress, with that device current; the CUDA
+ * runtime may load the library's kernels at that moment): make that first call during start-up, before any
+ * stream capture begins on that device.
+ * All calls on one device share the one array, and it keeps what the previous call left in it.  Nothing in it
+ * has to be zero at the start (each call rewrites every entry it later reads), but two calls whose kernels
+ * can run at the same time on the GPU -- different streams with no dependency between them, or two host
+ * threads -- overwrite each other's tables: order them (one stream, or an event between the streams).
+ * Results are bit-identical to fdas_prepare_spectrum's for the same X.
+ * FDAS_EARG: NULL pointers, spec_bf16 not 0/1, nbins < 1024.  FDAS_ECUDA: the lookup or a launch failed.
+ */
+int fdas_whiten_static(const float* d_X, int64_t nbins, void* d_spec, int spec_bf16, void* cuda_stream);
+
+/*
  * fdas_thresholds_from_sigma -- host helper (reading A13): h_thresholds_out[h-1] = T_h with
  * Q(h, T_h) = erfc(nsigma/sqrt2)/2, Q the survival function of a sum of h unit exponentials.
  */
@@ -229,6 +262,13 @@ int fdas_plan_templates_host(fdas_plan_t plan, double* h_out);
  * stored values (the prefilter only needs M >= P), 1023 means "no bound".  The buffer stays owned by the plan.
  */
 int fdas_plan_debug_maxplane(fdas_plan_t plan, const uint16_t** d_out, int64_t* pitch_out);
+
+/*
+ * fdas_plan_debug_rawspectrum -- diagnostic: device pointer to the plan-owned raw spectrum X (nfft/2 + 1
+ * complex float32, the cuFFT R2C output the last fdas_prepare_spectrum whitened) and its length in complex
+ * elements.  The buffer stays owned by the plan and is overwritten by the next prepare call.
+ */
+int fdas_plan_debug_rawspectrum(fdas_plan_t plan, const float** d_out, int64_t* ncomplex_out);
 
 /* Number of kernels the library launched on behalf of this plan since it was created. */
 int64_t fdas_plan_launch_count(fdas_plan_t plan);

@@ -375,6 +375,13 @@ int fdas_plan_debug_maxplane(fdas_plan_t plan, const uint16_t** d_out, int64_t* 
     return FDAS_OK;
 }
 
+int fdas_plan_debug_rawspectrum(fdas_plan_t plan, const float** d_out, int64_t* ncomplex_out) {
+    if (!plan || !d_out || !ncomplex_out) return FDAS_EARG;
+    *d_out = reinterpret_cast<const float*>(plan->d_X);
+    *ncomplex_out = plan->info.nfft / 2 + 1;
+    return FDAS_OK;
+}
+
 int64_t fdas_plan_launch_count(fdas_plan_t plan) { return plan ? plan->launches : -1; }
 
 int fdas_destroy(fdas_plan_t plan) {

@@ -6,6 +6,9 @@
 //        the first/last centre), w[k] = X[k] sqrt(ln2 / m(k)), w[0] = 0, stored fp32 or bf16 (RNE)
 #include <cuda_bf16.h>
 
+#include <mutex>
+#include <string>
+
 #include "fdas_kernels.h"
 
 namespace fdas {
@@ -170,3 +173,146 @@ cudaError_t launch_whiten(int precision, const WhitenParams& p, cudaStream_t st)
 }
 
 }  // namespace fdas
+
+// ---------------------------------------------------------------------------------------------------
+// fdas_whiten_static (include/fdas.h) -- K1 for callers that may not allocate device memory.
+//
+// The plan-based path keeps K1's scratch (block schedule + median table) in cudaMalloc'd buffers that
+// fdas_plan creates.  A caller that cannot create a plan -- a stage of a real-time backend whose HBM was
+// all handed to its own pool at start-up (a later cudaMalloc can fail there, and it synchronises the
+// whole device, stalling the ingest streams), or a plug-in that may only touch the buffers it is given --
+// gets the same two kernels with the scratch in the fixed array below.  The array is part of the
+// library image: every GPU that loads libfdas.so holds its 51 KB until the process exits.
+//
+// g_whiten_static_scratch is a DEVICE symbol.  In host code its name is only a host-side stand-in (the
+// address of a shadow variable), never a device address: the address the kernels receive comes from
+// cudaGetSymbolAddress, looked up once per device with that device current.
+// ---------------------------------------------------------------------------------------------------
+extern thread_local std::string g_detail;   // fdas_api.cu: text behind fdas_last_error_detail()
+
+namespace {
+
+constexpr int64_t kStaticMinBins = 1024;                 // smallest spectrum a plan can have (N >= 2 * 1024)
+constexpr int64_t kStaticMaxBins = (int64_t)1 << 24;     // stated maximum of the entry point
+constexpr int kStaticMaxBlocks = 4352;                   // the A3 schedule of 2^24 bins has 4124 blocks
+constexpr size_t kStaticSection = (size_t)kStaticMaxBlocks * 4;   // 17408 bytes = 68 x 256
+// three sections of kStaticSection bytes: blk_start (int32), blk_len (int32), blk_med (float)
+static __device__ __align__(256) unsigned char g_whiten_static_scratch[3 * kStaticSection];
+
+// Block schedule of reading A3 (the same rule as fdas::whitening_blocks on the host), written on the
+// device so that nothing is copied from pageable host memory: thread 0 walks the short blocks at the
+// low-frequency end (a few dozen), from the first 4096-bin block on the starts are an arithmetic series.
+__global__ void __launch_bounds__(256) static_schedule_kernel(int32_t* blk_start, int32_t* blk_len,
+                                                              long long nb, int nblk) {
+    __shared__ int s_i0;
+    __shared__ long long s_s0;
+    if (threadIdx.x == 0) {
+        long long s = 1;
+        int i = 0;
+        while (s < nb) {
+            const int lg = 63 - __clzll(s);
+            long long l = (lg >= 2) ? (1ll << (lg - 2)) : 1ll;
+            if (l < 32) l = 32;
+            if (l >= 4096) break;
+            if (s + l > nb) l = nb - s;
+            blk_start[i] = (int32_t)s;
+            blk_len[i] = (int32_t)l;
+            ++i;
+            s += l;
+        }
+        s_i0 = i;
+        s_s0 = s;
+    }
+    __syncthreads();
+    for (int i = s_i0 + (int)threadIdx.x; i < nblk; i += (int)blockDim.x) {
+        const long long s = s_s0 + (long long)(i - s_i0) * 4096;
+        blk_start[i] = (int32_t)s;
+        blk_len[i] = (int32_t)((nb - s < 4096) ? (nb - s) : 4096);
+    }
+}
+
+int static_block_count(int64_t nb) {   // host: number of blocks of the A3 schedule (no tables needed)
+    int64_t s = 1;
+    int n = 0;
+    while (s < nb) {
+        const int lg = 63 - __builtin_clzll((unsigned long long)s);
+        int64_t l = (lg >= 2) ? ((int64_t)1 << (lg - 2)) : 1;
+        if (l < 32) l = 32;
+        if (l > 4096) l = 4096;
+        if (s + l > nb) l = nb - s;
+        s += l;
+        ++n;
+    }
+    return n;
+}
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+unsigned char* g_static_ptr[kStaticMaxDevices] = {};   // device address of the scratch, per device ordinal
+
+}  // namespace
+
+extern "C" int fdas_whiten_static(const float* d_X, int64_t nbins, void* d_spec, int spec_bf16,
+                                  void* cuda_stream) {
+    if (!d_X || !d_spec || (spec_bf16 != 0 && spec_bf16 != 1)) return FDAS_EARG;
+    if (nbins < kStaticMinBins) {
+        g_detail = "fdas_whiten_static: nbins " + std::to_string(nbins) + " is below the minimum " +
+                   std::to_string(kStaticMinBins);
+        return FDAS_EARG;
+    }
+    if (nbins > kStaticMaxBins) {
+        g_detail = "fdas_whiten_static: nbins " + std::to_string(nbins) +
+                   " exceeds the fixed scratch array's maximum of " + std::to_string(kStaticMaxBins) +
+                   " bins (use a plan and fdas_prepare_spectrum for longer spectra)";
+        return FDAS_EUNSUPPORTED;
+    }
+    const int nblk = static_block_count(nbins);
+    if (nblk < 1 || nblk > kStaticMaxBlocks) {
+        g_detail = "fdas_whiten_static: block schedule does not fit the fixed scratch array";
+        return FDAS_EUNSUPPORTED;
+    }
+    // set-up, once per device: the device address of the scratch array on the CURRENT device
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess || dev < 0 || dev >= kStaticMaxDevices) {
+        g_detail = std::string("fdas_whiten_static: cudaGetDevice: ") +
+                   (e != cudaSuccess ? cudaGetErrorString(e) : "device ordinal out of range");
+        return FDAS_ECUDA;
+    }
+    unsigned char* base = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mutex);
+        if (!g_static_ptr[dev]) {
+            void* p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_whiten_static_scratch);
+            if (e != cudaSuccess || !p) {
+                g_detail = std::string("fdas_whiten_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e);
+                return FDAS_ECUDA;
+            }
+            g_static_ptr[dev] = static_cast<unsigned char*>(p);
+        }
+        base = g_static_ptr[dev];
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    fdas::WhitenParams w;
+    w.X = reinterpret_cast<const float2*>(d_X);
+    w.spec = d_spec;
+    int32_t* blk_start = reinterpret_cast<int32_t*>(base);
+    int32_t* blk_len = reinterpret_cast<int32_t*>(base + kStaticSection);
+    w.blk_start = blk_start;
+    w.blk_len = blk_len;
+    w.blk_med = reinterpret_cast<float*>(base + 2 * kStaticSection);
+    w.nblk = nblk;
+    w.nbins = nbins;
+    // Nothing in the scratch has to start at zero: the schedule kernel rewrites entries 0..nblk-1 of both
+    // tables and K1a rewrites medians 0..nblk-1 before K1b reads them; entries beyond nblk left by a
+    // longer earlier call are never read.
+    static_schedule_kernel<<<1, 256, 0, st>>>(blk_start, blk_len, (long long)nbins, nblk);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = fdas::launch_whiten(spec_bf16 ? FDAS_BF16 : FDAS_FP32, w, st);
+    if (e != cudaSuccess) {
+        g_detail = std::string("fdas_whiten_static: launch: ") + cudaGetErrorString(e);
+        return FDAS_ECUDA;
+    }
+    return FDAS_OK;
+}

@@ -25,7 +25,7 @@ FDAS_OK, FDAS_EARG, FDAS_EALLOC, FDAS_ECUDA, FDAS_ECUFFT, FDAS_EOVERFLOW, FDAS_E
 EXPORTS = (
     "fdas_plan", "fdas_plan_info", "fdas_prepare_spectrum", "fdas_convolve_plane",
     "fdas_harmonic_sum_peaks", "fdas_plan_invalidate_plane", "fdas_plan_set_harmonic_mode", "fdas_search_host", "fdas_search_batch", "fdas_thresholds_from_sigma",
-    "fdas_plan_templates_host", "fdas_plan_debug_maxplane", "fdas_plan_launch_count", "fdas_destroy", "fdas_strerror",
+    "fdas_whiten_static", "fdas_plan_templates_host", "fdas_plan_debug_maxplane", "fdas_plan_debug_rawspectrum", "fdas_plan_launch_count", "fdas_destroy", "fdas_strerror",
     "fdas_last_error_detail",
 )
 
@@ -70,6 +70,8 @@ def _load():
     L.fdas_thresholds_from_sigma.argtypes = [ci, dbl, C.POINTER(C.c_float)]
     L.fdas_plan_templates_host.argtypes = [vp, vp]
     L.fdas_plan_debug_maxplane.argtypes = [vp, C.POINTER(vp), C.POINTER(i64)]
+    L.fdas_plan_debug_rawspectrum.argtypes = [vp, C.POINTER(vp), C.POINTER(i64)]
+    L.fdas_whiten_static.argtypes = [vp, i64, vp, ci, vp]
     L.fdas_plan_launch_count.argtypes = [vp]
     L.fdas_plan_launch_count.restype = i64
     L.fdas_destroy.argtypes = [vp]
@@ -104,6 +106,21 @@ def _stream_ptr(stream) -> int:
     if stream is None:
         stream = torch.cuda.current_stream()
     return int(stream.cuda_stream)
+
+
+def whiten_static(d_X, nbins: int, d_spec, stream=None):
+    """fdas_whiten_static: whitening without a plan and without any allocation, for callers that may not
+    call cudaMalloc (see include/fdas.h: a real-time stage whose HBM is all in its own pool, a plug-in that
+    may only touch the buffers it is given).  d_X: raw spectrum, a float32 device tensor of >= nbins (re, im)
+    pairs or a raw device pointer (int); d_spec: (nbins, 2) float32 or bfloat16 device tensor (output).
+    At most 2^24 bins (the fixed scratch array's limit); calls on one device must not overlap on the GPU."""
+    import torch
+    x_ptr = d_X.data_ptr() if hasattr(d_X, "data_ptr") else int(d_X)
+    assert d_spec.is_cuda and d_spec.is_contiguous() and d_spec.numel() >= 2 * int(nbins)
+    assert d_spec.dtype in (torch.float32, torch.bfloat16)
+    _check(_lib.fdas_whiten_static(x_ptr, int(nbins), d_spec.data_ptr(),
+                                   1 if d_spec.dtype == torch.bfloat16 else 0, _stream_ptr(stream)),
+           "fdas_whiten_static")
 
 
 @dataclass
@@ -247,6 +264,12 @@ class Plan:
         ptr, pitch = C.c_void_p(), C.c_int64()
         _check(_lib.fdas_plan_debug_maxplane(self._h, C.byref(ptr), C.byref(pitch)), "fdas_plan_debug_maxplane")
         return int(ptr.value), int(pitch.value)
+
+    def debug_rawspectrum(self):
+        """(device pointer, complex length) of the plan-owned raw spectrum X of the last prepare (diagnostic)."""
+        ptr, n = C.c_void_p(), C.c_int64()
+        _check(_lib.fdas_plan_debug_rawspectrum(self._h, C.byref(ptr), C.byref(n)), "fdas_plan_debug_rawspectrum")
+        return int(ptr.value), int(n.value)
 
     def launch_count(self) -> int:
         return int(_lib.fdas_plan_launch_count(self._h))
