@@ -270,6 +270,13 @@ int fdas_plan_debug_maxplane(fdas_plan_t plan, const uint16_t** d_out, int64_t* 
  */
 int fdas_plan_debug_rawspectrum(fdas_plan_t plan, const float** d_out, int64_t* ncomplex_out);
 
+/*
+ * fdas_plan_debug_fail_prepare -- diagnostic, fault injection for the error paths: the (nth + 1)-th prepare step
+ * this plan enqueues from now on (through fdas_prepare_spectrum, fdas_search_host or fdas_search_batch) issues a
+ * CUDA call the runtime refuses and returns FDAS_ECUDA; the counter then disarms.  nth < 0 disarms at once.
+ */
+int fdas_plan_debug_fail_prepare(fdas_plan_t plan, int nth);
+
 /* Number of kernels the library launched on behalf of this plan since it was created. */
 int64_t fdas_plan_launch_count(fdas_plan_t plan);
 

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <cufft.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -21,7 +22,12 @@ using namespace fdas;
 
 thread_local std::string g_detail;
 
-static const int64_t kMaybeCapacity = 1 << 22;  // K3 prefilter survivors (fundamentals) listed per call
+// K3 prefilter survivors (fundamentals) listed per call: half of the plane's points, between 2^16 and 2^22
+// records of 8 bytes (a list that overflows falls back to the exact full scan, so the size is a speed matter)
+static int64_t maybe_capacity_for(const fdas_info_t& in) {
+    const int64_t half = (int64_t)in.nz * in.nbins / 2;
+    return std::min<int64_t>((int64_t)1 << 22, std::max<int64_t>((int64_t)1 << 16, half));
+}
 
 static void free_plan(fdas_plan_s* p) {
     if (!p) return;
@@ -106,12 +112,14 @@ static int build_plan(fdas_plan_s* p) {
         CU(cudaMalloc(&p->d_bank, packed.size() * sizeof(uint32_t)));
         CU(cudaMemcpy(p->d_bank, packed.data(), packed.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
     }
-    std::vector<float> t1, t2;
-    build_twiddles(in.seg_len, &t1, &t2);
-    CU(cudaMalloc(&p->d_tw1, t1.size() * sizeof(float)));
-    CU(cudaMalloc(&p->d_tw2, t2.size() * sizeof(float)));
-    CU(cudaMemcpy(p->d_tw1, t1.data(), t1.size() * sizeof(float), cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(p->d_tw2, t2.data(), t2.size() * sizeof(float), cudaMemcpyHostToDevice));
+    if (!fdas_is_tc(in.precision)) {   // twiddle tables of the segment FFT: the tensor-core path has no use for them
+        std::vector<float> t1, t2;
+        build_twiddles(in.seg_len, &t1, &t2);
+        CU(cudaMalloc(&p->d_tw1, t1.size() * sizeof(float)));
+        CU(cudaMalloc(&p->d_tw2, t2.size() * sizeof(float)));
+        CU(cudaMemcpy(p->d_tw1, t1.data(), t1.size() * sizeof(float), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(p->d_tw2, t2.data(), t2.size() * sizeof(float), cudaMemcpyHostToDevice));
+    }
 
     std::vector<int32_t> bs, bl;
     whitening_blocks(in.nbins, &bs, &bl);
@@ -123,7 +131,8 @@ static int build_plan(fdas_plan_s* p) {
     CU(cudaMemcpy(p->d_blk_len, bl.data(), bl.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
 
     CU(cudaMalloc(&p->d_maxplane, (size_t)in.nz * (size_t)(in.nbins / 8) * sizeof(unsigned short)));
-    CU(cudaMalloc(&p->d_maybe, (size_t)kMaybeCapacity * sizeof(uint2)));
+    p->maybe_capacity = maybe_capacity_for(in);
+    CU(cudaMalloc(&p->d_maybe, (size_t)p->maybe_capacity * sizeof(uint2)));
     CU(cudaMalloc(&p->d_maybe_count, 2 * sizeof(unsigned long long)));
     if (in.nbins % 64 == 0) {
         CU(cudaMalloc(&p->d_max2, (size_t)(in.nbins / 64) * (size_t)in.nz * sizeof(unsigned short)));
@@ -150,6 +159,11 @@ static int build_plan(fdas_plan_s* p) {
 }
 
 int fdas_enqueue_prepare(fdas_plan_s* plan, const float* d_series, void* d_spec, cudaStream_t st) {
+    if (plan->fail_prepare_in >= 0 && plan->fail_prepare_in-- == 0) {   // test hook, off (-1) unless armed
+        cudaMemcpyAsync(nullptr, nullptr, 1, cudaMemcpyDeviceToDevice, st);   // a real refused call: leaves its code in the last-error slot
+        g_detail = "injected failure (fdas_plan_debug_fail_prepare)";
+        return FDAS_ECUDA;
+    }
     CF(cufftSetStream(plan->fft, st));
     CF(cufftExecR2C(plan->fft, const_cast<float*>(d_series), reinterpret_cast<cufftComplex*>(plan->d_X)));
     WhitenParams w;
@@ -200,7 +214,7 @@ int fdas_enqueue_harmonic(fdas_plan_s* plan, const void* d_plane, unsigned short
     for (int i = 0; i < 32; ++i) hp.thr[i] = (i < H) ? h_thresholds[i] : INFINITY;
     hp.cands = d_cands; hp.capacity = capacity; hp.count = d_count;
     hp.maxplane = d_maxplane; hp.mpitch = plan->info.nbins / 8;
-    hp.maybe = plan->d_maybe; hp.maybe_capacity = kMaybeCapacity; hp.maybe_count = plan->d_maybe_count;
+    hp.maybe = plan->d_maybe; hp.maybe_capacity = plan->maybe_capacity; hp.maybe_count = plan->d_maybe_count;
     hp.overflow = reinterpret_cast<unsigned*>(plan->d_maybe_count + 1);
     hp.max2 = plan->d_max2;
     hp.nbr = plan->hsum_mode == FDAS_HSUM_NEIGHBOUR_MAX ? 1 : 0;
@@ -320,8 +334,18 @@ int fdas_search_host(fdas_plan_t plan, const float* h_series, int H, const float
                      void* cuda_stream) {
     if (!plan || !h_series || !h_thresholds || !h_count || capacity < 0 || (capacity > 0 && !h_cands))
         return FDAS_EARG;
+    // everything fdas_harmonic_sum_peaks would refuse is refused here, before any work is queued
+    if (H < 1 || H > 32 || r_lo < 0) return FDAS_EARG;
+    for (int i = 0; i < H; ++i)
+        if (std::isnan(h_thresholds[i])) return FDAS_EARG;
     const fdas_info_t& in = plan->info;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    // the workspace is the plan's: wait for the previous call's work (possibly on another stream) before
+    // the copy below overwrites its series
+    {
+        const int rc0 = order_before(plan, st);
+        if (rc0 != FDAS_OK) return rc0;
+    }
     if (!plan->ws_series) {
         CU(cudaMalloc(&plan->ws_series, (size_t)in.n_in * sizeof(float)));
         CU(cudaMalloc(&plan->ws_spec, (size_t)in.nbins * in.spec_elem_bytes));
@@ -379,6 +403,12 @@ int fdas_plan_debug_rawspectrum(fdas_plan_t plan, const float** d_out, int64_t* 
     if (!plan || !d_out || !ncomplex_out) return FDAS_EARG;
     *d_out = reinterpret_cast<const float*>(plan->d_X);
     *ncomplex_out = plan->info.nfft / 2 + 1;
+    return FDAS_OK;
+}
+
+int fdas_plan_debug_fail_prepare(fdas_plan_t plan, int nth) {
+    if (!plan) return FDAS_EARG;
+    plan->fail_prepare_in = nth;
     return FDAS_OK;
 }
 

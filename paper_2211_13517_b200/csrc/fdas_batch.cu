@@ -210,6 +210,9 @@ extern "C" int fdas_search_batch(fdas_plan_t plan, const float* const* series, i
         cudaStreamSynchronize(s->copy);
         cudaStreamSynchronize(s->a);
         cudaStreamSynchronize(s->b);
+        // the failed call left its code in the runtime's last-error slot: clear it, or the next kernel launch
+        // of this thread would report it (the launch checks read cudaGetLastError)
+        cudaGetLastError();
     }
     // every stream of the batch has been waited for: nothing of this plan is in flight
     plan->have_last = false;

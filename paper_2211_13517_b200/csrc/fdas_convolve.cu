@@ -227,11 +227,12 @@ static cudaError_t launch_one(const ConvParams& p, int64_t nseg, int nsplit, cud
     typedef SegGeom<L> G;
     constexpr int smem = 2 * G::XbufElems * (int)sizeof(float2);
     auto kern = convolve_kernel<PREC, L>;
-    static bool attr_set = false;       // per template instance
-    if (smem > 48 * 1024 && !attr_set) {
-        const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
+    if (smem > 48 * 1024) {
+        static PerDeviceOnce attr;      // per template instance, per device
+        const cudaError_t ea = attr.run([&] {
+            return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        });
+        if (ea != cudaSuccess) return ea;
     }
     kern<<<dim3((unsigned)nseg, (unsigned)nsplit), G::T, smem, st>>>(p);
     return cudaGetLastError();

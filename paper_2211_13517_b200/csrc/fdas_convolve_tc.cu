@@ -633,7 +633,10 @@ static cudaError_t make_plane_map(void* base, int plane16, int64_t cols, int64_t
 }
 
 // The tensor maps depend only on the output pointer and the plane geometry: they are encoded once per
-// plane buffer and kept in the plan's cache.
+// plane buffer and kept in the plan's cache.  Keying an entry by the pointer alone is safe because the
+// cache belongs to ONE plan and everything else a map encodes (element type, nbins, nz, pitch, box rows) is
+// a constant of that plan: a buffer that is freed and handed out again at the same address gets the same
+// map, and a map holds no reference to the memory behind it.
 static cudaError_t get_maps(TcMapCache* cache, int plane16, const ConvTcParams& p, const TcMapCache::Entry** out) {
     for (int i = 0; i < TcMapCache::kEntries; ++i) {
         const TcMapCache::Entry& e = cache->e[i];
@@ -662,12 +665,11 @@ template <int PLANE16, int NBUF>
 static cudaError_t launch_tc(const ConvTcParams& p, const TcMapCache::Entry& m, int nsm, cudaStream_t st) {
     const int smem = convolve_tc_smem_bytes(p.kp, p.npair, PLANE16);
     auto kern = tc::convolve_tc_kernel<PLANE16, NBUF>;
-    static bool attr_set = false;       // per template instance
-    if (!attr_set) {
-        const cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    static PerDeviceOnce attr;          // per template instance, per device
+    const cudaError_t ea = attr.run([&] {
+        return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    });
+    if (ea != cudaSuccess) return ea;
     const int64_t ntiles = p.nbins / tc::kTileR;
     const unsigned grid = (unsigned)(ntiles < nsm ? ntiles : nsm);
     // at least half of the SM's shared memory, so that two CTAs (2 x 512 TMEM columns) never share an SM

@@ -970,9 +970,12 @@ cudaError_t launch_harmonic(int plane_is_bf16, bool build_max, const HarmParams&
     if (coarse) {
         const int c2 = p.nz - 1;
         auto hz_of = [&](int j) { const int d = c2 - 2 * j; return d == 0 ? p.H : std::min(p.H, c2 / d); };
-        while (2 * nlow < p.nz - 1 && hz_of(nlow) <= kShallowDepth) ++nlow;
+        // (the centre row of an odd bank is classified like every other row: with H <= kShallowDepth it is
+        // shallow too, nlow reaches (nz + 1) / 2 and no row is left for the general prefilter -- the same
+        // partition as prefilter_coarse_kernel's `deep`, so that no fundamental is listed twice)
+        while (2 * nlow < p.nz && hz_of(nlow) <= kShallowDepth) ++nlow;
     }
-    const int ndeep = p.nz - 2 * nlow;          // rows with more than kShallowDepth harmonics
+    const int ndeep = std::max(0, p.nz - 2 * nlow);   // rows with more than kShallowDepth harmonics
     // of a deep row the general kernel takes the fundamentals r < 64 b_deep only (those that can have a fifth
     // harmonic inside the plane); the rest goes through the coarse level like the shallow rows
     unsigned b_deep = 0, q_end = (unsigned)(p.mpitch / 4);

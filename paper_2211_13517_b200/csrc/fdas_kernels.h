@@ -1,11 +1,30 @@
 // fdas_kernels.h -- launchers of the three sm_100a kernels behind the C ABI (internal).
 #pragma once
 #include <cuda_runtime.h>
+
+#include <atomic>
 #include <cstdint>
 
 #include "../../include/fdas.h"
 
 namespace fdas {
+
+// A function attribute (cudaFuncSetAttribute) belongs to one device: this remembers, per device ordinal, where
+// it has been set already (one bit per device, safe across host threads; ordinals >= 64 are set every time).
+struct PerDeviceOnce {
+    std::atomic<unsigned long long> mask{0ULL};
+    template <class F>
+    cudaError_t run(F&& set_attribute) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        const bool tracked = dev >= 0 && dev < 64;
+        if (tracked && ((mask.load(std::memory_order_acquire) >> dev) & 1ULL)) return cudaSuccess;
+        e = set_attribute();
+        if (e == cudaSuccess && tracked) mask.fetch_or(1ULL << dev, std::memory_order_release);
+        return e;
+    }
+};
 
 struct ConvParams {
     const void* spec;    // nbins complex: float2 (FDAS_FP32) or packed bf16x2 (re low, im high)

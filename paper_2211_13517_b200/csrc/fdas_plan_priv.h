@@ -49,7 +49,9 @@ struct fdas_plan_s {
     cudaStream_t last_stream = nullptr;
     bool have_last = false;
     unsigned short* d_max2 = nullptr;        // K3 coarse side plane M2 (nz x nbins/64 codes), rebuilt from M by every call
-    uint2* d_maybe = nullptr;                // K3 maybe list (kMaybeCapacity records)
+    uint2* d_maybe = nullptr;                // K3 maybe list (maybe_capacity records)
+    int64_t maybe_capacity = 0;
+    int fail_prepare_in = -1;                // diagnostic (fdas_plan_debug_fail_prepare): >= 0 counts prepares down to an injected failure
     unsigned long long* d_maybe_count = nullptr;
     // workspace of fdas_search_host (lazy)
     float* ws_series = nullptr;

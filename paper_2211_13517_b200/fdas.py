@@ -25,7 +25,7 @@ FDAS_OK, FDAS_EARG, FDAS_EALLOC, FDAS_ECUDA, FDAS_ECUFFT, FDAS_EOVERFLOW, FDAS_E
 EXPORTS = (
     "fdas_plan", "fdas_plan_info", "fdas_prepare_spectrum", "fdas_convolve_plane",
     "fdas_harmonic_sum_peaks", "fdas_plan_invalidate_plane", "fdas_plan_set_harmonic_mode", "fdas_search_host", "fdas_search_batch", "fdas_thresholds_from_sigma",
-    "fdas_whiten_static", "fdas_plan_templates_host", "fdas_plan_debug_maxplane", "fdas_plan_debug_rawspectrum", "fdas_plan_launch_count", "fdas_destroy", "fdas_strerror",
+    "fdas_whiten_static", "fdas_plan_templates_host", "fdas_plan_debug_maxplane", "fdas_plan_debug_rawspectrum", "fdas_plan_debug_fail_prepare", "fdas_plan_launch_count", "fdas_destroy", "fdas_strerror",
     "fdas_last_error_detail",
 )
 
@@ -72,6 +72,7 @@ def _load():
     L.fdas_plan_debug_maxplane.argtypes = [vp, C.POINTER(vp), C.POINTER(i64)]
     L.fdas_plan_debug_rawspectrum.argtypes = [vp, C.POINTER(vp), C.POINTER(i64)]
     L.fdas_whiten_static.argtypes = [vp, i64, vp, ci, vp]
+    L.fdas_plan_debug_fail_prepare.argtypes = [vp, ci]
     L.fdas_plan_launch_count.argtypes = [vp]
     L.fdas_plan_launch_count.restype = i64
     L.fdas_destroy.argtypes = [vp]
@@ -270,6 +271,10 @@ class Plan:
         ptr, n = C.c_void_p(), C.c_int64()
         _check(_lib.fdas_plan_debug_rawspectrum(self._h, C.byref(ptr), C.byref(n)), "fdas_plan_debug_rawspectrum")
         return int(ptr.value), int(n.value)
+
+    def debug_fail_prepare(self, nth: int):
+        """Fault injection (diagnostic): the (nth + 1)-th prepare step enqueued from now on fails with FDAS_ECUDA."""
+        _check(_lib.fdas_plan_debug_fail_prepare(self._h, int(nth)), "fdas_plan_debug_fail_prepare")
 
     def launch_count(self) -> int:
         return int(_lib.fdas_plan_launch_count(self._h))

@@ -23,9 +23,12 @@ def membership_window(thr, h, tol_abs, precision):
 
 
 def gpu_cand_dict(cands):
-    """structured CAND_DTYPE array -> {(r, j, h): (power, flag)}"""
-    return {(int(c["r"]), int(c["zidx"]), int(c["h"])): (float(c["power"]), int(c["flags"]) & 1)
-            for c in cands}
+    """structured CAND_DTYPE array -> {(r, j, h): (power, flag)}; a triple listed twice is an error
+    (the list is a set: fdas.h, "identical to evaluating every fundamental")."""
+    out = {(int(c["r"]), int(c["zidx"]), int(c["h"])): (float(c["power"]), int(c["flags"]) & 1)
+           for c in cands}
+    assert len(out) == len(cands), f"{len(cands) - len(out)} duplicated candidate records"
+    return out
 
 
 def local_amplitude(w, window=NOISE_WINDOW):
@@ -158,14 +161,46 @@ def oracle_margin_fn(oracle, P, H, r_lo):
 
 
 def record_stats(name, stats):
-    """Append one line of measured statistics to gpurun_out/parity_stats.jsonl (read back into
-    profiles/ by hand after a GPU run; best effort, never fails a test)."""
+    """Append one line of measured statistics to the file the environment variable FDAS_PARITY_STATS names
+    (nothing is written without it: a plain test run has no side effect).  `python tests/helpers.py FILE`
+    turns such a file into the markdown table kept under profiles/.  Best effort, never fails a test."""
     import json
     import os
+    path = os.environ.get("FDAS_PARITY_STATS")
+    if not path:
+        return
     try:
-        root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-        os.makedirs(os.path.join(root, "gpurun_out"), exist_ok=True)
-        with open(os.path.join(root, "gpurun_out", "parity_stats.jsonl"), "a") as f:
+        os.makedirs(os.path.dirname(os.path.abspath(path)), exist_ok=True)
+        with open(path, "a") as f:
             f.write(json.dumps({"test": name, **stats}) + "\n")
     except OSError:
         pass
+
+
+def stats_table(lines):
+    """Markdown table of the records record_stats wrote (the last record of each test wins)."""
+    import json
+    seen = {}
+    for line in lines:
+        if line.strip():
+            r = json.loads(line)
+            seen[r["test"]] = r
+
+    def f(r, k, fmt):
+        return fmt % r[k] if k in r else ""
+
+    out = ["| test | plane points | worst abs err / max | noise-floor ratio (A23) | plain ratio, P<30 | common | only GPU | "
+           "only oracle | outside strict window | widest window / T_h | worst rel power | flags checked |",
+           "|---|---|---|---|---|---|---|---|---|---|---|---|"]
+    for k, r in seen.items():
+        out.append(" ".join(str(c) for c in (
+            "|", k, "|", r.get("points", ""), "|", f(r, "worst_over_max", "%.2e"), "|", f(r, "noise_floor_ratio", "%.3f"),
+            "|", f(r, "plain_ratio_P_lt_30", "%.3g"), "|", r.get("common", ""), "|", r.get("only_gpu", ""), "|",
+            r.get("only_orc", ""), "|", r.get("outside_strict", ""), "|", f(r, "worst_window", "%.2e"), "|",
+            f(r, "worst_rel", "%.2e"), "|", r.get("flags_checked", ""), "|")))
+    return "\n".join(out)
+
+
+if __name__ == "__main__":
+    import sys
+    print(stats_table(open(sys.argv[1])))

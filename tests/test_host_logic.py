@@ -253,3 +253,17 @@ def test_bench_starts_its_own_ranks_and_shares_one_workload_string():
     assert t is not None and t["file"].startswith("profiles/") and 3.2e9 < t["traffic"] < 3.6e9
     assert "convolve_tc_kernel" in t["kernel"] and t["commit"]
     assert bench.ncu_traffic("tiny", "bf16_tc") is None
+
+
+def test_parity_stats_are_written_only_on_request_and_tabulated(tmp_path, monkeypatch):
+    import helpers
+    monkeypatch.delenv("FDAS_PARITY_STATS", raising=False)
+    helpers.record_stats("nowhere", {"points": 1})                       # no variable: no file anywhere
+    assert not os.path.exists(os.path.join(str(tmp_path), "stats.jsonl"))
+    path = os.path.join(str(tmp_path), "sub", "stats.jsonl")
+    monkeypatch.setenv("FDAS_PARITY_STATS", path)
+    helpers.record_stats("a", {"points": 10, "worst_over_max": 1e-3, "common": 5})
+    helpers.record_stats("a", {"points": 12, "worst_over_max": 2e-3, "common": 6})
+    helpers.record_stats("b", {"only_gpu": 1})
+    table = helpers.stats_table(open(path)).splitlines()
+    assert len(table) == 4 and table[2].startswith("| a | 12 | 2.00e-03") and "| b |" in table[3]
