@@ -43,6 +43,14 @@ TC_PRECISIONS = ("bf16_tc", "bf16_tc_plane16")
 PROFILES = os.path.join(ROOT, "profiles")
 
 
+# counters of an `ncu --set full` capture kept beside the DRAM traffic (write_traffic_json)
+COUNTER_PREFIXES = ("sm__pipe_tensor_cycles_active", "sm__pipe_fma_cycles_active", "sm__pipe_alu_cycles_active",
+                    "sm__pipe_fmaheavy_cycles_active", "smsp__issue_active", "l1tex__data_pipe_lsu_wavefronts.",
+                    "l1tex__data_pipe_lsu_wavefronts_mem_shared.", "smsp__inst_executed.sum", "sm__warps_active",
+                    "launch__registers_per_thread", "gpu__dram_throughput", "sm__throughput", "dram__throughput",
+                    "sm__cycles_active.avg", "smsp__cycles_active.avg")
+
+
 def ncu_traffic(workload: str, precision: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of ONE K2 launch, from the committed
     profiles/*_traffic.json files (written by `bench.py --traffic-from-ncu` out of an `ncu --set full`
@@ -77,8 +85,15 @@ def write_traffic_json(rep: str, out: str, workload: str, precision: str, comman
         def val(k):
             return float(r[hdr.index(k)]) * scale.get(units[hdr.index(k)], 1.0)
         rd, wr = val("dram__bytes_read.sum"), val("dram__bytes_write.sum")
+        counters = {}
+        for i, name in enumerate(hdr):
+            if name.startswith(COUNTER_PREFIXES) and not any(t in name for t in (".max.", ".min.", ".sum.pct_of_peak", ".sum.per_cycle")):
+                try:
+                    counters[name] = [float(r[i].replace(",", "")), units[i]]
+                except ValueError:
+                    pass
         recs.append({"kernel": r[hdr.index("Kernel Name")], "workload": workload, "precision": precision,
-                     "dram_bytes_read": rd, "dram_bytes_write": wr, "traffic": rd + wr,
+                     "dram_bytes_read": rd, "dram_bytes_write": wr, "traffic": rd + wr, "counters": counters,
                      "duration_us_under_ncu": float(r[hdr.index("gpu__time_duration.sum")]) *
                      {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}[units[hdr.index("gpu__time_duration.sum")]],
                      "command": command,
@@ -156,13 +171,15 @@ def trial_series(wl_name, trial, inputs):
 
 
 class ClockSampler(threading.Thread):
-    """Samples SM clock, power and throttle reasons through NVML while the timed region runs."""
+    """Samples SM clock, power and throttle reasons through NVML while the timed region runs; every sample
+    carries its host time (time.perf_counter) so that it can be paired with CUDA-event times."""
 
     def __init__(self, index: int, period: float = 0.02):
         super().__init__(daemon=True)
-        self.period, self.samples, self.reasons, self.power = period, [], set(), []
+        self.period, self.samples, self.reasons, self.power, self.t = period, [], set(), [], []
         self.stop_flag = threading.Event()
         self.ok = False
+        self.power_kind = "nvmlDeviceGetPowerUsage"
         try:
             import pynvml
             self.nv = pynvml
@@ -170,9 +187,24 @@ class ClockSampler(threading.Thread):
             self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
             self.sm_max = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
             self.ok = True
+            self.instant = getattr(pynvml, "NVML_FI_DEV_POWER_INSTANT", None)
+            if self.instant is not None and self._instant_power() is None:
+                self.instant = None
+            if self.instant is not None:
+                self.power_kind = "NVML_FI_DEV_POWER_INSTANT"
         except Exception as e:   # no NVML: clocks are reported as unavailable
             self.err = repr(e)
             self.sm_max = None
+
+    def _instant_power(self):
+        try:
+            v = self.nv.nvmlDeviceGetFieldValues(self.h, [self.instant])[0]
+            if int(v.nvmlReturn) != 0:
+                return None
+            mw = float(v.value.uiVal)
+            return mw / 1000.0 if mw > 0 else None
+        except Exception:
+            return None
 
     def energy_mj(self):
         try:
@@ -190,8 +222,13 @@ class ClockSampler(threading.Thread):
         }
         while not self.stop_flag.is_set():
             try:
-                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
-                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                mhz = int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                watts = self._instant_power() if self.instant is not None else None
+                if watts is None:
+                    watts = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                self.t.append(time.perf_counter())
+                self.samples.append(mhz)
+                self.power.append(watts)
                 try:
                     r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
                 except Exception:
@@ -207,8 +244,75 @@ class ClockSampler(threading.Thread):
         if not self.ok or not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["nvml_unavailable"]}
         return {"sm_mhz": int(statistics.median(self.samples)), "sm_max_mhz": self.sm_max,
+                "sm_mhz_min": min(self.samples), "sm_mhz_max_seen": max(self.samples),
                 "reasons": sorted(self.reasons), "power_w_mean": round(sum(self.power) / len(self.power), 1),
                 "samples": len(self.samples)}
+
+
+def sustained_loop(step, stream, torch, n_e, local_rank, every=16):
+    """`n_e` identical steps back to back (seconds long: the NVML energy counter needs that, and the board
+    settles at its power cap): J and ms per step, and -- from four CUDA events on every `every`-th step -- the
+    per-call split of the SUSTAINED step and a table of step time, power and J per step binned by the SM clock
+    NVML reported nearest to that step (the clock axis this pool allows: the power cap walks the clock by itself;
+    locking clocks is unavailable here)."""
+    es = ClockSampler(local_rank, period=0.01)
+    if not es.ok:
+        return None
+    marks = list(range(0, n_e, every)) if every > 0 else []
+    evs = {i: [torch.cuda.Event(enable_timing=True) for _ in range(4)] for i in marks}
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    es.start()
+    j0 = es.energy_mj()
+    t_host0 = time.perf_counter()
+    ev0.record(stream)
+    for i in range(n_e):
+        step(i, evs.get(i))
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    j1 = es.energy_mj()
+    es.stop_flag.set()
+    es.join(timeout=2.0)
+    sec = ev0.elapsed_time(ev1) * 1e-3
+    if j0 is None or j1 is None or j1 <= j0:
+        return None
+    if not marks:    # a loop of one call only (energy_by_kernel): no per-step split
+        return {"joules_per_step": (j1 - j0) / 1e3 / n_e, "mean_power_w": (j1 - j0) / 1e3 / sec, "steps": n_e,
+                "seconds": sec, "ms_per_step": 1e3 * sec / n_e, "clocks": es.summary()}
+    rows = []
+    ts = np.array(es.t) - t_host0
+    for i in marks:
+        e = evs[i]
+        rows.append((ev0.elapsed_time(e[0]) * 1e-3, e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2]),
+                     e[2].elapsed_time(e[3])))
+    rows = np.array(rows)
+    out = {"joules_per_step": (j1 - j0) / 1e3 / n_e, "mean_power_w": (j1 - j0) / 1e3 / sec,
+           "steps": n_e, "seconds": sec, "ms_per_step": 1e3 * sec / n_e,
+           "source": "NVML total energy counter over a separate, sustained loop of identical steps",
+           "kernel_ms_sustained": {"prepare_spectrum": float(rows[:, 1].mean()), "convolve_plane": float(rows[:, 2].mean()),
+                                   "harmonic_sum_peaks": float(rows[:, 3].mean()),
+                                   "sampled_steps": int(len(rows)), "every": every,
+                                   "second_half": {"prepare_spectrum": float(rows[len(rows) // 2:, 1].mean()),
+                                                   "convolve_plane": float(rows[len(rows) // 2:, 2].mean()),
+                                                   "harmonic_sum_peaks": float(rows[len(rows) // 2:, 3].mean())}},
+           "clocks": es.summary()}
+    if len(ts) >= 2:
+        mhz, watts = np.array(es.samples, dtype=float), np.array(es.power, dtype=float)
+        near = np.abs(rows[:, 0][:, None] - ts[None, :]).argmin(axis=1)
+        bins = {}
+        for r, k in zip(rows, near):
+            bins.setdefault(int(round(mhz[k] / 50.0) * 50), []).append((r[1] + r[2] + r[3], r[2], watts[k]))
+        table = []
+        for b in sorted(bins, reverse=True):
+            a = np.array(bins[b])
+            table.append({"sm_mhz": b, "n": int(len(a)), "ms_per_step": round(float(a[:, 0].mean()), 4),
+                          "convolve_plane_ms": round(float(a[:, 1].mean()), 4), "power_w": round(float(a[:, 2].mean()), 1),
+                          "joules_per_step": round(float(a[:, 0].mean() * a[:, 2].mean()) * 1e-3, 4)})
+        out["clock_bins"] = {"bin_mhz": 50, "power": es.power_kind, "rows": table,
+                             "note": "every 16th step of the sustained loop, paired with the NVML (SM MHz, W) sample "
+                                     "nearest in time; J per step = W x ms of that bin.  The clock moves only as the "
+                                     "1000 W cap moves it (locked clocks: unavailable on this pool)"}
+    return out
 
 
 # ------------------------------------------------------------------------------- CPU oracle arm
@@ -276,7 +380,8 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------------- CUDA arm
-def time_path(plan, fdas, torch, wl, dev_pool, thr, steps, warmup, energy_seconds, local_rank, barrier):
+def time_path(plan, fdas, torch, wl, dev_pool, thr, steps, warmup, energy_seconds, local_rank, barrier,
+              want_modes=True):
     """`steps` DM trials (prepare_spectrum -> convolve_plane -> harmonic_sum_peaks) of one plan on resident
     series: CUDA events on the launching stream around every call, NVML clocks during the timed region,
     and a second, seconds-long loop of the same steps for the energy per trial (the NVML counter needs
@@ -305,7 +410,7 @@ def time_path(plan, fdas, torch, wl, dev_pool, thr, steps, warmup, energy_second
         step(i)
     torch.cuda.synchronize()
     n_cands = int(d_n.item())
-    sampler = ClockSampler(local_rank)
+    sampler = ClockSampler(local_rank, period=0.001)
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
     launches0 = plan.launch_count()
     barrier()
@@ -328,25 +433,30 @@ def time_path(plan, fdas, torch, wl, dev_pool, thr, steps, warmup, energy_second
     }
     if sampler.ok and energy_seconds > 0:
         n_e = max(steps, int(energy_seconds * 1e3 / max(res["ms_per_step"], 1e-3)) + 1)
-        es = ClockSampler(local_rank, period=0.05)
-        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        es.start()
-        j0 = es.energy_mj()
-        ev0.record(stream)
-        for i in range(n_e):
-            step(i)
-        ev1.record(stream)
-        torch.cuda.synchronize()
-        j1 = es.energy_mj()
-        es.stop_flag.set()
-        es.join(timeout=2.0)
-        sec = ev0.elapsed_time(ev1) * 1e-3
-        if j0 is not None and j1 is not None and j1 > j0:
-            res["energy"] = {"joules_per_step": (j1 - j0) / 1e3 / n_e, "mean_power_w": (j1 - j0) / 1e3 / sec,
-                             "steps": n_e, "seconds": sec, "ms_per_step": 1e3 * sec / n_e,
-                             "source": "NVML total energy counter over a separate, sustained loop of identical steps",
-                             "clocks": es.summary()}
+        res["energy"] = sustained_loop(step, stream, torch, n_e, local_rank)
+    if not want_modes:
+        res["buffers"] = (d_spec, d_plane)
+        return res
+    if res["energy"] is not None and energy_seconds > 0:
+        # where the watts go (the sustained regime is power-bound): each call ALONE in its own seconds-long loop
+        calls = {"prepare_spectrum": lambda i, evs=None: plan.prepare_spectrum(dev_pool[i % pool_n], d_spec, stream),
+                 "convolve_plane": lambda i, evs=None: plan.convolve_plane(d_spec, d_plane, stream),
+                 "harmonic_sum_peaks": lambda i, evs=None: plan.harmonic_sum_peaks(d_plane, wl.nharm, thr, wl.r_lo,
+                                                                                  d_c, d_n, stream)}
+        by = {}
+        for name, fn in calls.items():
+            n_k = int(energy_seconds * 1e3 / max(res["kernel_ms"][name], 1e-3)) + 1
+            e = sustained_loop(fn, stream, torch, n_k, local_rank, every=0)
+            if e is not None:
+                by[name] = {"ms_per_call": e["ms_per_step"], "joules_per_call": e["joules_per_step"],
+                            "mean_power_w": e["mean_power_w"], "sm_mhz": e["clocks"].get("sm_mhz"),
+                            "reasons": e["clocks"].get("reasons"), "calls": e["steps"]}
+        if len(by) == 3:
+            by["sum_joules"] = sum(by[k]["joules_per_call"] for k in calls)
+            by["step_joules"] = res["energy"]["joules_per_step"]
+            by["note"] = ("each call of the step repeated alone for the same number of seconds (its own clock / power "
+                          "equilibrium); the sum against the J of the whole step in the sustained loop")
+            res["energy_by_kernel"] = by
     # both harmonic-sum modes on the plane of the last step: K3 alone, 10 launches each
     modes = {}
     for mode in ("plain", "neighbour_max"):
@@ -365,8 +475,43 @@ def time_path(plan, fdas, torch, wl, dev_pool, thr, steps, warmup, energy_second
     modes["note"] = ("neighbour_max: S'_h = sum_k max_{|d| <= k/2} P[k z][k r + d] (DESIGN.md reading A24), thresholds "
                      "= the plain ones raised by the growth of the noise mean")
     res["harmonic_modes"] = modes
+    res["k3_stress"] = k3_stress(plan, fdas, torch, wl, d_plane, d_c, d_n, stream,
+                                 res["kernel_ms"]["harmonic_sum_peaks"], n_cands)
     res["buffers"] = (d_spec, d_plane)
     return res
+
+
+def k3_stress(plan, fdas, torch, wl, d_plane, d_c, d_n, stream, base_ms, base_cands):
+    """K3 is a data-dependent branch-and-bound: the timed inputs (noise, about one candidate per trial at 6 sigma)
+    are its best case.  The same kernel on the last step's plane under conditions that are not: thresholds low
+    enough to list many fundamentals, low enough to overflow the prefilter's list (exact full scan), and a plane
+    with RFI-like columns far above the saturation value of the block-max codes (127.875)."""
+    def timed(thr, n):
+        plan.harmonic_sum_peaks(d_plane, wl.nharm, thr, wl.r_lo, d_c, d_n, stream)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(n):
+            plan.harmonic_sum_peaks(d_plane, wl.nharm, thr, wl.r_lo, d_c, d_n, stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        return {"harmonic_sum_peaks_ms": a.elapsed_time(b) / n, "candidates": int(d_n.item())}
+
+    out = {"baseline_6_sigma": {"harmonic_sum_peaks_ms": base_ms, "candidates": base_cands}}
+    for ns in (4.0, 3.0, 2.0):
+        out[f"threshold_{ns:g}_sigma"] = timed(fdas.thresholds_from_sigma(wl.nharm, ns), 3)
+    # RFI: 0.5 % of the columns (seeded) multiplied by 1000, in place; the block maxima are then rebuilt from the
+    # plane on every call (fdas_plan_invalidate_plane), which is part of the time below
+    g = torch.Generator(device="cpu")
+    g.manual_seed(2211)
+    nb = int(plan.info.nbins)
+    cols = torch.randperm(nb, generator=g)[: nb // 200].to(d_plane.device)
+    d_plane[:, cols] = d_plane[:, cols] * 1000.0
+    plan.invalidate_plane()
+    out["rfi_columns_6_sigma"] = dict(timed(fdas.thresholds_from_sigma(wl.nharm, wl.nsigma), 3),
+                                      columns=int(cols.numel()), includes="the rebuild of the block maxima from the plane")
+    out["note"] = ("candidate capacity 65536: `candidates` is the true count, only the first 65536 are stored and flagged; "
+                   "2 sigma overflows the 2^22-entry prefilter list, so pass B scans every fundamental")
+    return out
 
 
 def nbr_thresholds(thr):
@@ -380,18 +525,27 @@ def nbr_thresholds(thr):
     return np.array(out, dtype=np.float32)
 
 
-def k2_rooflines(info, precision, workload, t_conv_ms):
-    """The convolve kernel of one path against its binding roof and against HBM (north_star's yardstick)."""
+def k2_rooflines(info, precision, workload, t_conv_ms, t_conv_sustained_ms=None, sustained_clocks=None):
+    """The convolve kernel of one path against its binding roof and against HBM (north_star's yardstick).
+    `t_conv_sustained_ms`: the same launch timed inside the seconds-long, power-capped loop (every 16th step)."""
     points = int(info.nz) * int(info.nbins)
     hbm_peak, peak_kind = measured_peaks()
     gbs = HBM_BYTES_PER_POINT[precision] * points / (t_conv_ms * 1e-3) / 1e9
     traffic = ncu_traffic(workload, precision)
     hbm = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+           "launch_ms": t_conv_ms,
            "peak_kind": f"{peak_kind} copy bandwidth (MEASURED_PEAKS.json)",
            "bytes_per_point": HBM_BYTES_PER_POINT[precision], "bytes_per_launch": HBM_BYTES_PER_POINT[precision] * points,
            "frac_of_8TBs_nominal": gbs / 8000.0,
            "traffic": None if traffic is None else traffic["traffic"],
            "traffic_source": None if traffic is None else {k: traffic[k] for k in ("file", "kernel", "commit", "command")}}
+    if t_conv_sustained_ms:
+        gbs_s = HBM_BYTES_PER_POINT[precision] * points / (t_conv_sustained_ms * 1e-3) / 1e9
+        hbm.update({"launch_ms_sustained": t_conv_sustained_ms, "achieved_sustained": gbs_s,
+                    "frac_sustained": gbs_s / hbm_peak,
+                    "sustained_note": "the same launch inside the seconds-long loop of identical steps (board at its "
+                                      "power cap; CUDA events around every 16th step)",
+                    "sustained_clocks": sustained_clocks})
     if precision in TC_PRECISIONS:
         tpeak, tkind = measured_tensor_peak()
         tflops = tc_mma_flops(info) / (t_conv_ms * 1e-3) / 1e12
@@ -404,8 +558,22 @@ def k2_rooflines(info, precision, workload, t_conv_ms):
         main = {"kernel": "K2 convolve_kernel", "bound": "alu", "achieved": tflops, "peak": ALU_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": tflops / ALU_PEAK_TFLOPS,
                 "peak_kind": "derived: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz", "flops_per_launch": flops,
+                "launch_ms": t_conv_ms,
                 "traffic": hbm["traffic"], "traffic_source": hbm["traffic_source"]}
+        if t_conv_sustained_ms:
+            main.update({"launch_ms_sustained": t_conv_sustained_ms,
+                         "achieved_sustained": flops / (t_conv_sustained_ms * 1e-3) / 1e12,
+                         "frac_sustained": flops / (t_conv_sustained_ms * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+                         "sustained_clocks": sustained_clocks})
     return main, dict(hbm, kernel=main["kernel"])
+
+
+def sustained_of(m):
+    """(K2 launch ms inside the sustained loop, that loop's clocks) of a time_path result, or (None, None)."""
+    e = m.get("energy")
+    if not e or "kernel_ms_sustained" not in e:
+        return None, None
+    return e["kernel_ms_sustained"]["convolve_plane"], e.get("clocks")
 
 
 def seg_len_sweep(fdas, torch, wl, precision, d_x, launches=10):
@@ -437,20 +605,25 @@ def seg_len_sweep(fdas, torch, wl, precision, d_x, launches=10):
 
 
 def survey_block(fdas, torch, inputs, precision, trials_each, pool, thr, local_rank):
-    """configs[4] in small: `trials_each` DM trials of each resolution (64 us: N = 9,375,000; 128 us:
-    N = 4,687,500) through fdas_search_batch from PINNED HOST memory (the H2D copy of every series and the
-    D2H of every candidate list inside the timed region); series cycle a resident host pool."""
+    """configs[4]: DM trials of each resolution (64 us: N = 9,375,000; 128 us: N = 4,687,500) through
+    fdas_search_batch from PINNED HOST memory (the H2D copy of every series and the D2H of every candidate list
+    inside the timed region); series cycle a resident host pool.  trials_each < 0: the paper's counts, 3050 + 2875."""
     stream = torch.cuda.current_stream()
-    cap = 1 << 13
+    cap = 1 << 12
+    full = trials_each < 0
+    counts_of = {False: inputs.SURVEY_TRIALS_FULL if full else trials_each,
+                 True: inputs.SURVEY_TRIALS_HALF if full else trials_each}
     out = {"api": "fdas_search_batch, pinned host series in, candidates on the host out", "precision": precision,
-           "trials_each": trials_each, "shapes": [],
+           "trials": [counts_of[False], counts_of[True]], "whole_survey": full, "shapes": [],
            "note": f"the paper's survey is {inputs.SURVEY_TRIALS_FULL} + {inputs.SURVEY_TRIALS_HALF} trials "
-                   f"(PAPER.md:35, BASELINE.json configs[4]); this block runs {trials_each} of each shape, the "
-                   f"{pool} distinct seeded series of each shape cycled (throughput is data-independent apart "
-                   "from candidate counts); `survey_total_s_extrapolated` scales the per-trial times to the full counts"}
+                   f"(PAPER.md:35, BASELINE.json configs[4]); this block runs {counts_of[False]} + {counts_of[True]}, "
+                   f"the {pool} distinct seeded series of each shape cycled.  The inputs are noise with at most one weak "
+                   "signal (about one candidate per trial at 6 sigma): K3's branch-and-bound is at its best case here, "
+                   "see `k3_stress` for planes that are not"}
     sampler = ClockSampler(local_rank, period=0.05)
     plans = []
     for half in (False, True):
+        trials_each = counts_of[half]
         wl = inputs.ska(half_res=half)
         plan = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, precision)
         host = []
@@ -467,6 +640,7 @@ def survey_block(fdas, torch, inputs, precision, trials_each, pool, thr, local_r
     j0 = sampler.energy_mj() if sampler.ok else None
     t_all0 = time.perf_counter()
     for wl, plan, series, buf in plans:
+        trials_each = len(series)
         t0 = time.perf_counter()
         counts, _, st = plan.search_batch(series, wl.nharm, thr, wl.r_lo, capacity=cap, out=buf, stream=stream)
         torch.cuda.synchronize()
@@ -481,13 +655,18 @@ def survey_block(fdas, torch, inputs, precision, trials_each, pool, thr, local_r
     j1 = sampler.energy_mj() if sampler.ok else None
     sampler.stop_flag.set()
     sampler.join(timeout=2.0)
+    ntot = counts_of[False] + counts_of[True]
     out["total_seconds"] = total
-    out["ms_per_trial"] = 1e3 * total / (2 * trials_each)
+    out["ms_per_trial"] = 1e3 * total / ntot
     if j0 is not None and j1 is not None and j1 > j0:
-        out["joules_per_trial"] = (j1 - j0) / 1e3 / (2 * trials_each)
+        out["joules_per_trial"] = (j1 - j0) / 1e3 / ntot
+        out["joules_total"] = (j1 - j0) / 1e3
         out["mean_power_w"] = (j1 - j0) / 1e3 / total
-    out["survey_total_s_extrapolated"] = (inputs.SURVEY_TRIALS_FULL * out["shapes"][0]["ms_per_trial"]
-                                          + inputs.SURVEY_TRIALS_HALF * out["shapes"][1]["ms_per_trial"]) * 1e-3
+    if full:
+        out["survey_total_s"] = total          # measured: every one of the 5925 trials was run
+    else:
+        out["survey_total_s_extrapolated"] = (inputs.SURVEY_TRIALS_FULL * out["shapes"][0]["ms_per_trial"]
+                                              + inputs.SURVEY_TRIALS_HALF * out["shapes"][1]["ms_per_trial"]) * 1e-3
     out["clocks"] = sampler.summary()
     for _, plan, _, _ in plans:
         plan.close()
@@ -567,7 +746,7 @@ def run_cuda(args):
     torch.cuda.empty_cache()
 
     is_tc = precision in TC_PRECISIONS
-    roofline, roofline_hbm = k2_rooflines(info, precision, args.workload, m["kernel_ms"]["convolve_plane"])
+    roofline, roofline_hbm = k2_rooflines(info, precision, args.workload, m["kernel_ms"]["convolve_plane"], *sustained_of(m))
 
     # ---- beside the tensor-core path: north_star's literal kernel (overlap-save FFT, bf16 storage, fp32
     # arithmetic, no tensor cores) as a FULL record in the same run: step, kernel split, energy, rooflines
@@ -576,9 +755,9 @@ def run_cuda(args):
         fprec = "bf16_plane16" if precision.endswith("plane16") else "bf16"
         plan_f = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, fprec)
         mf = time_path(plan_f, fdas, torch, wl, dev_pool, thr, args.steps, args.warmup, args.energy_seconds,
-                       ctx.local_rank, lambda: None)
+                       ctx.local_rank, lambda: None, want_modes=False)
         mf.pop("buffers")
-        rf, rf_hbm = k2_rooflines(plan_f.info, fprec, args.workload, mf["kernel_ms"]["convolve_plane"])
+        rf, rf_hbm = k2_rooflines(plan_f.info, fprec, args.workload, mf["kernel_ms"]["convolve_plane"], *sustained_of(mf))
         fft_path = {"precision": fprec,
                     "kernel": "K2 convolve_kernel (overlap-save FFT, bf16 storage, fp32 arithmetic, no tensor cores): "
                               "north_star's literal convolve+power kernel",
@@ -586,15 +765,45 @@ def run_cuda(args):
                     "ms_per_step": mf["ms_per_step"], "kernel_ms": mf["kernel_ms"], "energy": mf["energy"],
                     "gpu_launches": int(mf["launches"]), "candidates_last_step": mf["candidates_last_step"],
                     "roofline": rf, "roofline_hbm": rf_hbm, "clocks": mf["clocks"],
-                    "ncu_counters": "profiles/r02b_k3_seglen.md (FMA pipe 63.3 %, LSU wavefronts 73.0 %, issue 52.4 %; SASS: 502 instructions per thread and template)"}
+                    "ncu_counters": None if rf.get("traffic_source") is None else
+                    dict(ncu_traffic(args.workload, fprec).get("counters") or {}, file=rf["traffic_source"]["file"])}
         plan_f.close()
         torch.cuda.empty_cache()
         # the same kernel at the other segment lengths (K2 alone, 10 launches each, same
         # spectrum; flop per plane point 5 L log2 L / (L - 2h) has its minimum near L = 1024-2048 for 129 taps)
         fft_path["seg_len_sweep"] = seg_len_sweep(fdas, torch, wl, fprec, dev_pool[0])
 
+    # ---- SURVEY.md 8(f) #4, precision axis: sustained ms / J per trial of EVERY precision in one record (the two
+    # paths above plus the three the line does not otherwise run), each with its sustained kernel split and its
+    # table binned by the SM clock the power cap produced
+    energy_grid = None
+    if ctx.world == 1 and not args.no_energy_grid and args.energy_seconds > 0 and m["energy"] is not None:
+        def grid_row(prec, burst_ms, e):
+            return {"precision": prec, "ms_per_step_burst": burst_ms, "ms_per_step_sustained": e["ms_per_step"],
+                    "joules_per_step": e["joules_per_step"], "mean_power_w": e["mean_power_w"],
+                    "sm_mhz": e["clocks"].get("sm_mhz"), "reasons": e["clocks"].get("reasons"),
+                    "kernel_ms_sustained": e["kernel_ms_sustained"], "clock_bins": e.get("clock_bins", {}).get("rows")}
+        rows = [grid_row(precision, m["ms_per_step"], m["energy"])]
+        if fft_path is not None and fft_path["energy"] is not None:
+            rows.append(grid_row(fft_path["precision"], fft_path["ms_per_step"], fft_path["energy"]))
+        for prec in ("bf16_tc", "bf16_tc_plane16", "bf16", "bf16_plane16", "fp32"):
+            if any(r["precision"] == prec for r in rows):
+                continue
+            plan_g = fdas.Plan(wl.n, wl.tsamp, wl.zmax, wl.zstep, wl.seg_len, prec)
+            mg = time_path(plan_g, fdas, torch, wl, dev_pool, thr, args.steps, args.warmup, args.energy_seconds,
+                           ctx.local_rank, lambda: None, want_modes=False)
+            mg.pop("buffers")
+            if mg["energy"] is not None:
+                rows.append(grid_row(prec, mg["ms_per_step"], mg["energy"]))
+            plan_g.close()
+            torch.cuda.empty_cache()
+        energy_grid = {"rows": rows, "seconds_each": args.energy_seconds,
+                       "note": "one sustained loop of identical SKA-like steps per precision at default clocks; the clock "
+                               "axis is what the 1000 W cap does by itself (clock_bins); locking clocks is unavailable "
+                               "on this pool (PAPER.md:27, :33-45)"}
+
     survey = None
-    if args.survey_trials > 0 and args.workload == "ska" and ctx.world == 1:
+    if args.survey_trials != 0 and args.workload == "ska" and ctx.world == 1:
         del dev_pool
         torch.cuda.empty_cache()
         survey = survey_block(fdas, torch, inputs, precision, args.survey_trials, min(4, args.pool), thr, ctx.local_rank)
@@ -621,6 +830,7 @@ def run_cuda(args):
         },
         "kernel_ms": m["kernel_ms"],
         "harmonic_modes": m["harmonic_modes"],
+        "k3_stress": m["k3_stress"],
         "candidates_last_step": m["candidates_last_step"],
         "gpu_launches": launches_total,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(info.nfft) * 4,
@@ -631,11 +841,12 @@ def run_cuda(args):
         "roofline": roofline,
         "roofline_hbm": roofline_hbm,
         "roofline_k3": {
-            "kernel": "K3 prefilter kernels + exact_kernel + flag_kernel", "bound": "hbm", "achieved": k3_gbs,
+            "kernel": "K3 prefilter kernels + exact_kernel + flag_kernel", "bound": "latency", "achieved": k3_gbs,
             "peak": hbm_peak, "unit": "GB/s", "frac": k3_gbs / hbm_peak,
-            "note": "algorithmic bytes = one read of the block-max side plane (nz x Nb/8 16-bit codes) that the "
-                    "branch-and-bound prefilter scans; K3 is bound by the latency of dependent loads and by its "
-                    "exact pass's random sector reads, not by DRAM bandwidth (profiles/r02b_k3_seglen.md)",
+            "note": "K3 is bound by the latency of its dependent loads and by the random 32-byte sector reads of its "
+                    "exact pass, not by DRAM bandwidth (profiles/r02b_k3_seglen.md): `achieved` / `frac` are context only "
+                    "-- one read of the block-max side plane (nz x Nb/8 16-bit codes, the bytes the branch-and-bound "
+                    "prefilter has to scan) over the measured K3 time, against the HBM peak",
         },
         "clocks": m["clocks"],
     }
@@ -643,8 +854,22 @@ def run_cuda(args):
         line["fft_path"] = fft_path
     if m["energy"] is not None:
         line["energy"] = m["energy"]
+    if "energy_by_kernel" in m:
+        line["energy_by_kernel"] = m["energy_by_kernel"]
+    if energy_grid is not None:
+        line["energy_grid"] = energy_grid
     if survey is not None:
         line["survey"] = survey
+    if ctx.world > 1:
+        line["config"]["omitted"] = ("with more than one rank the line carries no fft_path, energy_grid, survey or "
+                                     "cpu_baseline block (they are single-GPU records)")
+    if m["energy"] is not None:
+        line["sustained"] = {"ms_per_step": m["energy"]["ms_per_step"],
+                             "value": points / (m["energy"]["ms_per_step"] * 1e-3), "unit": UNIT,
+                             "joules_per_step": m["energy"]["joules_per_step"],
+                             "sm_mhz": m["energy"]["clocks"].get("sm_mhz"),
+                             "note": "the honest per-DM-trial figure of a survey: the seconds-long loop at the power "
+                                     "cap; `value` / `ms_per_step` of the line are the contract's K-step burst"}
     if ctx.rank == 0 and ctx.world == 1 and not args.no_cpu_baseline:
         v, cores, desc, _ = oracle_sample(host_pool[0].numpy(), wl, args.cpu_budget)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
@@ -825,11 +1050,14 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle plane work")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-fft-path", action="store_true", help="skip the full record of the FFT K2 path")
-    ap.add_argument("--survey-trials", type=int, default=768,
-                    help="ska workload, 1 GPU: DM trials of EACH resolution in the `survey` block (0 = off)")
+    ap.add_argument("--survey-trials", type=int, default=-1,
+                    help="ska workload, 1 GPU: DM trials of EACH resolution in the `survey` block "
+                         "(-1 = the paper's 3050 + 2875, 0 = off)")
+    ap.add_argument("--no-energy-grid", action="store_true",
+                    help="skip the sustained ms / J per trial of the precisions the line does not otherwise run")
     ap.add_argument("--traffic-from-ncu", default=None, metavar="REP",
                     help="write the DRAM traffic of the launches in an ncu report to --traffic-out and exit")
-    ap.add_argument("--traffic-out", default=os.path.join(PROFILES, "r02_traffic.json"))
+    ap.add_argument("--traffic-out", default=os.path.join(PROFILES, "r03_traffic.json"))
     ap.add_argument("--traffic-command", default="", help="the command the ncu report was captured with")
     args = ap.parse_args()
     if args.traffic_from_ncu:
