@@ -107,6 +107,30 @@ def test_whiten_static_at_its_maximum_size(fdas):
     plan.close()
 
 
+@pytest.mark.parametrize("spec_dtype", ["float32", "bfloat16"])
+@pytest.mark.parametrize("nbins", [1024, 100_003, 1_000_001])
+def test_whiten_static_against_the_oracle_on_lengths_a_plan_cannot_have(fdas, oracle, nbins, spec_dtype):
+    """A plan always has a power-of-two number of bins; this call takes any length from 1024 to 2^24, so the
+    lengths whose last block is cut short are compared with the CPU oracle's whitening (O2) directly, at the
+    tolerances of the parity tests (2e-5 of the largest modulus for fp32, 1e-2 for bf16 storage), with guard
+    rows behind the output that must stay untouched."""
+    import torch
+    rng = np.random.default_rng(nbins)
+    red = 1.0 + 30.0 / (1.0 + np.arange(nbins + 1) / 500.0)                     # a red-noise-like slope to whiten
+    X32 = np.stack([rng.standard_normal(nbins + 1) * red, rng.standard_normal(nbins + 1) * red], axis=1).astype(np.float32)
+    d_X = torch.from_numpy(X32).cuda()
+    w = oracle.whiten(X32[:nbins, 0].astype(np.float64) + 1j * X32[:nbins, 1].astype(np.float64))
+    dt = getattr(torch, spec_dtype)
+    buf = torch.full((nbins + 64, 2), float("nan"), dtype=dt, device="cuda")
+    fdas.whiten_static(d_X, nbins, buf[:nbins])
+    torch.cuda.synchronize()
+    got = buf[:nbins].float().cpu().numpy().astype(np.float64)
+    assert torch.isnan(buf[nbins:].float()).all().item()                        # nothing written past the end
+    assert not np.isnan(got).any() and got[0, 0] == 0.0 and got[0, 1] == 0.0
+    tol = (2e-5 if spec_dtype == "float32" else 1e-2) * np.abs(w).max()
+    assert np.abs(got[:, 0] + 1j * got[:, 1] - w).max() <= tol
+
+
 def test_whiten_static_refuses_sizes_beyond_the_fixed_array(fdas):
     import torch
     lib = fdas.lib()
