@@ -174,6 +174,8 @@ int fdas_plan_invalidate_plane(fdas_plan_t plan);
  * `cuda_stream`, copies the count and the first min(count, capacity) candidates back and waits for
  * them.  Device workspace (series, spectrum, plane, candidates) is allocated on first use and owned
  * by the plan.  Returns FDAS_EOVERFLOW (after copying `capacity` records) if count > capacity.
+ * FDAS_EARG (NULL pointers, capacity < 0, H outside 1..32, r_lo < 0, a NaN threshold) is returned before any
+ * work is queued; the call first orders itself after the plan's previous call, whatever stream that used.
  */
 int fdas_search_host(fdas_plan_t plan, const float* h_series, int H, const float* h_thresholds,
                      int64_t r_lo, fdas_cand_t* h_cands, int64_t capacity, int64_t* h_count,
